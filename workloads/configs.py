@@ -1,0 +1,169 @@
+"""Workload recipes (BASELINE.json `configs`).
+
+Stand-ins for the paper's Lorenz-driven Hodgkin-Huxley series,
+which is not available.  Everything is drawn from ``numpy.random.default_rng``
+with data seed = 11034887 + config index (+ 1000*chain for batched chains).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+MODEL_LINEAR = 0
+MODEL_HH = 1
+N_CONFIGS = 5
+DATA_SEED0 = 11034887
+
+# (gNa, gK, gL, ENa, EK, EL, C)  -- BASELINE.json config 0 "standard HH" values
+HH_P_TRUE = np.array([120.0, 36.0, 0.3, 50.0, -77.0, -54.4, 1.0])
+
+# tanh kinetics of PAPER.md:268-270 (Eq. 13-14) with Table 1
+# shifted by -65 mV: (V_a, dV_a, tau_a0, tau_a1)
+_KIN = {"m": (-40.0, 15.0, 0.1, 0.4), "h": (-60.0, -15.0, 1.0, 7.0), "n": (-55.0, 30.0, 1.0, 5.0)}
+
+
+def _hh_rhs_batch(x, I, p):
+    """Data-synthesis only.  x: (..., 4) = (V, m, h, n); I: (...,); p: (7,)."""
+    V, m, h, n = x[..., 0], x[..., 1], x[..., 2], x[..., 3]
+    gNa, gK, gL, ENa, EK, EL, C = p
+    out = np.empty_like(x)
+    out[..., 0] = (I + gNa * m**3 * h * (ENa - V) + gK * n**4 * (EK - V) + gL * (EL - V)) / C
+    for j, key in ((1, "m"), (2, "h"), (3, "n")):
+        Va, dVa, t0, t1 = _KIN[key]
+        th = np.tanh((V - Va) / dVa)
+        out[..., j] = (0.5 + 0.5 * th - x[..., j]) / (t0 + t1 * (1.0 - th * th))
+    return out
+
+
+def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1):
+    """Twin-experiment data: returns I (C,M+1), x_true (C,M+1,4), y (C,M+1).
+
+    Step current: 5 ms segments, segment k covers steps [k*5/dt, (k+1)*5/dt), amplitude U(0,15) uA/cm2.
+    Truth: RK4 at dt with midpoint current 0.5*(I_n + I_{n+1}); x(0) = rest at -65 mV.
+    Observation: V + N(0, 1 mV).
+    """
+    seg = int(round(5.0 / dt))
+    nseg = M // seg + 2
+    amp = rng.uniform(0.0, 15.0, size=(n_chains, nseg))
+    idx = np.arange(M + 1) // seg
+    I = amp[:, idx]
+    x = np.empty((n_chains, M + 1, 4))
+    V0 = -65.0
+    x[:, 0, 0] = V0
+    for j, key in ((1, "m"), (2, "h"), (3, "n")):
+        Va, dVa, _, _ = _KIN[key]
+        x[:, 0, j] = 0.5 + 0.5 * np.tanh((V0 - Va) / dVa)
+    p = HH_P_TRUE
+    for k in range(M):
+        xn = x[:, k]
+        I0, I1 = I[:, k], I[:, k + 1]
+        Ih = 0.5 * (I0 + I1)
+        k1 = _hh_rhs_batch(xn, I0, p)
+        k2 = _hh_rhs_batch(xn + 0.5 * dt * k1, Ih, p)
+        k3 = _hh_rhs_batch(xn + 0.5 * dt * k2, Ih, p)
+        k4 = _hh_rhs_batch(xn + dt * k3, I1, p)
+        x[:, k + 1] = xn + (dt / 6.0) * (k1 + 2 * k2 + 2 * k3 + k4)
+    y = x[:, :, 0] + rng.normal(0.0, 1.0, size=(n_chains, M + 1))
+    return I, x, y
+
+
+def linear_matrix(D: int = 2, rho: float = 0.99, theta: float = 0.05) -> np.ndarray:
+    """Config 1 map matrix A = 0.99 * R(0.05 rad) (row-major D*D; D=1 gives [[rho]])."""
+    if D == 1:
+        return np.array([[rho]])
+    A = np.eye(D)
+    c, s = np.cos(theta), np.sin(theta)
+    A[0, 0], A[0, 1], A[1, 0], A[1, 1] = c, -s, s, c
+    return rho * A
+
+
+def linear_truth(M: int, rng: np.random.Generator, D: int = 2, q_sd: float = 0.1, r_sd: float = 0.1):
+    """x_{n+1} = A x_n + N(0, q_sd^2 I), x_0 ~ N(0, I); y_n = x_{n,0} + N(0, r_sd^2)."""
+    A = linear_matrix(D)
+    x = np.empty((M + 1, D))
+    x[0] = rng.normal(size=D)
+    for k in range(M):
+        x[k + 1] = A @ x[k] + q_sd * rng.normal(size=D)
+    y = x[:, 0] + r_sd * rng.normal(size=M + 1)
+    return A, x, y
+
+
+@dataclass
+class Workload:
+    """Everything pimc_init / pimc_set_* need, as plain numpy arrays (fp64)."""
+    name: str
+    model: int
+    D: int
+    L: int
+    Np: int
+    M: int
+    dt: float
+    Rm: float
+    Rf: np.ndarray            # (D,)
+    n_chains: int
+    p0: np.ndarray            # (C, Np)
+    p_true: np.ndarray        # (Np,)
+    lo: np.ndarray            # (C, Np)
+    hi: np.ndarray            # (C, Np)
+    w_state: np.ndarray       # (D,)
+    w_param: np.ndarray       # (Np,)  0 = frozen
+    y: np.ndarray             # (C, M+1, L)
+    I: np.ndarray | None      # (C, M+1) or None
+    x0: np.ndarray            # (C, M+1, D) initial path
+    x_true: np.ndarray        # (C, M+1, D)
+    n_sweeps: int
+    chain_seed: int = 1       # Philox key; chain index goes in the counter
+    extra: dict = field(default_factory=dict)
+
+
+_WP_CFG2 = np.array([0.10, 0.03, 0.008, 0.025, 0.035, 0.5, 0.004])
+_WP_CFG3 = np.array([0.07, 0.02, 0.005, 0.018, 0.025, 0.4, 0.0026])
+
+
+def _hh_workload(name, cfg, M, dt, n_chains, w_param, n_sweeps, estimate, seed=None):
+    rng = np.random.default_rng(DATA_SEED0 + cfg if seed is None else seed)
+    I, xt, y = hh_truth(M, dt, rng, n_chains)
+    x0 = np.empty((n_chains, M + 1, 4))
+    x0[:, :, 0] = y
+    x0[:, :, 1:] = 0.5
+    pt = HH_P_TRUE
+    if estimate:
+        s = np.where(rng.random((n_chains, 7)) < 0.5, -1.0, 1.0)      # G8: +-20 % off truth
+        p0 = pt[None, :] * (1.0 + 0.2 * s)
+        wp = np.asarray(w_param, float)
+    else:
+        p0 = np.tile(pt, (n_chains, 1))
+        wp = np.zeros(7)
+    lo = np.tile(pt - 0.5 * np.abs(pt), (n_chains, 1))
+    hi = np.tile(pt + 0.5 * np.abs(pt), (n_chains, 1))
+    return Workload(name=name, model=MODEL_HH, D=4, L=1, Np=7, M=M, dt=dt, Rm=1.0,
+                    Rf=np.array([1e2, 1e4, 1e4, 1e4]), n_chains=n_chains, p0=p0, p_true=pt.copy(),
+                    lo=lo, hi=hi, w_state=np.array([0.5, 0.02, 0.02, 0.02]), w_param=wp,
+                    y=y[:, :, None].copy(), I=I, x0=x0, x_true=xt, n_sweeps=n_sweeps)
+
+
+def make_workload(cfg: int, *, M: int | None = None, n_chains: int | None = None,
+                  seed: int | None = None) -> Workload:
+    """BASELINE.json `configs[cfg]`; M / n_chains may be overridden to make small parity cases."""
+    if cfg == 0:
+        return _hh_workload("cfg0_hh_M256", 0, M or 256, 0.02, n_chains or 1, None, 2000, False, seed)
+    if cfg == 1:
+        M = M or 4096
+        rng = np.random.default_rng(DATA_SEED0 + 1 if seed is None else seed)
+        A, xt, y = linear_truth(M, rng)
+        x0 = np.zeros((1, M + 1, 2))
+        x0[0, :, 0] = y
+        return Workload(name="cfg1_linear_M4096", model=MODEL_LINEAR, D=2, L=1, Np=4, M=M, dt=1.0,
+                        Rm=100.0, Rf=np.array([100.0, 100.0]), n_chains=1, p0=A.reshape(1, 4).copy(),
+                        p_true=A.reshape(4).copy(), lo=np.full((1, 4), -2.0), hi=np.full((1, 4), 2.0),
+                        w_state=np.array([0.1, 0.1]), w_param=np.zeros(4), y=y[None, :, None].copy(),
+                        I=None, x0=x0, x_true=xt[None], n_sweeps=5000)
+    if cfg == 2:
+        return _hh_workload("cfg2_hh_M4096_params", 2, M or 4096, 0.02, n_chains or 1, _WP_CFG2, 20000, True, seed)
+    if cfg == 3:
+        return _hh_workload("cfg3_hh_M32768_params", 3, M or 32768, 0.01, n_chains or 1, _WP_CFG3, 10000, True, seed)
+    if cfg == 4:
+        return _hh_workload("cfg4_hh_128x8192_params", 4, M or 8192, 0.02, n_chains or 128,
+                            _WP_CFG2 / np.sqrt(2.0), 5000, True, seed)
+    raise ValueError(f"no config {cfg}")
