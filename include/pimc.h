@@ -1,0 +1,172 @@
+/* pimc.h -- C ABI of libpimc: B200-native (sm_100a) path-integral Monte Carlo hot path.
+ *
+ * Method: Quinn & Abarbanel, "Data Assimilation using a GPU Accelerated Path Integral Monte Carlo
+ * Approach", arXiv 1103.4887.  Citations are /root/reference/PAPER.md:<line> (not present at run time).
+ *
+ * What is sampled: paths X = {x_0..x_M} (D components per time step) and N_p model parameters p,
+ * distributed as exp(-A), with the action (Eq. for A_o, A_d; RK4-map form of the
+ * model error named by BASELINE.json's north_star):
+ *     A(X,p) = sum_{n=1..M} sum_{l<L} (Rm/2) (y_{n,l} - x_{n,l})^2
+ *            + sum_{n=0..M-1} sum_{a<D} (Rf_a/2) ((x_{n+1,a} - x_{n,a}) - g_a(x_n, p; I_n, I_{n+1}))^2
+ * where g is the increment of one model step (HH: one classical RK4 step of size dt; LINEAR: A x - x).
+ *
+ * One "sweep" (Fig. 1): Metropolis update of every even site, then of every odd site
+ * (joint Gaussian or uniform proposal of all D components, one accept per site, Eq. 9);
+ * then each parameter with non-zero width in sequence (proposals outside
+ * [lo,hi] are rejected); then, if enabled, accumulation of running moments and
+ * histograms.  All random numbers come from Philox4x32-10 keyed by
+ * (seed; site-or-parameter, sweep, chain, stream) so results do not depend on the launch shape.
+ *
+ * Conventions
+ *  - Every function returns PIMC_OK or a negative error; the first error message is kept and can be
+ *    read with pimc_last_error().  No C++ exception crosses this boundary.
+ *  - "dev" pointers are CUDA device pointers owned by the caller; "host" pointers are ordinary host
+ *    memory.  The library copies what it needs into the caller-provided workspace during the call
+ *    (asynchronously on `stream`), so inputs may be freed once the stream has passed the call.
+ *  - Arrays are row-major and contiguous.  Element type of x, y, I, p, trace arrays = `dtype`
+ *    (64: double, 32: float).  Moments are always double, counters unsigned 64-bit.
+ *  - All work is enqueued on the `stream` given to pimc_init (a cudaStream_t cast to void*; NULL =
+ *    the legacy default stream).  Nothing synchronises the host except where stated.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns PIMC_ECUDA.
+ */
+#ifndef PIMC_H
+#define PIMC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pimc_handle pimc_handle;
+
+enum { PIMC_OK = 0, PIMC_EINVAL = -1, PIMC_ESTATE = -2, PIMC_ECUDA = -3, PIMC_EUNSUPPORTED = -4, PIMC_ENOMEM = -5 };
+
+/* Models.  LINEAR: D in 1..4, parameters = the D*D map matrix (row-major), g = A x - x.
+ * HH: D = 4, x = (V,m,h,n), p = (gNa,gK,gL,ENa,EK,EL,C); tanh kinetics of PAPER.md:256-270 (Eq. 11-14)
+ * with Table 1 shifted by -65 mV; needs the injected current I. */
+enum { PIMC_MODEL_LINEAR = 0, PIMC_MODEL_HH = 1 };
+enum { PIMC_PROPOSAL_GAUSSIAN = 0, PIMC_PROPOSAL_UNIFORM = 1 };
+
+/* Number of parameters the model defines (HH: 7, LINEAR: D*D); negative on bad arguments. */
+int pimc_model_np(int model, int D);
+
+/* Bytes of device workspace pimc_init needs for this problem (0 on bad arguments). */
+size_t pimc_workspace_bytes(int model, int D, int L, int M, int n_chains, int dtype);
+
+/* Create a handle.  model/D/L/M: problem shape (x has M+1 time steps; the first L components are
+ * observed, h(x) = x[0:L]).  dt: time step of the RK4 map.  Rm: measurement precision
+ * (scalar, R_o of PAPER.md:135).  Rf: host, D model-error precisions (diagonal R_d).
+ * p0: host, n_chains*Np initial parameters.  dtype: 64 or 32.  workspace: dev, 256-byte aligned,
+ * at least pimc_workspace_bytes(); it is zero-filled here and owned by the caller, who must keep it
+ * alive until pimc_destroy.  Errors: PIMC_EINVAL (shape, non-finite dt/Rm/Rf, alignment, size),
+ * PIMC_EUNSUPPORTED (D the model does not define), PIMC_ECUDA (no device / CUDA failure). */
+int pimc_init(pimc_handle** h, int model, int D, int L, int M, double dt, double Rm, const double* Rf,
+              const double* p0, int n_chains, int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Observations y: dev (n_chains, M+1, L) (y_0 is never used by the action) and injected
+ * current I: dev (n_chains, M+1) or NULL (treated as 0).  Rebuilds the step cache if a path is set. */
+int pimc_set_data(pimc_handle* h, const void* y, const void* I);
+
+/* Current path x: dev (n_chains, M+1, D).  Copies in and rebuilds the cache g_n = g(x_n,p), n < M
+ * ("Calculate and store new RHS").  PIMC_ESTATE before pimc_set_data. */
+int pimc_set_path(pimc_handle* h, const void* x);
+
+/* Current parameters p: dev (n_chains, Np).  Copies in and rebuilds the cache. */
+int pimc_set_params(pimc_handle* h, const void* p);
+
+/* Copy out the current path (dev (n_chains, M+1, D)) and/or parameters (dev (n_chains, Np)); either may be NULL. */
+int pimc_get_path(pimc_handle* h, void* x_out, void* p_out);
+
+/* Copy out the current step cache g: dev (n_chains, M, D) (for cache-coherence checks). */
+int pimc_get_cache(pimc_handle* h, void* g_out);
+
+/* Proposal widths (PAPER.md:188 step (a), 226): w_state host D values >= 0; w_param host Np values >= 0
+ * or NULL (= all 0; a parameter with width 0 is frozen and never proposed); kind = PIMC_PROPOSAL_*. */
+int pimc_set_proposal(pimc_handle* h, const double* w_state, const double* w_param, int kind);
+
+/* Parameter bounds (uniform prior): host (n_chains, Np) each, lo <= hi.  Default: none. */
+int pimc_set_bounds(pimc_handle* h, const double* lo, const double* hi);
+
+/* Moment / histogram accumulation: enabled != 0 accumulates after every n_skip-th sweep,
+ * counted from the sweep at which it was (re)enabled or last reset. */
+int pimc_set_accum(pimc_handle* h, int enabled, long long n_skip);
+
+/* Zero the running sums and histogram counts and re-centre them on the current path and parameters. */
+int pimc_reset_moments(pimc_handle* h);
+
+/* Run n_sweeps sweeps on all chains (asynchronous on the stream; one persistent kernel launch).  The
+ * absolute sweep index (part of the RNG counter) continues across calls, so sweep(a)+sweep(b) ==
+ * sweep(a+b) bit for bit.  PIMC_ESTATE before set_data/set_path/set_proposal. */
+int pimc_sweep(pimc_handle* h, long long n_sweeps, unsigned long long seed);
+
+/* Only the state half-sweeps (rows A2/A3) or only the parameter moves (PAPER.md:199,
+ * 209; row A4) of pimc_sweep -- for measuring the two separately.  Same RNG counters as pimc_sweep. */
+int pimc_sweep_states_only(pimc_handle* h, long long n_sweeps, unsigned long long seed);
+int pimc_sweep_params_only(pimc_handle* h, long long n_sweeps, unsigned long long seed);
+
+/* Moments: out dev double, per chain [mean x (M+1,D), var x (M+1,D), mean p (Np), var p (Np)], chains
+ * concatenated; population variance.  n_samples_host (may be NULL) receives the sample count (host
+ * bookkeeping, no device sync). */
+int pimc_moments(pimc_handle* h, double* out, unsigned long long* n_samples_host);
+
+/* Acceptance counters: acc_out dev u64 (n_chains, 2, D+Np) = accepted, proposed per
+ * component class (joint proposals: all D entries equal) and per parameter. */
+int pimc_stats(pimc_handle* h, unsigned long long* acc_out);
+
+/* Histograms ("bin counts"): n_sel selections, host arrays: site[i] (>= 0: path site,
+ * -1: parameter), comp[i] (component or parameter index), range [lo[i],hi[i]), nbins bins plus an
+ * underflow and an overflow bin.  Applies to every chain.  n_sel = 0 disables.  n_sel <= 64. */
+int pimc_hist_config(pimc_handle* h, int n_sel, const int* site, const int* comp, const double* lo,
+                     const double* hi, int nbins);
+/* counts_out: dev u64 (n_chains, n_sel, nbins+2) = under, bins..., over. */
+int pimc_hist(pimc_handle* h, unsigned long long* counts_out);
+
+/* Debug trace, filled by the LAST sweep of each later pimc_sweep call (all-NULL disables; no cost then):
+ * dA_out dev (n_chains, M+1) per-site Delta-A; acc_out dev u8 (n_chains, M+1) decisions; xprop_out dev
+ * (n_chains, M+1, D) proposals or NULL; dA_param dev (n_chains, Np) (NaN = not evaluated: frozen or out of
+ * bounds); acc_param dev u8 (n_chains, Np); pprop_out dev (n_chains, Np) proposed parameter values or NULL. */
+int pimc_debug_trace(pimc_handle* h, void* dA_out, unsigned char* acc_out, void* xprop_out, void* dA_param,
+                     unsigned char* acc_param, void* pprop_out);
+
+/* Launch shape: CTAs per chain (0 = automatic) and threads per CTA (0 = automatic, multiple of 32,
+ * <= 1024).  More than one CTA per chain uses a cooperative launch with neighbour hand-off between
+ * half-sweeps; PIMC_EINVAL if the grid would not be co-resident. */
+int pimc_set_launch(pimc_handle* h, int ctas_per_chain, int threads_per_cta);
+/* Report the launch shape that pimc_sweep will use (any pointer may be NULL). */
+int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, int* tile_sites, int* smem_bytes);
+
+unsigned long long pimc_sweep_index(const pimc_handle* h);
+int pimc_set_sweep_index(pimc_handle* h, unsigned long long t);
+
+/* Number of kernels this handle has launched so far (for bench.py's gpu_launches). */
+unsigned long long pimc_launch_count(const pimc_handle* h);
+
+/* End-to-end convenience on HOST buffers (all host, dtype elements except moments): allocates its own
+ * device memory, copies y, I (may be NULL), x0, p0 in, runs n_burn sweeps, then n_sweeps sweeps with
+ * accumulation every sweep, copies moments_out (host double, layout of pimc_moments) and, if non-NULL,
+ * the final path x_out / parameters p_out back, synchronises and frees.  Uses the default stream. */
+int pimc_run_host(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype,
+                  const void* y, const void* I, const void* x0, const void* p0, const double* w_state,
+                  const double* w_param, const double* lo, const double* hi, int proposal_kind, long long n_burn,
+                  long long n_sweeps, unsigned long long seed, double* moments_out, void* x_out, void* p_out);
+
+/* RNG self-test entry (rows A1 / pin P4): fills out (dev u32, n*4) with Philox4x32-10(ctr[i], key), ctrs
+ * dev u32 (n,4); and the library's transforms: u_prop dev double n*4 = (w+0.5)2^-32 per word, u_acc dev
+ * double n = ((w1:w0 >> 12)+0.5)2^-52, z dev double n*4 = Box-Muller pairs (words 0,1) and (2,3).  Any
+ * output may be NULL. */
+int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned int key0, unsigned int key1,
+                      unsigned int* out, double* u_prop, double* u_acc, double* z, void* stream);
+
+/* Model self-test entry (row A0): g_out dev (n, D) = step increment at x dev (n, D) with parameters p dev (Np),
+ * currents I0, I1 dev (n) (NULL = 0), in `dtype` arithmetic. */
+int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p, const void* I0, const void* I1,
+                       double dt, unsigned long long n, void* g_out, void* stream);
+
+const char* pimc_last_error(const pimc_handle* h);   /* h may be NULL: last error of a failed pimc_init / static call */
+int pimc_destroy(pimc_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIMC_H */

@@ -1,0 +1,9 @@
+"""pimc-b200: B200-native (sm_100a) path-integral Monte Carlo data assimilation (arXiv 1103.4887).
+
+The product is ``libpimc.so`` (C ABI in ``include/pimc.h``); this package is the thin Python binding.
+There is no CPU fallback: every compute entry point runs CUDA kernels or raises.
+"""
+from .binding import (  # noqa: F401
+    MODEL_LINEAR, MODEL_HH, PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM, PimcError, Pimc, lib, library_path,
+    model_np, rng_selftest, step_selftest, run_host, exported_symbols,
+)

@@ -1,0 +1,636 @@
+// Host side of libpimc: the C ABI declared in include/pimc.h (argument checks, workspace carving, launch
+// configuration, absolute sweep counter).  All compute happens in the kernels of pimc_kernels.cuh; there
+// is no CPU fallback.
+#include "../../include/pimc.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pimc_kernels.cuh"
+
+using namespace pimc;
+
+namespace {
+
+thread_local std::string g_static_error;
+
+struct Carve {   // bump allocator over the caller's workspace; also used to size it
+    char* base;
+    size_t off = 0;
+    explicit Carve(char* b) : base(b) {}
+    template <typename T> T* take(size_t n) {
+        off = (off + 255) & ~(size_t)255;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+struct Layout {
+    void *x, *g0, *g1, *y, *I, *p;
+    int* cur;
+    double *lo, *hi, *cx, *S1x, *S2x, *cp, *S1p, *S2p;
+    unsigned long long* counters;
+    int *hsite, *hcomp;
+    double *hlo, *hhi, *hwidth;
+    unsigned long long* hist;
+    unsigned long long *hs_flag, *ar_flag, *ar_epoch;
+    double* ar_val;
+    size_t bytes;
+};
+
+constexpr int kMaxCtasPerChain = 1024;
+constexpr size_t kMaxHistWords = 1u << 20;   // u64 counters reserved for histograms (all chains)
+
+Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
+    const size_t es = dtype == 64 ? 8 : 4;
+    Carve c(base);
+    Layout o{};
+    const size_t nx = (size_t)C * (M + 1) * D, ng = (size_t)C * M * D;
+    o.x = c.take<char>(nx * es);
+    o.g0 = c.take<char>(ng * es);
+    o.g1 = c.take<char>(ng * es);
+    o.y = c.take<char>((size_t)C * (M + 1) * (L > 0 ? L : 1) * es);
+    o.I = c.take<char>((size_t)C * (M + 1) * es);
+    o.p = c.take<char>((size_t)C * Np * es);
+    o.cur = c.take<int>(C);
+    o.lo = c.take<double>((size_t)C * Np);
+    o.hi = c.take<double>((size_t)C * Np);
+    o.cx = c.take<double>(nx);
+    o.S1x = c.take<double>(nx);
+    o.S2x = c.take<double>(nx);
+    o.cp = c.take<double>((size_t)C * Np);
+    o.S1p = c.take<double>((size_t)C * Np);
+    o.S2p = c.take<double>((size_t)C * Np);
+    o.counters = c.take<unsigned long long>((size_t)C * 2 * (D + Np));
+    o.hsite = c.take<int>(kMaxHistSel);
+    o.hcomp = c.take<int>(kMaxHistSel);
+    o.hlo = c.take<double>(kMaxHistSel);
+    o.hhi = c.take<double>(kMaxHistSel);
+    o.hwidth = c.take<double>(kMaxHistSel);
+    o.hist = c.take<unsigned long long>(kMaxHistWords);
+    o.hs_flag = c.take<unsigned long long>((size_t)C * kMaxCtasPerChain);
+    o.ar_flag = c.take<unsigned long long>((size_t)C * 2 * kMaxCtasPerChain);
+    o.ar_val = c.take<double>((size_t)C * 2 * kMaxCtasPerChain);
+    o.ar_epoch = c.take<unsigned long long>(C);
+    o.bytes = (c.off + 255) & ~(size_t)255;
+    return o;
+}
+
+bool shape_ok(int model, int D, int L, int M, int C, int dtype, int* why) {
+    *why = PIMC_EINVAL;
+    if (!(model == PIMC_MODEL_LINEAR || model == PIMC_MODEL_HH)) return false;
+    if (D < 1 || L < 0 || L > D || M < 1 || C < 1 || !(dtype == 64 || dtype == 32)) return false;
+    *why = PIMC_EUNSUPPORTED;
+    if (model == PIMC_MODEL_HH && D != 4) return false;
+    if (model == PIMC_MODEL_LINEAR && D > 4) return false;
+    if ((long long)C * ((long long)M + 1) > (1ll << 31)) return false;
+    return true;
+}
+
+}  // namespace
+
+struct pimc_handle {
+    int model, D, L, M, Np, C, dtype;
+    double dt, Rm, Rf[kMaxD];
+    cudaStream_t stream;
+    Layout lay;
+    double wx[kMaxD], wp[kMaxNp];
+    int kind = 0;
+    bool have_data = false, have_path = false, have_prop = false, have_I = false;
+    int accum = 0;
+    unsigned long long n_skip = 1, t_enable = 0, n_samples = 0, t = 0;
+    int n_sel = 0, nbins = 0;
+    void *tr_dA = nullptr, *tr_xprop = nullptr, *tr_dAp = nullptr, *tr_pprop = nullptr;
+    unsigned char *tr_acc = nullptr, *tr_accp = nullptr;
+    int G_user = 0, T_user = 0;
+    unsigned long long hs_base = 0, launches = 0;
+    int sm_count = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(pimc_handle* h, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (h) { if (h->err.empty()) h->err = buf; }
+    else g_static_error = buf;
+    return code;
+}
+#define PIMC_CUDA(h, call)                                                                        \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) return fail(h, PIMC_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+// ---- model / dtype dispatch --------------------------------------------------------------------------
+template <typename F> int dispatch(int model, int D, int dtype, F&& f) {
+    if (model == PIMC_MODEL_HH) {
+        if (dtype == 64) return f(HHModel<double>{}, double{});
+        return f(HHModel<float>{}, float{});
+    }
+    switch (D * 100 + dtype) {
+        case 164: return f(LinearModel<double, 1>{}, double{});
+        case 264: return f(LinearModel<double, 2>{}, double{});
+        case 364: return f(LinearModel<double, 3>{}, double{});
+        case 464: return f(LinearModel<double, 4>{}, double{});
+        case 132: return f(LinearModel<float, 1>{}, float{});
+        case 232: return f(LinearModel<float, 2>{}, float{});
+        case 332: return f(LinearModel<float, 3>{}, float{});
+        case 432: return f(LinearModel<float, 4>{}, float{});
+    }
+    return PIMC_EUNSUPPORTED;
+}
+
+struct LaunchShape { int G, T, tile; bool cooperative; };
+
+// Choose CTAs per chain, threads per CTA and the tile length (even).
+template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape* out) {
+    int T = h->T_user;
+    int G = h->G_user;
+    const int sites = h->M + 1;
+    int per_sm = 0;
+    if (G == 0) {
+        // many chains: one CTA per chain, no inter-CTA traffic.  few chains: spread each over the SMs.
+        if (h->C >= h->sm_count / 2) G = 1;
+        else {
+            if (T == 0) T = 128;
+            PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R>, T, 0));
+            const int cap = per_sm > 0 ? h->sm_count : 0;    // one CTA per SM: the FP64 pipe is the shared resource
+            G = (sites + 2 * T - 1) / (2 * T);
+            if (G > cap / h->C) G = cap / h->C;
+            if (G < 1) G = 1;
+        }
+    }
+    if (T == 0) T = (G == 1) ? kMaxThreads : 128;
+    if (T % 32 != 0 || T < 32 || T > kMaxThreads) return fail(h, PIMC_EINVAL, "threads_per_cta must be a multiple of 32 in [32,%d]", kMaxThreads);
+    if (G > kMaxCtasPerChain) return fail(h, PIMC_EINVAL, "ctas_per_chain > %d", kMaxCtasPerChain);
+    int tile = (sites + G - 1) / G;
+    tile += tile & 1;
+    G = (sites + tile - 1) / tile;     // drop empty tiles
+    out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1;
+    if (G > 1) {
+        PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R>, T, 0));
+        if ((long long)G * h->C > (long long)per_sm * h->sm_count)
+            return fail(h, PIMC_EINVAL, "grid of %d CTAs is not co-resident (capacity %d)", G * h->C, per_sm * h->sm_count);
+    }
+    return PIMC_OK;
+}
+
+template <class Model, typename R> int rebuild_cache(pimc_handle* h) {
+    const size_t total = (size_t)h->C * h->M;
+    const int threads = 128;
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, 148 * 16);
+    // after a rebuild, buffer 0 is current
+    build_cache_kernel<Model, R><<<blocks, threads, 0, h->stream>>>((const R*)h->lay.x, h->have_I ? (const R*)h->lay.I : nullptr,
+                                                                     (const R*)h->lay.p, (R*)h->lay.g0, h->M, h->C, (R)h->dt);
+    h->launches++;
+    PIMC_CUDA(h, cudaGetLastError());
+    PIMC_CUDA(h, cudaMemsetAsync(h->lay.cur, 0, sizeof(int) * h->C, h->stream));
+    return PIMC_OK;
+}
+
+int rebuild(pimc_handle* h) {
+    return dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return rebuild_cache<decltype(model), decltype(real)>(h); });
+}
+
+template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
+    LaunchShape ls;
+    int rc = choose_shape<Model, R>(h, &ls);
+    if (rc != PIMC_OK) return rc;
+    SweepArgs<R> a{};
+    a.M = h->M; a.L = h->L; a.n_chains = h->C; a.G = ls.G; a.tile = ls.tile; a.kind = h->kind;
+    a.dt = (R)h->dt; a.Rm = (R)h->Rm;
+    for (int c = 0; c < h->D; ++c) { a.Rf[c] = (R)h->Rf[c]; a.wx[c] = (R)h->wx[c]; }
+    for (int l = 0; l < h->Np; ++l) a.wp[l] = h->wp[l];
+    a.x = (R*)h->lay.x; a.g[0] = (R*)h->lay.g0; a.g[1] = (R*)h->lay.g1;
+    a.y = (const R*)h->lay.y; a.I = h->have_I ? (const R*)h->lay.I : nullptr;
+    a.p = (R*)h->lay.p; a.cur = h->lay.cur; a.lo = h->lay.lo; a.hi = h->lay.hi;
+    a.accum = h->accum; a.n_skip = h->n_skip; a.t_enable = h->t_enable;
+    a.cx = h->lay.cx; a.S1x = h->lay.S1x; a.S2x = h->lay.S2x; a.cp = h->lay.cp; a.S1p = h->lay.S1p; a.S2p = h->lay.S2p;
+    a.counters = h->lay.counters;
+    a.n_sel = h->n_sel; a.nbins = h->nbins;
+    a.hsite = h->lay.hsite; a.hcomp = h->lay.hcomp; a.hlo = h->lay.hlo; a.hhi = h->lay.hhi; a.hwidth = h->lay.hwidth; a.hist = h->lay.hist;
+    a.tr_dA = (R*)h->tr_dA; a.tr_acc = h->tr_acc; a.tr_xprop = (R*)h->tr_xprop;
+    a.tr_dAp = (R*)h->tr_dAp; a.tr_accp = h->tr_accp; a.tr_pprop = (R*)h->tr_pprop;
+    a.t0 = h->t; a.seed = seed; a.n_sweeps = n_sweeps; a.do_states = do_states; a.do_params = do_params;
+    a.hs_flag = h->lay.hs_flag; a.ar_val = h->lay.ar_val; a.ar_flag = h->lay.ar_flag; a.ar_epoch = h->lay.ar_epoch;
+    a.hs_base = h->hs_base;
+
+    const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
+    if (ls.cooperative) {
+        void* params[] = {&a};
+        PIMC_CUDA(h, cudaLaunchCooperativeKernel((const void*)sweep_kernel<Model, R>, grid, block, params, 0, h->stream));
+    } else {
+        sweep_kernel<Model, R><<<grid, block, 0, h->stream>>>(a);
+        PIMC_CUDA(h, cudaGetLastError());
+    }
+    h->launches++;
+    if (do_states) h->hs_base += 2ull * (unsigned long long)n_sweeps;
+    if (h->accum) {   // host bookkeeping of the sample count: sweeps t in [t0, t0+n) with (t - t_enable) % n_skip == 0
+        const unsigned long long first = h->t - h->t_enable, last = first + (unsigned long long)n_sweeps;   // [first, last)
+        const unsigned long long k = h->n_skip;
+        h->n_samples += (last + k - 1) / k - (first + k - 1) / k;
+    }
+    h->t += (unsigned long long)n_sweeps;
+    return PIMC_OK;
+}
+
+int sweep_common(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
+    if (!h) return PIMC_EINVAL;
+    if (n_sweeps < 0) return fail(h, PIMC_EINVAL, "n_sweeps < 0");
+    if (!h->have_data || !h->have_path || !h->have_prop) return fail(h, PIMC_ESTATE, "pimc_sweep before set_data / set_path / set_proposal");
+    if (n_sweeps == 0) return PIMC_OK;
+    if (((h->t + (unsigned long long)n_sweeps) >> 48) != 0) return fail(h, PIMC_EINVAL, "sweep index exceeds 48 bits");
+    return dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) {
+        return run_sweeps<decltype(model), decltype(real)>(h, n_sweeps, seed, do_states, do_params);
+    });
+}
+
+int recentre(pimc_handle* h) {
+    const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
+    const int threads = 256;
+    const int bx = (int)std::min<size_t>((nx + threads - 1) / threads, 148 * 8), bp = (int)((np + threads - 1) / threads);
+    if (h->dtype == 64) {
+        widen_kernel<double><<<bx, threads, 0, h->stream>>>((const double*)h->lay.x, h->lay.cx, nx);
+        if (np) widen_kernel<double><<<bp, threads, 0, h->stream>>>((const double*)h->lay.p, h->lay.cp, np);
+    } else {
+        widen_kernel<float><<<bx, threads, 0, h->stream>>>((const float*)h->lay.x, h->lay.cx, nx);
+        if (np) widen_kernel<float><<<bp, threads, 0, h->stream>>>((const float*)h->lay.p, h->lay.cp, np);
+    }
+    h->launches += np ? 2 : 1;
+    PIMC_CUDA(h, cudaGetLastError());
+    return PIMC_OK;
+}
+
+bool finite_all(const double* v, int n) {
+    for (int i = 0; i < n; ++i) if (!std::isfinite(v[i])) return false;
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pimc_model_np(int model, int D) {
+    if (model == PIMC_MODEL_HH) return D == 4 ? 7 : -1;
+    if (model == PIMC_MODEL_LINEAR) return (D >= 1 && D <= 4) ? D * D : -1;
+    return -1;
+}
+
+size_t pimc_workspace_bytes(int model, int D, int L, int M, int n_chains, int dtype) {
+    int why;
+    if (!shape_ok(model, D, L, M, n_chains, dtype, &why)) return 0;
+    return carve(nullptr, D, L, M, pimc_model_np(model, D), n_chains, dtype).bytes;
+}
+
+int pimc_init(pimc_handle** out, int model, int D, int L, int M, double dt, double Rm, const double* Rf, const double* p0,
+              int n_chains, int dtype, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!out) return fail(nullptr, PIMC_EINVAL, "null handle pointer");
+    *out = nullptr;
+    int why;
+    if (!shape_ok(model, D, L, M, n_chains, dtype, &why)) return fail(nullptr, why, "bad or unsupported shape (model=%d D=%d L=%d M=%d chains=%d dtype=%d)", model, D, L, M, n_chains, dtype);
+    if (!Rf || !p0) return fail(nullptr, PIMC_EINVAL, "Rf and p0 are required");
+    if (!std::isfinite(dt) || !std::isfinite(Rm) || Rm < 0 || !finite_all(Rf, D)) return fail(nullptr, PIMC_EINVAL, "dt, Rm, Rf must be finite (Rm, Rf >= 0)");
+    for (int c = 0; c < D; ++c) if (Rf[c] < 0) return fail(nullptr, PIMC_EINVAL, "Rf must be >= 0");
+    const int Np = pimc_model_np(model, D);
+    if (!finite_all(p0, n_chains * Np)) return fail(nullptr, PIMC_EINVAL, "p0 must be finite");
+    const size_t need = carve(nullptr, D, L, M, Np, n_chains, dtype).bytes;
+    if (!workspace || ((uintptr_t)workspace & 255) != 0) return fail(nullptr, PIMC_EINVAL, "workspace must be a 256-byte aligned device pointer");
+    if (workspace_bytes < need) return fail(nullptr, PIMC_EINVAL, "workspace too small: %zu < %zu", workspace_bytes, need);
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(nullptr, PIMC_ECUDA, "no CUDA device: libpimc has no CPU fallback");
+    pimc_handle* h = new (std::nothrow) pimc_handle();
+    if (!h) return fail(nullptr, PIMC_ENOMEM, "out of host memory");
+    h->model = model; h->D = D; h->L = L; h->M = M; h->Np = Np; h->C = n_chains; h->dtype = dtype;
+    h->dt = dt; h->Rm = Rm;
+    for (int c = 0; c < D; ++c) h->Rf[c] = Rf[c];
+    for (int c = 0; c < kMaxD; ++c) h->wx[c] = 0.0;
+    for (int l = 0; l < kMaxNp; ++l) h->wp[l] = 0.0;
+    h->stream = (cudaStream_t)stream;
+    h->lay = carve((char*)workspace, D, L, M, Np, n_chains, dtype);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaMemsetAsync(workspace, 0, need, h->stream);
+    // parameters and (infinite) bounds
+    std::vector<double> lo((size_t)n_chains * Np, -INFINITY), hi((size_t)n_chains * Np, INFINITY);
+    if (e == cudaSuccess && Np) {
+        if (dtype == 64) e = cudaMemcpyAsync(h->lay.p, p0, sizeof(double) * n_chains * Np, cudaMemcpyHostToDevice, h->stream);
+        else {
+            std::vector<float> pf(p0, p0 + (size_t)n_chains * Np);
+            e = cudaMemcpyAsync(h->lay.p, pf.data(), sizeof(float) * n_chains * Np, cudaMemcpyHostToDevice, h->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);   // pf is a temporary
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h->lay.lo, lo.data(), sizeof(double) * lo.size(), cudaMemcpyHostToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h->lay.hi, hi.data(), sizeof(double) * hi.size(), cudaMemcpyHostToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);       // host temporaries go out of scope
+    }
+    if (e != cudaSuccess) {
+        fail(nullptr, PIMC_ECUDA, "pimc_init: %s", cudaGetErrorString(e));
+        delete h;
+        return PIMC_ECUDA;
+    }
+    *out = h;
+    return PIMC_OK;
+}
+
+int pimc_set_data(pimc_handle* h, const void* y, const void* I) {
+    if (!h) return PIMC_EINVAL;
+    if (h->L > 0 && !y) return fail(h, PIMC_EINVAL, "y is required when L > 0");
+    const size_t es = h->dtype == 64 ? 8 : 4;
+    if (h->L > 0) PIMC_CUDA(h, cudaMemcpyAsync(h->lay.y, y, (size_t)h->C * (h->M + 1) * h->L * es, cudaMemcpyDeviceToDevice, h->stream));
+    if (h->model == PIMC_MODEL_HH && !I) return fail(h, PIMC_EINVAL, "the HH model needs the injected current I");
+    h->have_I = I != nullptr;
+    if (I) PIMC_CUDA(h, cudaMemcpyAsync(h->lay.I, I, (size_t)h->C * (h->M + 1) * es, cudaMemcpyDeviceToDevice, h->stream));
+    h->have_data = true;
+    if (h->have_path) return rebuild(h);
+    return PIMC_OK;
+}
+
+int pimc_set_path(pimc_handle* h, const void* x) {
+    if (!h || !x) return fail(h, PIMC_EINVAL, "null argument");
+    if (!h->have_data) return fail(h, PIMC_ESTATE, "pimc_set_path before pimc_set_data");
+    const size_t es = h->dtype == 64 ? 8 : 4;
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.x, x, (size_t)h->C * (h->M + 1) * h->D * es, cudaMemcpyDeviceToDevice, h->stream));
+    h->have_path = true;
+    return rebuild(h);
+}
+
+int pimc_set_params(pimc_handle* h, const void* p) {
+    if (!h || !p) return fail(h, PIMC_EINVAL, "null argument");
+    const size_t es = h->dtype == 64 ? 8 : 4;
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.p, p, (size_t)h->C * h->Np * es, cudaMemcpyDeviceToDevice, h->stream));
+    if (h->have_path) return rebuild(h);
+    return PIMC_OK;
+}
+
+int pimc_get_path(pimc_handle* h, void* x_out, void* p_out) {
+    if (!h) return PIMC_EINVAL;
+    const size_t es = h->dtype == 64 ? 8 : 4;
+    if (x_out) PIMC_CUDA(h, cudaMemcpyAsync(x_out, h->lay.x, (size_t)h->C * (h->M + 1) * h->D * es, cudaMemcpyDeviceToDevice, h->stream));
+    if (p_out) PIMC_CUDA(h, cudaMemcpyAsync(p_out, h->lay.p, (size_t)h->C * h->Np * es, cudaMemcpyDeviceToDevice, h->stream));
+    return PIMC_OK;
+}
+
+int pimc_get_cache(pimc_handle* h, void* g_out) {
+    if (!h || !g_out) return fail(h, PIMC_EINVAL, "null argument");
+    if (!h->have_path) return fail(h, PIMC_ESTATE, "no path set");
+    const size_t es = h->dtype == 64 ? 8 : 4;
+    // the selector lives on the device; chains may differ, so copy chain by chain after reading it back
+    std::vector<int> cur(h->C);
+    PIMC_CUDA(h, cudaMemcpyAsync(cur.data(), h->lay.cur, sizeof(int) * h->C, cudaMemcpyDeviceToHost, h->stream));
+    PIMC_CUDA(h, cudaStreamSynchronize(h->stream));
+    const size_t per = (size_t)h->M * h->D * es;
+    for (int c = 0; c < h->C; ++c) {
+        const char* src = (const char*)(cur[c] ? h->lay.g1 : h->lay.g0) + per * c;
+        PIMC_CUDA(h, cudaMemcpyAsync((char*)g_out + per * c, src, per, cudaMemcpyDeviceToDevice, h->stream));
+    }
+    return PIMC_OK;
+}
+
+int pimc_set_proposal(pimc_handle* h, const double* w_state, const double* w_param, int kind) {
+    if (!h || !w_state) return fail(h, PIMC_EINVAL, "null argument");
+    if (!(kind == PIMC_PROPOSAL_GAUSSIAN || kind == PIMC_PROPOSAL_UNIFORM)) return fail(h, PIMC_EINVAL, "unknown proposal kind");
+    for (int c = 0; c < h->D; ++c) if (!(w_state[c] >= 0) || !std::isfinite(w_state[c])) return fail(h, PIMC_EINVAL, "w_state must be finite and >= 0");
+    if (w_param) for (int l = 0; l < h->Np; ++l) if (!(w_param[l] >= 0) || !std::isfinite(w_param[l])) return fail(h, PIMC_EINVAL, "w_param must be finite and >= 0");
+    for (int c = 0; c < h->D; ++c) h->wx[c] = w_state[c];
+    for (int l = 0; l < h->Np; ++l) h->wp[l] = w_param ? w_param[l] : 0.0;
+    h->kind = kind;
+    h->have_prop = true;
+    return PIMC_OK;
+}
+
+int pimc_set_bounds(pimc_handle* h, const double* lo, const double* hi) {
+    if (!h || !lo || !hi) return fail(h, PIMC_EINVAL, "null argument");
+    const size_t n = (size_t)h->C * h->Np;
+    for (size_t i = 0; i < n; ++i) if (!(lo[i] <= hi[i])) return fail(h, PIMC_EINVAL, "bounds need lo <= hi");
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.lo, lo, sizeof(double) * n, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.hi, hi, sizeof(double) * n, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaStreamSynchronize(h->stream));   // lo/hi are pageable host memory owned by the caller
+    return PIMC_OK;
+}
+
+int pimc_set_accum(pimc_handle* h, int enabled, long long n_skip) {
+    if (!h) return PIMC_EINVAL;
+    if (n_skip < 1) return fail(h, PIMC_EINVAL, "n_skip must be >= 1");
+    if (enabled && !h->accum) h->t_enable = h->t;
+    h->accum = enabled ? 1 : 0;
+    h->n_skip = (unsigned long long)n_skip;
+    return PIMC_OK;
+}
+
+int pimc_reset_moments(pimc_handle* h) {
+    if (!h) return PIMC_EINVAL;
+    if (!h->have_path) return fail(h, PIMC_ESTATE, "no path set");
+    const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
+    PIMC_CUDA(h, cudaMemsetAsync(h->lay.S1x, 0, sizeof(double) * nx, h->stream));
+    PIMC_CUDA(h, cudaMemsetAsync(h->lay.S2x, 0, sizeof(double) * nx, h->stream));
+    if (np) {
+        PIMC_CUDA(h, cudaMemsetAsync(h->lay.S1p, 0, sizeof(double) * np, h->stream));
+        PIMC_CUDA(h, cudaMemsetAsync(h->lay.S2p, 0, sizeof(double) * np, h->stream));
+    }
+    if (h->n_sel) PIMC_CUDA(h, cudaMemsetAsync(h->lay.hist, 0, sizeof(unsigned long long) * (size_t)h->C * h->n_sel * (h->nbins + 2), h->stream));
+    h->n_samples = 0;
+    h->t_enable = h->t;
+    return recentre(h);
+}
+
+int pimc_sweep(pimc_handle* h, long long n_sweeps, unsigned long long seed) { return sweep_common(h, n_sweeps, seed, 1, 1); }
+int pimc_sweep_states_only(pimc_handle* h, long long n_sweeps, unsigned long long seed) { return sweep_common(h, n_sweeps, seed, 1, 0); }
+int pimc_sweep_params_only(pimc_handle* h, long long n_sweeps, unsigned long long seed) { return sweep_common(h, n_sweeps, seed, 0, 1); }
+
+int pimc_moments(pimc_handle* h, double* out, unsigned long long* n_samples_host) {
+    if (!h || !out) return fail(h, PIMC_EINVAL, "null argument");
+    const size_t nx = (size_t)(h->M + 1) * h->D;
+    const size_t total = (size_t)h->C * (nx + h->Np);
+    const int threads = 256;
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, 148 * 8);
+    moments_kernel<<<blocks, threads, 0, h->stream>>>(h->lay.cx, h->lay.S1x, h->lay.S2x, h->lay.cp, h->lay.S1p, h->lay.S2p, nx, h->Np,
+                                                      h->C, (double)h->n_samples, out);
+    h->launches++;
+    PIMC_CUDA(h, cudaGetLastError());
+    if (n_samples_host) *n_samples_host = h->n_samples;
+    return PIMC_OK;
+}
+
+int pimc_stats(pimc_handle* h, unsigned long long* acc_out) {
+    if (!h || !acc_out) return fail(h, PIMC_EINVAL, "null argument");
+    PIMC_CUDA(h, cudaMemcpyAsync(acc_out, h->lay.counters, sizeof(unsigned long long) * (size_t)h->C * 2 * (h->D + h->Np),
+                                 cudaMemcpyDeviceToDevice, h->stream));
+    return PIMC_OK;
+}
+
+int pimc_hist_config(pimc_handle* h, int n_sel, const int* site, const int* comp, const double* lo, const double* hi, int nbins) {
+    if (!h) return PIMC_EINVAL;
+    if (n_sel < 0 || n_sel > kMaxHistSel) return fail(h, PIMC_EINVAL, "n_sel must be in [0,%d]", kMaxHistSel);
+    if (n_sel == 0) { h->n_sel = 0; return PIMC_OK; }
+    if (!site || !comp || !lo || !hi || nbins < 1) return fail(h, PIMC_EINVAL, "bad histogram arguments");
+    if ((size_t)h->C * n_sel * (nbins + 2) > kMaxHistWords) return fail(h, PIMC_EINVAL, "histogram storage exceeds %zu counters", kMaxHistWords);
+    std::vector<double> width(n_sel);
+    for (int i = 0; i < n_sel; ++i) {
+        if (site[i] > h->M || site[i] < -1) return fail(h, PIMC_EINVAL, "histogram site out of range");
+        if (comp[i] < 0 || comp[i] >= (site[i] < 0 ? h->Np : h->D)) return fail(h, PIMC_EINVAL, "histogram component out of range");
+        if (!(lo[i] < hi[i])) return fail(h, PIMC_EINVAL, "histogram range needs lo < hi");
+        width[i] = (hi[i] - lo[i]) / nbins;
+    }
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.hsite, site, sizeof(int) * n_sel, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.hcomp, comp, sizeof(int) * n_sel, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.hlo, lo, sizeof(double) * n_sel, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.hhi, hi, sizeof(double) * n_sel, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaMemcpyAsync(h->lay.hwidth, width.data(), sizeof(double) * n_sel, cudaMemcpyHostToDevice, h->stream));
+    PIMC_CUDA(h, cudaMemsetAsync(h->lay.hist, 0, sizeof(unsigned long long) * (size_t)h->C * n_sel * (nbins + 2), h->stream));
+    PIMC_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->n_sel = n_sel; h->nbins = nbins;
+    return PIMC_OK;
+}
+
+int pimc_hist(pimc_handle* h, unsigned long long* counts_out) {
+    if (!h || !counts_out) return fail(h, PIMC_EINVAL, "null argument");
+    if (!h->n_sel) return fail(h, PIMC_ESTATE, "no histogram configured");
+    PIMC_CUDA(h, cudaMemcpyAsync(counts_out, h->lay.hist, sizeof(unsigned long long) * (size_t)h->C * h->n_sel * (h->nbins + 2),
+                                 cudaMemcpyDeviceToDevice, h->stream));
+    return PIMC_OK;
+}
+
+int pimc_debug_trace(pimc_handle* h, void* dA_out, unsigned char* acc_out, void* xprop_out, void* dA_param, unsigned char* acc_param,
+                     void* pprop_out) {
+    if (!h) return PIMC_EINVAL;
+    h->tr_dA = dA_out; h->tr_acc = acc_out; h->tr_xprop = xprop_out; h->tr_dAp = dA_param; h->tr_accp = acc_param; h->tr_pprop = pprop_out;
+    return PIMC_OK;
+}
+
+int pimc_set_launch(pimc_handle* h, int ctas_per_chain, int threads_per_cta) {
+    if (!h) return PIMC_EINVAL;
+    if (ctas_per_chain < 0 || ctas_per_chain > kMaxCtasPerChain) return fail(h, PIMC_EINVAL, "ctas_per_chain out of range");
+    if (threads_per_cta != 0 && (threads_per_cta % 32 != 0 || threads_per_cta < 32 || threads_per_cta > kMaxThreads))
+        return fail(h, PIMC_EINVAL, "threads_per_cta must be 0 or a multiple of 32 in [32,%d]", kMaxThreads);
+    const int G0 = h->G_user, T0 = h->T_user;
+    h->G_user = ctas_per_chain; h->T_user = threads_per_cta;
+    LaunchShape ls;
+    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    if (rc != PIMC_OK) { h->G_user = G0; h->T_user = T0; }
+    return rc;
+}
+
+int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, int* tile_sites, int* smem_bytes) {
+    if (!h) return PIMC_EINVAL;
+    LaunchShape ls;
+    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    if (rc != PIMC_OK) return rc;
+    if (ctas_per_chain) *ctas_per_chain = ls.G;
+    if (threads_per_cta) *threads_per_cta = ls.T;
+    if (tile_sites) *tile_sites = ls.tile;
+    if (smem_bytes) *smem_bytes = 0;
+    return PIMC_OK;
+}
+
+unsigned long long pimc_sweep_index(const pimc_handle* h) { return h ? h->t : 0; }
+int pimc_set_sweep_index(pimc_handle* h, unsigned long long t) {
+    if (!h) return PIMC_EINVAL;
+    if ((t >> 48) != 0) return fail(h, PIMC_EINVAL, "sweep index exceeds 48 bits");
+    h->t = t;
+    return PIMC_OK;
+}
+unsigned long long pimc_launch_count(const pimc_handle* h) { return h ? h->launches : 0; }
+
+int pimc_run_host(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype, const void* y,
+                  const void* I, const void* x0, const void* p0, const double* w_state, const double* w_param, const double* lo,
+                  const double* hi, int proposal_kind, long long n_burn, long long n_sweeps, unsigned long long seed, double* moments_out,
+                  void* x_out, void* p_out) {
+    int why;
+    if (!shape_ok(model, D, L, M, n_chains, dtype, &why)) return fail(nullptr, why, "bad or unsupported shape");
+    if (!x0 || !p0 || !w_state || !moments_out || (L > 0 && !y)) return fail(nullptr, PIMC_EINVAL, "null argument");
+    const int Np = pimc_model_np(model, D);
+    const size_t es = dtype == 64 ? 8 : 4;
+    const size_t nx = (size_t)n_chains * (M + 1) * D, ny = (size_t)n_chains * (M + 1) * (L > 0 ? L : 1), nI = (size_t)n_chains * (M + 1);
+    const size_t nmom = (size_t)n_chains * (2 * (size_t)(M + 1) * D + 2 * (size_t)Np);
+    const size_t ws = pimc_workspace_bytes(model, D, L, M, n_chains, dtype);
+    char* dev = nullptr;
+    const size_t o_x = 0, o_y = o_x + ((nx * es + 255) & ~(size_t)255), o_I = o_y + ((ny * es + 255) & ~(size_t)255),
+                 o_p = o_I + ((nI * es + 255) & ~(size_t)255), o_m = o_p + (((size_t)n_chains * Np * es + 255) & ~(size_t)255),
+                 o_ws = o_m + ((nmom * 8 + 255) & ~(size_t)255);
+    if (cudaMalloc(&dev, o_ws + ws) != cudaSuccess) return fail(nullptr, PIMC_ENOMEM, "cudaMalloc of %zu bytes failed", o_ws + ws);
+    pimc_handle* h = nullptr;
+    int rc = PIMC_OK;
+    cudaError_t e = cudaSuccess;
+    // parameters as doubles for pimc_init (host side)
+    std::vector<double> p0d((size_t)n_chains * Np);
+    for (size_t i = 0; i < p0d.size(); ++i) p0d[i] = dtype == 64 ? ((const double*)p0)[i] : (double)((const float*)p0)[i];
+    do {
+        if ((e = cudaMemcpyAsync(dev + o_x, x0, nx * es, cudaMemcpyHostToDevice, 0)) != cudaSuccess) break;
+        if (L > 0 && (e = cudaMemcpyAsync(dev + o_y, y, ny * es, cudaMemcpyHostToDevice, 0)) != cudaSuccess) break;
+        if (I && (e = cudaMemcpyAsync(dev + o_I, I, nI * es, cudaMemcpyHostToDevice, 0)) != cudaSuccess) break;
+        if ((rc = pimc_init(&h, model, D, L, M, dt, Rm, Rf, p0d.data(), n_chains, dtype, dev + o_ws, ws, nullptr)) != PIMC_OK) break;
+        if ((rc = pimc_set_data(h, dev + o_y, I ? dev + o_I : nullptr)) != PIMC_OK) break;
+        if ((rc = pimc_set_proposal(h, w_state, w_param, proposal_kind)) != PIMC_OK) break;
+        if (lo && hi && (rc = pimc_set_bounds(h, lo, hi)) != PIMC_OK) break;
+        if ((rc = pimc_set_path(h, dev + o_x)) != PIMC_OK) break;
+        if ((rc = pimc_sweep(h, n_burn, seed)) != PIMC_OK) break;
+        if ((rc = pimc_set_accum(h, 1, 1)) != PIMC_OK) break;
+        if ((rc = pimc_reset_moments(h)) != PIMC_OK) break;
+        if ((rc = pimc_sweep(h, n_sweeps, seed)) != PIMC_OK) break;
+        if ((rc = pimc_moments(h, (double*)(dev + o_m), nullptr)) != PIMC_OK) break;
+        if ((e = cudaMemcpyAsync(moments_out, dev + o_m, nmom * 8, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) break;
+        if (x_out || p_out) {
+            if ((rc = pimc_get_path(h, x_out ? dev + o_x : nullptr, p_out ? dev + o_p : nullptr)) != PIMC_OK) break;
+            if (x_out && (e = cudaMemcpyAsync(x_out, dev + o_x, nx * es, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) break;
+            if (p_out && (e = cudaMemcpyAsync(p_out, dev + o_p, (size_t)n_chains * Np * es, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) break;
+        }
+        e = cudaStreamSynchronize(0);
+    } while (0);
+    if (rc != PIMC_OK && h) g_static_error = h->err;
+    if (e != cudaSuccess) { rc = fail(nullptr, PIMC_ECUDA, "pimc_run_host: %s", cudaGetErrorString(e)); }
+    if (h) pimc_destroy(h);
+    cudaFree(dev);
+    return rc;
+}
+
+int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned int key0, unsigned int key1, unsigned int* out,
+                      double* u_prop, double* u_acc, double* z, void* stream) {
+    if (!ctrs) return fail(nullptr, PIMC_EINVAL, "null argument");
+    if (n == 0) return PIMC_OK;
+    const int threads = 256;
+    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, 148ull * 8);
+    rng_selftest_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(ctrs, n, key0, key1, out, u_prop, u_acc, z);
+    PIMC_CUDA(nullptr, cudaGetLastError());
+    return PIMC_OK;
+}
+
+int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p, const void* I0, const void* I1, double dt,
+                       unsigned long long n, void* g_out, void* stream) {
+    if (!x || !p || !g_out) return fail(nullptr, PIMC_EINVAL, "null argument");
+    if (pimc_model_np(model, D) < 0 || !(dtype == 64 || dtype == 32)) return fail(nullptr, PIMC_EUNSUPPORTED, "unsupported model / D / dtype");
+    if (n == 0) return PIMC_OK;
+    const int threads = 128;
+    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, 148ull * 16);
+    return dispatch(model, D, dtype, [&](auto m, auto real) {
+        using Model = decltype(m);
+        using R = decltype(real);
+        step_selftest_kernel<Model, R><<<blocks, threads, 0, (cudaStream_t)stream>>>((const R*)x, (const R*)p, (const R*)I0, (const R*)I1,
+                                                                                     (R)dt, n, (R*)g_out);
+        PIMC_CUDA(nullptr, cudaGetLastError());
+        return (int)PIMC_OK;
+    });
+}
+
+const char* pimc_last_error(const pimc_handle* h) { return h ? h->err.c_str() : g_static_error.c_str(); }
+
+int pimc_destroy(pimc_handle* h) {
+    if (!h) return PIMC_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    delete h;
+    return PIMC_OK;
+}
+
+}  // extern "C"

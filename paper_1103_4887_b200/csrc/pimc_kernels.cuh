@@ -1,0 +1,504 @@
+// Device side of libpimc: the persistent sweep kernel (rows A2-A6 of SURVEY.md §8(a)) and small helpers.
+//
+// Work decomposition.  A chain's M+1 time steps are cut into G contiguous tiles of `tile` sites (tile even,
+// so every tile starts on an even site); tile b of chain c is CTA c*G + b.  Inside a half-sweep every
+// site of one parity is independent, so the threads of a CTA stride over the tile's
+// sites of that parity.  The whole pimc_sweep call is ONE launch: the CTA loops over sweeps; between
+// half-sweeps it only has to agree with its two neighbour tiles (row A3), not with the whole grid:
+//   * the even half-sweep of tile b reads x,g of site s-1  (last written by tile b-1's odd half-sweep),
+//   * the odd  half-sweep of tile b reads x   of site e    (last written by tile b+1's even half-sweep),
+// so each CTA publishes a monotonically increasing half-sweep count with a release store and the
+// neighbour polls it with an acquire load.  Parameter moves need one scalar
+// all-reduce per parameter: every CTA publishes its partial Delta-A, then every CTA sums all G partials in
+// index order, so all CTAs take the same decision from bit-identical totals without a broadcast step
+// (replaces the paper's second, single-thread kernel).  The two cache copies + selector of PAPER.md:244
+// are kept: g[cur] is current, g[cur^1] receives the proposal's increments, accept flips cur.
+// With G = 1 (batched chains, one CTA per chain) there is no inter-CTA traffic at all.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "pimc_model.cuh"
+#include "pimc_rng.cuh"
+
+namespace pimc {
+
+constexpr int kMaxD = 4;
+constexpr int kMaxNp = 16;
+constexpr int kMaxThreads = 512;
+constexpr int kMaxHistSel = 64;
+
+template <typename R> struct SweepArgs {
+    // problem
+    int M, L, n_chains, G, tile, kind;
+    R dt, Rm, Rf[kMaxD], wx[kMaxD];
+    double wp[kMaxNp];
+    // device state (per chain, chains concatenated)
+    R* x;                 // (C, M+1, D)
+    R* g[2];              // (C, M, D) x 2: step-increment caches (ping-pong)
+    const R* y;           // (C, M+1, L)
+    const R* I;           // (C, M+1) or nullptr
+    R* p;                 // (C, Np)
+    int* cur;             // (C) which cache is current
+    const double* lo;     // (C, Np)
+    const double* hi;
+    // statistics
+    int accum;
+    unsigned long long n_skip, t_enable;
+    double *cx, *S1x, *S2x;      // (C, M+1, D)
+    double *cp, *S1p, *S2p;      // (C, Np)
+    unsigned long long* counters;  // (C, 2, D+Np) accepted, proposed
+    int n_sel, nbins;
+    const int* hsite; const int* hcomp; const double* hlo; const double* hhi; const double* hwidth;
+    unsigned long long* hist;    // (C, n_sel, nbins+2)
+    // debug trace of the last sweep (all nullptr = off)
+    R* tr_dA; unsigned char* tr_acc; R* tr_xprop; R* tr_dAp; unsigned char* tr_accp; R* tr_pprop;
+    // run
+    unsigned long long t0, seed;
+    long long n_sweeps;
+    int do_states, do_params;
+    // inter-CTA hand-off (G > 1)
+    unsigned long long* hs_flag;  // (C, G) completed half-sweeps
+    double* ar_val;               // (C, 2, G) partial Delta-A
+    unsigned long long* ar_flag;  // (C, 2, G)
+    unsigned long long* ar_epoch; // (C) all-reduce events performed so far (device-side bookkeeping)
+    unsigned long long hs_base;
+};
+
+// ---- memory-model helpers ------------------------------------------------------------------------
+__device__ __forceinline__ void st_release_gpu(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_acquire_gpu(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+// Path and cache values may have been written by a neighbour CTA: read them from L2, never from a stale L1 line.
+template <typename R, int D> __device__ __forceinline__ void load_vec(const R* base, size_t site, R out[D]) {
+    const R* q = base + site * D;
+    if constexpr (D == 4 && sizeof(R) == 8) {
+        const double2 a = __ldcg(reinterpret_cast<const double2*>(q));
+        const double2 b = __ldcg(reinterpret_cast<const double2*>(q) + 1);
+        out[0] = a.x; out[1] = a.y; out[2] = b.x; out[3] = b.y;
+    } else if constexpr (D == 4 && sizeof(R) == 4) {
+        const float4 a = __ldcg(reinterpret_cast<const float4*>(q));
+        out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+    } else if constexpr (D == 2 && sizeof(R) == 8) {
+        const double2 a = __ldcg(reinterpret_cast<const double2*>(q));
+        out[0] = a.x; out[1] = a.y;
+    } else {
+#pragma unroll
+        for (int a = 0; a < D; ++a) out[a] = __ldcg(q + a);
+    }
+}
+template <typename R, int D> __device__ __forceinline__ void store_vec(R* base, size_t site, const R v[D]) {
+    R* q = base + site * D;
+    if constexpr (D == 4 && sizeof(R) == 8) {
+        reinterpret_cast<double2*>(q)[0] = make_double2(v[0], v[1]);
+        reinterpret_cast<double2*>(q)[1] = make_double2(v[2], v[3]);
+    } else if constexpr (D == 4 && sizeof(R) == 4) {
+        reinterpret_cast<float4*>(q)[0] = make_float4(v[0], v[1], v[2], v[3]);
+    } else if constexpr (D == 2 && sizeof(R) == 8) {
+        reinterpret_cast<double2*>(q)[0] = make_double2(v[0], v[1]);
+    } else {
+#pragma unroll
+        for (int a = 0; a < D; ++a) q[a] = v[a];
+    }
+}
+
+// ---- deterministic block sum: fixed xor tree inside a warp, then warps added in index order --------
+__device__ __forceinline__ double block_sum(double v, double* red /* >= 32 doubles of shared memory */) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+    const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    if ((threadIdx.x & 31) == 0) red[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+    for (int w = 0; w < nwarps; ++w) tot += red[w];
+    __syncthreads();
+    return tot;
+}
+
+// ---- proposals (Fig. 1 (a)) ---------------------------------------------------------------
+template <typename R, int D>
+__device__ __forceinline__ void propose_state(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n,
+                                              const R xn[D], R xp[D]) {
+    const Words4 w = draw(a.seed, t, chain, n, kStreamStateProposal, 0);
+    if (a.kind == 1) {   // uniform: x' = x + w (2u - 1)
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], __dmul_rn(a.wx[c], 2.0 * unit_open(w.w[c]) - 1.0));   // no FMA: bit-reproducible
+            else xp[c] = __fadd_rn(xn[c], __fmul_rn(a.wx[c], __fsub_rn(__fmul_rn(2.0f, unit_openf(w.w[c])), 1.0f)));
+        }
+    } else {             // Gaussian: Box-Muller pairs from words (0,1) and (2,3)
+        R z[4];
+        if constexpr (sizeof(R) == 8) {
+            normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z[0], z[1]);
+            if constexpr (D > 2) normal_pair(unit_open(w.w[2]), unit_open(w.w[3]), z[2], z[3]);
+        } else {
+            normal_pair(unit_openf(w.w[0]), unit_openf(w.w[1]), z[0], z[1]);
+            if constexpr (D > 2) normal_pair(unit_openf(w.w[2]), unit_openf(w.w[3]), z[2], z[3]);
+        }
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], __dmul_rn(a.wx[c], z[c]));
+            else xp[c] = __fadd_rn(xn[c], __fmul_rn(a.wx[c], z[c]));
+        }
+    }
+}
+
+template <typename R> __device__ __forceinline__ R log_accept_uniform(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n) {
+    const Words4 w = draw(a.seed, t, chain, n, kStreamStateAccept, 0);
+    if constexpr (sizeof(R) == 8) return log(unit_open52(w.w[0], w.w[1]));
+    else return logf(unit_openf(w.w[0]));
+}
+
+// ---- one Metropolis site update: Fig. 1 (a)-(i) ----------------------------------------------------------
+template <class Model, typename R>
+__device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __restrict__ prm, unsigned long long t,
+                                            uint32_t chain, int n, R* __restrict__ x, R* __restrict__ g, const R* __restrict__ y,
+                                            const R* __restrict__ I, bool trace, size_t chain_site0) {
+    constexpr int D = Model::D;
+    const int M = a.M;
+    R xn[D], xp[D], gp[D];
+    load_vec<R, D>(x, n, xn);
+    propose_state<R, D>(a, t, chain, (uint32_t)n, xn, xp);
+    R dA = R(0);
+    if (n >= 1) {
+        R xm[D], gm[D];
+        load_vec<R, D>(x, n - 1, xm);
+        load_vec<R, D>(g, n - 1, gm);
+#pragma unroll
+        for (int c = 0; c < D; ++c) {   // model-error term n-1 -> n
+            const R r_new = (xp[c] - xm[c]) - gm[c];
+            const R r_old = (xn[c] - xm[c]) - gm[c];
+            dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+        }
+        for (int l = 0; l < a.L; ++l) {  // measurement term n (the action sums n = 1..M)
+            const R yn = __ldg(y + (size_t)n * a.L + l);
+            const R d_new = yn - xp[l], d_old = yn - xn[l];
+            dA += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
+        }
+    }
+    if (n <= M - 1) {
+        R xq[D], gn[D];
+        load_vec<R, D>(x, n + 1, xq);
+        load_vec<R, D>(g, n, gn);
+        const R I0 = I ? __ldg(I + n) : R(0), I1 = I ? __ldg(I + n + 1) : R(0);
+        Model::increment(xp, prm, I0, I1, a.dt, gp);
+#pragma unroll
+        for (int c = 0; c < D; ++c) {   // model-error term n -> n+1
+            const R r_new = (xq[c] - xp[c]) - gp[c];
+            const R r_old = (xq[c] - xn[c]) - gn[c];
+            dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+        }
+    }
+    const R logu = log_accept_uniform<R>(a, t, chain, (uint32_t)n);
+    const bool accept = logu < -dA;      // NaN or +inf rejects; dA <= 0 always accepts
+    if (accept) {
+        store_vec<R, D>(x, n, xp);
+        if (n <= M - 1) store_vec<R, D>(g, n, gp);
+    }
+    if (trace) {
+        const size_t gs = chain_site0 + (size_t)n;
+        if (a.tr_dA) a.tr_dA[gs] = dA;
+        if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
+        if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
+    }
+    return accept;
+}
+
+// ---- the persistent sweep kernel ---------------------------------------------------------------------------
+template <class Model, typename R>
+__global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a) {
+    constexpr int D = Model::D;
+    constexpr int NP = Model::NP;
+    __shared__ double red[32];
+    __shared__ R ps[NP];          // current parameters
+    __shared__ R ps_prop[NP];     // parameters with the proposed entry
+    __shared__ unsigned int s_pacc[NP], s_pprop[NP];
+    __shared__ double bcast[4];
+    __shared__ int s_cur;
+
+    const int G = a.G, M = a.M, T = blockDim.x, tid = threadIdx.x;
+    const uint32_t chain = blockIdx.x / G;
+    const int b = blockIdx.x % G;
+    const int s = b * a.tile;
+    const int e = min(s + a.tile, M + 1);
+    const size_t site0 = (size_t)chain * (M + 1);
+
+    R* x = a.x + site0 * D;
+    R* gbuf[2] = {a.g[0] + (size_t)chain * M * D, a.g[1] + (size_t)chain * M * D};
+    const R* y = a.y + site0 * a.L;
+    const R* I = a.I ? a.I + site0 : nullptr;
+    unsigned long long* hs_flag = a.hs_flag + (size_t)chain * G;
+
+    if (tid < NP) { ps[tid] = a.p[(size_t)chain * NP + tid]; s_pacc[tid] = 0; s_pprop[tid] = 0; }
+    if (tid == 0) s_cur = a.cur[chain];
+    __syncthreads();
+    int cur = s_cur;
+    unsigned int n_acc_state = 0;
+    unsigned long long ar_count = a.ar_epoch[chain];   // all-reduce events this chain has performed so far
+
+    for (long long i = 0; i < a.n_sweeps; ++i) {
+        const unsigned long long t = a.t0 + (unsigned long long)i;
+        const bool trace = (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
+
+        // ---------------- A2/A3: even half-sweep, then odd half-sweep ----------------
+        if (a.do_states) {
+            for (int parity = 0; parity < 2; ++parity) {
+                if (G > 1) {
+                    if (tid == 0) {
+                        const unsigned long long need = a.hs_base + 2ull * (unsigned long long)i + (unsigned long long)parity;
+                        if (parity == 0 && b > 0) while (ld_acquire_gpu(hs_flag + b - 1) < need) {}
+                        if (parity == 1 && b < G - 1) while (ld_acquire_gpu(hs_flag + b + 1) < need) {}
+                    }
+                    __syncthreads();
+                }
+                for (int n = s + parity + 2 * tid; n < e; n += 2 * T)
+                    n_acc_state += update_site<Model, R>(a, ps, t, chain, n, x, gbuf[cur], y, I, trace, site0) ? 1u : 0u;
+                __syncthreads();
+                if (G > 1 && tid == 0)
+                    st_release_gpu(hs_flag + b, a.hs_base + 2ull * (unsigned long long)i + (unsigned long long)parity + 1ull);
+            }
+        }
+
+        // ---------------- A4: parameter moves, in sequence ----------------
+        if (a.do_params) {
+            for (int l = 0; l < NP; ++l) {
+                if (!(a.wp[l] > 0.0)) continue;
+                // one thread draws the proposal and the accept uniform; everybody needs p', log u and the bounds verdict
+                if (tid == 0) {
+                    const Words4 w = draw(a.seed, t, chain, (uint32_t)l, kStreamParam, 0);
+                    double step;
+                    if (a.kind == 1) step = __dmul_rn(a.wp[l], 2.0 * unit_open(w.w[0]) - 1.0);
+                    else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(a.wp[l], z0); }
+                    double pl;
+                    if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)ps[l], step);
+                    else pl = (double)__fadd_rn(ps[l], (float)step);
+                    const double lo = a.lo[(size_t)chain * NP + l], hi = a.hi[(size_t)chain * NP + l];
+                    bcast[0] = pl;
+                    bcast[1] = log(unit_open52(w.w[2], w.w[3]));
+                    bcast[2] = (pl >= lo && pl <= hi) ? 1.0 : 0.0;
+                }
+                if (tid < NP) ps_prop[tid] = ps[tid];
+                __syncthreads();
+                const double pl = bcast[0], logu = bcast[1];
+                const bool inside = bcast[2] != 0.0;
+                bool accept = false;
+                double dA = __longlong_as_double(0x7FF8000000000000ll);   // NaN = not evaluated
+                if (inside) {   // a proposal outside the bounds is rejected (without evaluating the model)
+                    if (tid == 0) ps_prop[l] = (R)pl;
+                    __syncthreads();
+                    R* gcur = gbuf[cur];
+                    R* galt = gbuf[cur ^ 1];
+                    double part = 0.0;
+                    const int e_fwd = min(e, M);
+                    for (int n = s + tid; n < e_fwd; n += T) {
+                        R xn[D], xq[D], gn[D], gp[D];
+                        load_vec<R, D>(x, n, xn);
+                        load_vec<R, D>(x, n + 1, xq);
+                        load_vec<R, D>(gcur, n, gn);
+                        const R I0 = I ? __ldg(I + n) : R(0), I1 = I ? __ldg(I + n + 1) : R(0);
+                        Model::increment(xn, ps_prop, I0, I1, a.dt, gp);
+                        store_vec<R, D>(galt, n, gp);
+                        R acc = R(0);
+#pragma unroll
+                        for (int c = 0; c < D; ++c) {
+                            const R d = xq[c] - xn[c];
+                            const R r_new = d - gp[c], r_old = d - gn[c];
+                            acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                        }
+                        part += (double)acc;
+                    }
+                    dA = block_sum(part, red);
+                    if (G > 1) {   // all-gather of the G partials, summed in index order by every CTA
+                        const int slot = (int)(ar_count & 1ull);
+                        double* val = a.ar_val + ((size_t)chain * 2 + slot) * G;
+                        unsigned long long* flg = a.ar_flag + ((size_t)chain * 2 + slot) * G;
+                        if (tid == 0) {
+                            val[b] = dA;
+                            st_release_gpu(flg + b, ar_count + 1ull);
+                        }
+                        double mine = 0.0;
+                        for (int j = tid; j < G; j += T) {
+                            while (ld_acquire_gpu(flg + j) < ar_count + 1ull) {}
+                            mine += __ldcg(val + j);
+                        }
+                        dA = block_sum(mine, red);
+                        ar_count += 1ull;
+                    }
+                    accept = logu < -dA;
+                    if (accept) cur ^= 1;
+                }
+                if (tid == 0) {
+                    if (accept) ps[l] = (R)pl;
+                    if (b == 0) {
+                        s_pprop[l] += 1;
+                        if (accept) s_pacc[l] += 1;
+                        if (trace) {
+                            if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)dA;
+                            if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = accept ? 1 : 0;
+                            if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = (R)pl;
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+            if (trace && b == 0 && tid == 0) {
+                for (int l = 0; l < NP; ++l)
+                    if (!(a.wp[l] > 0.0)) {
+                        if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)__longlong_as_double(0x7FF8000000000000ll);
+                        if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = 0;
+                        if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = ps[l];
+                    }
+            }
+        }
+
+        // ---------------- A5: running moments and histograms ----------------
+        if (a.accum && ((t - a.t_enable) % a.n_skip) == 0ull) {
+            // own sites only; they were last written by this CTA (visible after the barriers above)
+            for (int idx = s * D + tid; idx < e * D; idx += T) {
+                const size_t gi = site0 * D + (size_t)idx;
+                const double d = (double)__ldcg(x + idx) - a.cx[gi];
+                a.S1x[gi] += d;
+                a.S2x[gi] += d * d;
+            }
+            if (b == 0 && tid < NP) {
+                const size_t gi = (size_t)chain * NP + tid;
+                const double d = (double)ps[tid] - a.cp[gi];
+                a.S1p[gi] += d;
+                a.S2p[gi] += d * d;
+            }
+            for (int sel = tid; sel < a.n_sel; sel += T) {
+                const int site = a.hsite[sel], comp = a.hcomp[sel];
+                const bool mine = site < 0 ? (b == 0) : (site >= s && site < e);
+                if (mine) {
+                    const double v = site < 0 ? (double)ps[comp] : (double)__ldcg(x + (size_t)site * D + comp);
+                    unsigned long long* bins = a.hist + ((size_t)chain * a.n_sel + sel) * (size_t)(a.nbins + 2);
+                    const double lo = a.hlo[sel], hi = a.hhi[sel];
+                    int bin;
+                    if (!(v >= lo)) bin = 0;
+                    else if (v >= hi) bin = a.nbins + 1;
+                    else {
+                        long long q = (long long)floor((v - lo) / a.hwidth[sel]);
+                        if (q >= a.nbins) q = a.nbins - 1;
+                        bin = 1 + (int)q;
+                    }
+                    bins[bin] += 1ull;     // one owner thread per selection: no atomics needed
+                }
+            }
+            __syncthreads();   // the next half-sweep overwrites x
+        }
+    }
+
+    // ---------------- A6 + state write-back ----------------
+    {
+        const double acc_total = block_sum((double)n_acc_state, red);   // exact: counts < 2^53
+        if (tid == 0) {
+            unsigned long long* cnt = a.counters + (size_t)chain * 2 * (D + NP);
+            const unsigned long long acc_u = (unsigned long long)acc_total;
+            unsigned long long prop_u = 0;
+            if (a.do_states) prop_u = (unsigned long long)(e - s) * (unsigned long long)a.n_sweeps;
+            for (int c = 0; c < D; ++c) {
+                if (acc_u) atomicAdd(cnt + c, acc_u);
+                if (prop_u) atomicAdd(cnt + (D + NP) + c, prop_u);
+            }
+            if (b == 0) {
+                for (int l = 0; l < NP; ++l) {
+                    cnt[D + l] += s_pacc[l];
+                    cnt[(D + NP) + D + l] += s_pprop[l];
+                    a.p[(size_t)chain * NP + l] = ps[l];
+                }
+                a.cur[chain] = cur;
+                a.ar_epoch[chain] = ar_count;
+            }
+        }
+    }
+}
+
+// ---- A0: (re)build the step cache of every chain ---------------------------------------------------------
+template <class Model, typename R>
+__global__ void build_cache_kernel(const R* __restrict__ x, const R* __restrict__ I, const R* __restrict__ p, R* __restrict__ g,
+                                   int M, int n_chains, R dt) {
+    constexpr int D = Model::D;
+    constexpr int NP = Model::NP;
+    const size_t total = (size_t)n_chains * M;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t chain = idx / M;
+        const int n = (int)(idx % M);
+        const R* prm = p + chain * NP;
+        R xn[D], gn[D];
+#pragma unroll
+        for (int c = 0; c < D; ++c) xn[c] = x[(chain * (M + 1) + n) * D + c];
+        const R I0 = I ? I[chain * (M + 1) + n] : R(0), I1 = I ? I[chain * (M + 1) + n + 1] : R(0);
+        Model::increment(xn, prm, I0, I1, dt, gn);
+#pragma unroll
+        for (int c = 0; c < D; ++c) g[(chain * M + n) * D + c] = gn[c];
+    }
+}
+
+// ---- stand-alone step increment on arbitrary states (self-test entry) -------------------------------------
+template <class Model, typename R>
+__global__ void step_selftest_kernel(const R* __restrict__ x, const R* __restrict__ p, const R* __restrict__ I0,
+                                     const R* __restrict__ I1, R dt, unsigned long long n, R* __restrict__ g) {
+    constexpr int D = Model::D;
+    constexpr int NP = Model::NP;
+    const R* prm = p;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
+        R xn[D], gn[D];
+#pragma unroll
+        for (int c = 0; c < D; ++c) xn[c] = x[i * D + c];
+        Model::increment(xn, prm, I0 ? I0[i] : R(0), I1 ? I1[i] : R(0), dt, gn);
+#pragma unroll
+        for (int c = 0; c < D; ++c) g[i * D + c] = gn[c];
+    }
+}
+
+// ---- RNG self-test ------------------------------------------------------------------------------------------
+__global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, unsigned long long n, uint32_t k0, uint32_t k1,
+                                    uint32_t* __restrict__ out, double* __restrict__ u_prop, double* __restrict__ u_acc,
+                                    double* __restrict__ z) {
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
+        const Words4 w = philox4x32_10(ctrs[4 * i], ctrs[4 * i + 1], ctrs[4 * i + 2], ctrs[4 * i + 3], k0, k1);
+        if (out) for (int j = 0; j < 4; ++j) out[4 * i + j] = w.w[j];
+        if (u_prop) for (int j = 0; j < 4; ++j) u_prop[4 * i + j] = unit_open(w.w[j]);
+        if (u_acc) u_acc[i] = unit_open52(w.w[0], w.w[1]);
+        if (z) {
+            normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z[4 * i], z[4 * i + 1]);
+            normal_pair(unit_open(w.w[2]), unit_open(w.w[3]), z[4 * i + 2], z[4 * i + 3]);
+        }
+    }
+}
+
+// ---- moments read-out: mean = c + S1/N, var = S2/N - (S1/N)^2 ---------------------------------------------
+__global__ void moments_kernel(const double* __restrict__ cx, const double* __restrict__ S1x, const double* __restrict__ S2x,
+                               const double* __restrict__ cp, const double* __restrict__ S1p, const double* __restrict__ S2p,
+                               size_t nx /* (M+1)*D */, int np, int n_chains, double N, double* __restrict__ out) {
+    const size_t per_chain = 2 * nx + 2 * (size_t)np;
+    const size_t total = (size_t)n_chains * (nx + np);
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t chain = idx / (nx + np), r = idx % (nx + np);
+        double c, s1, s2;
+        size_t o_mean, o_var;
+        if (r < nx) {
+            c = cx[chain * nx + r]; s1 = S1x[chain * nx + r]; s2 = S2x[chain * nx + r];
+            o_mean = chain * per_chain + r; o_var = o_mean + nx;
+        } else {
+            const size_t l = r - nx;
+            c = cp[chain * np + l]; s1 = S1p[chain * np + l]; s2 = S2p[chain * np + l];
+            o_mean = chain * per_chain + 2 * nx + l; o_var = o_mean + np;
+        }
+        const double m1 = N > 0.0 ? s1 / N : 0.0;
+        out[o_mean] = c + m1;
+        out[o_var] = N > 0.0 ? s2 / N - m1 * m1 : 0.0;
+    }
+}
+
+// type conversion copy (double <- R) for re-centring the moments
+template <typename R> __global__ void widen_kernel(const R* __restrict__ in, double* __restrict__ out, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) out[i] = (double)in[i];
+}
+
+}  // namespace pimc

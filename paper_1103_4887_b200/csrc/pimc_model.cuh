@@ -1,0 +1,72 @@
+// Model step increments g(x, p; I_n, I_{n+1}) for the PIMC kernels (row A0 of SURVEY.md §8(a)).
+//   HH     : tanh-kinetics Hodgkin-Huxley neuron, PAPER.md:256-270 (Eq. 11-14), Table 1
+//            shifted by -65 mV; one classical RK4 step of size dt, current at the half step = mean of the ends.
+//   LINEAR : x -> A x with A = p (row-major D x D); g = A x - x.
+// The caches hold the INCREMENT g, not f = x + g: the residual (x_{n+1} - x_n) - g_n then loses no bits to the
+// +-65 mV offset of V (matters in fp32).
+#pragma once
+
+namespace pimc {
+
+template <typename R> __device__ __forceinline__ R tanh_(R v);
+template <> __device__ __forceinline__ double tanh_<double>(double v) { return tanh(v); }
+template <> __device__ __forceinline__ float tanh_<float>(float v) { return tanhf(v); }
+
+// ---------------------------------------------------------------------------------------------------
+template <typename R> struct HHModel {
+    static constexpr int D = 4;
+    static constexpr int NP = 7;
+
+    // The parameter vector lives in shared memory (one copy per CTA); p[] = (gNa, gK, gL, ENa, EK, EL, C).
+    // d a / dt = (a_inf(V) - a) / tau_a(V);  a_inf = 1/2 + 1/2 tanh(s), tau = tau0 + tau1 (1 - tanh^2 s), s = (V - Va)/dVa
+    static __device__ __forceinline__ R gate(R V, R a, R Va, R dVa, R tau0, R tau1) {
+        const R th = tanh_<R>((V - Va) / dVa);
+        const R ainf = R(0.5) + R(0.5) * th;
+        const R tau = tau0 + tau1 * (R(1) - th * th);
+        return (ainf - a) / tau;
+    }
+    static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R I, R F[4]) {
+        const R V = x[0], m = x[1], h = x[2], n = x[3];
+        const R n2 = n * n;
+        const R cur = I + p[0] * (m * m * m) * h * (p[3] - V) + p[1] * (n2 * n2) * (p[4] - V) + p[2] * (p[5] - V);
+        F[0] = cur / p[6];
+        F[1] = gate(V, m, R(-40.0), R(15.0), R(0.1), R(0.4));
+        F[2] = gate(V, h, R(-60.0), R(-15.0), R(1.0), R(7.0));
+        F[3] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
+    }
+    static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
+        const R Ih = R(0.5) * (I0 + I1);
+        const R hdt = R(0.5) * dt;
+        R k[4], xs[4], acc[4];
+        rhs(x, p, I0, k);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { acc[a] = k[a]; xs[a] = x[a] + hdt * k[a]; }
+        rhs(xs, p, Ih, k);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + hdt * k[a]; }
+        rhs(xs, p, Ih, k);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + dt * k[a]; }
+        rhs(xs, p, I1, k);
+        const R dt6 = dt / R(6);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) g[a] = dt6 * (acc[a] + k[a]);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------
+template <typename R, int D_> struct LinearModel {
+    static constexpr int D = D_;
+    static constexpr int NP = D_ * D_;
+    static __device__ __forceinline__ void increment(const R x[D_], const R* __restrict__ p, R, R, R, R g[D_]) {
+#pragma unroll
+        for (int a = 0; a < D_; ++a) {
+            R f = R(0);
+#pragma unroll
+            for (int b = 0; b < D_; ++b) f += p[a * D_ + b] * x[b];
+            g[a] = f - x[a];
+        }
+    }
+};
+
+}  // namespace pimc
