@@ -1,0 +1,283 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of libpimc on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--sweeps-per-step S]
+
+Metric (BASELINE.json): Metropolis site-updates/s and sweeps/s, Hodgkin-Huxley, M = 32768, fp64, states + 7
+parameters (configs[3]); one "step" = one pimc_sweep call of S full sweeps (even + odd half-sweep, 7 sequential
+parameter moves, moment accumulation) over the seeded synthetic workload, i.e. one pass of every §8(a) row.
+Rank 0 prints ONE JSON line.  N > 1 runs N independent replicas (the path does not shard: "replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from workloads import make_workload  # noqa: E402
+
+METRIC = "Metropolis site-updates/sec and sweeps/sec (HH, M=32768, fp64) vs FP64 roofline"
+UNIT = "site-updates/s"
+
+# Algorithmic work per unit, fixed once (SURVEY.md §8(d) "Algorithmic work"): FP64 pipe slots
+# (1 slot = one FMA/ADD/MUL lane-operation = 2 FLOP at peak) per joint site-update and per parameter-move model evaluation.
+W_SITE_SLOTS = 800.0
+W_EVAL_SLOTS = 560.0
+# FP64 peak derived from unit counts and clocks: 148 SMs x 64 FP64 lanes/clk/SM x 1.965 GHz, 2 FLOP per lane-FMA.
+FP64_LANES_PER_SM_CLK = 64
+SM_COUNT = 148
+SM_MAX_HZ = 1.965e9
+PEAK_TFLOPS_DERIVED = SM_COUNT * FP64_LANES_PER_SM_CLK * SM_MAX_HZ * 2 / 1e12
+
+
+def rank_info():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.05):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons, self.stop_flag = index, period, [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap", nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_rate(w, budget_s, chain=0):
+    """Time the CPU oracle, as it stands, on a bounded sample of the same workload.  Returns (site-updates/s, sweeps, seconds)."""
+    from oracle import OracleChain
+    o = OracleChain.from_workload(w, chain=chain)
+    t0 = time.perf_counter()
+    o.sweep(2, seed=w.chain_seed)                       # warm-up + first estimate
+    per = (time.perf_counter() - t0) / 2
+    n = max(2, int(budget_s / max(per, 1e-6)))
+    t0 = time.perf_counter()
+    o.sweep(n, seed=w.chain_seed)
+    dt = time.perf_counter() - t0
+    return (w.M + 1) * n / dt, n, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle (as it stands) on the host cores, bounded sample per step.  Rank 0 only."""
+    rank, _, world = rank_info()
+    if rank != 0:
+        return
+    from oracle import OracleChain
+    w = make_workload(args.config)
+    o = OracleChain.from_workload(w, chain=0)
+    t0 = time.perf_counter(); o.sweep(1, seed=1); per = time.perf_counter() - t0
+    n_per_step = max(1, int(min(args.ref_budget / (args.steps + args.warmup), 60.0) / per))
+    for _ in range(args.warmup):
+        o.sweep(n_per_step, seed=1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.sweep(n_per_step, seed=1)
+    dt = time.perf_counter() - t0
+    value = (w.M + 1) * n_per_step * args.steps / dt
+    sample = f"{n_per_step} full sweeps per step of chain 0 of {w.name} (states + 7 parameter moves), serial fp64 C++ -O2"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": w.name, "M": w.M, "n_chains": 1, "sweeps_per_step": n_per_step},
+        "sweeps_per_s": n_per_step * args.steps / dt,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def reduce_over_ranks(local_seconds, local_units, world, dist=None):
+    """Whole-job throughput = units processed by all ranks / max over ranks of the timed seconds."""
+    if world == 1 or dist is None:
+        return local_seconds, local_units
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([local_seconds], dtype=torch.float64, device=dev)
+    u = torch.tensor([local_units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def run_ours(args):
+    import torch
+    import paper_1103_4887_b200 as P
+    rank, local_rank, world = rank_info()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (libpimc has no CPU fallback)")
+    dev_index = torch.cuda.current_device()
+
+    # replicas only: every rank runs the same shape with its own data realisation and Philox key
+    w = make_workload(args.config, seed=None if rank == 0 else 11034887 + args.config + 7919 * rank)
+    seed = w.chain_seed + rank
+    S = args.sweeps_per_step
+    h = P.Pimc.from_workload(w, dtype=64)
+    h.set_accum(True, 1)
+    h.reset_moments()
+    shape = h.get_launch()
+    units_per_step = float(w.n_chains) * (w.M + 1) * S
+    n_active = int(np.count_nonzero(w.w_param))
+    evals_per_step = float(w.n_chains) * w.M * S * n_active
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def one_step(fn, n=S):
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream); fn(n, seed); e1.record(stream)
+        return e0, e1
+
+    for _ in range(args.warmup):
+        one_step(h.sweep)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(dev_index)
+    sampler.start()
+    launches0 = h.launch_count
+    t_wall0 = time.perf_counter()
+    evs = [one_step(h.sweep) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t_wall = time.perf_counter() - t_wall0
+    sampler.stop_flag = True
+    sampler.join()
+    launches = h.launch_count - launches0
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    local_s = sum(step_ms) * 1e-3
+    tot_s, tot_units = reduce_over_ranks(local_s, units_per_step * args.steps, world, dist)
+    value = tot_units / tot_s
+    ms_per_step = tot_s / args.steps * 1e3
+
+    # rows A2 and A4 on their own (same launch shape, same data), for the breakdown the north_star asks for
+    def rate(fn, units, reps=3):
+        fn(max(1, S // 10), seed); torch.cuda.synchronize()
+        ms = []
+        for _ in range(reps):
+            a, b = one_step(fn); torch.cuda.synchronize(); ms.append(a.elapsed_time(b))
+        return units / (min(ms) * 1e-3), min(ms)
+    a2_rate, a2_ms = rate(h.sweep_states_only, units_per_step)
+    a4_rate, a4_ms = (rate(h.sweep_params_only, evals_per_step) if n_active else (0.0, 0.0))
+
+    # roofline of the dominant (only) kernel of the step: the persistent sweep kernel
+    slots_per_launch = units_per_step * W_SITE_SLOTS + evals_per_step * W_EVAL_SLOTS
+    achieved_tflops = 2.0 * slots_per_launch / (float(np.mean(step_ms)) * 1e-3) / 1e12
+    measured_peak = P.fp64_peak(150) * 2 / 1e12 if rank == 0 else None
+    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": PEAK_TFLOPS_DERIVED, "unit": "TFLOP/s",
+                "frac": achieved_tflops / PEAK_TFLOPS_DERIVED, "traffic": None,
+                "peak_source": "derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json",
+                "peak_measured_dfma_tflops": measured_peak,
+                "frac_of_measured_dfma": (achieved_tflops / measured_peak) if measured_peak else None,
+                "kernel": "pimc::sweep_kernel<HHModel<double>,double>",
+                "work_model": {"slots_per_site_update": W_SITE_SLOTS, "slots_per_param_eval": W_EVAL_SLOTS,
+                               "site_updates_per_launch": units_per_step, "param_evals_per_launch": evals_per_step},
+                "a2_only": {"site_updates_per_s": a2_rate, "ms_per_launch": a2_ms,
+                            "frac": 2 * a2_rate * W_SITE_SLOTS / 1e12 / PEAK_TFLOPS_DERIVED},
+                "a4_only": {"param_evals_per_s": a4_rate, "ms_per_launch": a4_ms,
+                            "frac": 2 * a4_rate * W_EVAL_SLOTS / 1e12 / PEAK_TFLOPS_DERIVED}}
+
+    # end to end through the C ABI on HOST buffers: H2D of y, I, x0, p0 + sweeps + D2H of the moments inside the timed region
+    e2e = None
+    if rank == 0 or world > 1:
+        P.run_host(w, 0, max(1, S // 10), seed)         # warm-up (context, allocator)
+        reps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            out = P.run_host(w, 0, S, seed)
+        dt_e2e = time.perf_counter() - t0
+        s_e2e, u_e2e = reduce_over_ranks(dt_e2e, units_per_step * reps, world, dist)
+        e2e = {"value": u_e2e / s_e2e, "unit": UNIT, "h2d_bytes_per_step": out["h2d_bytes"], "d2h_bytes_per_step": out["d2h_bytes"],
+               "ms_per_step": s_e2e / reps * 1e3, "call": "pimc_run_host (cudaMalloc + H2D + pimc_sweep + pimc_moments + D2H + sync)"}
+
+    if rank == 0:
+        cpu_rate, cpu_n, cpu_s = oracle_rate(w, args.cpu_budget)
+        cpu = {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{cpu_n} full sweeps of chain 0 of {w.name} in {cpu_s:.1f} s (serial fp64 C++ -O2, {os.cpu_count()} cores present)"}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
+                       "accumulate_every": 1, "launch": shape, "l2": "flushed between timed steps (256 MiB fill)",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "sweeps_per_s": value / (w.M + 1),
+            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu,
+            "wall_s_timed_region": t_wall, "speedup_vs_oracle_1core": value / cpu_rate,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--sweeps-per-step", type=int, default=1000)
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--ref-budget", type=float, default=120.0, help="seconds of oracle time for --impl reference")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        from paper_1103_4887_b200 import build
+        rank, _, world = rank_info()
+        if rank == 0:
+            build.build()
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -163,6 +163,11 @@ int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned i
 int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p, const void* I0, const void* I1,
                        double dt, unsigned long long n, void* g_out, void* stream);
 
+/* Roofline denominator probe: runs a register-only chain of independent double-precision FMAs on every SM for
+ * roughly `millis` milliseconds and writes the sustained rate in lane-FMA per second (one lane-FMA = one FP64 pipe
+ * slot of one thread) to *lane_fma_per_s (host).  Synchronises the device. */
+int pimc_fp64_peak_selftest(int millis, double* lane_fma_per_s);
+
 const char* pimc_last_error(const pimc_handle* h);   /* h may be NULL: last error of a failed pimc_init / static call */
 int pimc_destroy(pimc_handle* h);
 

@@ -47,6 +47,7 @@ _SIGNATURES = {
                                 _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp]),
     "pimc_rng_selftest": (C.c_int, [_vp, C.c_ulonglong, C.c_uint, C.c_uint, _vp, _vp, _vp, _vp, _vp]),
     "pimc_step_selftest": (C.c_int, [C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp, C.c_double, C.c_ulonglong, _vp, _vp]),
+    "pimc_fp64_peak_selftest": (C.c_int, [C.c_int, _dp]),
     "pimc_last_error": (C.c_char_p, [_vp]),
     "pimc_destroy": (C.c_int, [_vp]),
 }
@@ -300,6 +301,13 @@ def step_selftest(model, x, p, I0, I1, dt):
     _check(lib().pimc_step_selftest(model, D, dtype, _ptr(x), _ptr(p), _ptr(I0), _ptr(I1), float(dt), n, _ptr(g),
                                     C.c_void_p(torch.cuda.current_stream().cuda_stream)))
     return g
+
+
+def fp64_peak(millis=200):
+    """Measured sustained FP64 FMA rate of this device in lane-FMA/s (roofline denominator probe)."""
+    v = C.c_double()
+    _check(lib().pimc_fp64_peak_selftest(int(millis), C.byref(v)))
+    return v.value
 
 
 def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_path=False):

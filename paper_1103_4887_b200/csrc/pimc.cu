@@ -624,6 +624,37 @@ int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p
     });
 }
 
+int pimc_fp64_peak_selftest(int millis, double* lane_fma_per_s) {
+    if (!lane_fma_per_s || millis < 1) return fail(nullptr, PIMC_EINVAL, "bad argument");
+    int dev = 0, sms = 0;
+    PIMC_CUDA(nullptr, cudaGetDevice(&dev));
+    PIMC_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* sink = nullptr;
+    PIMC_CUDA(nullptr, cudaMalloc(&sink, 64));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int threads = 1024, iters = 40000;
+    fp64_peak_kernel<<<sms, threads>>>(sink, iters, 1.0000001, 1e-9);   // warm-up
+    cudaDeviceSynchronize();
+    double best = 0.0, elapsed = 0.0;
+    while (elapsed < (double)millis) {
+        cudaEventRecord(e0);
+        fp64_peak_kernel<<<sms, threads>>>(sink, iters, 1.0000001, 1e-9);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        elapsed += ms;
+        const double rate = (double)sms * threads * 8.0 * iters / (ms * 1e-3);
+        if (rate > best) best = rate;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    PIMC_CUDA(nullptr, cudaGetLastError());
+    *lane_fma_per_s = best;
+    return PIMC_OK;
+}
+
 const char* pimc_last_error(const pimc_handle* h) { return h ? h->err.c_str() : g_static_error.c_str(); }
 
 int pimc_destroy(pimc_handle* h) {

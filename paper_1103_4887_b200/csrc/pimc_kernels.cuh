@@ -472,6 +472,21 @@ __global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, unsigned 
     }
 }
 
+// ---- FP64 pipe probe: 8 independent FMA chains per thread, no memory traffic ------------------------------
+__global__ void fp64_peak_kernel(double* sink, int iters, double a, double b) {
+    double v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = threadIdx.x * 1e-3 + i;
+    for (int k = 0; k < iters; ++k) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = fma(v[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += v[i];
+    if (s == 1234.5) sink[0] = s;   // never true; keeps the chains alive
+}
+
 // ---- moments read-out: mean = c + S1/N, var = S2/N - (S1/N)^2 ---------------------------------------------
 __global__ void moments_kernel(const double* __restrict__ cx, const double* __restrict__ S1x, const double* __restrict__ S2x,
                                const double* __restrict__ cp, const double* __restrict__ S1p, const double* __restrict__ S2p,
