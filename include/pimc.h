@@ -163,6 +163,11 @@ int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned i
 int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p, const void* I0, const void* I1,
                        double dt, unsigned long long n, void* g_out, void* stream);
 
+/* Elementary-function self-test: x dev double (n), out dev double (n,7) = the kernels' own branch-free
+ * exp(x) (x clamped to +-700), log|x|, sqrt|x|, sin(min(|x|,7.9)), cos(min(|x|,7.9)), 1/|x|, and the HH m-gate rate
+ * (m_inf(V) - 0.3)/tau_m(V) at V = x (Eq. 12-14). */
+int pimc_math_selftest(const double* x, unsigned long long n, double* out, void* stream);
+
 /* Roofline denominator probe: runs a register-only chain of independent double-precision FMAs on every SM for
  * roughly `millis` milliseconds and writes the sustained rate in lane-FMA per second (one lane-FMA = one FP64 pipe
  * slot of one thread) to *lane_fma_per_s (host).  Synchronises the device. */

@@ -5,5 +5,5 @@ There is no CPU fallback: every compute entry point runs CUDA kernels or raises.
 """
 from .binding import (  # noqa: F401
     MODEL_LINEAR, MODEL_HH, PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM, PimcError, Pimc, lib, library_path,
-    model_np, rng_selftest, step_selftest, run_host, exported_symbols, fp64_peak,
+    model_np, rng_selftest, step_selftest, run_host, exported_symbols, fp64_peak, math_selftest,
 )

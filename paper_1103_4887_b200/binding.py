@@ -47,6 +47,7 @@ _SIGNATURES = {
                                 _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp]),
     "pimc_rng_selftest": (C.c_int, [_vp, C.c_ulonglong, C.c_uint, C.c_uint, _vp, _vp, _vp, _vp, _vp]),
     "pimc_step_selftest": (C.c_int, [C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp, C.c_double, C.c_ulonglong, _vp, _vp]),
+    "pimc_math_selftest": (C.c_int, [_vp, C.c_ulonglong, _vp, _vp]),
     "pimc_fp64_peak_selftest": (C.c_int, [C.c_int, _dp]),
     "pimc_last_error": (C.c_char_p, [_vp]),
     "pimc_destroy": (C.c_int, [_vp]),
@@ -301,6 +302,15 @@ def step_selftest(model, x, p, I0, I1, dt):
     _check(lib().pimc_step_selftest(model, D, dtype, _ptr(x), _ptr(p), _ptr(I0), _ptr(I1), float(dt), n, _ptr(g),
                                     C.c_void_p(torch.cuda.current_stream().cuda_stream)))
     return g
+
+
+def math_selftest(x):
+    """x: CUDA float64 tensor (n,) -> (n,7): exp, log|x|, sqrt|x|, sin, cos, 1/|x|, HH m-gate rate (kernel math)."""
+    import torch
+    assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+    out = torch.empty((x.numel(), 7), dtype=torch.float64, device=x.device)
+    _check(lib().pimc_math_selftest(_ptr(x), x.numel(), _ptr(out), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    return out
 
 
 def fp64_peak(millis=200):

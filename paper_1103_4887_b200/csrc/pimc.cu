@@ -624,6 +624,16 @@ int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p
     });
 }
 
+int pimc_math_selftest(const double* x, unsigned long long n, double* out, void* stream) {
+    if (!x || !out) return fail(nullptr, PIMC_EINVAL, "null argument");
+    if (n == 0) return PIMC_OK;
+    const int threads = 256;
+    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, 148ull * 8);
+    math_selftest_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(x, n, out);
+    PIMC_CUDA(nullptr, cudaGetLastError());
+    return PIMC_OK;
+}
+
 int pimc_fp64_peak_selftest(int millis, double* lane_fma_per_s) {
     if (!lane_fma_per_s || millis < 1) return fail(nullptr, PIMC_EINVAL, "bad argument");
     int dev = 0, sms = 0;

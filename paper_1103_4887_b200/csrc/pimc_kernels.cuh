@@ -150,7 +150,7 @@ __device__ __forceinline__ void propose_state(const SweepArgs<R>& a, unsigned lo
 
 template <typename R> __device__ __forceinline__ R log_accept_uniform(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n) {
     const Words4 w = draw(a.seed, t, chain, n, kStreamStateAccept, 0);
-    if constexpr (sizeof(R) == 8) return log(unit_open52(w.w[0], w.w[1]));
+    if constexpr (sizeof(R) == 8) return log_fast(unit_open52(w.w[0], w.w[1]));
     else return logf(unit_openf(w.w[0]));
 }
 
@@ -175,10 +175,13 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
             const R r_old = (xn[c] - xm[c]) - gm[c];
             dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
         }
-        for (int l = 0; l < a.L; ++l) {  // measurement term n (the action sums n = 1..M)
-            const R yn = __ldg(y + (size_t)n * a.L + l);
-            const R d_new = yn - xp[l], d_old = yn - xn[l];
-            dA += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
+#pragma unroll
+        for (int l = 0; l < D; ++l) {    // measurement term n (the action sums n = 1..M); the first L components are observed
+            if (l < a.L) {
+                const R yn = __ldg(y + (size_t)n * a.L + l);
+                const R d_new = yn - xp[l], d_old = yn - xn[l];
+                dA += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
+            }
         }
     }
     if (n <= M - 1) {
@@ -229,7 +232,8 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     const size_t site0 = (size_t)chain * (M + 1);
 
     R* x = a.x + site0 * D;
-    R* gbuf[2] = {a.g[0] + (size_t)chain * M * D, a.g[1] + (size_t)chain * M * D};
+    R* const g_a = a.g[0] + (size_t)chain * M * D;
+    R* const g_b = a.g[1] + (size_t)chain * M * D;
     const R* y = a.y + site0 * a.L;
     const R* I = a.I ? a.I + site0 : nullptr;
     unsigned long long* hs_flag = a.hs_flag + (size_t)chain * G;
@@ -257,7 +261,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     __syncthreads();
                 }
                 for (int n = s + parity + 2 * tid; n < e; n += 2 * T)
-                    n_acc_state += update_site<Model, R>(a, ps, t, chain, n, x, gbuf[cur], y, I, trace, site0) ? 1u : 0u;
+                    n_acc_state += update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0) ? 1u : 0u;
                 __syncthreads();
                 if (G > 1 && tid == 0)
                     st_release_gpu(hs_flag + b, a.hs_base + 2ull * (unsigned long long)i + (unsigned long long)parity + 1ull);
@@ -279,7 +283,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     else pl = (double)__fadd_rn(ps[l], (float)step);
                     const double lo = a.lo[(size_t)chain * NP + l], hi = a.hi[(size_t)chain * NP + l];
                     bcast[0] = pl;
-                    bcast[1] = log(unit_open52(w.w[2], w.w[3]));
+                    bcast[1] = log_fast(unit_open52(w.w[2], w.w[3]));
                     bcast[2] = (pl >= lo && pl <= hi) ? 1.0 : 0.0;
                 }
                 if (tid < NP) ps_prop[tid] = ps[tid];
@@ -291,8 +295,8 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                 if (inside) {   // a proposal outside the bounds is rejected (without evaluating the model)
                     if (tid == 0) ps_prop[l] = (R)pl;
                     __syncthreads();
-                    R* gcur = gbuf[cur];
-                    R* galt = gbuf[cur ^ 1];
+                    R* gcur = cur ? g_b : g_a;
+                    R* galt = cur ? g_a : g_b;
                     double part = 0.0;
                     const int e_fwd = min(e, M);
                     for (int n = s + tid; n < e_fwd; n += T) {
@@ -469,6 +473,23 @@ __global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, unsigned 
             normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z[4 * i], z[4 * i + 1]);
             normal_pair(unit_open(w.w[2]), unit_open(w.w[3]), z[4 * i + 2], z[4 * i + 3]);
         }
+    }
+}
+
+// ---- elementary-function self-test: out (n,7) = exp, log, sqrt, sin, cos, 1/x, HH gate m-rate at (x, a = 0.3) ----
+__global__ void math_selftest_kernel(const double* __restrict__ x, unsigned long long n, double* __restrict__ out) {
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
+        const double v = x[i];
+        const double av = fabs(v);
+        double s, c;
+        sincos_fast(fmin(av, 7.9), s, c);
+        out[7 * i + 0] = exp_fast(fmin(fmax(v, -700.0), 700.0));
+        out[7 * i + 1] = log_fast(fmax(av, 1e-300));
+        out[7 * i + 2] = sqrt_fast(fmax(av, 1e-300));
+        out[7 * i + 3] = s;
+        out[7 * i + 4] = c;
+        out[7 * i + 5] = rcp_fast(fmax(av, 1e-300));
+        out[7 * i + 6] = HHModel<double>::gate_fast(v, 0.3, -40.0, 15.0, 0.1, 0.4);
     }
 }
 

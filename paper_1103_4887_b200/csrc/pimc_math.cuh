@@ -1,0 +1,120 @@
+// Branch-free double-precision elementary functions for the PIMC kernels.
+//
+// Why not libdevice: exp/tanh/log/sincos/division from the CUDA math library carry special-case branches
+// (BSSY/BSYNC/BRA), materialise every polynomial coefficient with two UMOVs and serialise the three
+// independent gate evaluations of the Hodgkin-Huxley right-hand side.  In the v1 profile
+// (profiles/r01_v1_baseline.md) only 34 % of the executed warp instructions were FP64-pipe instructions.
+// These versions assume what the sampler guarantees (finite, range-limited arguments), keep coefficients in
+// constant memory (a free DFMA operand) and contain no branches, so the compiler can interleave independent
+// chains.  Each is accurate to about 1 ulp, far inside the 1e-12 Delta-A tolerance; tests/test_gpu_math.py
+// checks them against the host libm through the pimc_math_selftest entry point.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pimc {
+
+#define PIMC_COEF(name, n) __constant__ double name[n]
+#include "pimc_math_coef.inc"
+#undef PIMC_COEF
+
+__device__ __forceinline__ double rcp_seed(double d) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+    return y;
+}
+__device__ __forceinline__ double rsqrt_seed(double d) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+    return y;
+}
+
+// 1/d for normal d (no zero / inf / nan handling): MUFU seed (~20 bits) + two Newton steps.
+__device__ __forceinline__ double rcp_fast(double d) {
+    double y = rcp_seed(d);
+    double e = fma(-d, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-d, y, 1.0);
+    y = fma(y, e, y);
+    return y;
+}
+// n/d with one residual correction of the quotient.
+__device__ __forceinline__ double div_fast(double n, double d) {
+    const double y = rcp_fast(d);
+    const double q = n * y;
+    const double r = fma(-d, q, n);
+    return fma(r, y, q);
+}
+
+// exp(x) for |x| <= 700: x = k ln2 + r, |r| <= ln2/2; e^r = 1 + r + r^2 P(r); scale by 2^k through the exponent field.
+__device__ __forceinline__ double exp_fast(double x) {
+    constexpr double kMagic = 6755399441055744.0;                 // 1.5 * 2^52: adds round-to-nearest-integer
+    constexpr double kLog2e = 1.4426950408889634074;
+    constexpr double kLn2Hi = 0x1.62e42fefa39efp-1, kLn2Lo = 0x1.abc9e3b39803fp-56;
+    const double t = fma(x, kLog2e, kMagic);
+    const int k = __double2loint(t);
+    const double kd = t - kMagic;
+    double r = fma(kd, -kLn2Hi, x);
+    r = fma(kd, -kLn2Lo, r);
+    double p = kExpP[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) p = fma(p, r, kExpP[i]);
+    const double e = fma(p, r * r, r);                             // e^r - 1
+    const double s = __hiloint2double((k + 1023) << 20, 0);        // 2^k
+    return fma(e, s, s);
+}
+
+// log(u) for normal positive u (here u in (0,1)): u = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh((m-1)/(m+1)).
+__device__ __forceinline__ double log_fast(double u) {
+    constexpr double kLn2Hi = 6.93147180369123816490e-01, kLn2Lo = 1.90821492927058770002e-10;   // hi has 21 trailing zero bits
+    int hi = __double2hiint(u);
+    const int lo = __double2loint(u);
+    int e = (hi >> 20) - 1023;
+    hi = (hi & 0x000FFFFF) | 0x3FF00000;                           // m in [1,2)
+    const int big = hi >= 0x3FF6A09F ? 1 : 0;                      // m >= ~sqrt(2): halve it
+    hi -= big << 20;
+    e += big;
+    const double m = __hiloint2double(hi, lo);
+    const double f = div_fast(m - 1.0, m + 1.0);
+    const double w = f * f;
+    double L = kLogL[8];
+#pragma unroll
+    for (int i = 7; i >= 0; --i) L = fma(L, w, kLogL[i]);
+    const double lm = fma(f * w, L, f + f);                        // 2 f + f^3 L(w)
+    const double ed = (double)e;
+    return fma(ed, kLn2Hi, fma(ed, kLn2Lo, lm));
+}
+
+// sqrt(x) for normal positive x: MUFU seed, two coupled Newton steps on (sqrt, 1/(2 sqrt)), one residual correction.
+__device__ __forceinline__ double sqrt_fast(double x) {
+    const double y = rsqrt_seed(x);
+    double g = x * y, h = 0.5 * y;
+    double r = fma(-h, g, 0.5);
+    g = fma(g, r, g); h = fma(h, r, h);
+    r = fma(-h, g, 0.5);
+    g = fma(g, r, g); h = fma(h, r, h);
+    const double d = fma(-g, g, x);
+    return fma(d, h, g);
+}
+
+// sin and cos of a in [0, 8): a = k pi/2 + r, |r| <= pi/4.
+__device__ __forceinline__ void sincos_fast(double a, double& s_out, double& c_out) {
+    constexpr double kMagic = 6755399441055744.0;
+    constexpr double kTwoOverPi = 0.63661977236758134308;
+    constexpr double kPio2Hi = 0x1.921fb54442d18p+0, kPio2Lo = 0x1.1a62633145c07p-54;
+    const double t = fma(a, kTwoOverPi, kMagic);
+    const int k = __double2loint(t);
+    const double kd = t - kMagic;
+    double r = fma(kd, -kPio2Hi, a);
+    r = fma(kd, -kPio2Lo, r);
+    const double w = r * r;
+    double S = kSinS[5], C = kCosC[5];
+#pragma unroll
+    for (int i = 4; i >= 0; --i) { S = fma(S, w, kSinS[i]); C = fma(C, w, kCosC[i]); }
+    const double s = fma(r * w, S, r);
+    const double c = fma(w * w, C, fma(w, -0.5, 1.0));
+    const double sa = (k & 1) ? c : s, ca = (k & 1) ? s : c;
+    s_out = (k & 2) ? -sa : sa;
+    c_out = ((k + 1) & 2) ? -ca : ca;
+}
+
+}  // namespace pimc

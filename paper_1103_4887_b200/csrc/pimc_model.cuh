@@ -5,6 +5,7 @@
 // The caches hold the INCREMENT g, not f = x + g: the residual (x_{n+1} - x_n) - g_n then loses no bits to the
 // +-65 mV offset of V (matters in fp32).
 #pragma once
+#include "pimc_math.cuh"
 
 namespace pimc {
 
@@ -25,29 +26,51 @@ template <typename R> struct HHModel {
         const R tau = tau0 + tau1 * (R(1) - th * th);
         return (ainf - a) / tau;
     }
-    static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R I, R F[4]) {
+    // Double precision: one exponential and one reciprocal per gate.  With e = exp(2 s), q = e + 1:
+    //   tanh s = (e-1)/q, a_inf = e/q, 1 - tanh^2 s = 4 e / q^2  =>  (a_inf - a)/tau = (e - a q) q / (tau0 q^2 + 4 tau1 e).
+    // |2 s| is clamped at 80, where tanh s = +-1 to 1e-35 (far below half an ulp), so nothing overflows.
+    static __device__ __forceinline__ double gate_fast(double V, double a, double Va, double dVa, double tau0, double tau1) {
+        const double c1 = 2.0 / dVa, c0 = -2.0 * Va / dVa;
+        double s2 = fma(V, c1, c0);
+        s2 = fmin(fmax(s2, -80.0), 80.0);
+        const double e = exp_fast(s2);
+        const double q = e + 1.0;
+        const double num = fma(-a, q, e) * q;
+        const double den = fma(tau0 * q, q, (4.0 * tau1) * e);
+        return num * rcp_fast(den);
+    }
+    static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R inv_C, R I, R F[4]) {
         const R V = x[0], m = x[1], h = x[2], n = x[3];
         const R n2 = n * n;
         const R cur = I + p[0] * (m * m * m) * h * (p[3] - V) + p[1] * (n2 * n2) * (p[4] - V) + p[2] * (p[5] - V);
-        F[0] = cur / p[6];
-        F[1] = gate(V, m, R(-40.0), R(15.0), R(0.1), R(0.4));
-        F[2] = gate(V, h, R(-60.0), R(-15.0), R(1.0), R(7.0));
-        F[3] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
+        if constexpr (sizeof(R) == 8) {
+            F[0] = cur * inv_C;
+            F[1] = gate_fast(V, m, -40.0, 15.0, 0.1, 0.4);
+            F[2] = gate_fast(V, h, -60.0, -15.0, 1.0, 7.0);
+            F[3] = gate_fast(V, n, -55.0, 30.0, 1.0, 5.0);
+        } else {
+            F[0] = cur / p[6];
+            F[1] = gate(V, m, R(-40.0), R(15.0), R(0.1), R(0.4));
+            F[2] = gate(V, h, R(-60.0), R(-15.0), R(1.0), R(7.0));
+            F[3] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
+        }
     }
     static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
         const R Ih = R(0.5) * (I0 + I1);
         const R hdt = R(0.5) * dt;
+        R inv_C = R(0);
+        if constexpr (sizeof(R) == 8) inv_C = div_fast(1.0, p[6]);
         R k[4], xs[4], acc[4];
-        rhs(x, p, I0, k);
+        rhs(x, p, inv_C, I0, k);
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] = k[a]; xs[a] = x[a] + hdt * k[a]; }
-        rhs(xs, p, Ih, k);
+        rhs(xs, p, inv_C, Ih, k);
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + hdt * k[a]; }
-        rhs(xs, p, Ih, k);
+        rhs(xs, p, inv_C, Ih, k);
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + dt * k[a]; }
-        rhs(xs, p, I1, k);
+        rhs(xs, p, inv_C, I1, k);
         const R dt6 = dt / R(6);
 #pragma unroll
         for (int a = 0; a < 4; ++a) g[a] = dt6 * (acc[a] + k[a]);

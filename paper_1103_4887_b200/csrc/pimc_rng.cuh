@@ -5,6 +5,8 @@
 #pragma once
 #include <cstdint>
 
+#include "pimc_math.cuh"
+
 namespace pimc {
 
 enum : uint32_t { kStreamStateProposal = 0, kStreamStateAccept = 1, kStreamParam = 2 };
@@ -48,9 +50,9 @@ __device__ __forceinline__ float unit_openf(uint32_t w) { return (__uint2float_r
 
 // Box-Muller pair from two uniforms: radius sqrt(-2 ln u1), angle 2 pi u2.
 __device__ __forceinline__ void normal_pair(double u1, double u2, double& z0, double& z1) {
-    const double radius = sqrt(-2.0 * log(u1));
+    const double radius = sqrt_fast(-2.0 * log_fast(u1));
     double s, c;
-    sincos(6.283185307179586476925286766559 * u2, &s, &c);
+    sincos_fast(6.283185307179586476925286766559 * u2, s, c);
     z0 = radius * c;
     z1 = radius * s;
 }
