@@ -47,6 +47,12 @@ enum { PIMC_OK = 0, PIMC_EINVAL = -1, PIMC_ESTATE = -2, PIMC_ECUDA = -3, PIMC_EU
  * with Table 1 shifted by -65 mV; needs the injected current I. */
 enum { PIMC_MODEL_LINEAR = 0, PIMC_MODEL_HH = 1 };
 enum { PIMC_PROPOSAL_GAUSSIAN = 0, PIMC_PROPOSAL_UNIFORM = 1 };
+/* Sweep engines (same results, different data placement).  GLOBAL: path and cache stay
+ * in global memory (L2), threads stride over the tile, neighbour tiles synchronise every half-sweep with
+ * release/acquire flags; any tile length.  TILE: each CTA keeps its tile plus h halo sites in shared memory, one
+ * (even, odd) site pair per compute thread, halos updated redundantly and exchanged every h half-sweeps as tagged
+ * 8-byte packets; needs tile + 2h <= threads_per_cta <= 512.  AUTO: TILE when it fits, else GLOBAL. */
+enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2 };
 
 /* Number of parameters the model defines (HH: 7, LINEAR: D*D); negative on bad arguments. */
 int pimc_model_np(int model, int D);
@@ -135,6 +141,15 @@ int pimc_debug_trace(pimc_handle* h, void* dA_out, unsigned char* acc_out, void*
 int pimc_set_launch(pimc_handle* h, int ctas_per_chain, int threads_per_cta);
 /* Report the launch shape that pimc_sweep will use (any pointer may be NULL). */
 int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, int* tile_sites, int* smem_bytes);
+
+/* Choose the sweep engine (PIMC_ENGINE_*) and the halo depth of the TILE engine (-1 = automatic, else even, <= 16:
+ * half-sweeps between halo exchanges, row A3).  PIMC_EUNSUPPORTED if the problem does not fit the TILE engine. */
+int pimc_set_engine(pimc_handle* h, int engine, int halo);
+/* Report the engine and halo depth pimc_sweep will use (any pointer may be NULL). */
+int pimc_get_engine(pimc_handle* h, int* engine, int* halo);
+/* Synchronise the stream and report whether any inter-CTA hand-off timed out (*fault_host != 0 => PIMC_ECUDA;
+ * the chain state is then undefined).  A diagnostic: hand-offs cannot be lost in a co-resident (cooperative) launch. */
+int pimc_fault(pimc_handle* h, int* fault_host);
 
 unsigned long long pimc_sweep_index(const pimc_handle* h);
 int pimc_set_sweep_index(pimc_handle* h, unsigned long long t);

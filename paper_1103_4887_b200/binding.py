@@ -9,6 +9,7 @@ import numpy as np
 
 MODEL_LINEAR, MODEL_HH = 0, 1
 PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM = 0, 1
+ENGINE_AUTO, ENGINE_GLOBAL, ENGINE_TILE = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libpimc.so")
@@ -40,6 +41,9 @@ _SIGNATURES = {
     "pimc_debug_trace": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "pimc_set_launch": (C.c_int, [_vp, C.c_int, C.c_int]),
     "pimc_get_launch": (C.c_int, [_vp, _ip, _ip, _ip, _ip]),
+    "pimc_set_engine": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
+    "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
     "pimc_set_sweep_index": (C.c_int, [_vp, C.c_ulonglong]),
     "pimc_launch_count": (C.c_ulonglong, [_vp]),
@@ -198,6 +202,20 @@ class Pimc:
         v = [C.c_int() for _ in range(4)]
         _check(lib().pimc_get_launch(self._h, *[C.byref(q) for q in v]), self._h)
         return dict(ctas_per_chain=v[0].value, threads_per_cta=v[1].value, tile_sites=v[2].value, smem_bytes=v[3].value)
+
+    def set_engine(self, engine=ENGINE_AUTO, halo=-1):
+        _check(lib().pimc_set_engine(self._h, int(engine), int(halo)), self._h)
+
+    def get_engine(self):
+        e, hh = C.c_int(), C.c_int()
+        _check(lib().pimc_get_engine(self._h, C.byref(e), C.byref(hh)), self._h)
+        return dict(engine=e.value, halo=hh.value)
+
+    def fault(self):
+        """Synchronise the stream; raises PimcError if an inter-CTA hand-off was lost."""
+        f = C.c_int()
+        _check(lib().pimc_fault(self._h, C.byref(f)), self._h)
+        return f.value
 
     # ---- the hot path ----
     def sweep(self, n_sweeps, seed):

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpimc.so")
 SOURCES = ["pimc.cu"]
-DEPS = ["pimc.cu", "pimc_kernels.cuh", "pimc_model.cuh", "pimc_rng.cuh", "pimc_math.cuh", "pimc_math_coef.inc", os.path.join("..", "..", "include", "pimc.h")]
+DEPS = ["pimc.cu", "pimc_kernels.cuh", "pimc_tile_kernel.cuh", "pimc_model.cuh", "pimc_rng.cuh", "pimc_math.cuh", "pimc_math_coef.inc", os.path.join("..", "..", "include", "pimc.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "pimc_kernels.cuh"
+#include "pimc_tile_kernel.cuh"
 
 using namespace pimc;
 
@@ -41,6 +42,8 @@ struct Layout {
     unsigned long long* hist;
     unsigned long long *hs_flag, *ar_flag, *ar_epoch;
     double* ar_val;
+    unsigned long long *hx_words, *hx_epoch, *ar_words;
+    int* fault;
     size_t bytes;
 };
 
@@ -78,6 +81,10 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     o.ar_flag = c.take<unsigned long long>((size_t)C * 2 * kMaxCtasPerChain);
     o.ar_val = c.take<double>((size_t)C * 2 * kMaxCtasPerChain);
     o.ar_epoch = c.take<unsigned long long>(C);
+    o.hx_epoch = c.take<unsigned long long>(C);
+    o.hx_words = c.take<unsigned long long>((size_t)kTileMaxCtas * 2 * 2 * kHaloWordsPerSide);
+    o.ar_words = c.take<unsigned long long>((size_t)C * 2 * kTileMaxCtas * 2);
+    o.fault = c.take<int>(4);
     o.bytes = (c.off + 255) & ~(size_t)255;
     return o;
 }
@@ -108,7 +115,7 @@ struct pimc_handle {
     int n_sel = 0, nbins = 0;
     void *tr_dA = nullptr, *tr_xprop = nullptr, *tr_dAp = nullptr, *tr_pprop = nullptr;
     unsigned char *tr_acc = nullptr, *tr_accp = nullptr;
-    int G_user = 0, T_user = 0;
+    int G_user = 0, T_user = 0, engine_user = PIMC_ENGINE_AUTO, halo_user = -1;
     unsigned long long hs_base = 0, launches = 0;
     int sm_count = 0;
     std::string err;
@@ -151,10 +158,10 @@ template <typename F> int dispatch(int model, int D, int dtype, F&& f) {
     return PIMC_EUNSUPPORTED;
 }
 
-struct LaunchShape { int G, T, tile; bool cooperative; };
+struct LaunchShape { int G, T, tile; bool cooperative; int engine, h; size_t smem; };
 
 // Choose CTAs per chain, threads per CTA and the tile length (even).
-template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape* out) {
+template <class Model, typename R> int choose_shape_global(pimc_handle* h, LaunchShape* out) {
     int T = h->T_user;
     int G = h->G_user;
     const int sites = h->M + 1;
@@ -178,12 +185,67 @@ template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape*
     tile += tile & 1;
     G = (sites + tile - 1) / tile;     // drop empty tiles
     out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1;
+    out->engine = PIMC_ENGINE_GLOBAL; out->h = 0; out->smem = 0;
     if (G > 1) {
         PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R>, T, 0));
         if ((long long)G * h->C > (long long)per_sm * h->sm_count)
             return fail(h, PIMC_EINVAL, "grid of %d CTAs is not co-resident (capacity %d)", G * h->C, per_sm * h->sm_count);
     }
     return PIMC_OK;
+}
+
+// Tile-resident engine: G tiles per chain, each tile plus 2 h halo sites fits the 2 TC = T threads of its CTA
+// (one (even, odd) site pair per compute thread).  Returns PIMC_EUNSUPPORTED (without touching the error string)
+// when the problem does not fit, so that the automatic choice can fall back to the global-memory engine.
+template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchShape* out, bool quiet) {
+    const int sites = h->M + 1;
+    const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
+    auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
+    if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
+    int T = h->T_user, G = h->G_user;
+    if (T != 0 && (T % 64 != 0 || T > 512)) return no("threads_per_cta must be a multiple of 64, at most 512");
+    const int Tmax = T ? T : 512;
+    const int h_want = h->halo_user >= 0 ? h->halo_user : kTileHaloMax;
+    if (G == 0) {
+        if (sites <= (T ? T : 256)) G = 1;                          // whole chain in one CTA: no hand-off at all
+        else {
+            G = cap_ctas / h->C;                                    // spread each chain over as many SMs as there are
+            const int min_tile = 32;
+            if (G > (sites + min_tile - 1) / min_tile) G = (sites + min_tile - 1) / min_tile;
+            if (G < 1) G = 1;
+        }
+    }
+    if ((long long)G * h->C > cap_ctas && G > 1) return no("grid would not be co-resident");
+    int tile = (sites + G - 1) / G;
+    tile += tile & 1;
+    for (;;) {                                                      // the last tile must not be shorter than 2 sites
+        G = (sites + tile - 1) / tile;
+        const int last = sites - (G - 1) * tile;
+        if (G == 1 || last >= 2) break;
+        tile += 2;
+    }
+    int hh = 0;
+    if (G > 1) {
+        const int last = sites - (G - 1) * tile;
+        hh = std::min(h_want, kTileHaloMax) & ~1;
+        hh = std::min(hh, last & ~1);
+        hh = std::min(hh, tile & ~1);
+        hh = std::min(hh, ((Tmax - tile) / 2) & ~1);
+        if (hh < 2) return no("tile plus halos does not fit the CTA");
+    }
+    if (T == 0) T = std::max(64, (tile + 2 * hh + 63) / 64 * 64);
+    if (tile + 2 * hh > T || T > 512) return no("tile plus halos does not fit the CTA");
+    out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1; out->engine = PIMC_ENGINE_TILE; out->h = hh;
+    out->smem = tile_smem_bytes<R>(T, h->D, h->L);
+    if (out->smem > 227 * 1024) return no("shared memory");
+    return PIMC_OK;
+}
+
+template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape* out) {
+    if (h->engine_user == PIMC_ENGINE_GLOBAL) return choose_shape_global<Model, R>(h, out);
+    if (h->engine_user == PIMC_ENGINE_TILE) return choose_shape_tile<Model, R>(h, out, false);
+    if (choose_shape_tile<Model, R>(h, out, true) == PIMC_OK) return PIMC_OK;
+    return choose_shape_global<Model, R>(h, out);
 }
 
 template <class Model, typename R> int rebuild_cache(pimc_handle* h) {
@@ -225,17 +287,18 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     a.t0 = h->t; a.seed = seed; a.n_sweeps = n_sweeps; a.do_states = do_states; a.do_params = do_params;
     a.hs_flag = h->lay.hs_flag; a.ar_val = h->lay.ar_val; a.ar_flag = h->lay.ar_flag; a.ar_epoch = h->lay.ar_epoch;
     a.hs_base = h->hs_base;
+    a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault;
 
     const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
-    if (ls.cooperative) {
-        void* params[] = {&a};
-        PIMC_CUDA(h, cudaLaunchCooperativeKernel((const void*)sweep_kernel<Model, R>, grid, block, params, 0, h->stream));
-    } else {
-        sweep_kernel<Model, R><<<grid, block, 0, h->stream>>>(a);
-        PIMC_CUDA(h, cudaGetLastError());
-    }
+    const void* fn = ls.engine == PIMC_ENGINE_TILE
+                         ? (ls.T <= 256 ? (const void*)tile_sweep_kernel<Model, R, 256> : (const void*)tile_sweep_kernel<Model, R, 512>)
+                         : (const void*)sweep_kernel<Model, R>;
+    if (ls.smem > 48 * 1024) PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
+    void* params[] = {&a};
+    if (ls.cooperative) PIMC_CUDA(h, cudaLaunchCooperativeKernel(fn, grid, block, params, ls.smem, h->stream));
+    else PIMC_CUDA(h, cudaLaunchKernel(fn, grid, block, params, ls.smem, h->stream));
     h->launches++;
-    if (do_states) h->hs_base += 2ull * (unsigned long long)n_sweeps;
+    if (do_states && ls.engine == PIMC_ENGINE_GLOBAL) h->hs_base += 2ull * (unsigned long long)n_sweeps;
     if (h->accum) {   // host bookkeeping of the sample count: sweeps t in [t0, t0+n) with (t - t_enable) % n_skip == 0
         const unsigned long long first = h->t - h->t_enable, last = first + (unsigned long long)n_sweeps;   // [first, last)
         const unsigned long long k = h->n_skip;
@@ -531,7 +594,37 @@ int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, i
     if (ctas_per_chain) *ctas_per_chain = ls.G;
     if (threads_per_cta) *threads_per_cta = ls.T;
     if (tile_sites) *tile_sites = ls.tile;
-    if (smem_bytes) *smem_bytes = 0;
+    if (smem_bytes) *smem_bytes = (int)ls.smem;
+    return PIMC_OK;
+}
+
+int pimc_set_engine(pimc_handle* h, int engine, int halo) {
+    if (!h) return PIMC_EINVAL;
+    if (engine < PIMC_ENGINE_AUTO || engine > PIMC_ENGINE_TILE) return fail(h, PIMC_EINVAL, "unknown engine");
+    if (halo < -1 || halo > kTileHaloMax || (halo > 0 && (halo & 1))) return fail(h, PIMC_EINVAL, "halo must be -1 (automatic) or an even number in [0,%d]", kTileHaloMax);
+    const int e0 = h->engine_user, h0 = h->halo_user;
+    h->engine_user = engine; h->halo_user = halo;
+    LaunchShape ls;
+    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    if (rc != PIMC_OK) { h->engine_user = e0; h->halo_user = h0; }
+    return rc;
+}
+
+int pimc_get_engine(pimc_handle* h, int* engine, int* halo) {
+    if (!h) return PIMC_EINVAL;
+    LaunchShape ls;
+    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    if (rc != PIMC_OK) return rc;
+    if (engine) *engine = ls.engine;
+    if (halo) *halo = ls.h;
+    return PIMC_OK;
+}
+
+int pimc_fault(pimc_handle* h, int* fault_host) {
+    if (!h || !fault_host) return fail(h, PIMC_EINVAL, "null argument");
+    PIMC_CUDA(h, cudaMemcpyAsync(fault_host, h->lay.fault, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    PIMC_CUDA(h, cudaStreamSynchronize(h->stream));
+    if (*fault_host) return fail(h, PIMC_ECUDA, "a hand-off between CTAs was never delivered (fault flag %d)", *fault_host);
     return PIMC_OK;
 }
 

@@ -63,6 +63,12 @@ template <typename R> struct SweepArgs {
     unsigned long long* ar_flag;  // (C, 2, G)
     unsigned long long* ar_epoch; // (C) all-reduce events performed so far (device-side bookkeeping)
     unsigned long long hs_base;
+    // tile-resident engine (pimc_tile_kernel.cuh): halo depth, tagged-packet mailboxes, fault flag
+    int h;
+    unsigned long long* hx_words;   // (kTileMaxCtas, 2 sides, 2 slots, kHaloWordsPerSide)
+    unsigned long long* hx_epoch;   // (C) halo exchanges performed so far
+    unsigned long long* ar_words;   // (C, 2 slots, kTileMaxCtas, 2) Delta-A partials
+    int* fault;                     // set to 1 if a hand-off was never delivered
 };
 
 // ---- memory-model helpers ------------------------------------------------------------------------

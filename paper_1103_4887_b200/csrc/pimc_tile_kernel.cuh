@@ -1,0 +1,516 @@
+// Tile-resident persistent sweep kernel (engine PIMC_ENGINE_TILE): rows A1-A6 of SURVEY.md §8(a) with the
+// path tile, the step cache, the data and the running moments of a CTA held in shared memory for the whole
+// pimc_sweep call.
+//
+// Why.  With one chain of M = 32768 there are only M/2 independent site-updates per half-sweep
+// (PAPER.md:185, 207): about one per thread on 148 SMs.  The half-sweep time is therefore the LATENCY of one
+// site-update, and the global-memory engine (pimc_kernels.cuh) spends it on three dependent L2 round trips,
+// a gpu-scope fence + flag per half-sweep and a serial Philox -> Box-Muller -> RK4 chain
+// (profiles/r01_v2_*.md).  This engine removes each of those from the critical path:
+//   * the tile [s_ext, e_ext) = owned sites [s, e) plus `h` halo sites on each side lives in shared memory;
+//     a neighbour value costs one LDS;
+//   * the CTA is warp-specialised inside the state half-sweeps: threads [0, TC) own one (even, odd) site pair
+//     each and run the Metropolis update; threads [TC, 2 TC) draw the proposals and log-uniforms of the NEXT
+//     sweep (Philox is stateless, PAPER.md:234 replaced per SURVEY Delta-8) into a double-buffered ring, so
+//     no random number is ever generated on the critical path;
+//   * halo sites are updated REDUNDANTLY by both neighbours (same Philox counters => same bits), which
+//     is correct for k half-sweeps on sites at least k away from the tile edge; the tiles only exchange their
+//     h edge sites every h half-sweeps (row A3) instead of synchronising every half-sweep;
+//   * every inter-CTA message (halo values, Delta-A partials of the parameter all-reduce) is a set of 8-byte
+//     packets {32 payload bits, 32-bit epoch tag} written with relaxed stores and polled with relaxed loads:
+//     one L2 round trip, no fence, no separate flag (an aligned 8-byte access is single-copy atomic).
+// Parameter moves (row A4) use all 2 TC threads, one tile site each.
+#pragma once
+#include "pimc_kernels.cuh"
+
+namespace pimc {
+
+constexpr int kTileHaloMax = 16;                                   // largest halo depth h
+constexpr int kTileMaxCtas = 2048;                                 // inbox slots (global CTA index)
+constexpr int kHaloWordsPerSide = kTileHaloMax * 2 * kMaxD * 2;    // h sites x (x, g) x D values x 2 words
+constexpr unsigned long long kSpinLimit = 20ull * 1000 * 1000;    // polls before a hand-off is declared lost
+
+// ---- 8-byte tagged packets ---------------------------------------------------------------------------------
+__device__ __forceinline__ void ll_store(unsigned long long* p, uint32_t payload, uint32_t tag) {
+    const unsigned long long v = ((unsigned long long)tag << 32) | (unsigned long long)payload;
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ll_load(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+// Poll until the packet carries `tag`; returns the payload.  Gives up (and raises the fault flag) after kSpinLimit polls.
+__device__ __forceinline__ uint32_t ll_wait(const unsigned long long* p, uint32_t tag, int* fault) {
+    unsigned long long v = ll_load(p);
+    unsigned long long spins = 0;
+    while ((uint32_t)(v >> 32) != tag) {
+        ++spins;
+        if (spins > kSpinLimit) { atomicExch(fault, 1); break; }
+        if ((spins & 0xFFFFull) == 0 && *reinterpret_cast<volatile int*>(fault) != 0) break;   // somebody else already gave up
+        v = ll_load(p);
+    }
+    return (uint32_t)v;
+}
+__device__ __forceinline__ void bar_compute(int n_threads) {     // named barrier 1: the compute warps only
+    asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory");
+}
+
+template <typename R> struct TileSmem {
+    double *S1, *S2, *cc;       // [E*D] running moments of the tile (fp64 always)
+    double* red;                // [32]
+    double* pdraw;              // [2 sets][kMaxNp][2] = (step, log u) of the parameter moves
+    double *blo, *bhi;          // [kMaxNp] bounds
+    R *xs, *g0, *g1;            // [(E+1)*D]
+    R *Is, *ys;                 // [E+2], [E*L]
+    R *rstep, *rlogu;           // [2 sets][2 parities][TC][D], [2][2][TC]
+    unsigned int* cnt;          // [2]: accepted owned state updates (lo, unused)
+};
+
+template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L) {
+    const size_t E = (size_t)T, TC = (size_t)T / 2;
+    size_t dbl = 3 * E * D + 32 + 2 * kMaxNp * 2 + 2 * kMaxNp + 2;
+    size_t real = 3 * (E + 1) * D + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * TC * D + 4 * TC;
+    return dbl * 8 + ((real * sizeof(R) + 15) & ~(size_t)15) + 16;
+}
+
+template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L) {
+    const size_t E = (size_t)T, TC = (size_t)T / 2;
+    TileSmem<R> m;
+    double* d = reinterpret_cast<double*>(base);
+    m.S1 = d; d += E * D;
+    m.S2 = d; d += E * D;
+    m.cc = d; d += E * D;
+    m.red = d; d += 32;
+    m.pdraw = d; d += 2 * kMaxNp * 2;
+    m.blo = d; d += kMaxNp;
+    m.bhi = d; d += kMaxNp;
+    m.cnt = reinterpret_cast<unsigned int*>(d); d += 2;
+    R* r = reinterpret_cast<R*>(d);
+    m.xs = r; r += (E + 1) * D;
+    m.g0 = r; r += (E + 1) * D;
+    m.g1 = r; r += (E + 1) * D;
+    m.Is = r; r += E + 2;
+    m.ys = r; r += E * (size_t)(L > 0 ? L : 1);
+    m.rstep = r; r += 4 * TC * D;
+    m.rlogu = r; r += 4 * TC;
+    return m;
+}
+
+template <typename R, int D> __device__ __forceinline__ void lds_vec(const R* base, int row, R out[D]) {
+#pragma unroll
+    for (int c = 0; c < D; ++c) out[c] = base[row * D + c];
+}
+template <typename R, int D> __device__ __forceinline__ void sts_vec(R* base, int row, const R v[D]) {
+#pragma unroll
+    for (int c = 0; c < D; ++c) base[row * D + c] = v[c];
+}
+
+// ---- producer: proposal steps w_a z_a and log u for one site of one half-sweep (row A1) ----------------------
+template <typename R, int D>
+__device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n, R* step_out, R* logu_out) {
+    const Words4 w = draw(a.seed, t, chain, n, kStreamStateProposal, 0);
+    R st[4] = {R(0), R(0), R(0), R(0)};
+    if (a.kind == 1) {
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            if constexpr (sizeof(R) == 8) st[c] = __dmul_rn(a.wx[c], 2.0 * unit_open(w.w[c]) - 1.0);
+            else st[c] = __fmul_rn(a.wx[c], __fsub_rn(__fmul_rn(2.0f, unit_openf(w.w[c])), 1.0f));
+        }
+    } else {
+        R z[4] = {R(0), R(0), R(0), R(0)};
+        if constexpr (sizeof(R) == 8) {
+            normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z[0], z[1]);
+            if constexpr (D > 2) normal_pair(unit_open(w.w[2]), unit_open(w.w[3]), z[2], z[3]);
+        } else {
+            normal_pair(unit_openf(w.w[0]), unit_openf(w.w[1]), z[0], z[1]);
+            if constexpr (D > 2) normal_pair(unit_openf(w.w[2]), unit_openf(w.w[3]), z[2], z[3]);
+        }
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            if constexpr (sizeof(R) == 8) st[c] = __dmul_rn(a.wx[c], z[c]);
+            else st[c] = __fmul_rn(a.wx[c], z[c]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < D; ++c) step_out[c] = st[c];
+    *logu_out = log_accept_uniform<R>(a, t, chain, n);
+}
+
+// ---- the kernel ----------------------------------------------------------------------------------------------
+template <class Model, typename R, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
+    constexpr int D = Model::D;
+    constexpr int NP = Model::NP;
+    extern __shared__ __align__(16) unsigned char tile_smem_raw[];
+    const int T = blockDim.x, TC = T >> 1, tid = threadIdx.x;
+    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L);
+
+    const int G = a.G, M = a.M, L = a.L, h = a.h;
+    const uint32_t chain = blockIdx.x / G;
+    const int b = blockIdx.x % G;
+    const int s = b * a.tile, e = min(s + a.tile, M + 1);
+    const int s_ext = max(0, s - h), e_ext = min(M + 1, e + h), n_ext = e_ext - s_ext;
+    const size_t site0 = (size_t)chain * (M + 1);
+    const bool edge_lo = s_ext == 0, edge_hi = e_ext == M + 1;
+
+    R* const gx = a.x + site0 * D;
+    R* const gg0 = a.g[0] + (size_t)chain * M * D;
+    R* const gg1 = a.g[1] + (size_t)chain * M * D;
+    int cur = a.cur[chain];
+
+    // ---- load the extended tile ----
+    for (int idx = tid; idx < n_ext * D; idx += T) sm.xs[idx] = gx[(size_t)s_ext * D + idx];
+    {
+        const R* gsrc = cur ? gg1 : gg0;
+        R* gdst = cur ? sm.g1 : sm.g0;
+        const int ng = min(e_ext, M) - s_ext;      // cache entries exist for n <= M-1
+        for (int idx = tid; idx < ng * D; idx += T) gdst[idx] = gsrc[(size_t)s_ext * D + idx];
+    }
+    for (int i = tid; i <= n_ext; i += T) {
+        const int n = s_ext + i;
+        sm.Is[i] = (a.I && n <= M) ? a.I[site0 + n] : R(0);
+    }
+    for (int idx = tid; idx < n_ext * L; idx += T) sm.ys[idx] = a.y[(site0 + s_ext) * L + idx];
+    if (a.accum) {
+        for (int idx = tid; idx < n_ext * D; idx += T) {
+            const size_t gi = (site0 + s_ext) * D + idx;
+            sm.S1[idx] = a.S1x[gi]; sm.S2[idx] = a.S2x[gi]; sm.cc[idx] = a.cx[gi];
+        }
+    }
+    if (tid < NP) { sm.blo[tid] = a.lo[(size_t)chain * NP + tid]; sm.bhi[tid] = a.hi[(size_t)chain * NP + tid]; }
+    if (tid == 0) { sm.cnt[0] = 0; }
+    R prm[NP];                                     // every thread keeps the (identical) parameter vector in registers
+#pragma unroll
+    for (int k = 0; k < NP; ++k) prm[k] = a.p[(size_t)chain * NP + k];
+
+    unsigned long long ar_count = a.ar_epoch[chain];
+    unsigned long long hx_count = a.hx_epoch[chain];
+    unsigned int n_acc_state = 0, pacc[NP], pprop[NP];
+#pragma unroll
+    for (int k = 0; k < NP; ++k) { pacc[k] = 0; pprop[k] = 0; }
+
+    // ---- producers: fill RNG set `set` for sweep t ----
+    auto produce = [&](int set, unsigned long long t) {
+        const int j = tid - TC;
+        if (a.do_states) {
+#pragma unroll 1
+            for (int parity = 0; parity < 2; ++parity) {
+                const int n = s_ext + 2 * j + parity;
+                if (n <= M && 2 * j + parity < n_ext)
+                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.rstep + ((size_t)(set * 2 + parity) * TC + j) * D,
+                                       sm.rlogu + (size_t)(set * 2 + parity) * TC + j);
+            }
+        }
+        if (a.do_params && j < NP && a.wp[j] > 0.0) {
+            const Words4 w = draw(a.seed, t, chain, (uint32_t)j, kStreamParam, 0);
+            double step;
+            if (a.kind == 1) step = __dmul_rn(a.wp[j], 2.0 * unit_open(w.w[0]) - 1.0);
+            else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(a.wp[j], z0); }
+            sm.pdraw[(set * kMaxNp + j) * 2 + 0] = step;
+            sm.pdraw[(set * kMaxNp + j) * 2 + 1] = log_fast(unit_open52(w.w[2], w.w[3]));
+        }
+    };
+    if (tid >= TC) produce(0, a.t0);
+    __syncthreads();
+
+    int k_phase = 0;                               // half-sweeps since the halos were last exact
+    for (long long i = 0; i < a.n_sweeps; ++i) {
+        const unsigned long long t = a.t0 + (unsigned long long)i;
+        const int set = (int)(i & 1);
+        const bool trace = (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
+
+        if (tid < TC) {
+            // ---------------- A2: even half-sweep, then odd half-sweep (compute warps) ----------------
+            if (a.do_states) {
+#pragma unroll 1
+                for (int parity = 0; parity < 2; ++parity) {
+                    const int k = k_phase + parity + 1;      // half-sweeps run on the current halos, this one included
+                    const int iloc = 2 * tid + parity, n = s_ext + iloc;
+                    const bool ok = n <= M && iloc < n_ext && (edge_lo || iloc >= k) && (edge_hi || iloc < n_ext - k);
+                    if (ok) {
+                        R* gc = cur ? sm.g1 : sm.g0;
+                        R xn[D], xp[D], gp[D];
+                        lds_vec<R, D>(sm.xs, iloc, xn);
+                        const R* st = sm.rstep + ((size_t)(set * 2 + parity) * TC + tid) * D;
+#pragma unroll
+                        for (int c = 0; c < D; ++c) {
+                            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], st[c]);
+                            else xp[c] = __fadd_rn(xn[c], st[c]);
+                        }
+                        R dA = R(0);
+                        if (n >= 1) {
+                            R xm[D], gm[D];
+                            lds_vec<R, D>(sm.xs, iloc - 1, xm);
+                            lds_vec<R, D>(gc, iloc - 1, gm);
+#pragma unroll
+                            for (int c = 0; c < D; ++c) {
+                                const R r_new = (xp[c] - xm[c]) - gm[c];
+                                const R r_old = (xn[c] - xm[c]) - gm[c];
+                                dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            }
+#pragma unroll
+                            for (int l = 0; l < D; ++l) {
+                                if (l < L) {
+                                    const R yn = sm.ys[iloc * L + l];
+                                    const R d_new = yn - xp[l], d_old = yn - xn[l];
+                                    dA += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
+                                }
+                            }
+                        }
+                        if (n <= M - 1) {
+                            R xq[D], gn[D];
+                            lds_vec<R, D>(sm.xs, iloc + 1, xq);
+                            lds_vec<R, D>(gc, iloc, gn);
+                            Model::increment(xp, prm, sm.Is[iloc], sm.Is[iloc + 1], a.dt, gp);
+#pragma unroll
+                            for (int c = 0; c < D; ++c) {
+                                const R r_new = (xq[c] - xp[c]) - gp[c];
+                                const R r_old = (xq[c] - xn[c]) - gn[c];
+                                dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            }
+                        }
+                        const R logu = sm.rlogu[(size_t)(set * 2 + parity) * TC + tid];
+                        const bool accept = logu < -dA;
+                        if (accept) {
+                            sts_vec<R, D>(sm.xs, iloc, xp);
+                            if (n <= M - 1) sts_vec<R, D>(gc, iloc, gp);
+                        }
+                        const bool owned = n >= s && n < e;
+                        if (owned) {
+                            n_acc_state += accept ? 1u : 0u;
+                            if (trace) {
+                                const size_t gs = site0 + (size_t)n;
+                                if (a.tr_dA) a.tr_dA[gs] = dA;
+                                if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
+                                if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
+                            }
+                        }
+                    }
+                    bar_compute(TC);
+                }
+            }
+        } else {
+            // ---------------- A1: proposals and uniforms of the next sweep (producer warps) ----------------
+            if (i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull);
+        }
+        if (a.do_states) k_phase += 2;               // every thread keeps the count: the hand-off below is CTA-uniform
+        __syncthreads();
+
+        // ---------------- A4: parameter moves, in sequence; one tile site per thread ----------------
+        if (a.do_params) {
+            const int r = tid, n = s_ext + r;
+            const bool can_eval = r < n_ext && n <= M - 1;
+            const bool owned = n >= s && n < e && n <= M - 1;
+#pragma unroll 1
+            for (int l = 0; l < NP; ++l) {
+                if (!(a.wp[l] > 0.0)) continue;
+                const double step = sm.pdraw[(set * kMaxNp + l) * 2 + 0], logu = sm.pdraw[(set * kMaxNp + l) * 2 + 1];
+                R pcur = R(0);
+#pragma unroll
+                for (int k = 0; k < NP; ++k) pcur = (k == l) ? prm[k] : pcur;
+                double pl;
+                if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)pcur, step);
+                else pl = (double)__fadd_rn(pcur, (float)step);
+                const bool inside = pl >= sm.blo[l] && pl <= sm.bhi[l];
+                bool accept = false;
+                double dA = __longlong_as_double(0x7FF8000000000000ll);
+                if (inside) {
+                    R pp[NP];
+#pragma unroll
+                    for (int k = 0; k < NP; ++k) pp[k] = (k == l) ? (R)pl : prm[k];
+                    R* gc = cur ? sm.g1 : sm.g0;
+                    R* ga = cur ? sm.g0 : sm.g1;
+                    double part = 0.0;
+                    if (can_eval) {
+                        R xn[D], gp[D];
+                        lds_vec<R, D>(sm.xs, r, xn);
+                        Model::increment(xn, pp, sm.Is[r], sm.Is[r + 1], a.dt, gp);
+                        sts_vec<R, D>(ga, r, gp);
+                        if (owned) {
+                            R xq[D], gn[D];
+                            lds_vec<R, D>(sm.xs, r + 1, xq);
+                            lds_vec<R, D>(gc, r, gn);
+                            R acc = R(0);
+#pragma unroll
+                            for (int c = 0; c < D; ++c) {
+                                const R d = xq[c] - xn[c];
+                                const R r_new = d - gp[c], r_old = d - gn[c];
+                                acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            }
+                            part = (double)acc;
+                        }
+                    }
+                    dA = block_sum(part, sm.red);
+                    if (G > 1) {   // all-gather of the G partials as tagged packets; every CTA sums them in index order
+                        const uint32_t tag = (uint32_t)(ar_count + 1ull);
+                        unsigned long long* base = a.ar_words + ((size_t)chain * 2 + (size_t)(ar_count & 1ull)) * (size_t)kTileMaxCtas * 2;
+                        if (tid == 0) {
+                            const unsigned long long bits = (unsigned long long)__double_as_longlong(dA);
+                            ll_store(base + 2 * b, (uint32_t)bits, tag);
+                            ll_store(base + 2 * b + 1, (uint32_t)(bits >> 32), tag);
+                        }
+                        double mine = 0.0;
+                        for (int j = tid; j < G; j += T) {
+                            const uint32_t lo = ll_wait(base + 2 * j, tag, a.fault);
+                            const uint32_t hi = ll_wait(base + 2 * j + 1, tag, a.fault);
+                            mine += __longlong_as_double((long long)(((unsigned long long)hi << 32) | lo));
+                        }
+                        dA = block_sum(mine, sm.red);
+                        ar_count += 1ull;
+                    }
+                    accept = logu < -dA;
+                    if (accept) cur ^= 1;
+                }
+#pragma unroll
+                for (int k = 0; k < NP; ++k) {
+                    if (k == l) {
+                        pprop[k] += 1;
+                        if (accept) { prm[k] = (R)pl; pacc[k] += 1; }
+                    }
+                }
+                if (trace && b == 0 && tid == 0) {
+                    if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)dA;
+                    if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = accept ? 1 : 0;
+                    if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = (R)pl;
+                }
+            }
+            if (trace && b == 0 && tid == 0) {
+#pragma unroll
+                for (int l = 0; l < NP; ++l)
+                    if (!(a.wp[l] > 0.0)) {
+                        if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)__longlong_as_double(0x7FF8000000000000ll);
+                        if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = 0;
+                        if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = prm[l];
+                    }
+            }
+        }
+
+        // ---------------- A3: refresh the halos from the neighbour tiles ----------------
+        // needed once h half-sweeps have been run on the current halos.  Parameter moves do not shorten that: they
+        // re-evaluate the cache of every tile site from its own state, so sites inside the still-exact cone stay exact.
+        if (G > 1 && a.do_states && i + 1 < a.n_sweeps && k_phase + 2 > h) {
+            const uint32_t tag = (uint32_t)(hx_count + 1ull);
+            const size_t slot = (size_t)(hx_count & 1ull);
+            constexpr int WPV = sizeof(R) / 4;               // packets per value
+            const int nwords = h * 2 * D * WPV;              // per direction
+            const R* gc = cur ? sm.g1 : sm.g0;
+            const uint32_t* xs32 = reinterpret_cast<const uint32_t*>(sm.xs);
+            const uint32_t* gc32 = reinterpret_cast<const uint32_t*>(gc);
+            // send: word w <-> (site offset o, which (0: x, 1: g), component c, half)
+            for (int w = tid; w < 2 * nwords; w += T) {
+                const int dir = w / nwords, q = w % nwords;      // dir 0: to the left neighbour, 1: to the right
+                if ((dir == 0 && b == 0) || (dir == 1 && b == G - 1)) continue;
+                const int o = q / (2 * D * WPV), rem = q % (2 * D * WPV);
+                const int which = rem / (D * WPV), cw = rem % (D * WPV);
+                const int nsite = dir == 0 ? s + o : e - h + o;
+                const int iloc = nsite - s_ext;
+                uint32_t payload = 0;
+                if (which == 0) payload = xs32[iloc * D * WPV + cw];
+                else if (nsite <= M - 1) payload = gc32[iloc * D * WPV + cw];
+                const int dst_cta = (int)blockIdx.x + (dir == 0 ? -1 : 1);
+                const int dst_side = dir == 0 ? 1 : 0;           // my left neighbour receives "from its right"
+                unsigned long long* box = a.hx_words + (((size_t)dst_cta * 2 + dst_side) * 2 + slot) * (size_t)kHaloWordsPerSide;
+                ll_store(box + q, payload, tag);
+            }
+            // receive
+            uint32_t* xd32 = reinterpret_cast<uint32_t*>(sm.xs);
+            uint32_t* gd32 = reinterpret_cast<uint32_t*>(cur ? sm.g1 : sm.g0);
+            for (int w = tid; w < 2 * nwords; w += T) {
+                const int side = w / nwords, q = w % nwords;     // side 0: from the left neighbour, 1: from the right
+                if ((side == 0 && b == 0) || (side == 1 && b == G - 1)) continue;
+                const int o = q / (2 * D * WPV), rem = q % (2 * D * WPV);
+                const int which = rem / (D * WPV), cw = rem % (D * WPV);
+                const int nsite = side == 0 ? s - h + o : e + o;
+                const int iloc = nsite - s_ext;
+                const unsigned long long* box = a.hx_words + (((size_t)blockIdx.x * 2 + side) * 2 + slot) * (size_t)kHaloWordsPerSide;
+                const uint32_t payload = ll_wait(box + q, tag, a.fault);
+                if (which == 0) xd32[iloc * D * WPV + cw] = payload;
+                else if (nsite <= M - 1) gd32[iloc * D * WPV + cw] = payload;
+            }
+            hx_count += 1ull;
+            k_phase = 0;
+            __syncthreads();
+        }
+
+        // ---------------- A5: running moments and histograms (owned sites) ----------------
+        if (a.accum && ((t - a.t_enable) % a.n_skip) == 0ull) {
+            for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) {
+                const double d = (double)sm.xs[idx] - sm.cc[idx];
+                sm.S1[idx] += d;
+                sm.S2[idx] += d * d;
+            }
+            if (b == 0 && tid < NP) {
+                const size_t gi = (size_t)chain * NP + tid;
+                double pv = 0.0;
+#pragma unroll
+                for (int k = 0; k < NP; ++k) pv = (k == tid) ? (double)prm[k] : pv;
+                const double d = pv - a.cp[gi];
+                a.S1p[gi] += d;
+                a.S2p[gi] += d * d;
+            }
+            for (int sel = tid; sel < a.n_sel; sel += T) {
+                const int site = a.hsite[sel], comp = a.hcomp[sel];
+                const bool mine = site < 0 ? (b == 0) : (site >= s && site < e);
+                if (mine) {
+                    double v = 0.0;
+                    if (site < 0) {
+#pragma unroll
+                        for (int k = 0; k < NP; ++k) v = (k == comp) ? (double)prm[k] : v;
+                    } else v = (double)sm.xs[(site - s_ext) * D + comp];
+                    unsigned long long* bins = a.hist + ((size_t)chain * a.n_sel + sel) * (size_t)(a.nbins + 2);
+                    const double lo = a.hlo[sel], hi = a.hhi[sel];
+                    int bin;
+                    if (!(v >= lo)) bin = 0;
+                    else if (v >= hi) bin = a.nbins + 1;
+                    else {
+                        long long q = (long long)floor((v - lo) / a.hwidth[sel]);
+                        if (q >= a.nbins) q = a.nbins - 1;
+                        bin = 1 + (int)q;
+                    }
+                    bins[bin] += 1ull;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---------------- write the tile back; A6 counters ----------------
+    for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) gx[(size_t)s_ext * D + idx] = sm.xs[idx];
+    {
+        R* gdst = cur ? gg1 : gg0;
+        const R* gsrc = cur ? sm.g1 : sm.g0;
+        const int hi_g = min(e, M);
+        for (int idx = (s - s_ext) * D + tid; idx < (hi_g - s_ext) * D; idx += T) gdst[(size_t)s_ext * D + idx] = gsrc[idx];
+    }
+    if (a.accum) {
+        for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) {
+            const size_t gi = (site0 + s_ext) * D + idx;
+            a.S1x[gi] = sm.S1[idx]; a.S2x[gi] = sm.S2[idx];
+        }
+    }
+    if (n_acc_state) atomicAdd(sm.cnt, n_acc_state);
+    __syncthreads();
+    if (tid == 0) {
+        unsigned long long* cnt = a.counters + (size_t)chain * 2 * (D + NP);
+        const unsigned long long acc_u = sm.cnt[0];
+        const unsigned long long prop_u = a.do_states ? (unsigned long long)(e - s) * (unsigned long long)a.n_sweeps : 0ull;
+        for (int c = 0; c < D; ++c) {
+            if (acc_u) atomicAdd(cnt + c, acc_u);
+            if (prop_u) atomicAdd(cnt + (D + NP) + c, prop_u);
+        }
+        if (b == 0) {
+#pragma unroll
+            for (int l = 0; l < NP; ++l) {
+                cnt[D + l] += pacc[l];
+                cnt[(D + NP) + D + l] += pprop[l];
+                a.p[(size_t)chain * NP + l] = prm[l];
+            }
+            a.cur[chain] = cur;
+            a.ar_epoch[chain] = ar_count;
+            a.hx_epoch[chain] = hx_count;
+        }
+    }
+}
+
+}  // namespace pimc
