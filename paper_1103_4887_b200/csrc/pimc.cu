@@ -83,7 +83,7 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     o.ar_epoch = c.take<unsigned long long>(C);
     o.hx_epoch = c.take<unsigned long long>(C);
     o.hx_words = c.take<unsigned long long>((size_t)kTileMaxCtas * 2 * 2 * kHaloWordsPerSide);
-    o.ar_words = c.take<unsigned long long>((size_t)C * 2 * kTileMaxCtas * 2);
+    o.ar_words = c.take<unsigned long long>((size_t)2 * kTileMaxCtas * kArSlotWords);
     o.fault = c.take<int>(4);
     o.bytes = (c.off + 255) & ~(size_t)255;
     return o;

@@ -67,7 +67,7 @@ template <typename R> struct SweepArgs {
     int h;
     unsigned long long* hx_words;   // (kTileMaxCtas, 2 sides, 2 slots, kHaloWordsPerSide)
     unsigned long long* hx_epoch;   // (C) halo exchanges performed so far
-    unsigned long long* ar_words;   // (C, 2 slots, kTileMaxCtas, 2) Delta-A partials
+    unsigned long long* ar_words;   // (2 slots, kTileMaxCtas, kArSlotWords) Delta-A partials, one 128-byte line per CTA
     int* fault;                     // set to 1 if a hand-off was never delivered
 };
 

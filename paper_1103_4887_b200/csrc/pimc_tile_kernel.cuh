@@ -26,7 +26,8 @@
 namespace pimc {
 
 constexpr int kTileHaloMax = 16;                                   // largest halo depth h
-constexpr int kTileMaxCtas = 2048;                                 // inbox slots (global CTA index)
+constexpr int kTileMaxCtas = 256;                                  // inbox slots (global CTA index); the grid is co-resident, one CTA per SM
+constexpr int kArSlotWords = 16;                                   // one 128-byte line per CTA: slots sharing a line serialise in L2 (measured 2x slower)
 constexpr int kHaloWordsPerSide = kTileHaloMax * 2 * kMaxD * 2;    // h sites x (x, g) x D values x 2 words
 constexpr unsigned long long kSpinLimit = 20ull * 1000 * 1000;    // polls before a hand-off is declared lost
 
@@ -51,6 +52,22 @@ __device__ __forceinline__ uint32_t ll_wait(const unsigned long long* p, uint32_
         v = ll_load(p);
     }
     return (uint32_t)v;
+}
+// A double as two tagged packets in one 16-byte access (each 8-byte half is single-copy atomic and carries its own tag).
+__device__ __forceinline__ void ll_store_f64(unsigned long long* p, double v, uint32_t tag) {
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(v), t = (unsigned long long)tag << 32;
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(t | (bits & 0xFFFFFFFFull)), "l"(t | (bits >> 32)) : "memory");
+}
+__device__ __forceinline__ double ll_wait_f64(const unsigned long long* p, uint32_t tag, int* fault) {
+    unsigned long long a, b, spins = 0;
+    for (;;) {
+        asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+        if ((uint32_t)(a >> 32) == tag && (uint32_t)(b >> 32) == tag) break;
+        ++spins;
+        if (spins > kSpinLimit) { atomicExch(fault, 1); break; }
+        if ((spins & 0xFFFFull) == 0 && *reinterpret_cast<volatile int*>(fault) != 0) break;
+    }
+    return __longlong_as_double((long long)((b << 32) | (a & 0xFFFFFFFFull)));
 }
 __device__ __forceinline__ void bar_compute(int n_threads) {     // named barrier 1: the compute warps only
     asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory");
@@ -344,18 +361,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     dA = block_sum(part, sm.red);
                     if (G > 1) {   // all-gather of the G partials as tagged packets; every CTA sums them in index order
                         const uint32_t tag = (uint32_t)(ar_count + 1ull);
-                        unsigned long long* base = a.ar_words + ((size_t)chain * 2 + (size_t)(ar_count & 1ull)) * (size_t)kTileMaxCtas * 2;
-                        if (tid == 0) {
-                            const unsigned long long bits = (unsigned long long)__double_as_longlong(dA);
-                            ll_store(base + 2 * b, (uint32_t)bits, tag);
-                            ll_store(base + 2 * b + 1, (uint32_t)(bits >> 32), tag);
-                        }
+                        unsigned long long* base = a.ar_words + ((size_t)(ar_count & 1ull) * kTileMaxCtas + (size_t)chain * G) * kArSlotWords;
+                        if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
                         double mine = 0.0;
-                        for (int j = tid; j < G; j += T) {
-                            const uint32_t lo = ll_wait(base + 2 * j, tag, a.fault);
-                            const uint32_t hi = ll_wait(base + 2 * j + 1, tag, a.fault);
-                            mine += __longlong_as_double((long long)(((unsigned long long)hi << 32) | lo));
-                        }
+                        for (int j = tid; j < G; j += T) mine += ll_wait_f64(base + (size_t)j * kArSlotWords, tag, a.fault);
                         dA = block_sum(mine, sm.red);
                         ar_count += 1ull;
                     }
