@@ -277,7 +277,7 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     a.x = (R*)h->lay.x; a.g[0] = (R*)h->lay.g0; a.g[1] = (R*)h->lay.g1;
     a.y = (const R*)h->lay.y; a.I = h->have_I ? (const R*)h->lay.I : nullptr;
     a.p = (R*)h->lay.p; a.cur = h->lay.cur; a.lo = h->lay.lo; a.hi = h->lay.hi;
-    a.accum = h->accum; a.n_skip = h->n_skip; a.t_enable = h->t_enable;
+    a.accum = h->accum; a.n_skip = h->n_skip; a.t_enable = h->t_enable; a.skip0 = h->accum ? (h->t - h->t_enable) % h->n_skip : 0ull;
     a.cx = h->lay.cx; a.S1x = h->lay.S1x; a.S2x = h->lay.S2x; a.cp = h->lay.cp; a.S1p = h->lay.S1p; a.S2p = h->lay.S2p;
     a.counters = h->lay.counters;
     a.n_sel = h->n_sel; a.nbins = h->nbins;

@@ -45,6 +45,7 @@ template <typename R> struct SweepArgs {
     // statistics
     int accum;
     unsigned long long n_skip, t_enable;
+    unsigned long long skip0;    // (t0 - t_enable) mod n_skip: the tile engine counts from here instead of dividing every sweep
     double *cx, *S1x, *S2x;      // (C, M+1, D)
     double *cp, *S1p, *S2p;      // (C, Np)
     unsigned long long* counters;  // (C, 2, D+Np) accepted, proposed
@@ -170,7 +171,7 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
     R xn[D], xp[D], gp[D];
     load_vec<R, D>(x, n, xn);
     propose_state<R, D>(a, t, chain, (uint32_t)n, xn, xp);
-    R dA = R(0);
+    R dL = R(0), dR = R(0);     // left part (term n-1 -> n and measurement n) and right part (term n -> n+1), summed separately
     if (n >= 1) {
         R xm[D], gm[D];
         load_vec<R, D>(x, n - 1, xm);
@@ -179,14 +180,14 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
         for (int c = 0; c < D; ++c) {   // model-error term n-1 -> n
             const R r_new = (xp[c] - xm[c]) - gm[c];
             const R r_old = (xn[c] - xm[c]) - gm[c];
-            dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+            dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
         }
 #pragma unroll
         for (int l = 0; l < D; ++l) {    // measurement term n (the action sums n = 1..M); the first L components are observed
             if (l < a.L) {
                 const R yn = __ldg(y + (size_t)n * a.L + l);
                 const R d_new = yn - xp[l], d_old = yn - xn[l];
-                dA += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
+                dL += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
             }
         }
     }
@@ -200,9 +201,10 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
         for (int c = 0; c < D; ++c) {   // model-error term n -> n+1
             const R r_new = (xq[c] - xp[c]) - gp[c];
             const R r_old = (xq[c] - xn[c]) - gn[c];
-            dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+            dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
         }
     }
+    const R dA = dL + dR;
     const R logu = log_accept_uniform<R>(a, t, chain, (uint32_t)n);
     const bool accept = logu < -dA;      // NaN or +inf rejects; dA <= 0 always accepts
     if (accept) {

@@ -73,59 +73,80 @@ __device__ __forceinline__ void bar_compute(int n_threads) {     // named barrie
     asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory");
 }
 
+// Shared-memory layout.  Every per-site array (x, both caches, moment sums) is stored as parity planes in
+// structure-of-arrays form: element (local site i, component c) lives at ((i & 1) * D + c) * P + (i >> 1), P = the
+// plane pitch.  Compute thread j owns local sites 2j and 2j+1, so all its accesses (own site, left and right
+// neighbour) are unit-stride across the warp: no bank conflicts (the site-major layout of v3 had 8-way conflicts
+// on every 8-byte access, profiles/r01_v3_tile_engine.md).
 template <typename R> struct TileSmem {
-    double *S1, *S2, *cc;       // [E*D] running moments of the tile (fp64 always)
+    double *S1, *S2, *cc;       // [2*D*P] running moments of the tile (fp64 always)
     double* red;                // [32]
     double* pdraw;              // [2 sets][kMaxNp][2] = (step, log u) of the parameter moves
     double *blo, *bhi;          // [kMaxNp] bounds
-    R *xs, *g0, *g1;            // [(E+1)*D]
+    double *pS1, *pS2, *pcc;    // [kMaxNp] running moments of the parameters (tile 0 of each chain)
+    R *xs, *g0, *g1;            // [2*D*P]
     R *Is, *ys;                 // [E+2], [E*L]
-    R *rstep, *rlogu;           // [2 sets][2 parities][TC][D], [2][2][TC]
+    R *rstep, *rlogu;           // [2 sets][2 parities][D][TC], [2][2][TC]
     unsigned int* cnt;          // [2]: accepted owned state updates (lo, unused)
+    int P;
 };
 
+// the pitch is a compile-time constant of the kernel instantiation (MAXT = 256 or 512), so plane offsets are immediates
+__host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512) / 2 + 2; }
+
 template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L) {
-    const size_t E = (size_t)T, TC = (size_t)T / 2;
-    size_t dbl = 3 * E * D + 32 + 2 * kMaxNp * 2 + 2 * kMaxNp + 2;
-    size_t real = 3 * (E + 1) * D + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * TC * D + 4 * TC;
+    const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
+    size_t dbl = 3 * 2 * D * P + 32 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
+    const size_t RP = P - 2;
+    size_t real = 3 * 2 * D * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
+    (void)TC;
     return dbl * 8 + ((real * sizeof(R) + 15) & ~(size_t)15) + 16;
 }
 
 template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L) {
-    const size_t E = (size_t)T, TC = (size_t)T / 2;
+    const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     TileSmem<R> m;
+    m.P = (int)P;
     double* d = reinterpret_cast<double*>(base);
-    m.S1 = d; d += E * D;
-    m.S2 = d; d += E * D;
-    m.cc = d; d += E * D;
+    m.S1 = d; d += 2 * D * P;
+    m.S2 = d; d += 2 * D * P;
+    m.cc = d; d += 2 * D * P;
     m.red = d; d += 32;
     m.pdraw = d; d += 2 * kMaxNp * 2;
     m.blo = d; d += kMaxNp;
     m.bhi = d; d += kMaxNp;
+    m.pS1 = d; d += kMaxNp;
+    m.pS2 = d; d += kMaxNp;
+    m.pcc = d; d += kMaxNp;
     m.cnt = reinterpret_cast<unsigned int*>(d); d += 2;
     R* r = reinterpret_cast<R*>(d);
-    m.xs = r; r += (E + 1) * D;
-    m.g0 = r; r += (E + 1) * D;
-    m.g1 = r; r += (E + 1) * D;
+    m.xs = r; r += 2 * D * P;
+    m.g0 = r; r += 2 * D * P;
+    m.g1 = r; r += 2 * D * P;
     m.Is = r; r += E + 2;
     m.ys = r; r += E * (size_t)(L > 0 ? L : 1);
-    m.rstep = r; r += 4 * TC * D;
-    m.rlogu = r; r += 4 * TC;
+    m.rstep = r; r += 4 * (P - 2) * D;
+    m.rlogu = r; r += 4 * (P - 2);
+    (void)TC;
     return m;
 }
 
-template <typename R, int D> __device__ __forceinline__ void lds_vec(const R* base, int row, R out[D]) {
+// offset of (local site i, component c) in a parity-plane array
+template <int D> __device__ __forceinline__ int so(int i, int c, int P) { return ((i & 1) * D + c) * P + (i >> 1); }
+
+// all D components of the site at plane `q`, pair index `j`
+template <typename R, int D> __device__ __forceinline__ void lds_site(const R* base, int q, int j, int P, R out[D]) {
 #pragma unroll
-    for (int c = 0; c < D; ++c) out[c] = base[row * D + c];
+    for (int c = 0; c < D; ++c) out[c] = base[(q * D + c) * P + j];
 }
-template <typename R, int D> __device__ __forceinline__ void sts_vec(R* base, int row, const R v[D]) {
+template <typename R, int D> __device__ __forceinline__ void sts_site(R* base, int q, int j, int P, const R v[D]) {
 #pragma unroll
-    for (int c = 0; c < D; ++c) base[row * D + c] = v[c];
+    for (int c = 0; c < D; ++c) base[(q * D + c) * P + j] = v[c];
 }
 
 // ---- producer: proposal steps w_a z_a and log u for one site of one half-sweep (row A1) ----------------------
 template <typename R, int D>
-__device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n, R* step_out, R* logu_out) {
+__device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n, R* step_out, int stride, R* logu_out) {
     const Words4 w = draw(a.seed, t, chain, n, kStreamStateProposal, 0);
     R st[4] = {R(0), R(0), R(0), R(0)};
     if (a.kind == 1) {
@@ -150,9 +171,10 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
         }
     }
 #pragma unroll
-    for (int c = 0; c < D; ++c) step_out[c] = st[c];
+    for (int c = 0; c < D; ++c) step_out[c * stride] = st[c];
     *logu_out = log_accept_uniform<R>(a, t, chain, n);
 }
+
 
 // ---- the kernel ----------------------------------------------------------------------------------------------
 template <class Model, typename R, int MAXT>
@@ -162,12 +184,14 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     extern __shared__ __align__(16) unsigned char tile_smem_raw[];
     const int T = blockDim.x, TC = T >> 1, tid = threadIdx.x;
     const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L);
+    constexpr int RP = MAXT / 2;                   // pitch of the random-number ring
+    constexpr int P = MAXT / 2 + 2;                // == tile_pitch(T): the launcher picks MAXT = 256 for T <= 256, else 512
 
     const int G = a.G, M = a.M, L = a.L, h = a.h;
     const uint32_t chain = blockIdx.x / G;
     const int b = blockIdx.x % G;
     const int s = b * a.tile, e = min(s + a.tile, M + 1);
-    const int s_ext = max(0, s - h), e_ext = min(M + 1, e + h), n_ext = e_ext - s_ext;
+    const int s_ext = max(0, s - h), e_ext = min(M + 1, e + h), n_ext = e_ext - s_ext;   // s_ext is even (tile and h are)
     const size_t site0 = (size_t)chain * (M + 1);
     const bool edge_lo = s_ext == 0, edge_hi = e_ext == M + 1;
 
@@ -176,13 +200,13 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     R* const gg1 = a.g[1] + (size_t)chain * M * D;
     int cur = a.cur[chain];
 
-    // ---- load the extended tile ----
-    for (int idx = tid; idx < n_ext * D; idx += T) sm.xs[idx] = gx[(size_t)s_ext * D + idx];
+    // ---- load the extended tile (site-major in global memory -> parity planes in shared memory) ----
+    for (int idx = tid; idx < n_ext * D; idx += T) sm.xs[so<D>(idx / D, idx % D, P)] = gx[(size_t)s_ext * D + idx];
     {
         const R* gsrc = cur ? gg1 : gg0;
         R* gdst = cur ? sm.g1 : sm.g0;
         const int ng = min(e_ext, M) - s_ext;      // cache entries exist for n <= M-1
-        for (int idx = tid; idx < ng * D; idx += T) gdst[idx] = gsrc[(size_t)s_ext * D + idx];
+        for (int idx = tid; idx < ng * D; idx += T) gdst[so<D>(idx / D, idx % D, P)] = gsrc[(size_t)s_ext * D + idx];
     }
     for (int i = tid; i <= n_ext; i += T) {
         const int n = s_ext + i;
@@ -192,7 +216,12 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     if (a.accum) {
         for (int idx = tid; idx < n_ext * D; idx += T) {
             const size_t gi = (site0 + s_ext) * D + idx;
-            sm.S1[idx] = a.S1x[gi]; sm.S2[idx] = a.S2x[gi]; sm.cc[idx] = a.cx[gi];
+            const int o = so<D>(idx / D, idx % D, P);
+            sm.S1[o] = a.S1x[gi]; sm.S2[o] = a.S2x[gi]; sm.cc[o] = a.cx[gi];
+        }
+        if (tid < NP) {
+            const size_t gi = (size_t)chain * NP + tid;
+            sm.pS1[tid] = a.S1p[gi]; sm.pS2[tid] = a.S2p[gi]; sm.pcc[tid] = a.cp[gi];
         }
     }
     if (tid < NP) { sm.blo[tid] = a.lo[(size_t)chain * NP + tid]; sm.bhi[tid] = a.hi[(size_t)chain * NP + tid]; }
@@ -203,6 +232,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
 
     unsigned long long ar_count = a.ar_epoch[chain];
     unsigned long long hx_count = a.hx_epoch[chain];
+    unsigned long long skip_ctr = a.skip0;         // (t - t_enable) mod n_skip, kept as a counter (no 64-bit division in the loop)
     unsigned int n_acc_state = 0, pacc[NP], pprop[NP];
 #pragma unroll
     for (int k = 0; k < NP; ++k) { pacc[k] = 0; pprop[k] = 0; }
@@ -215,8 +245,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             for (int parity = 0; parity < 2; ++parity) {
                 const int n = s_ext + 2 * j + parity;
                 if (n <= M && 2 * j + parity < n_ext)
-                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.rstep + ((size_t)(set * 2 + parity) * TC + j) * D,
-                                       sm.rlogu + (size_t)(set * 2 + parity) * TC + j);
+                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.rstep + (size_t)(set * 2 + parity) * D * RP + j, RP,
+                                       sm.rlogu + (size_t)(set * 2 + parity) * RP + j);
             }
         }
         if (a.do_params && j < NP && a.wp[j] > 0.0) {
@@ -231,77 +261,91 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     if (tid >= TC) produce(0, a.t0);
     __syncthreads();
 
+    // compute thread `tid` owns the local site pair (2 tid, 2 tid + 1); thread r of a parameter move evaluates local
+    // site prm_site: the even sites on threads [0, TC), the odd sites on [TC, T) (unit-stride plane accesses)
+    const int prm_q = tid >= TC ? 1 : 0, prm_j = tid - prm_q * TC, prm_iloc = 2 * prm_j + prm_q;
+
     int k_phase = 0;                               // half-sweeps since the halos were last exact
     for (long long i = 0; i < a.n_sweeps; ++i) {
         const unsigned long long t = a.t0 + (unsigned long long)i;
         const int set = (int)(i & 1);
         const bool trace = (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
+        const bool acc_now = a.accum && skip_ctr == 0ull;
+        skip_ctr = (skip_ctr + 1ull == a.n_skip) ? 0ull : skip_ctr + 1ull;
 
         if (tid < TC) {
             // ---------------- A2: even half-sweep, then odd half-sweep (compute warps) ----------------
             if (a.do_states) {
 #pragma unroll 1
-                for (int parity = 0; parity < 2; ++parity) {
-                    const int k = k_phase + parity + 1;      // half-sweeps run on the current halos, this one included
-                    const int iloc = 2 * tid + parity, n = s_ext + iloc;
+                for (int q = 0; q < 2; ++q) {
+                    const int k = k_phase + q + 1;           // half-sweeps run on the current halos, this one included
+                    const int iloc = 2 * tid + q, n = s_ext + iloc;
                     const bool ok = n <= M && iloc < n_ext && (edge_lo || iloc >= k) && (edge_hi || iloc < n_ext - k);
                     if (ok) {
+                        // One straight-line block: every load is issued up front, the model step runs on the proposal,
+                        // and the neighbour values, moment sums and log u are consumed after it (off the critical path).
+                        // Edge sites (n = 0: no left term and no measurement; n = M: no right term) are handled by selects.
                         R* gc = cur ? sm.g1 : sm.g0;
-                        R xn[D], xp[D], gp[D];
-                        lds_vec<R, D>(sm.xs, iloc, xn);
-                        const R* st = sm.rstep + ((size_t)(set * 2 + parity) * TC + tid) * D;
+                        const bool has_l = n >= 1, has_r = n <= M - 1;
+                        const int jl = max(tid - 1 + q, 0), jr = tid + q;   // pair index of the left / right neighbour (plane 1 - q)
+                        const int own = q * D * P + tid, oth = (1 - q) * D * P;
+                        const R* ring = sm.rstep + (size_t)(set * 2 + q) * D * RP + tid;
+                        R xn[D], xp[D], gp[D], xm[D], gm[D], xq[D], gn[D];
+                        double mc[D], m1[D], m2[D];
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
-                            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], st[c]);
-                            else xp[c] = __fadd_rn(xn[c], st[c]);
+                            xn[c] = sm.xs[own + c * P];
+                            const R st = ring[c * RP];
+                            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], st);
+                            else xp[c] = __fadd_rn(xn[c], st);
                         }
-                        R dA = R(0);
-                        if (n >= 1) {
-                            R xm[D], gm[D];
-                            lds_vec<R, D>(sm.xs, iloc - 1, xm);
-                            lds_vec<R, D>(gc, iloc - 1, gm);
+                        const R I0 = sm.Is[iloc], I1 = sm.Is[iloc + 1];
 #pragma unroll
-                            for (int c = 0; c < D; ++c) {
-                                const R r_new = (xp[c] - xm[c]) - gm[c];
-                                const R r_old = (xn[c] - xm[c]) - gm[c];
-                                dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
-                            }
-#pragma unroll
-                            for (int l = 0; l < D; ++l) {
-                                if (l < L) {
-                                    const R yn = sm.ys[iloc * L + l];
-                                    const R d_new = yn - xp[l], d_old = yn - xn[l];
-                                    dA += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
-                                }
-                            }
+                        for (int c = 0; c < D; ++c) {
+                            xm[c] = sm.xs[oth + c * P + jl]; gm[c] = gc[oth + c * P + jl];
+                            xq[c] = sm.xs[oth + c * P + jr]; gn[c] = gc[own + c * P];
+                            mc[c] = sm.cc[own + c * P]; m1[c] = sm.S1[own + c * P]; m2[c] = sm.S2[own + c * P];
                         }
-                        if (n <= M - 1) {
-                            R xq[D], gn[D];
-                            lds_vec<R, D>(sm.xs, iloc + 1, xq);
-                            lds_vec<R, D>(gc, iloc, gn);
-                            Model::increment(xp, prm, sm.Is[iloc], sm.Is[iloc + 1], a.dt, gp);
+                        const R logu = sm.rlogu[(size_t)(set * 2 + q) * RP + tid];
+                        Model::increment(xp, prm, I0, I1, a.dt, gp);
+                        R dL = R(0), dR = R(0);
 #pragma unroll
-                            for (int c = 0; c < D; ++c) {
-                                const R r_new = (xq[c] - xp[c]) - gp[c];
-                                const R r_old = (xq[c] - xn[c]) - gn[c];
-                                dA += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                        for (int c = 0; c < D; ++c) {
+                            const R r_new = (xp[c] - xm[c]) - gm[c];
+                            const R r_old = (xn[c] - xm[c]) - gm[c];
+                            dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                        }
+#pragma unroll
+                        for (int l = 0; l < D; ++l) {
+                            if (l < L) {
+                                const R yn = sm.ys[iloc * L + l];
+                                const R d_new = yn - xp[l], d_old = yn - xn[l];
+                                dL += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
                             }
                         }
-                        const R logu = sm.rlogu[(size_t)(set * 2 + parity) * TC + tid];
+#pragma unroll
+                        for (int c = 0; c < D; ++c) {
+                            const R r_new = (xq[c] - xp[c]) - gp[c];
+                            const R r_old = (xq[c] - xn[c]) - gn[c];
+                            dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                        }
+                        const R dA = (has_l ? dL : R(0)) + (has_r ? dR : R(0));
                         const bool accept = logu < -dA;
-                        if (accept) {
-                            sts_vec<R, D>(sm.xs, iloc, xp);
-                            if (n <= M - 1) sts_vec<R, D>(gc, iloc, gp);
+#pragma unroll
+                        for (int c = 0; c < D; ++c) {
+                            if (accept) sm.xs[own + c * P] = xp[c];
+                            if (accept && has_r) gc[own + c * P] = gp[c];
+                            // A5 for this site: its value is final for sweep t (parameter moves do not touch x)
+                            const double d = (double)(accept ? xp[c] : xn[c]) - mc[c];
+                            if (acc_now) { sm.S1[own + c * P] = m1[c] + d; sm.S2[own + c * P] = m2[c] + d * d; }
                         }
                         const bool owned = n >= s && n < e;
-                        if (owned) {
-                            n_acc_state += accept ? 1u : 0u;
-                            if (trace) {
-                                const size_t gs = site0 + (size_t)n;
-                                if (a.tr_dA) a.tr_dA[gs] = dA;
-                                if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
-                                if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
-                            }
+                        n_acc_state += (owned && accept) ? 1u : 0u;
+                        if (trace && owned) {
+                            const size_t gs = site0 + (size_t)n;
+                            if (a.tr_dA) a.tr_dA[gs] = dA;
+                            if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
+                            if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
                         }
                     }
                     bar_compute(TC);
@@ -316,8 +360,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
 
         // ---------------- A4: parameter moves, in sequence; one tile site per thread ----------------
         if (a.do_params) {
-            const int r = tid, n = s_ext + r;
-            const bool can_eval = r < n_ext && n <= M - 1;
+            const int n = s_ext + prm_iloc;
+            const bool can_eval = prm_iloc < n_ext && n <= M - 1;
             const bool owned = n >= s && n < e && n <= M - 1;
 #pragma unroll 1
             for (int l = 0; l < NP; ++l) {
@@ -341,13 +385,13 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     double part = 0.0;
                     if (can_eval) {
                         R xn[D], gp[D];
-                        lds_vec<R, D>(sm.xs, r, xn);
-                        Model::increment(xn, pp, sm.Is[r], sm.Is[r + 1], a.dt, gp);
-                        sts_vec<R, D>(ga, r, gp);
+                        lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
+                        Model::increment(xn, pp, sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp);
+                        sts_site<R, D>(ga, prm_q, prm_j, P, gp);
                         if (owned) {
                             R xq[D], gn[D];
-                            lds_vec<R, D>(sm.xs, r + 1, xq);
-                            lds_vec<R, D>(gc, r, gn);
+                            lds_site<R, D>(sm.xs, 1 - prm_q, prm_j + prm_q, P, xq);
+                            lds_site<R, D>(gc, prm_q, prm_j, P, gn);
                             R acc = R(0);
 #pragma unroll
                             for (int c = 0; c < D; ++c) {
@@ -413,10 +457,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 const int o = q / (2 * D * WPV), rem = q % (2 * D * WPV);
                 const int which = rem / (D * WPV), cw = rem % (D * WPV);
                 const int nsite = dir == 0 ? s + o : e - h + o;
-                const int iloc = nsite - s_ext;
+                const int widx = so<D>(nsite - s_ext, cw / WPV, P) * WPV + cw % WPV;
                 uint32_t payload = 0;
-                if (which == 0) payload = xs32[iloc * D * WPV + cw];
-                else if (nsite <= M - 1) payload = gc32[iloc * D * WPV + cw];
+                if (which == 0) payload = xs32[widx];
+                else if (nsite <= M - 1) payload = gc32[widx];
                 const int dst_cta = (int)blockIdx.x + (dir == 0 ? -1 : 1);
                 const int dst_side = dir == 0 ? 1 : 0;           // my left neighbour receives "from its right"
                 unsigned long long* box = a.hx_words + (((size_t)dst_cta * 2 + dst_side) * 2 + slot) * (size_t)kHaloWordsPerSide;
@@ -431,11 +475,11 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 const int o = q / (2 * D * WPV), rem = q % (2 * D * WPV);
                 const int which = rem / (D * WPV), cw = rem % (D * WPV);
                 const int nsite = side == 0 ? s - h + o : e + o;
-                const int iloc = nsite - s_ext;
+                const int widx = so<D>(nsite - s_ext, cw / WPV, P) * WPV + cw % WPV;
                 const unsigned long long* box = a.hx_words + (((size_t)blockIdx.x * 2 + side) * 2 + slot) * (size_t)kHaloWordsPerSide;
                 const uint32_t payload = ll_wait(box + q, tag, a.fault);
-                if (which == 0) xd32[iloc * D * WPV + cw] = payload;
-                else if (nsite <= M - 1) gd32[iloc * D * WPV + cw] = payload;
+                if (which == 0) xd32[widx] = payload;
+                else if (nsite <= M - 1) gd32[widx] = payload;
             }
             hx_count += 1ull;
             k_phase = 0;
@@ -443,59 +487,70 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         }
 
         // ---------------- A5: running moments and histograms (owned sites) ----------------
-        if (a.accum && ((t - a.t_enable) % a.n_skip) == 0ull) {
-            for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) {
-                const double d = (double)sm.xs[idx] - sm.cc[idx];
-                sm.S1[idx] += d;
-                sm.S2[idx] += d * d;
+        // the state moments of a sweep with state updates were accumulated by the compute threads above
+        if (acc_now) {
+            if (!a.do_states) {
+                for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) {
+                    const int o = so<D>(idx / D, idx % D, P);
+                    const double d = (double)sm.xs[o] - sm.cc[o];
+                    sm.S1[o] += d;
+                    sm.S2[o] += d * d;
+                }
             }
-            if (b == 0 && tid < NP) {
-                const size_t gi = (size_t)chain * NP + tid;
+            if (tid < NP) {
                 double pv = 0.0;
 #pragma unroll
                 for (int k = 0; k < NP; ++k) pv = (k == tid) ? (double)prm[k] : pv;
-                const double d = pv - a.cp[gi];
-                a.S1p[gi] += d;
-                a.S2p[gi] += d * d;
+                const double d = pv - sm.pcc[tid];
+                sm.pS1[tid] += d;
+                sm.pS2[tid] += d * d;
             }
-            for (int sel = tid; sel < a.n_sel; sel += T) {
-                const int site = a.hsite[sel], comp = a.hcomp[sel];
-                const bool mine = site < 0 ? (b == 0) : (site >= s && site < e);
-                if (mine) {
-                    double v = 0.0;
-                    if (site < 0) {
+            if (a.n_sel > 0) {
+                for (int sel = tid; sel < a.n_sel; sel += T) {
+                    const int site = a.hsite[sel], comp = a.hcomp[sel];
+                    const bool mine = site < 0 ? (b == 0) : (site >= s && site < e);
+                    if (mine) {
+                        double v = 0.0;
+                        if (site < 0) {
 #pragma unroll
-                        for (int k = 0; k < NP; ++k) v = (k == comp) ? (double)prm[k] : v;
-                    } else v = (double)sm.xs[(site - s_ext) * D + comp];
-                    unsigned long long* bins = a.hist + ((size_t)chain * a.n_sel + sel) * (size_t)(a.nbins + 2);
-                    const double lo = a.hlo[sel], hi = a.hhi[sel];
-                    int bin;
-                    if (!(v >= lo)) bin = 0;
-                    else if (v >= hi) bin = a.nbins + 1;
-                    else {
-                        long long q = (long long)floor((v - lo) / a.hwidth[sel]);
-                        if (q >= a.nbins) q = a.nbins - 1;
-                        bin = 1 + (int)q;
+                            for (int k = 0; k < NP; ++k) v = (k == comp) ? (double)prm[k] : v;
+                        } else v = (double)sm.xs[so<D>(site - s_ext, comp, P)];
+                        unsigned long long* bins = a.hist + ((size_t)chain * a.n_sel + sel) * (size_t)(a.nbins + 2);
+                        const double lo = a.hlo[sel], hi = a.hhi[sel];
+                        int bin;
+                        if (!(v >= lo)) bin = 0;
+                        else if (v >= hi) bin = a.nbins + 1;
+                        else {
+                            long long q = (long long)floor((v - lo) / a.hwidth[sel]);
+                            if (q >= a.nbins) q = a.nbins - 1;
+                            bin = 1 + (int)q;
+                        }
+                        bins[bin] += 1ull;
                     }
-                    bins[bin] += 1ull;
                 }
+                __syncthreads();   // the next half-sweep overwrites x
             }
-            __syncthreads();
         }
     }
 
     // ---------------- write the tile back; A6 counters ----------------
-    for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) gx[(size_t)s_ext * D + idx] = sm.xs[idx];
+    __syncthreads();
+    for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) gx[(size_t)s_ext * D + idx] = sm.xs[so<D>(idx / D, idx % D, P)];
     {
         R* gdst = cur ? gg1 : gg0;
         const R* gsrc = cur ? sm.g1 : sm.g0;
         const int hi_g = min(e, M);
-        for (int idx = (s - s_ext) * D + tid; idx < (hi_g - s_ext) * D; idx += T) gdst[(size_t)s_ext * D + idx] = gsrc[idx];
+        for (int idx = (s - s_ext) * D + tid; idx < (hi_g - s_ext) * D; idx += T) gdst[(size_t)s_ext * D + idx] = gsrc[so<D>(idx / D, idx % D, P)];
     }
     if (a.accum) {
         for (int idx = (s - s_ext) * D + tid; idx < (e - s_ext) * D; idx += T) {
             const size_t gi = (site0 + s_ext) * D + idx;
-            a.S1x[gi] = sm.S1[idx]; a.S2x[gi] = sm.S2[idx];
+            const int o = so<D>(idx / D, idx % D, P);
+            a.S1x[gi] = sm.S1[o]; a.S2x[gi] = sm.S2[o];
+        }
+        if (b == 0 && tid < NP) {
+            const size_t gi = (size_t)chain * NP + tid;
+            a.S1p[gi] = sm.pS1[tid]; a.S2p[gi] = sm.pS2[tid];
         }
     }
     if (n_acc_state) atomicAdd(sm.cnt, n_acc_state);
