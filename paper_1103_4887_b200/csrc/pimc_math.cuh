@@ -45,7 +45,24 @@ __device__ __forceinline__ double div_fast(double n, double d) {
     return fma(r, y, q);
 }
 
-// exp(x) for |x| <= 700: x = k ln2 + r, |r| <= ln2/2; e^r = 1 + r + r^2 P(r); scale by 2^k through the exponent field.
+// e^r - 1 for |r| <= ~0.36: r + r^2 P(r), P of degree 9 evaluated by Estrin's scheme (dependent depth 5 instead of 11).
+__device__ __forceinline__ double expm1_small(double r) {
+    const double r2 = r * r;
+    const double a0 = fma(kExpP[1], r, kExpP[0]);
+    const double a1 = fma(kExpP[3], r, kExpP[2]);
+    const double a2 = fma(kExpP[5], r, kExpP[4]);
+    const double a3 = fma(kExpP[7], r, kExpP[6]);
+    const double a4 = fma(kExpP[9], r, kExpP[8]);
+    const double r4 = r2 * r2;
+    const double b0 = fma(a1, r2, a0);
+    const double b1 = fma(a3, r2, a2);
+    const double r8 = r4 * r4;
+    const double c0 = fma(b1, r4, b0);
+    const double p = fma(a4, r8, c0);
+    return fma(p, r2, r);
+}
+
+// exp(x) for |x| <= 700: x = k ln2 + r, |r| <= ln2/2; scale by 2^k through the exponent field.
 __device__ __forceinline__ double exp_fast(double x) {
     constexpr double kMagic = 6755399441055744.0;                 // 1.5 * 2^52: adds round-to-nearest-integer
     constexpr double kLog2e = 1.4426950408889634074;
@@ -55,12 +72,42 @@ __device__ __forceinline__ double exp_fast(double x) {
     const double kd = t - kMagic;
     double r = fma(kd, -kLn2Hi, x);
     r = fma(kd, -kLn2Lo, r);
-    double p = kExpP[9];
-#pragma unroll
-    for (int i = 8; i >= 0; --i) p = fma(p, r, kExpP[i]);
-    const double e = fma(p, r * r, r);                             // e^r - 1
+    const double e = expm1_small(r);                               // e^r - 1
     const double s = __hiloint2double((k + 1023) << 20, 0);        // 2^k
     return fma(e, s, s);
+}
+
+// exp(c1 V + c0) for any finite V with the result SATURATED to [2^-300, 2^301): used where only e/(1+e)-type
+// ratios of the result matter (the Hodgkin-Huxley gates), which are exact to rounding long before saturation.
+// The clamp is integer arithmetic on k, off the floating-point dependency chain.  Requires |c1 V + c0| < 2^31 ln 2
+// (the caller guards).
+__device__ __forceinline__ double exp_affine_sat(double V, double c1, double c0) {
+    constexpr double kMagic = 6755399441055744.0;
+    constexpr double kLog2e = 1.4426950408889634074;
+    constexpr double kLn2Hi = 0x1.62e42fefa39efp-1, kLn2Lo = 0x1.abc9e3b39803fp-56;
+    const double x = fma(V, c1, c0);
+    const double t = fma(x, kLog2e, kMagic);
+    int k = __double2loint(t);
+    const double kd = t - kMagic;
+    double r = fma(kd, -kLn2Hi, x);
+    r = fma(kd, -kLn2Lo, r);
+    const double e = expm1_small(r);
+    k = min(max(k, -300), 300);
+    const double s = __hiloint2double((k + 1023) << 20, 0);
+    return fma(e, s, s);
+}
+
+// num / den for normal den: MUFU seed y0 (measured relative error ~2^-13), then
+// num y0 (1 + e + e^2 + e^3 + e^4) with e = 1 - den y0 (relative error e^5 < 2^-64): four dependent FP64 operations
+// after the seed, and the numerator rides along for free.
+__device__ __forceinline__ double div_series(double num, double den) {
+    const double y0 = rcp_seed(den);
+    const double e = fma(-den, y0, 1.0);
+    const double t = num * y0;
+    const double p = fma(e, e, e);
+    const double e2 = e * e;
+    const double S = fma(p, e2, p);
+    return fma(t, S, t);
 }
 
 // log(u) for normal positive u (here u in (0,1)): u = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh((m-1)/(m+1)).

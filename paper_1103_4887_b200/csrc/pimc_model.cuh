@@ -27,17 +27,16 @@ template <typename R> struct HHModel {
         return (ainf - a) / tau;
     }
     // Double precision: one exponential and one reciprocal per gate.  With e = exp(2 s), q = e + 1:
-    //   tanh s = (e-1)/q, a_inf = e/q, 1 - tanh^2 s = 4 e / q^2  =>  (a_inf - a)/tau = (e - a q) q / (tau0 q^2 + 4 tau1 e).
-    // |2 s| is clamped at 80, where tanh s = +-1 to 1e-35 (far below half an ulp), so nothing overflows.
+    //   tanh s = (e-1)/q, a_inf = e/q, 1 - tanh^2 s = 4 e / q^2  =>  (a_inf - a)/tau = (e - a q) q / (tau0 q^2 + 4 tau1 e),
+    //   and tau0 q^2 + 4 tau1 e = tau0 + e (2 tau0 + 4 tau1 + tau0 e) (two FMAs straight from e).
+    // e saturates at 2^+-300 (exp_affine_sat), where tanh s = +-1 far below half an ulp, so nothing overflows.
     static __device__ __forceinline__ double gate_fast(double V, double a, double Va, double dVa, double tau0, double tau1) {
         const double c1 = 2.0 / dVa, c0 = -2.0 * Va / dVa;
-        double s2 = fma(V, c1, c0);
-        s2 = fmin(fmax(s2, -80.0), 80.0);
-        const double e = exp_fast(s2);
+        const double e = exp_affine_sat(V, c1, c0);
         const double q = e + 1.0;
+        const double den = fma(e, fma(e, tau0, 2.0 * tau0 + 4.0 * tau1), tau0);
         const double num = fma(-a, q, e) * q;
-        const double den = fma(tau0 * q, q, (4.0 * tau1) * e);
-        return num * rcp_fast(den);
+        return div_series(num, den);
     }
     static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R inv_C, R I, R F[4]) {
         const R V = x[0], m = x[1], h = x[2], n = x[3];
@@ -55,25 +54,44 @@ template <typename R> struct HHModel {
             F[3] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
         }
     }
-    static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
+    // Quantities that depend only on (p, dt): computed once per parameter vector, not once per site.
+    struct Prep { R inv_C, hdt, dt6; };
+    static __device__ __forceinline__ Prep prepare(const R* __restrict__ p, R dt) {
+        Prep q;
+        q.inv_C = R(0);
+        if constexpr (sizeof(R) == 8) q.inv_C = div_fast(1.0, p[6]);
+        q.hdt = R(0.5) * dt;
+        q.dt6 = dt / R(6);
+        return q;
+    }
+    // Domain guard of the double-precision gates: a stage voltage beyond +-1e8 mV (or NaN) makes the whole increment
+    // NaN, i.e. the proposal is rejected; inside the guard the gates saturate exactly like tanh.
+    static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, const Prep& q, R I0, R I1, R dt, R g[4]) {
         const R Ih = R(0.5) * (I0 + I1);
-        const R hdt = R(0.5) * dt;
-        R inv_C = R(0);
-        if constexpr (sizeof(R) == 8) inv_C = div_fast(1.0, p[6]);
         R k[4], xs[4], acc[4];
-        rhs(x, p, inv_C, I0, k);
+        bool sane = true;
+        rhs(x, p, q.inv_C, I0, k);
+        if constexpr (sizeof(R) == 8) sane = sane && fabs(x[0]) < 1e8;
 #pragma unroll
-        for (int a = 0; a < 4; ++a) { acc[a] = k[a]; xs[a] = x[a] + hdt * k[a]; }
-        rhs(xs, p, inv_C, Ih, k);
+        for (int a = 0; a < 4; ++a) { acc[a] = k[a]; xs[a] = x[a] + q.hdt * k[a]; }
+        rhs(xs, p, q.inv_C, Ih, k);
+        if constexpr (sizeof(R) == 8) sane = sane && fabs(xs[0]) < 1e8;
 #pragma unroll
-        for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + hdt * k[a]; }
-        rhs(xs, p, inv_C, Ih, k);
+        for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + q.hdt * k[a]; }
+        rhs(xs, p, q.inv_C, Ih, k);
+        if constexpr (sizeof(R) == 8) sane = sane && fabs(xs[0]) < 1e8;
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + dt * k[a]; }
-        rhs(xs, p, inv_C, I1, k);
-        const R dt6 = dt / R(6);
+        rhs(xs, p, q.inv_C, I1, k);
+        if constexpr (sizeof(R) == 8) sane = sane && fabs(xs[0]) < 1e8;
 #pragma unroll
-        for (int a = 0; a < 4; ++a) g[a] = dt6 * (acc[a] + k[a]);
+        for (int a = 0; a < 4; ++a) {
+            g[a] = q.dt6 * (acc[a] + k[a]);
+            if constexpr (sizeof(R) == 8) g[a] = sane ? g[a] : __longlong_as_double(0x7FF8000000000000ll);
+        }
+    }
+    static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
+        increment(x, p, prepare(p, dt), I0, I1, dt, g);
     }
 };
 
@@ -81,6 +99,11 @@ template <typename R> struct HHModel {
 template <typename R, int D_> struct LinearModel {
     static constexpr int D = D_;
     static constexpr int NP = D_ * D_;
+    struct Prep {};
+    static __device__ __forceinline__ Prep prepare(const R* __restrict__, R) { return Prep{}; }
+    static __device__ __forceinline__ void increment(const R x[D_], const R* __restrict__ p, const Prep&, R I0, R I1, R dt, R g[D_]) {
+        increment(x, p, I0, I1, dt, g);
+    }
     static __device__ __forceinline__ void increment(const R x[D_], const R* __restrict__ p, R, R, R, R g[D_]) {
 #pragma unroll
         for (int a = 0; a < D_; ++a) {

@@ -276,6 +276,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         if (tid < TC) {
             // ---------------- A2: even half-sweep, then odd half-sweep (compute warps) ----------------
             if (a.do_states) {
+                const typename Model::Prep prep = Model::prepare(prm, a.dt);
 #pragma unroll 1
                 for (int q = 0; q < 2; ++q) {
                     const int k = k_phase + q + 1;           // half-sweeps run on the current halos, this one included
@@ -307,7 +308,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             mc[c] = sm.cc[own + c * P]; m1[c] = sm.S1[own + c * P]; m2[c] = sm.S2[own + c * P];
                         }
                         const R logu = sm.rlogu[(size_t)(set * 2 + q) * RP + tid];
-                        Model::increment(xp, prm, I0, I1, a.dt, gp);
+                        Model::increment(xp, prm, prep, I0, I1, a.dt, gp);
                         R dL = R(0), dR = R(0);
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
