@@ -73,6 +73,21 @@ __device__ __forceinline__ void bar_compute(int n_threads) {     // named barrie
     asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory");
 }
 
+// Deterministic block sum with ONE barrier: the warp partials go to one of two alternating buffers, so the buffer of
+// call k is only rewritten by call k+2, after every thread has passed the barrier of call k+1.
+__device__ __forceinline__ double block_sum_db(double v, double* red /* 64 doubles */, unsigned& phase) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+    double* buf = red + (phase & 1u) * 32;
+    phase ^= 1u;
+    const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    if ((threadIdx.x & 31) == 0) buf[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+    for (int w = 0; w < nwarps; ++w) tot += buf[w];
+    return tot;
+}
+
 // Shared-memory layout.  Every per-site array (x, both caches, moment sums) is stored as parity planes in
 // structure-of-arrays form: element (local site i, component c) lives at ((i & 1) * D + c) * P + (i >> 1), P = the
 // plane pitch.  Compute thread j owns local sites 2j and 2j+1, so all its accesses (own site, left and right
@@ -80,7 +95,7 @@ __device__ __forceinline__ void bar_compute(int n_threads) {     // named barrie
 // on every 8-byte access, profiles/r01_v3_tile_engine.md).
 template <typename R> struct TileSmem {
     double *S1, *S2, *cc;       // [2*D*P] running moments of the tile (fp64 always)
-    double* red;                // [32]
+    double* red;                // [2][32]
     double* pdraw;              // [2 sets][kMaxNp][2] = (step, log u) of the parameter moves
     double *blo, *bhi;          // [kMaxNp] bounds
     double *pS1, *pS2, *pcc;    // [kMaxNp] running moments of the parameters (tile 0 of each chain)
@@ -96,7 +111,7 @@ __host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512)
 
 template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
-    size_t dbl = 3 * 2 * D * P + 32 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
+    size_t dbl = 3 * 2 * D * P + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
     const size_t RP = P - 2;
     size_t real = 3 * 2 * D * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
     (void)TC;
@@ -111,7 +126,7 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.S1 = d; d += 2 * D * P;
     m.S2 = d; d += 2 * D * P;
     m.cc = d; d += 2 * D * P;
-    m.red = d; d += 32;
+    m.red = d; d += 64;
     m.pdraw = d; d += 2 * kMaxNp * 2;
     m.blo = d; d += kMaxNp;
     m.bhi = d; d += kMaxNp;
@@ -266,6 +281,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     const int prm_q = tid >= TC ? 1 : 0, prm_j = tid - prm_q * TC, prm_iloc = 2 * prm_j + prm_q;
 
     int k_phase = 0;                               // half-sweeps since the halos were last exact
+    unsigned red_phase = 0;
     for (long long i = 0; i < a.n_sweeps; ++i) {
         const unsigned long long t = a.t0 + (unsigned long long)i;
         const int set = (int)(i & 1);
@@ -403,14 +419,14 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             part = (double)acc;
                         }
                     }
-                    dA = block_sum(part, sm.red);
+                    dA = block_sum_db(part, sm.red, red_phase);
                     if (G > 1) {   // all-gather of the G partials as tagged packets; every CTA sums them in index order
                         const uint32_t tag = (uint32_t)(ar_count + 1ull);
                         unsigned long long* base = a.ar_words + ((size_t)(ar_count & 1ull) * kTileMaxCtas + (size_t)chain * G) * kArSlotWords;
                         if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
                         double mine = 0.0;
                         for (int j = tid; j < G; j += T) mine += ll_wait_f64(base + (size_t)j * kArSlotWords, tag, a.fault);
-                        dA = block_sum(mine, sm.red);
+                        dA = block_sum_db(mine, sm.red, red_phase);
                         ar_count += 1ull;
                     }
                     accept = logu < -dA;
