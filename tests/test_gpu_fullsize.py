@@ -1,0 +1,96 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times, and the fp32 variant of config 3.
+
+Full-size cases use what the oracle can still do in seconds: a few teacher-forced sweeps (every site compared), and
+free-running sweeps with UNIFORM proposals, which are bit-reproducible, so path, parameters, counters and the traced
+Delta-A of every site must agree."""
+import numpy as np
+import pytest
+
+from helpers import TOL32, TOL64, gpu_handle, oracle_chains, teacher_forced
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    import paper_1103_4887_b200 as P
+    assert torch.cuda.is_available()
+    P.lib()
+    return P
+
+
+def test_cfg3_full_size_teacher_forced_in_bench_launch(P):
+    # config 3: HH, M = 32768, dt = 0.01, states + 7 parameters; automatic launch = the one bench.py times
+    w = make_workload(3)
+    h = gpu_handle(w)
+    shape = h.get_launch()
+    assert w.M == 32768 and shape["ctas_per_chain"] >= 100, shape      # spread over the SMs, tile-resident engine
+    rep = teacher_forced(w, h, oracle_chains(w), 3, seed=20110347)
+    print("cfg3 full size", shape, rep)
+    assert rep["sites"] == 3 * (w.M + 1)
+    assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0 and rep["ties"] <= 1, rep
+    assert rep["param_moves"] > 0 and rep["max_param_rel"] <= TOL64, rep
+    assert rep["max_xprop_ulp"] <= 4.0 and rep["max_path_diff"] <= 1e-12, rep
+
+
+def _free_running_uniform(P, w, n_sweeps, seed, chains=None):
+    h = gpu_handle(w, kind=1)
+    tr = h.enable_trace()
+    h.set_accum(True, 1); h.reset_moments()
+    h.sweep(n_sweeps, seed=seed)
+    xg, pg = [a.cpu().numpy() for a in h.get_path()]
+    st = h.stats().cpu().numpy().astype(np.uint64)
+    dA = tr["dA"].cpu().numpy(); acc = tr["acc"].cpu().numpy()
+    mx, mp, n = h.moments()
+    mx = mx.cpu().numpy()
+    orcs = oracle_chains(w, kind=1)
+    worst = 0.0
+    for c in (range(w.n_chains) if chains is None else chains):
+        o = orcs[c]
+        o.set_accum(True, 1); o.reset_moments()
+        o.sweep(n_sweeps, seed=seed)
+        xo, po = o.get_path()
+        assert np.array_equal(xg[c], xo), (c, np.abs(xg[c] - xo).max())
+        assert np.array_equal(pg[c], po), c
+        assert np.array_equal(st[c], o.stats()), c
+        ot = o.trace()                                   # last sweep: same state on both sides, so every site compares
+        assert np.array_equal(acc[c], ot["acc"]), c
+        err = np.abs(dA[c] - ot["dA"]) / np.maximum(np.maximum(np.abs(ot["dA"]), ot["S"]), 1e-300)
+        worst = max(worst, float(err.max()))
+        ox, op, on = o.moments()
+        assert n == on == n_sweeps
+        assert np.allclose(mx[c], ox, rtol=1e-13, atol=1e-13)
+    assert worst <= TOL64, worst
+    return worst
+
+
+def test_cfg3_full_size_free_running_bit_identical(P):
+    w = make_workload(3)
+    worst = _free_running_uniform(P, w, 24, seed=7)       # 24 sweeps: three halo exchanges of the tile engine
+    print("cfg3 free-running, max dA error / scale:", worst)
+
+
+def test_cfg4_full_size_batched_chains_bit_identical(P):
+    # config 4: 128 independent chains x M = 8192; every chain's path after 2 sweeps, 16 of them against the oracle
+    w = make_workload(4)
+    assert w.n_chains == 128 and w.M == 8192
+    worst = _free_running_uniform(P, w, 2, seed=11, chains=list(range(0, 128, 8)))
+    print("cfg4 free-running, max dA error / scale:", worst)
+
+
+@pytest.mark.parametrize("cfg,M,launch,with_params", [(2, 600, None, True), (2, 601, (5, 64), True), (0, 256, None, False),
+                                                      (1, 1000, None, False), (3, 4000, None, True)])
+def test_fp32_teacher_forced_parity(P, cfg, M, launch, with_params):
+    # config 3's fp32 variant: per-site Delta-A within 1e-5 of the fp64 oracle evaluated on the same fp32 states and the
+    # GPU's own fp32 proposals (probe A.5)
+    w = make_workload(cfg, M=M)
+    h = gpu_handle(w, dtype=32, with_params=with_params, launch=launch)
+    orcs = oracle_chains(w, state_dtype=32, with_params=with_params)
+    rep = teacher_forced(w, h, orcs, 20, seed=3, tol=TOL32, do_params=with_params, state_dtype=32)
+    print("fp32", cfg, M, h.get_launch(), rep)
+    assert rep["max_rel"] <= TOL32, rep
+    assert rep["mismatch_outside_window"] == 0, rep
+    if with_params:
+        assert rep["param_moves"] > 0 and rep["max_param_rel"] <= 10 * TOL32, rep
