@@ -36,6 +36,7 @@ FP64_LANES_PER_SM_CLK = 64
 SM_COUNT = 148
 SM_MAX_HZ = 1.965e9
 PEAK_TFLOPS_DERIVED = SM_COUNT * FP64_LANES_PER_SM_CLK * SM_MAX_HZ * 2 / 1e12
+NCU_DRAM_BYTES_PER_LAUNCH = 5968384.0   # cfg3 full sweep launch: 5.923 MB read + 45 KB written (profiles/r01_v4_tile_engine_soa.md)
 
 
 def rank_info():
@@ -155,7 +156,8 @@ def run_ours(args):
     w = make_workload(args.config, seed=None if rank == 0 else 11034887 + args.config + 7919 * rank)
     seed = w.chain_seed + rank
     S = args.sweeps_per_step
-    h = P.Pimc.from_workload(w, dtype=64)
+    h = P.Pimc.from_workload(w, dtype=args.dtype)
+    peak_tflops = PEAK_TFLOPS_DERIVED * (1.0 if args.dtype == 64 else 2.0)   # fp32: 128 FP32 lanes/clk/SM
     h.set_accum(True, 1)
     h.reset_moments()
     shape = h.get_launch()
@@ -209,27 +211,28 @@ def run_ours(args):
     slots_per_launch = units_per_step * W_SITE_SLOTS + evals_per_step * W_EVAL_SLOTS
     achieved_tflops = 2.0 * slots_per_launch / (float(np.mean(step_ms)) * 1e-3) / 1e12
     measured_peak = P.fp64_peak(150) * 2 / 1e12 if rank == 0 else None
-    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": PEAK_TFLOPS_DERIVED, "unit": "TFLOP/s",
-                "frac": achieved_tflops / PEAK_TFLOPS_DERIVED, "traffic": None,
-                "peak_source": "derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json",
+    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved_tflops / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == 3 and args.dtype == 64) else None,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r01_v4_tile_engine_soa.md (tile loaded once, written back once: independent of the sweeps per launch)",
+                "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
                 "peak_measured_dfma_tflops": measured_peak,
                 "frac_of_measured_dfma": (achieved_tflops / measured_peak) if measured_peak else None,
-                "kernel": "pimc::sweep_kernel<HHModel<double>,double>",
+                "kernel": "pimc::tile_sweep_kernel<HHModel<double>,double,256>" if shape.get("smem_bytes", 0) else "pimc::sweep_kernel<HHModel<double>,double>",
                 "work_model": {"slots_per_site_update": W_SITE_SLOTS, "slots_per_param_eval": W_EVAL_SLOTS,
                                "site_updates_per_launch": units_per_step, "param_evals_per_launch": evals_per_step},
                 "a2_only": {"site_updates_per_s": a2_rate, "ms_per_launch": a2_ms,
-                            "frac": 2 * a2_rate * W_SITE_SLOTS / 1e12 / PEAK_TFLOPS_DERIVED},
+                            "frac": 2 * a2_rate * W_SITE_SLOTS / 1e12 / peak_tflops},
                 "a4_only": {"param_evals_per_s": a4_rate, "ms_per_launch": a4_ms,
-                            "frac": 2 * a4_rate * W_EVAL_SLOTS / 1e12 / PEAK_TFLOPS_DERIVED}}
+                            "frac": 2 * a4_rate * W_EVAL_SLOTS / 1e12 / peak_tflops}}
 
     # end to end through the C ABI on HOST buffers: H2D of y, I, x0, p0 + sweeps + D2H of the moments inside the timed region
     e2e = None
     if rank == 0 or world > 1:
-        P.run_host(w, 0, max(1, S // 10), seed)         # warm-up (context, allocator)
+        P.run_host(w, 0, max(1, S // 10), seed, dtype=args.dtype)         # warm-up (context, allocator)
         reps = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
         for _ in range(reps):
-            out = P.run_host(w, 0, S, seed)
+            out = P.run_host(w, 0, S, seed, dtype=args.dtype)
         dt_e2e = time.perf_counter() - t0
         s_e2e, u_e2e = reduce_over_ranks(dt_e2e, units_per_step * reps, world, dist)
         e2e = {"value": u_e2e / s_e2e, "unit": UNIT, "h2d_bytes_per_step": out["h2d_bytes"], "d2h_bytes_per_step": out["d2h_bytes"],
@@ -241,7 +244,7 @@ def run_ours(args):
                "sample": f"{cpu_n} full sweeps of chain 0 of {w.name} in {cpu_s:.1f} s (serial fp64 C++ -O2, {os.cpu_count()} cores present)"}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.dtype == 64 else "f32",
             "data": "synthetic",
             "config": {"workload": w.name, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
                        "accumulate_every": 1, "launch": shape, "l2": "flushed between timed steps (256 MiB fill)",
@@ -263,6 +266,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--dtype", type=int, default=64, choices=[64, 32], help="arithmetic type of the path (config 3 is also quoted in fp32)")
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=120.0, help="seconds of oracle time for --impl reference")
