@@ -281,6 +281,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     const int prm_q = tid >= TC ? 1 : 0, prm_j = tid - prm_q * TC, prm_iloc = 2 * prm_j + prm_q;
 
     int k_phase = 0;                               // half-sweeps since the halos were last exact
+    typename Model::Prep prep = Model::prepare(prm, a.dt);   // refreshed whenever a parameter move is accepted
     unsigned red_phase = 0;
     for (long long i = 0; i < a.n_sweeps; ++i) {
         const unsigned long long t = a.t0 + (unsigned long long)i;
@@ -292,7 +293,6 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         if (tid < TC) {
             // ---------------- A2: even half-sweep, then odd half-sweep (compute warps) ----------------
             if (a.do_states) {
-                const typename Model::Prep prep = Model::prepare(prm, a.dt);
 #pragma unroll 1
                 for (int q = 0; q < 2; ++q) {
                     const int k = k_phase + q + 1;           // half-sweeps run on the current halos, this one included
@@ -348,13 +348,17 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         }
                         const R dA = (has_l ? dL : R(0)) + (has_r ? dR : R(0));
                         const bool accept = logu < -dA;
+                        const bool keep_g = accept && has_r;
+                        // unconditional stores of selected values: no divergent branch in the tail of the update
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
-                            if (accept) sm.xs[own + c * P] = xp[c];
-                            if (accept && has_r) gc[own + c * P] = gp[c];
+                            const R xf = accept ? xp[c] : xn[c];
+                            sm.xs[own + c * P] = xf;
+                            gc[own + c * P] = keep_g ? gp[c] : gn[c];
                             // A5 for this site: its value is final for sweep t (parameter moves do not touch x)
-                            const double d = (double)(accept ? xp[c] : xn[c]) - mc[c];
-                            if (acc_now) { sm.S1[own + c * P] = m1[c] + d; sm.S2[own + c * P] = m2[c] + d * d; }
+                            const double d = (double)xf - mc[c];
+                            sm.S1[own + c * P] = acc_now ? m1[c] + d : m1[c];
+                            sm.S2[own + c * P] = acc_now ? m2[c] + d * d : m2[c];
                         }
                         const bool owned = n >= s && n < e;
                         n_acc_state += (owned && accept) ? 1u : 0u;
@@ -380,6 +384,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             const int n = s_ext + prm_iloc;
             const bool can_eval = prm_iloc < n_ext && n <= M - 1;
             const bool owned = n >= s && n < e && n <= M - 1;
+            bool params_changed = false;
 #pragma unroll 1
             for (int l = 0; l < NP; ++l) {
                 if (!(a.wp[l] > 0.0)) continue;
@@ -431,6 +436,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     }
                     accept = logu < -dA;
                     if (accept) cur ^= 1;
+                    params_changed = params_changed || accept;
                 }
 #pragma unroll
                 for (int k = 0; k < NP; ++k) {
@@ -445,6 +451,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = (R)pl;
                 }
             }
+            if (params_changed) prep = Model::prepare(prm, a.dt);
             if (trace && b == 0 && tid == 0) {
 #pragma unroll
                 for (int l = 0; l < NP; ++l)
