@@ -236,7 +236,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     if (T == 0) T = std::max(64, (tile + 2 * hh + 63) / 64 * 64);
     if (tile + 2 * hh > T || T > 512) return no("tile plus halos does not fit the CTA");
     out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1; out->engine = PIMC_ENGINE_TILE; out->h = hh;
-    out->smem = tile_smem_bytes<R>(T, h->D, h->L);
+    out->smem = tile_smem_bytes<R>(T, h->D, h->L, Model::NK);
     if (out->smem > 227 * 1024) return no("shared memory");
     return PIMC_OK;
 }

@@ -38,22 +38,35 @@ template <typename R> struct HHModel {
         const double num = fma(-a, q, e) * q;
         return div_series(num, den);
     }
-    static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R inv_C, R I, R F[4]) {
+    // dV/dt (Eq. 11 with the config's physical parameters): the only place the parameters enter
+    static __device__ __forceinline__ R rhs_V(const R x[4], const R* __restrict__ p, R inv_C, R I) {
         const R V = x[0], m = x[1], h = x[2], n = x[3];
         const R n2 = n * n;
         const R cur = I + p[0] * (m * m * m) * h * (p[3] - V) + p[1] * (n2 * n2) * (p[4] - V) + p[2] * (p[5] - V);
+        if constexpr (sizeof(R) == 8) return cur * inv_C;
+        else return cur / p[6];
+    }
+    // d(m,h,n)/dt (Eq. 12-14): functions of the state only, not of the parameters
+    static __device__ __forceinline__ void rhs_gates(const R x[4], R Fg[3]) {
+        const R V = x[0], m = x[1], h = x[2], n = x[3];
         if constexpr (sizeof(R) == 8) {
-            F[0] = cur * inv_C;
-            F[1] = gate_fast(V, m, -40.0, 15.0, 0.1, 0.4);
-            F[2] = gate_fast(V, h, -60.0, -15.0, 1.0, 7.0);
-            F[3] = gate_fast(V, n, -55.0, 30.0, 1.0, 5.0);
+            Fg[0] = gate_fast(V, m, -40.0, 15.0, 0.1, 0.4);
+            Fg[1] = gate_fast(V, h, -60.0, -15.0, 1.0, 7.0);
+            Fg[2] = gate_fast(V, n, -55.0, 30.0, 1.0, 5.0);
         } else {
-            F[0] = cur / p[6];
-            F[1] = gate(V, m, R(-40.0), R(15.0), R(0.1), R(0.4));
-            F[2] = gate(V, h, R(-60.0), R(-15.0), R(1.0), R(7.0));
-            F[3] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
+            Fg[0] = gate(V, m, R(-40.0), R(15.0), R(0.1), R(0.4));
+            Fg[1] = gate(V, h, R(-60.0), R(-15.0), R(1.0), R(7.0));
+            Fg[2] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
         }
     }
+    static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R inv_C, R I, R F[4]) {
+        F[0] = rhs_V(x, p, inv_C, I);
+        rhs_gates(x, F + 1);
+    }
+    // The first RK4 stage evaluates the gate rates at x itself: they do not depend on the parameters, so a parameter
+    // move (row A4: same x, seven different p per sweep) can reuse them.  NK values per site are cached by the tile engine.
+    static constexpr int NK = 3;
+    static __device__ __forceinline__ void stage1_cache(const R x[4], R kg[3]) { rhs_gates(x, kg); }
     // Quantities that depend only on (p, dt): computed once per parameter vector, not once per site.
     struct Prep { R inv_C, hdt, dt6; };
     static __device__ __forceinline__ Prep prepare(const R* __restrict__ p, R dt) {
@@ -66,11 +79,22 @@ template <typename R> struct HHModel {
     }
     // Domain guard of the double-precision gates: a stage voltage beyond +-1e8 mV (or NaN) makes the whole increment
     // NaN, i.e. the proposal is rejected; inside the guard the gates saturate exactly like tanh.
-    static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, const Prep& q, R I0, R I1, R dt, R g[4]) {
+    // kg_in: stage-1 gate rates computed earlier at this same x (bit-identical to recomputing them); kg_out: receives them
+    template <bool IN, bool OUT>
+    static __device__ __forceinline__ void increment_k(const R x[4], const R* __restrict__ p, const Prep& q, R I0, R I1, R dt, R g[4],
+                                                       const R* kg_in, R* kg_out) {
         const R Ih = R(0.5) * (I0 + I1);
         R k[4], xs[4], acc[4];
         bool sane = true;
-        rhs(x, p, q.inv_C, I0, k);
+        if constexpr (IN) {
+            k[0] = rhs_V(x, p, q.inv_C, I0);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) k[1 + a] = kg_in[a];
+        } else rhs(x, p, q.inv_C, I0, k);
+        if constexpr (OUT) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) kg_out[a] = k[1 + a];
+        }
         if constexpr (sizeof(R) == 8) sane = sane && fabs(x[0]) < 1e8;
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] = k[a]; xs[a] = x[a] + q.hdt * k[a]; }
@@ -90,6 +114,9 @@ template <typename R> struct HHModel {
             if constexpr (sizeof(R) == 8) g[a] = sane ? g[a] : __longlong_as_double(0x7FF8000000000000ll);
         }
     }
+    static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, const Prep& q, R I0, R I1, R dt, R g[4]) {
+        increment_k<false, false>(x, p, q, I0, I1, dt, g, nullptr, nullptr);
+    }
     static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
         increment(x, p, prepare(p, dt), I0, I1, dt, g);
     }
@@ -101,6 +128,12 @@ template <typename R, int D_> struct LinearModel {
     static constexpr int NP = D_ * D_;
     struct Prep {};
     static __device__ __forceinline__ Prep prepare(const R* __restrict__, R) { return Prep{}; }
+    static constexpr int NK = 0;                   // nothing parameter-independent worth caching
+    static __device__ __forceinline__ void stage1_cache(const R*, R*) {}
+    template <bool IN, bool OUT>
+    static __device__ __forceinline__ void increment_k(const R x[D_], const R* __restrict__ p, const Prep&, R I0, R I1, R dt, R g[D_], const R*, R*) {
+        increment(x, p, I0, I1, dt, g);
+    }
     static __device__ __forceinline__ void increment(const R x[D_], const R* __restrict__ p, const Prep&, R I0, R I1, R dt, R g[D_]) {
         increment(x, p, I0, I1, dt, g);
     }

@@ -100,6 +100,7 @@ template <typename R> struct TileSmem {
     double *blo, *bhi;          // [kMaxNp] bounds
     double *pS1, *pS2, *pcc;    // [kMaxNp] running moments of the parameters (tile 0 of each chain)
     R *xs, *g0, *g1;            // [2*D*P]
+    R *kg;                      // [2*NK*P] parameter-independent first-stage rates of every tile site (Model::stage1_cache)
     R *Is, *ys;                 // [E+2], [E*L]
     R *rstep, *rlogu;           // [2 sets][2 parities][D][TC], [2][2][TC]
     unsigned int* cnt;          // [2]: accepted owned state updates (lo, unused)
@@ -109,16 +110,16 @@ template <typename R> struct TileSmem {
 // the pitch is a compile-time constant of the kernel instantiation (MAXT = 256 or 512), so plane offsets are immediates
 __host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512) / 2 + 2; }
 
-template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L) {
+template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     size_t dbl = 3 * 2 * D * P + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
     const size_t RP = P - 2;
-    size_t real = 3 * 2 * D * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
+    size_t real = 3 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
     (void)TC;
     return dbl * 8 + ((real * sizeof(R) + 15) & ~(size_t)15) + 16;
 }
 
-template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L) {
+template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L, int NK) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     TileSmem<R> m;
     m.P = (int)P;
@@ -138,6 +139,7 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.xs = r; r += 2 * D * P;
     m.g0 = r; r += 2 * D * P;
     m.g1 = r; r += 2 * D * P;
+    m.kg = r; r += 2 * (size_t)NK * P;
     m.Is = r; r += E + 2;
     m.ys = r; r += E * (size_t)(L > 0 ? L : 1);
     m.rstep = r; r += 4 * (P - 2) * D;
@@ -198,7 +200,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     constexpr int NP = Model::NP;
     extern __shared__ __align__(16) unsigned char tile_smem_raw[];
     const int T = blockDim.x, TC = T >> 1, tid = threadIdx.x;
-    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L);
+    constexpr int NK = Model::NK;
+    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK);
     constexpr int RP = MAXT / 2;                   // pitch of the random-number ring
     constexpr int P = MAXT / 2 + 2;                // == tile_pitch(T): the launcher picks MAXT = 256 for T <= 256, else 512
 
@@ -280,6 +283,22 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     // site prm_site: the even sites on threads [0, TC), the odd sites on [TC, T) (unit-stride plane accesses)
     const int prm_q = tid >= TC ? 1 : 0, prm_j = tid - prm_q * TC, prm_iloc = 2 * prm_j + prm_q;
 
+    // first-stage rates of this thread's tile site, from its current state (kernel start and after every halo refresh;
+    // in between, the site updates keep them current)
+    auto refresh_stage1 = [&]() {
+        if constexpr (NK > 0) {
+            if (prm_iloc < n_ext) {
+                R xn[D], kk[NK > 0 ? NK : 1];
+                lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
+                Model::stage1_cache(xn, kk);
+#pragma unroll
+                for (int c = 0; c < NK; ++c) sm.kg[(prm_q * NK + c) * P + prm_j] = kk[c];
+            }
+        }
+    };
+    refresh_stage1();
+    __syncthreads();
+
     int k_phase = 0;                               // half-sweeps since the halos were last exact
     typename Model::Prep prep = Model::prepare(prm, a.dt);   // refreshed whenever a parameter move is accepted
     unsigned red_phase = 0;
@@ -324,7 +343,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             mc[c] = sm.cc[own + c * P]; m1[c] = sm.S1[own + c * P]; m2[c] = sm.S2[own + c * P];
                         }
                         const R logu = sm.rlogu[(size_t)(set * 2 + q) * RP + tid];
-                        Model::increment(xp, prm, prep, I0, I1, a.dt, gp);
+                        R kgo[NK > 0 ? NK : 1], kgn[NK > 0 ? NK : 1];
+#pragma unroll
+                        for (int c = 0; c < NK; ++c) kgo[c] = sm.kg[(q * NK + c) * P + tid];
+                        Model::template increment_k<false, true>(xp, prm, prep, I0, I1, a.dt, gp, nullptr, kgn);
                         R dL = R(0), dR = R(0);
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
@@ -349,6 +371,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         const R dA = (has_l ? dL : R(0)) + (has_r ? dR : R(0));
                         const bool accept = logu < -dA;
                         const bool keep_g = accept && has_r;
+#pragma unroll
+                        for (int c = 0; c < NK; ++c) sm.kg[(q * NK + c) * P + tid] = accept ? kgn[c] : kgo[c];
                         // unconditional stores of selected values: no divergent branch in the tail of the update
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
@@ -408,7 +432,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     if (can_eval) {
                         R xn[D], gp[D];
                         lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
-                        Model::increment(xn, pp, sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp);
+                        R kk[NK > 0 ? NK : 1];
+#pragma unroll
+                        for (int c = 0; c < NK; ++c) kk[c] = sm.kg[(prm_q * NK + c) * P + prm_j];
+                        Model::template increment_k<(NK > 0), false>(xn, pp, Model::prepare(pp, a.dt), sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp, kk, nullptr);
                         sts_site<R, D>(ga, prm_q, prm_j, P, gp);
                         if (owned) {
                             R xq[D], gn[D];
@@ -508,6 +535,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             hx_count += 1ull;
             k_phase = 0;
             __syncthreads();
+            if constexpr (NK > 0) { refresh_stage1(); __syncthreads(); }
         }
 
         // ---------------- A5: running moments and histograms (owned sites) ----------------
