@@ -53,6 +53,9 @@ def lib():
             "orc_site_delta_A": (C.c_double, [C.c_void_p, C.c_int, dp, dp]),
             "orc_param_delta_A": (C.c_double, [C.c_void_p, C.c_int, C.c_double, dp]),
             "orc_full_action": (None, [C.c_void_p, dp, dp, dp, dp]),
+            "orc_cache_len": (C.c_int, [C.c_void_p]),
+            "orc_set_discretisation": (C.c_int, [C.c_void_p, C.c_int]),
+            "orc_half_rhs": (None, [C.c_int, C.c_int, dp, dp, C.c_double, C.c_double, dp]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name)
@@ -176,9 +179,13 @@ class OracleChain:
         return x, p
 
     def get_cache(self):
-        g = np.empty((self.M, self.D))
+        g = np.empty((lib().orc_cache_len(self._h), self.D))     # M rows (RK4 map) or M + 1 (trapezoid)
         lib().orc_get_cache(self._h, _dp(g))
         return g
+
+    def set_discretisation(self, disc):
+        """0 = explicit RK4 map (default), 1 = the paper's trapezoid rule (Eq. 7)."""
+        assert lib().orc_set_discretisation(self._h, int(disc)) == 0
 
     def set_proposal(self, w_state, w_param=None, kind=0):
         ws = _f64(w_state).reshape(-1)

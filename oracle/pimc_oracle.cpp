@@ -167,6 +167,7 @@ struct Chain {
     double Rf[MAXD];
     std::vector<double> x, g, y, I, p, lo, hi, wx, wp;
     int proposal_kind = 0;                    // 0 gaussian, 1 uniform
+    int disc = 0;                             // model-error discretisation: 0 = explicit RK4 map (north_star), 1 = trapezoid rule (Eq. 7)
     uint64_t t = 0;                           // absolute sweep index
     uint32_t chain_id = 0;
     bool have_data = false, have_path = false;
@@ -185,10 +186,35 @@ struct Chain {
 
 double I_at(const Chain& c, int n) { return c.I.empty() ? 0.0 : c.I[n]; }
 
+// The model-error term between steps n and n+1 is (Rf_a/2) r_a^2 with
+//   disc 0 (RK4 map, BASELINE north_star):   r = (x_{n+1} - x_n) - g_n,            g_n = RK4 increment at x_n      (n = 0..M-1)
+//   disc 1 (trapezoid, Eq. 7):  r = (x_{n+1} - x_n) - c_n - c_{n+1},  c_n = (dt/2) F(x_n, p; I_n)     (n = 0..M)
+// i.e. the paper's eps_{n+1} = x_{n+1} - x_n - (dt/2)[F(x_{n+1}) + F(x_n)].  The cache array `g` holds g_n or c_n
+// (the paper caches F_n).  Linear model in trapezoid form: F(x) = (A x - x)/dt, so c = (A x - x)/2.
+int cache_len(const Chain& c) { return c.disc == 1 ? c.M + 1 : c.M; }
+
+void half_rhs(int model, int D, const double* x, const double* p, double I, double dt, double* out) {
+    if (model == MODEL_LINEAR) {
+        for (int a = 0; a < D; ++a) {
+            double f = 0.0;
+            for (int b = 0; b < D; ++b) f += p[a * D + b] * x[b];
+            out[a] = 0.5 * (f - x[a]);
+        }
+        return;
+    }
+    double F[4];
+    hh_rhs(x, p, I, F);
+    for (int a = 0; a < 4; ++a) out[a] = 0.5 * dt * F[a];
+}
+
+// cache entry n of the chain's discretisation at state x (n <= M-1 for disc 0, n <= M for disc 1)
+void cache_value(const Chain& c, int n, const double* x, const double* p, double* out) {
+    if (c.disc == 1) half_rhs(c.model, c.D, x, p, I_at(c, n), c.dt, out);
+    else step_increment(c.model, c.D, x, p, I_at(c, n), I_at(c, n + 1), c.dt, out);
+}
+
 void rebuild_cache(Chain& c) {
-    for (int n = 0; n < c.M; ++n)
-        step_increment(c.model, c.D, &c.x[(size_t)n * c.D], c.p.data(), I_at(c, n), I_at(c, n + 1), c.dt,
-                       &c.g[(size_t)n * c.D]);
+    for (int n = 0; n < cache_len(c); ++n) cache_value(c, n, &c.x[(size_t)n * c.D], c.p.data(), &c.g[(size_t)n * c.D]);
 }
 
 // Local change of the action if x_n is replaced by xp (Fig. 1 (c)-(g)).
@@ -197,6 +223,39 @@ double site_delta_A(const Chain& c, int n, const double* xp, double* gp, double*
     const int D = c.D, M = c.M;
     const double* xn = &c.x[(size_t)n * D];
     double dA = 0.0, S = 0.0;
+    if (c.disc == 1) {
+        // Fig. 1 (b)-(f) as printed: F' = F(x'_n); eps'_n, eps_n (term n-1 -> n), eps'_{n+1}, eps_{n+1} (term n -> n+1), delta'_n, delta_n
+        cache_value(c, n, xp, c.p.data(), gp);                         // c'_n = (dt/2) F(x'_n): needed at every n, n = M included
+        const double* cn = &c.g[(size_t)n * D];
+        if (n >= 1) {
+            const double* xm = &c.x[(size_t)(n - 1) * D];
+            const double* cm = &c.g[(size_t)(n - 1) * D];
+            for (int a = 0; a < D; ++a) {
+                const double r_new = ((xp[a] - xm[a]) - cm[a]) - gp[a];
+                const double r_old = ((xn[a] - xm[a]) - cm[a]) - cn[a];
+                const double t_new = 0.5 * c.Rf[a] * r_new * r_new, t_old = 0.5 * c.Rf[a] * r_old * r_old;
+                dA += t_new - t_old; S += t_new + t_old;
+            }
+            for (int l = 0; l < c.L; ++l) {
+                const double d_new = c.y[(size_t)n * c.L + l] - xp[l];
+                const double d_old = c.y[(size_t)n * c.L + l] - xn[l];
+                const double t_new = 0.5 * c.Rm * d_new * d_new, t_old = 0.5 * c.Rm * d_old * d_old;
+                dA += t_new - t_old; S += t_new + t_old;
+            }
+        }
+        if (n <= M - 1) {
+            const double* xq = &c.x[(size_t)(n + 1) * D];
+            const double* cq = &c.g[(size_t)(n + 1) * D];
+            for (int a = 0; a < D; ++a) {
+                const double r_new = ((xq[a] - xp[a]) - gp[a]) - cq[a];
+                const double r_old = ((xq[a] - xn[a]) - cn[a]) - cq[a];
+                const double t_new = 0.5 * c.Rf[a] * r_new * r_new, t_old = 0.5 * c.Rf[a] * r_old * r_old;
+                dA += t_new - t_old; S += t_new + t_old;
+            }
+        }
+        if (S_out) *S_out = S;
+        return dA;
+    }
     if (n >= 1) {
         const double* xm = &c.x[(size_t)(n - 1) * D];
         const double* gm = &c.g[(size_t)(n - 1) * D];
@@ -296,7 +355,7 @@ void update_site(Chain& c, uint64_t seed, int n) {
     for (int a = 0; a < D; ++a) { c.prop[a] += 1; if (accept) c.acc[a] += 1; }
     if (accept) {
         for (int a = 0; a < D; ++a) c.x[(size_t)n * D + a] = xp[a];
-        if (n <= c.M - 1) for (int a = 0; a < D; ++a) c.g[(size_t)n * D + a] = gp[a];
+        if (n < cache_len(c)) for (int a = 0; a < D; ++a) c.g[(size_t)n * D + a] = gp[a];
     }
 }
 
@@ -316,10 +375,30 @@ void half_sweep(Chain& c, uint64_t seed, int parity, int order) {
     for (int n : sites) update_site(c, seed, n);
 }
 
+// Change of the action when the parameter vector becomes pnew on the current path: every model-error term changes
+// (PAPER.md:199, 209).  gnew receives the cache under pnew; the sum runs over the terms in index order (Neumaier).
+double param_delta_sum(const Chain& c, const double* pnew, std::vector<double>& gnew, double* S_out) {
+    const int D = c.D, M = c.M, nc = cache_len(c);
+    gnew.resize((size_t)(M + 1) * D);          // always room for the longer (trapezoid) cache: the arrays are swapped on accept
+    for (int n = 0; n < nc; ++n) cache_value(c, n, &c.x[(size_t)n * D], pnew, &gnew[(size_t)n * D]);
+    Neumaier sum; double S = 0.0;
+    for (int n = 0; n < M; ++n)
+        for (int a = 0; a < D; ++a) {
+            const double d = c.x[(size_t)(n + 1) * D + a] - c.x[(size_t)n * D + a];
+            double r_new = d - gnew[(size_t)n * D + a];
+            double r_old = d - c.g[(size_t)n * D + a];
+            if (c.disc == 1) { r_new -= gnew[(size_t)(n + 1) * D + a]; r_old -= c.g[(size_t)(n + 1) * D + a]; }
+            const double t_new = 0.5 * c.Rf[a] * r_new * r_new, t_old = 0.5 * c.Rf[a] * r_old * r_old;
+            sum.add(t_new - t_old); S += t_new + t_old;
+        }
+    if (S_out) *S_out = S;
+    return sum.value();
+}
+
 // S4. Sequential parameter moves (row A4).
 void parameter_moves(Chain& c, uint64_t seed) {
-    const int D = c.D, M = c.M;
-    std::vector<double> gnew((size_t)M * D), pnew(c.Np);
+    const int D = c.D;
+    std::vector<double> gnew, pnew(c.Np);
     for (int l = 0; l < c.Np; ++l) {
         c.tr_dAp[l] = std::numeric_limits<double>::quiet_NaN(); c.tr_Sp[l] = 0.0;
         c.tr_logup[l] = 0.0; c.tr_accp[l] = 0; c.tr_pprop[l] = c.p[l];
@@ -336,19 +415,8 @@ void parameter_moves(Chain& c, uint64_t seed) {
         c.prop[D + l] += 1;
         if (!(pl >= c.lo[l] && pl <= c.hi[l])) continue;               // outside bounds => rejected
         pnew = c.p; pnew[l] = pl;
-        Neumaier sum; double S = 0.0;
-        for (int n = 0; n < M; ++n) {
-            step_increment(c.model, D, &c.x[(size_t)n * D], pnew.data(), I_at(c, n), I_at(c, n + 1), c.dt,
-                           &gnew[(size_t)n * D]);
-            for (int a = 0; a < D; ++a) {
-                const double d = c.x[(size_t)(n + 1) * D + a] - c.x[(size_t)n * D + a];
-                const double r_new = d - gnew[(size_t)n * D + a];
-                const double r_old = d - c.g[(size_t)n * D + a];
-                const double t_new = 0.5 * c.Rf[a] * r_new * r_new, t_old = 0.5 * c.Rf[a] * r_old * r_old;
-                sum.add(t_new - t_old); S += t_new + t_old;
-            }
-        }
-        const double dA = sum.value();
+        double S = 0.0;
+        const double dA = param_delta_sum(c, pnew.data(), gnew, &S);
         const bool accept = logu < -dA;
         c.tr_dAp[l] = dA; c.tr_Sp[l] = S; c.tr_accp[l] = accept ? 1 : 0;
         if (accept) { c.p[l] = pl; c.g.swap(gnew); c.acc[D + l] += 1; }
@@ -392,11 +460,13 @@ long double full_action(const Chain& c, const double* x, const double* p) {
             const long double d = (long double)c.y[(size_t)n * c.L + l] - (long double)x[(size_t)n * D + l];
             A += 0.5L * (long double)c.Rm * d * d;
         }
-    double g[MAXD];
+    double g[MAXD], g1[MAXD];
     for (int n = 0; n < c.M; ++n) {
-        step_increment(c.model, D, &x[(size_t)n * D], p, I_at(c, n), I_at(c, n + 1), c.dt, g);
+        cache_value(c, n, &x[(size_t)n * D], p, g);
+        if (c.disc == 1) cache_value(c, n + 1, &x[(size_t)(n + 1) * D], p, g1);
         for (int a = 0; a < D; ++a) {
-            const long double r = ((long double)x[(size_t)(n + 1) * D + a] - (long double)x[(size_t)n * D + a]) - (long double)g[a];
+            long double r = ((long double)x[(size_t)(n + 1) * D + a] - (long double)x[(size_t)n * D + a]) - (long double)g[a];
+            if (c.disc == 1) r -= (long double)g1[a];
             A += 0.5L * (long double)c.Rf[a] * r * r;
         }
     }
@@ -438,7 +508,7 @@ void* orc_create(int model, int D, int L, int M, double dt, double Rm, const dou
     c->dt = dt; c->Rm = Rm; c->chain_id = chain_id;
     for (int a = 0; a < D; ++a) c->Rf[a] = Rf[a];
     const size_t nx = (size_t)(M + 1) * D;
-    c->x.assign(nx, 0.0); c->g.assign((size_t)M * D, 0.0); c->y.assign((size_t)(M + 1) * (L > 0 ? L : 1), 0.0);
+    c->x.assign(nx, 0.0); c->g.assign((size_t)(M + 1) * D, 0.0); c->y.assign((size_t)(M + 1) * (L > 0 ? L : 1), 0.0);
     c->p.assign(p0, p0 + c->Np);
     if (state_dtype == 32) for (double& v : c->p) v = (double)(float)v;
     c->lo.assign(c->Np, -std::numeric_limits<double>::infinity());
@@ -481,7 +551,18 @@ void orc_get_path(void* h, double* x, double* p) {
     if (x) std::memcpy(x, c.x.data(), c.x.size() * sizeof(double));
     if (p) std::memcpy(p, c.p.data(), c.p.size() * sizeof(double));
 }
-void orc_get_cache(void* h, double* g) { Chain& c = *(Chain*)h; std::memcpy(g, c.g.data(), c.g.size() * sizeof(double)); }
+// cache entries in use: M (RK4 map) or M+1 (trapezoid) rows of D values
+int orc_cache_len(void* h) { return cache_len(*(Chain*)h); }
+void orc_get_cache(void* h, double* g) { Chain& c = *(Chain*)h; std::memcpy(g, c.g.data(), (size_t)cache_len(c) * c.D * sizeof(double)); }
+// 0 = explicit RK4 map (default), 1 = trapezoid rule of the paper (Eq. 7)
+int orc_set_discretisation(void* h, int disc) {
+    Chain& c = *(Chain*)h;
+    if (!(disc == 0 || disc == 1)) return -1;
+    c.disc = disc;
+    if (c.have_path) rebuild_cache(c);
+    return 0;
+}
+void orc_half_rhs(int model, int D, const double* x, const double* p, double I, double dt, double* out) { half_rhs(model, D, x, p, I, dt, out); }
 void orc_set_proposal(void* h, const double* w_state, const double* w_param, int kind) {
     Chain& c = *(Chain*)h;
     c.wx.assign(w_state, w_state + c.D);
@@ -569,19 +650,8 @@ double orc_site_delta_A(void* h, int n, const double* xp, double* S) {
 // Parameter-move dA of replacing p_l by pl on the current path (no RNG, no state change).
 double orc_param_delta_A(void* h, int l, double pl, double* S_out) {
     Chain& c = *(Chain*)h;
-    std::vector<double> pnew = c.p; pnew[l] = pl;
-    Neumaier sum; double S = 0.0, g[MAXD];
-    for (int n = 0; n < c.M; ++n) {
-        step_increment(c.model, c.D, &c.x[(size_t)n * c.D], pnew.data(), I_at(c, n), I_at(c, n + 1), c.dt, g);
-        for (int a = 0; a < c.D; ++a) {
-            const double d = c.x[(size_t)(n + 1) * c.D + a] - c.x[(size_t)n * c.D + a];
-            const double r_new = d - g[a], r_old = d - c.g[(size_t)n * c.D + a];
-            const double t_new = 0.5 * c.Rf[a] * r_new * r_new, t_old = 0.5 * c.Rf[a] * r_old * r_old;
-            sum.add(t_new - t_old); S += t_new + t_old;
-        }
-    }
-    if (S_out) *S_out = S;
-    return sum.value();
+    std::vector<double> pnew = c.p, gnew; pnew[l] = pl;
+    return param_delta_sum(c, pnew.data(), gnew, S_out);
 }
 // Full action of an arbitrary (x, p) with this chain's data, accumulated in long double; returned as
 // hi + lo doubles so ctypes callers keep the extra bits.
