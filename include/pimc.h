@@ -53,6 +53,14 @@ enum { PIMC_PROPOSAL_GAUSSIAN = 0, PIMC_PROPOSAL_UNIFORM = 1 };
  * (even, odd) site pair per compute thread, halos updated redundantly and exchanged every h half-sweeps as tagged
  * 8-byte packets; needs tile + 2h <= threads_per_cta <= 512.  AUTO: TILE when it fits, else GLOBAL. */
 enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2 };
+/* Discretisation of the model-error term between steps n and n+1, (Rf_a/2) r_a^2:
+ *  RK4MAP    (default; BASELINE north_star): r = (x_{n+1} - x_n) - g_n, g_n = the increment of one RK4 step from x_n
+ *            (LINEAR: g = A x - x); the cache holds g_n, n = 0..M-1.
+ *  TRAPEZOID (the paper's own rule, Eq. 7): r = x_{n+1} - x_n - (dt/2)[F(x_{n+1}) + F(x_n)], F the model's
+ *            vector field with the current I_n at step n (LINEAR: F(x) = (A x - x)/dt); the cache holds
+ *            c_n = (dt/2) F(x_n), n = 0..M (PAPER.md:189, 242 caches F_n).  One right-hand side per proposal instead of
+ *            four.  Runs on the GLOBAL engine (PIMC_EUNSUPPORTED if the TILE engine is forced). */
+enum { PIMC_DISC_RK4MAP = 0, PIMC_DISC_TRAPEZOID = 1 };
 
 /* Number of parameters the model defines (HH: 7, LINEAR: D*D); negative on bad arguments. */
 int pimc_model_np(int model, int D);
@@ -84,8 +92,12 @@ int pimc_set_params(pimc_handle* h, const void* p);
 /* Copy out the current path (dev (n_chains, M+1, D)) and/or parameters (dev (n_chains, Np)); either may be NULL. */
 int pimc_get_path(pimc_handle* h, void* x_out, void* p_out);
 
-/* Copy out the current step cache g: dev (n_chains, M, D) (for cache-coherence checks). */
+/* Copy out the current step cache: dev (n_chains, M, D) for PIMC_DISC_RK4MAP, dev (n_chains, M+1, D) for
+ * PIMC_DISC_TRAPEZOID (for cache-coherence checks).  Synchronises the stream. */
 int pimc_get_cache(pimc_handle* h, void* g_out);
+
+/* Select the discretisation (PIMC_DISC_*); rebuilds the cache if a path is set.  PIMC_EINVAL on an unknown value. */
+int pimc_set_discretisation(pimc_handle* h, int disc);
 
 /* Proposal widths (PAPER.md:188 step (a), 226): w_state host D values >= 0; w_param host Np values >= 0
  * or NULL (= all 0; a parameter with width 0 is frozen and never proposed); kind = PIMC_PROPOSAL_*. */

@@ -10,6 +10,7 @@ import numpy as np
 MODEL_LINEAR, MODEL_HH = 0, 1
 PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM = 0, 1
 ENGINE_AUTO, ENGINE_GLOBAL, ENGINE_TILE = 0, 1, 2
+DISC_RK4MAP, DISC_TRAPEZOID = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libpimc.so")
@@ -42,6 +43,7 @@ _SIGNATURES = {
     "pimc_set_launch": (C.c_int, [_vp, C.c_int, C.c_int]),
     "pimc_get_launch": (C.c_int, [_vp, _ip, _ip, _ip, _ip]),
     "pimc_set_engine": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "pimc_set_discretisation": (C.c_int, [_vp, C.c_int]),
     "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
     "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
@@ -235,9 +237,15 @@ class Pimc:
         return x, p
 
     def get_cache(self):
-        g = self.torch.empty((self.C, self.M, self.D), dtype=self.tdtype, device=self.device)
+        rows = self.M + 1 if getattr(self, "disc", DISC_RK4MAP) == DISC_TRAPEZOID else self.M
+        g = self.torch.empty((self.C, rows, self.D), dtype=self.tdtype, device=self.device)
         _check(lib().pimc_get_cache(self._h, _ptr(g)), self._h)
         return g
+
+    def set_discretisation(self, disc):
+        """DISC_RK4MAP (default) or DISC_TRAPEZOID (the paper's rule, Eq. 7; GLOBAL engine)."""
+        _check(lib().pimc_set_discretisation(self._h, int(disc)), self._h)
+        self.disc = int(disc)
 
     def moments(self):
         """-> (mean_x, var_x) each (C, M+1, D); (mean_p, var_p) each (C, Np); n_samples."""

@@ -54,7 +54,7 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     const size_t es = dtype == 64 ? 8 : 4;
     Carve c(base);
     Layout o{};
-    const size_t nx = (size_t)C * (M + 1) * D, ng = (size_t)C * M * D;
+    const size_t nx = (size_t)C * (M + 1) * D, ng = (size_t)C * (M + 1) * D;   // caches: room for the trapezoid form's M + 1 entries
     o.x = c.take<char>(nx * es);
     o.g0 = c.take<char>(ng * es);
     o.g1 = c.take<char>(ng * es);
@@ -109,6 +109,7 @@ struct pimc_handle {
     Layout lay;
     double wx[kMaxD], wp[kMaxNp];
     int kind = 0;
+    int disc = PIMC_DISC_RK4MAP;
     bool have_data = false, have_path = false, have_prop = false, have_I = false;
     int accum = 0;
     unsigned long long n_skip = 1, t_enable = 0, n_samples = 0, t = 0;
@@ -201,6 +202,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int sites = h->M + 1;
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
+    if (h->disc != PIMC_DISC_RK4MAP) return no("the trapezoid discretisation runs on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
     if (T != 0 && (T % 64 != 0 || T > 512)) return no("threads_per_cta must be a multiple of 64, at most 512");
@@ -249,12 +251,12 @@ template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape*
 }
 
 template <class Model, typename R> int rebuild_cache(pimc_handle* h) {
-    const size_t total = (size_t)h->C * h->M;
+    const size_t total = (size_t)h->C * (h->M + 1);
     const int threads = 128;
     const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, 148 * 16);
     // after a rebuild, buffer 0 is current
     build_cache_kernel<Model, R><<<blocks, threads, 0, h->stream>>>((const R*)h->lay.x, h->have_I ? (const R*)h->lay.I : nullptr,
-                                                                     (const R*)h->lay.p, (R*)h->lay.g0, h->M, h->C, (R)h->dt);
+                                                                     (const R*)h->lay.p, (R*)h->lay.g0, h->M, h->C, (R)h->dt, h->disc);
     h->launches++;
     PIMC_CUDA(h, cudaGetLastError());
     PIMC_CUDA(h, cudaMemsetAsync(h->lay.cur, 0, sizeof(int) * h->C, h->stream));
@@ -271,6 +273,7 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     if (rc != PIMC_OK) return rc;
     SweepArgs<R> a{};
     a.M = h->M; a.L = h->L; a.n_chains = h->C; a.G = ls.G; a.tile = ls.tile; a.kind = h->kind;
+    a.disc = h->disc; a.nc = h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M;
     a.dt = (R)h->dt; a.Rm = (R)h->Rm;
     for (int c = 0; c < h->D; ++c) { a.Rf[c] = (R)h->Rf[c]; a.wx[c] = (R)h->wx[c]; }
     for (int l = 0; l < h->Np; ++l) a.wp[l] = h->wp[l];
@@ -454,11 +457,21 @@ int pimc_get_cache(pimc_handle* h, void* g_out) {
     std::vector<int> cur(h->C);
     PIMC_CUDA(h, cudaMemcpyAsync(cur.data(), h->lay.cur, sizeof(int) * h->C, cudaMemcpyDeviceToHost, h->stream));
     PIMC_CUDA(h, cudaStreamSynchronize(h->stream));
-    const size_t per = (size_t)h->M * h->D * es;
+    const size_t per = (size_t)(h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M) * h->D * es;
     for (int c = 0; c < h->C; ++c) {
         const char* src = (const char*)(cur[c] ? h->lay.g1 : h->lay.g0) + per * c;
         PIMC_CUDA(h, cudaMemcpyAsync((char*)g_out + per * c, src, per, cudaMemcpyDeviceToDevice, h->stream));
     }
+    return PIMC_OK;
+}
+
+int pimc_set_discretisation(pimc_handle* h, int disc) {
+    if (!h) return PIMC_EINVAL;
+    if (!(disc == PIMC_DISC_RK4MAP || disc == PIMC_DISC_TRAPEZOID)) return fail(h, PIMC_EINVAL, "unknown discretisation %d", disc);
+    if (disc == PIMC_DISC_TRAPEZOID && h->engine_user == PIMC_ENGINE_TILE)
+        return fail(h, PIMC_EUNSUPPORTED, "the trapezoid discretisation runs on the GLOBAL engine");
+    h->disc = disc;
+    if (h->have_path) return rebuild(h);
     return PIMC_OK;
 }
 

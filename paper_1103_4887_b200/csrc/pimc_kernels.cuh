@@ -31,11 +31,13 @@ constexpr int kMaxHistSel = 64;
 template <typename R> struct SweepArgs {
     // problem
     int M, L, n_chains, G, tile, kind;
+    int disc;             // model-error discretisation: 0 = explicit RK4 map, 1 = trapezoid rule (Eq. 7)
+    int nc;               // cache entries per chain: M (disc 0: g_n, n <= M-1) or M + 1 (disc 1: c_n = (dt/2) F(x_n), n <= M)
     R dt, Rm, Rf[kMaxD], wx[kMaxD];
     double wp[kMaxNp];
     // device state (per chain, chains concatenated)
     R* x;                 // (C, M+1, D)
-    R* g[2];              // (C, M, D) x 2: step-increment caches (ping-pong)
+    R* g[2];              // (C, nc, D) x 2: step caches (ping-pong)
     const R* y;           // (C, M+1, L)
     const R* I;           // (C, M+1) or nullptr
     R* p;                 // (C, Np)
@@ -172,6 +174,44 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
     load_vec<R, D>(x, n, xn);
     propose_state<R, D>(a, t, chain, (uint32_t)n, xn, xp);
     R dL = R(0), dR = R(0);     // left part (term n-1 -> n and measurement n) and right part (term n -> n+1), summed separately
+    if (a.disc == 1) {
+        // trapezoid rule, Fig. 1 (b)-(f) as printed: c' = (dt/2) F(x'_n) enters BOTH neighbouring terms; every residual is
+        // (x_{k+1} - x_k) - c_k - c_{k+1}
+        R cn[D];
+        load_vec<R, D>(g, n, cn);
+        const R I0 = I ? __ldg(I + n) : R(0);
+        Model::half_rhs(xp, prm, Model::prepare(prm, a.dt), I0, gp);
+        if (n >= 1) {
+            R xm[D], cm[D];
+            load_vec<R, D>(x, n - 1, xm);
+            load_vec<R, D>(g, n - 1, cm);
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                const R r_new = ((xp[c] - xm[c]) - cm[c]) - gp[c];
+                const R r_old = ((xn[c] - xm[c]) - cm[c]) - cn[c];
+                dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+            }
+#pragma unroll
+            for (int l = 0; l < D; ++l) {
+                if (l < a.L) {
+                    const R yn = __ldg(y + (size_t)n * a.L + l);
+                    const R d_new = yn - xp[l], d_old = yn - xn[l];
+                    dL += R(0.5) * a.Rm * (d_new * d_new - d_old * d_old);
+                }
+            }
+        }
+        if (n <= M - 1) {
+            R xq[D], cq[D];
+            load_vec<R, D>(x, n + 1, xq);
+            load_vec<R, D>(g, n + 1, cq);
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                const R r_new = ((xq[c] - xp[c]) - gp[c]) - cq[c];
+                const R r_old = ((xq[c] - xn[c]) - cn[c]) - cq[c];
+                dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+            }
+        }
+    } else {
     if (n >= 1) {
         R xm[D], gm[D];
         load_vec<R, D>(x, n - 1, xm);
@@ -204,12 +244,13 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
             dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
         }
     }
+    }
     const R dA = dL + dR;
     const R logu = log_accept_uniform<R>(a, t, chain, (uint32_t)n);
     const bool accept = logu < -dA;      // NaN or +inf rejects; dA <= 0 always accepts
     if (accept) {
         store_vec<R, D>(x, n, xp);
-        if (n <= M - 1) store_vec<R, D>(g, n, gp);
+        if (n < a.nc) store_vec<R, D>(g, n, gp);
     }
     if (trace) {
         const size_t gs = chain_site0 + (size_t)n;
@@ -240,8 +281,8 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     const size_t site0 = (size_t)chain * (M + 1);
 
     R* x = a.x + site0 * D;
-    R* const g_a = a.g[0] + (size_t)chain * M * D;
-    R* const g_b = a.g[1] + (size_t)chain * M * D;
+    R* const g_a = a.g[0] + (size_t)chain * a.nc * D;
+    R* const g_b = a.g[1] + (size_t)chain * a.nc * D;
     const R* y = a.y + site0 * a.L;
     const R* I = a.I ? a.I + site0 : nullptr;
     unsigned long long* hs_flag = a.hs_flag + (size_t)chain * G;
@@ -307,6 +348,30 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     R* galt = cur ? g_a : g_b;
                     double part = 0.0;
                     const int e_fwd = min(e, M);
+                    if (a.disc == 1) {
+                        // trapezoid rule: term n -> n+1 needs c'_n and c'_{n+1}; the thread of site n evaluates both (the field is
+                        // one right-hand side, a quarter of an RK4 step) and stores c'_n (and c'_M with the last term)
+                        const typename Model::Prep pq = Model::prepare(ps_prop, a.dt);
+                        for (int n = s + tid; n < e_fwd; n += T) {
+                            R xn[D], xq[D], cn[D], cq[D], cpn[D], cpq[D];
+                            load_vec<R, D>(x, n, xn);
+                            load_vec<R, D>(x, n + 1, xq);
+                            load_vec<R, D>(gcur, n, cn);
+                            load_vec<R, D>(gcur, n + 1, cq);
+                            Model::half_rhs(xn, ps_prop, pq, I ? __ldg(I + n) : R(0), cpn);
+                            Model::half_rhs(xq, ps_prop, pq, I ? __ldg(I + n + 1) : R(0), cpq);
+                            store_vec<R, D>(galt, n, cpn);
+                            if (n + 1 == M) store_vec<R, D>(galt, n + 1, cpq);
+                            R acc = R(0);
+#pragma unroll
+                            for (int c = 0; c < D; ++c) {
+                                const R d = xq[c] - xn[c];
+                                const R r_new = (d - cpn[c]) - cpq[c], r_old = (d - cn[c]) - cq[c];
+                                acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            }
+                            part += (double)acc;
+                        }
+                    } else
                     for (int n = s + tid; n < e_fwd; n += T) {
                         R xn[D], xq[D], gn[D], gp[D];
                         load_vec<R, D>(x, n, xn);
@@ -433,21 +498,23 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
 // ---- A0: (re)build the step cache of every chain ---------------------------------------------------------
 template <class Model, typename R>
 __global__ void build_cache_kernel(const R* __restrict__ x, const R* __restrict__ I, const R* __restrict__ p, R* __restrict__ g,
-                                   int M, int n_chains, R dt) {
+                                   int M, int n_chains, R dt, int disc) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
-    const size_t total = (size_t)n_chains * M;
+    const int nc = disc == 1 ? M + 1 : M;          // entries per chain
+    const size_t total = (size_t)n_chains * nc;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
-        const size_t chain = idx / M;
-        const int n = (int)(idx % M);
+        const size_t chain = idx / nc;
+        const int n = (int)(idx % nc);
         const R* prm = p + chain * NP;
         R xn[D], gn[D];
 #pragma unroll
         for (int c = 0; c < D; ++c) xn[c] = x[(chain * (M + 1) + n) * D + c];
-        const R I0 = I ? I[chain * (M + 1) + n] : R(0), I1 = I ? I[chain * (M + 1) + n + 1] : R(0);
-        Model::increment(xn, prm, I0, I1, dt, gn);
+        const R I0 = I ? I[chain * (M + 1) + n] : R(0), I1 = (I && n < M) ? I[chain * (M + 1) + n + 1] : R(0);
+        if (disc == 1) Model::half_rhs(xn, prm, Model::prepare(prm, dt), I0, gn);
+        else Model::increment(xn, prm, I0, I1, dt, gn);
 #pragma unroll
-        for (int c = 0; c < D; ++c) g[(chain * M + n) * D + c] = gn[c];
+        for (int c = 0; c < D; ++c) g[(chain * nc + n) * D + c] = gn[c];
     }
 }
 

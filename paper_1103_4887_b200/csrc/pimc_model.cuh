@@ -120,6 +120,18 @@ template <typename R> struct HHModel {
     static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
         increment(x, p, prepare(p, dt), I0, I1, dt, g);
     }
+    // Trapezoid discretisation (Eq. 7): the cached quantity is c = (dt/2) F(x, p; I)
+    static __device__ __forceinline__ void half_rhs(const R x[4], const R* __restrict__ p, const Prep& q, R I, R c[4]) {
+        R F[4];
+        rhs(x, p, q.inv_C, I, F);
+        bool sane = true;
+        if constexpr (sizeof(R) == 8) sane = fabs(x[0]) < 1e8;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            c[a] = q.hdt * F[a];
+            if constexpr (sizeof(R) == 8) c[a] = sane ? c[a] : __longlong_as_double(0x7FF8000000000000ll);
+        }
+    }
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -128,6 +140,16 @@ template <typename R, int D_> struct LinearModel {
     static constexpr int NP = D_ * D_;
     struct Prep {};
     static __device__ __forceinline__ Prep prepare(const R* __restrict__, R) { return Prep{}; }
+    // Trapezoid form of the linear model: F(x) = (A x - x)/dt, so c = (dt/2) F = (A x - x)/2
+    static __device__ __forceinline__ void half_rhs(const R x[D_], const R* __restrict__ p, const Prep&, R, R c[D_]) {
+#pragma unroll
+        for (int a = 0; a < D_; ++a) {
+            R f = R(0);
+#pragma unroll
+            for (int b = 0; b < D_; ++b) f += p[a * D_ + b] * x[b];
+            c[a] = R(0.5) * (f - x[a]);
+        }
+    }
     static constexpr int NK = 0;                   // nothing parameter-independent worth caching
     static __device__ __forceinline__ void stage1_cache(const R*, R*) {}
     template <bool IN, bool OUT>

@@ -214,8 +214,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     const bool edge_lo = s_ext == 0, edge_hi = e_ext == M + 1;
 
     R* const gx = a.x + site0 * D;
-    R* const gg0 = a.g[0] + (size_t)chain * M * D;
-    R* const gg1 = a.g[1] + (size_t)chain * M * D;
+    R* const gg0 = a.g[0] + (size_t)chain * a.nc * D;     // this engine runs the RK4-map discretisation only: nc == M
+    R* const gg1 = a.g[1] + (size_t)chain * a.nc * D;
     int cur = a.cur[chain];
 
     // ---- load the extended tile (site-major in global memory -> parity planes in shared memory) ----

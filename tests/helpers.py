@@ -10,19 +10,23 @@ TOL32 = 1e-5       # fp32
 TIE64 = 1e-9       # near-tie window |dA + log u|
 
 
-def gpu_handle(w, dtype=64, with_params=True, launch=None, kind=0):
+def gpu_handle(w, dtype=64, with_params=True, launch=None, kind=0, disc=0):
     import paper_1103_4887_b200 as P
     h = P.Pimc.from_workload(w, dtype=dtype, with_params=with_params)
+    if disc:
+        h.set_discretisation(disc)
     h.set_proposal(w.w_state, w.w_param if with_params else None, kind)
     if launch:
         h.set_launch(*launch)
     return h
 
 
-def oracle_chains(w, state_dtype=64, with_params=True, kind=0):
+def oracle_chains(w, state_dtype=64, with_params=True, kind=0, disc=0):
     out = []
     for c in range(w.n_chains):
         o = OracleChain.from_workload(w, chain=c, state_dtype=state_dtype, with_params=with_params)
+        if disc:
+            o.set_discretisation(disc)
         o.set_proposal(w.w_state, w.w_param if with_params else None, kind)
         out.append(o)
     return out
@@ -38,7 +42,7 @@ def ulp_diff(a, b):
     return np.abs(a - b) / np.maximum(np.spacing(np.maximum(np.abs(a), np.abs(b))), 1e-300)
 
 
-def teacher_forced(w, h, orcs, n_sweeps, seed, tol=TOL64, tie=TIE64, do_params=True, state_dtype=64):
+def teacher_forced(w, h, orcs, n_sweeps, seed, tol=TOL64, tie=TIE64, do_params=True, state_dtype=64, disc=0):
     """SURVEY.md §8(c) T1.  For every sweep: force the GPU to the oracle's state, run one sweep on both with the
     trace on, and compare per-site Delta-A (evaluated by the oracle AT THE GPU's proposals, on the path as it stood
     when the site was visited), decisions, parameter moves and the resulting path.  Returns a report dict."""
@@ -47,6 +51,9 @@ def teacher_forced(w, h, orcs, n_sweeps, seed, tol=TOL64, tie=TIE64, do_params=T
     rep = dict(sites=0, max_rel=0.0, ties=0, mismatch_outside_window=0, max_xprop_ulp=0.0, max_param_rel=0.0, param_ties=0,
                param_moves=0, max_path_diff=0.0, accepted=0)
     helper = [OracleChain.from_workload(w, chain=c, state_dtype=state_dtype, with_params=do_params) for c in range(C)]
+    for hc in helper:
+        if disc:
+            hc.set_discretisation(disc)
     for t in range(n_sweeps):
         X = np.stack([o.get_path()[0] for o in orcs]); Pp = np.stack([o.get_path()[1] for o in orcs])
         h.set_params(to_dev(Pp, h)); h.set_path(to_dev(X, h))

@@ -1,0 +1,105 @@
+"""GPU parity for the paper's trapezoid discretisation (PIMC_DISC_TRAPEZOID; Eq. 7)
+against the oracle's set_discretisation(1): teacher-forced per-site and parameter Delta-A, free-running bit-identical
+chains with uniform proposals, cache coherence (c_n = (dt/2) F(x_n), n = 0..M), batched chains, fp32, edge sizes."""
+import numpy as np
+import pytest
+
+from helpers import TOL32, TOL64, gpu_handle, oracle_chains, teacher_forced
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+TRAP = 1
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    import paper_1103_4887_b200 as P
+    assert torch.cuda.is_available()
+    P.lib()
+    return P
+
+
+CASES = [
+    ("cfg0_M256_auto", 0, 256, None, False, 40),
+    ("cfg0_M257_3ctas", 0, 257, (3, 32), False, 20),
+    ("cfg2_M600_auto", 2, 600, None, True, 40),
+    ("cfg2_M601_5ctas", 2, 601, (5, 64), True, 20),
+    ("cfg2_M333_1cta", 2, 333, (1, 96), True, 20),
+    ("cfg1_M999_7ctas", 1, 999, (7, 32), False, 20),
+]
+
+
+@pytest.mark.parametrize("name,cfg,M,launch,with_params,n_sweeps", CASES, ids=[c[0] for c in CASES])
+def test_teacher_forced_parity_trapezoid(P, name, cfg, M, launch, with_params, n_sweeps):
+    w = make_workload(cfg, M=M)
+    h = gpu_handle(w, with_params=with_params, launch=launch, disc=TRAP)
+    assert h.get_engine()["engine"] == P.ENGINE_GLOBAL
+    orcs = oracle_chains(w, with_params=with_params, disc=TRAP)
+    rep = teacher_forced(w, h, orcs, n_sweeps, seed=20110347, do_params=with_params, disc=TRAP)
+    print(name, h.get_launch(), rep)
+    assert rep["sites"] == n_sweeps * (M + 1)
+    assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0 and rep["ties"] <= 2, rep
+    assert rep["max_xprop_ulp"] <= 4.0 and rep["accepted"] > 0, rep
+    if with_params:
+        assert rep["param_moves"] > 0 and rep["max_param_rel"] <= TOL64, rep
+    assert rep["max_path_diff"] <= 1e-12
+
+
+@pytest.mark.parametrize("cfg,M,launch", [(0, 256, None), (2, 500, (4, 64)), (1, 700, (3, 128)), (3, 4001, None)])
+def test_free_running_uniform_bit_identical_trapezoid(P, cfg, M, launch):
+    w = make_workload(cfg, M=M)
+    h = gpu_handle(w, launch=launch, kind=1, disc=TRAP)
+    o = oracle_chains(w, kind=1, disc=TRAP)[0]
+    h.set_accum(True, 2); o.set_accum(True, 2)
+    h.reset_moments(); o.reset_moments()
+    h.sweep(60, seed=5); o.sweep(60, seed=5)
+    xg, pg = [a.cpu().numpy() for a in h.get_path()]
+    xo, po = o.get_path()
+    assert np.array_equal(xg[0], xo), np.abs(xg[0] - xo).max()
+    assert np.array_equal(pg[0], po)
+    assert np.array_equal(h.stats().cpu().numpy()[0].astype(np.uint64), o.stats())
+    mx, mp, n = h.moments()
+    ox, op, on = o.moments()
+    assert n == on == 30
+    assert np.allclose(mx.cpu().numpy()[0], ox, rtol=1e-13, atol=1e-13)
+    # cache coherence on the device: c_n = (dt/2) F(x_n, p; I_n) for n = 0..M, against the oracle's recomputation
+    g = h.get_cache().cpu().numpy()[0]
+    og = o.get_cache()
+    assert g.shape == og.shape == (M + 1, w.D)
+    # (the gate rates (a_inf - a)/tau cancel, so the error is relative to the scale of the terms: (dt/2) x (100 mV/ms, 1/ms))
+    scale = np.maximum(np.abs(og), 0.5 * w.dt * (np.array([100.0, 1.0, 1.0, 1.0]) if w.D == 4 else np.ones(w.D)))
+    assert np.max(np.abs(g - og) / scale) < 1e-13
+
+
+def test_batched_chains_and_fp32_trapezoid(P):
+    w = make_workload(4, M=300, n_chains=5)
+    h = gpu_handle(w, launch=(1, 64), disc=TRAP)
+    rep = teacher_forced(w, h, oracle_chains(w, disc=TRAP), 15, seed=99, disc=TRAP)
+    assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0 and rep["max_param_rel"] <= TOL64, rep
+    w = make_workload(2, M=600)
+    h = gpu_handle(w, dtype=32, disc=TRAP)
+    rep = teacher_forced(w, h, oracle_chains(w, state_dtype=32, disc=TRAP), 15, seed=3, tol=TOL32, state_dtype=32, disc=TRAP)
+    assert rep["max_rel"] <= TOL32 and rep["mismatch_outside_window"] == 0, rep
+
+
+def test_edge_sizes_switching_and_engine_rule_trapezoid(P):
+    import paper_1103_4887_b200 as Pm
+    for M in (1, 2, 5):
+        w = make_workload(0, M=M)
+        h = gpu_handle(w, with_params=False, disc=TRAP)
+        rep = teacher_forced(w, h, oracle_chains(w, with_params=False, disc=TRAP), 10, seed=3, do_params=False, disc=TRAP)
+        assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0, (M, rep)
+    # switching the discretisation on a live handle rebuilds the cache; the TILE engine refuses the trapezoid form
+    w = make_workload(2, M=300)
+    h = gpu_handle(w)
+    h.sweep(3, seed=1)
+    h.set_discretisation(Pm.DISC_TRAPEZOID)
+    assert h.get_cache().shape == (1, 301, 4) and h.get_engine()["engine"] == Pm.ENGINE_GLOBAL
+    with pytest.raises(Pm.PimcError):
+        h.set_engine(Pm.ENGINE_TILE)
+    h.sweep(3, seed=1)
+    h.set_discretisation(Pm.DISC_RK4MAP)
+    assert h.get_cache().shape == (1, 300, 4)
+    with pytest.raises(Pm.PimcError):
+        h.set_discretisation(7)
