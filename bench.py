@@ -31,6 +31,10 @@ UNIT = "site-updates/s"
 # (1 slot = one FMA/ADD/MUL lane-operation = 2 FLOP at peak) per joint site-update and per parameter-move model evaluation.
 W_SITE_SLOTS = 800.0
 W_EVAL_SLOTS = 560.0
+# trapezoid discretisation (--disc trapezoid, the paper's own rule): one right-hand side per proposal instead of four
+# (108 + Delta-A 97 + RNG 175), one per parameter-move evaluation (108 + 32)
+W_SITE_SLOTS_TRAP = 380.0
+W_EVAL_SLOTS_TRAP = 140.0
 # FP64 peak derived from unit counts and clocks: 148 SMs x 64 FP64 lanes/clk/SM x 1.965 GHz, 2 FLOP per lane-FMA.
 FP64_LANES_PER_SM_CLK = 64
 SM_COUNT = 148
@@ -83,10 +87,12 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def oracle_rate(w, budget_s, chain=0):
+def oracle_rate(w, budget_s, chain=0, disc=0):
     """Time the CPU oracle, as it stands, on a bounded sample of the same workload.  Returns (site-updates/s, sweeps, seconds)."""
     from oracle import OracleChain
     o = OracleChain.from_workload(w, chain=chain)
+    if disc:
+        o.set_discretisation(disc)
     t0 = time.perf_counter()
     o.sweep(2, seed=w.chain_seed)                       # warm-up + first estimate
     per = (time.perf_counter() - t0) / 2
@@ -118,7 +124,7 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": w.name, "M": w.M, "n_chains": 1, "sweeps_per_step": n_per_step},
+        "data": "synthetic", "config": {"workload": w.name + ("_trapezoid" if trap else ""), "discretisation": args.disc, "M": w.M, "n_chains": 1, "sweeps_per_step": n_per_step},
         "sweeps_per_s": n_per_step * args.steps / dt,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -157,6 +163,10 @@ def run_ours(args):
     seed = w.chain_seed + rank
     S = args.sweeps_per_step
     h = P.Pimc.from_workload(w, dtype=args.dtype)
+    trap = args.disc == "trapezoid"
+    if trap:
+        h.set_discretisation(P.DISC_TRAPEZOID)
+    w_site, w_eval = (W_SITE_SLOTS_TRAP, W_EVAL_SLOTS_TRAP) if trap else (W_SITE_SLOTS, W_EVAL_SLOTS)
     peak_tflops = PEAK_TFLOPS_DERIVED * (1.0 if args.dtype == 64 else 2.0)   # fp32: 128 FP32 lanes/clk/SM
     h.set_accum(True, 1)
     h.reset_moments()
@@ -208,26 +218,26 @@ def run_ours(args):
     a4_rate, a4_ms = (rate(h.sweep_params_only, evals_per_step) if n_active else (0.0, 0.0))
 
     # roofline of the dominant (only) kernel of the step: the persistent sweep kernel
-    slots_per_launch = units_per_step * W_SITE_SLOTS + evals_per_step * W_EVAL_SLOTS
+    slots_per_launch = units_per_step * w_site + evals_per_step * w_eval
     achieved_tflops = 2.0 * slots_per_launch / (float(np.mean(step_ms)) * 1e-3) / 1e12
     measured_peak = P.fp64_peak(150) * 2 / 1e12 if rank == 0 else None
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved_tflops / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == 3 and args.dtype == 64) else None,
+                "frac": achieved_tflops / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == 3 and args.dtype == 64 and not trap) else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r01_v5_tile_engine_stage1_cache.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
                 "peak_measured_dfma_tflops": measured_peak,
                 "frac_of_measured_dfma": (achieved_tflops / measured_peak) if measured_peak else None,
                 "kernel": "pimc::tile_sweep_kernel<HHModel<double>,double,256>" if shape.get("smem_bytes", 0) else "pimc::sweep_kernel<HHModel<double>,double>",
-                "work_model": {"slots_per_site_update": W_SITE_SLOTS, "slots_per_param_eval": W_EVAL_SLOTS,
+                "work_model": {"slots_per_site_update": w_site, "slots_per_param_eval": w_eval,
                                "site_updates_per_launch": units_per_step, "param_evals_per_launch": evals_per_step},
                 "a2_only": {"site_updates_per_s": a2_rate, "ms_per_launch": a2_ms,
-                            "frac": 2 * a2_rate * W_SITE_SLOTS / 1e12 / peak_tflops},
+                            "frac": 2 * a2_rate * w_site / 1e12 / peak_tflops},
                 "a4_only": {"param_evals_per_s": a4_rate, "ms_per_launch": a4_ms,
-                            "frac": 2 * a4_rate * W_EVAL_SLOTS / 1e12 / peak_tflops}}
+                            "frac": 2 * a4_rate * w_eval / 1e12 / peak_tflops}}
 
     # end to end through the C ABI on HOST buffers: H2D of y, I, x0, p0 + sweeps + D2H of the moments inside the timed region
     e2e = None
-    if rank == 0 or world > 1:
+    if (rank == 0 or world > 1) and not trap:     # pimc_run_host is the RK4-map convenience call
         P.run_host(w, 0, max(1, S // 10), seed, dtype=args.dtype)         # warm-up (context, allocator)
         reps = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
@@ -239,14 +249,14 @@ def run_ours(args):
                "ms_per_step": s_e2e / reps * 1e3, "call": "pimc_run_host (cudaMalloc + H2D + pimc_sweep + pimc_moments + D2H + sync)"}
 
     if rank == 0:
-        cpu_rate, cpu_n, cpu_s = oracle_rate(w, args.cpu_budget)
+        cpu_rate, cpu_n, cpu_s = oracle_rate(w, args.cpu_budget, disc=1 if trap else 0)
         cpu = {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{cpu_n} full sweeps of chain 0 of {w.name} in {cpu_s:.1f} s (serial fp64 C++ -O2, {os.cpu_count()} cores present)"}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.dtype == 64 else "f32",
             "data": "synthetic",
-            "config": {"workload": w.name, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
+            "config": {"workload": w.name + ("_trapezoid" if trap else ""), "discretisation": args.disc, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
                        "accumulate_every": 1, "launch": shape, "l2": "flushed between timed steps (256 MiB fill)",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "sweeps_per_s": value / (w.M + 1),
@@ -266,6 +276,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--disc", default="rk4", choices=["rk4", "trapezoid"], help="model-error discretisation: the north_star's RK4 map or the paper's trapezoid rule")
     ap.add_argument("--dtype", type=int, default=64, choices=[64, 32], help="arithmetic type of the path (config 3 is also quoted in fp32)")
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
