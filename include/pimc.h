@@ -59,7 +59,7 @@ enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2 };
  *  TRAPEZOID (the paper's own rule, Eq. 7): r = x_{n+1} - x_n - (dt/2)[F(x_{n+1}) + F(x_n)], F the model's
  *            vector field with the current I_n at step n (LINEAR: F(x) = (A x - x)/dt); the cache holds
  *            c_n = (dt/2) F(x_n), n = 0..M (PAPER.md:189, 242 caches F_n).  One right-hand side per proposal instead of
- *            four.  Runs on the GLOBAL engine (PIMC_EUNSUPPORTED if the TILE engine is forced). */
+ *            four.  Both engines support both discretisations. */
 enum { PIMC_DISC_RK4MAP = 0, PIMC_DISC_TRAPEZOID = 1 };
 
 /* Number of parameters the model defines (HH: 7, LINEAR: D*D); negative on bad arguments. */

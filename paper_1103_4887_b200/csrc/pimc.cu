@@ -202,7 +202,6 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int sites = h->M + 1;
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
-    if (h->disc != PIMC_DISC_RK4MAP) return no("the trapezoid discretisation runs on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
     if (T != 0 && (T % 64 != 0 || T > 512)) return no("threads_per_cta must be a multiple of 64, at most 512");
@@ -238,7 +237,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     if (T == 0) T = std::max(64, (tile + 2 * hh + 63) / 64 * 64);
     if (tile + 2 * hh > T || T > 512) return no("tile plus halos does not fit the CTA");
     out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1; out->engine = PIMC_ENGINE_TILE; out->h = hh;
-    out->smem = tile_smem_bytes<R>(T, h->D, h->L, Model::NK);
+    out->smem = tile_smem_bytes<R>(T, h->D, h->L, h->disc == PIMC_DISC_TRAPEZOID ? 0 : Model::NK);
     if (out->smem > 227 * 1024) return no("shared memory");
     return PIMC_OK;
 }
@@ -293,9 +292,12 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault;
 
     const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
-    const void* fn = ls.engine == PIMC_ENGINE_TILE
-                         ? (ls.T <= 256 ? (const void*)tile_sweep_kernel<Model, R, 256> : (const void*)tile_sweep_kernel<Model, R, 512>)
-                         : (const void*)sweep_kernel<Model, R>;
+    const bool trap = h->disc == PIMC_DISC_TRAPEZOID;
+    const void* fn = (const void*)sweep_kernel<Model, R>;
+    if (ls.engine == PIMC_ENGINE_TILE) {
+        if (ls.T <= 256) fn = trap ? (const void*)tile_sweep_kernel<Model, R, 256, true> : (const void*)tile_sweep_kernel<Model, R, 256, false>;
+        else fn = trap ? (const void*)tile_sweep_kernel<Model, R, 512, true> : (const void*)tile_sweep_kernel<Model, R, 512, false>;
+    }
     if (ls.smem > 48 * 1024) PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
     void* params[] = {&a};
     if (ls.cooperative) PIMC_CUDA(h, cudaLaunchCooperativeKernel(fn, grid, block, params, ls.smem, h->stream));
@@ -468,8 +470,6 @@ int pimc_get_cache(pimc_handle* h, void* g_out) {
 int pimc_set_discretisation(pimc_handle* h, int disc) {
     if (!h) return PIMC_EINVAL;
     if (!(disc == PIMC_DISC_RK4MAP || disc == PIMC_DISC_TRAPEZOID)) return fail(h, PIMC_EINVAL, "unknown discretisation %d", disc);
-    if (disc == PIMC_DISC_TRAPEZOID && h->engine_user == PIMC_ENGINE_TILE)
-        return fail(h, PIMC_EUNSUPPORTED, "the trapezoid discretisation runs on the GLOBAL engine");
     h->disc = disc;
     if (h->have_path) return rebuild(h);
     return PIMC_OK;

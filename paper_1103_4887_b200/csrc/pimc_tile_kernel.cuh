@@ -194,13 +194,15 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
 
 
 // ---- the kernel ----------------------------------------------------------------------------------------------
-template <class Model, typename R, int MAXT>
+// TRAP selects the paper's trapezoid discretisation (Eq. 7): the cache holds c_n = (dt/2) F(x_n) for n = 0..M,
+// every residual is (x_{k+1} - x_k) - c_k - c_{k+1}, the model step is ONE right-hand side, and there is no stage-1 cache.
+template <class Model, typename R, int MAXT, bool TRAP>
 __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
     extern __shared__ __align__(16) unsigned char tile_smem_raw[];
     const int T = blockDim.x, TC = T >> 1, tid = threadIdx.x;
-    constexpr int NK = Model::NK;
+    constexpr int NK = TRAP ? 0 : Model::NK;
     const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK);
     constexpr int RP = MAXT / 2;                   // pitch of the random-number ring
     constexpr int P = MAXT / 2 + 2;                // == tile_pitch(T): the launcher picks MAXT = 256 for T <= 256, else 512
@@ -223,7 +225,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     {
         const R* gsrc = cur ? gg1 : gg0;
         R* gdst = cur ? sm.g1 : sm.g0;
-        const int ng = min(e_ext, M) - s_ext;      // cache entries exist for n <= M-1
+        const int ng = min(e_ext, TRAP ? M + 1 : M) - s_ext;      // cache entries exist for n <= M-1 (trapezoid: n <= M)
         for (int idx = tid; idx < ng * D; idx += T) gdst[so<D>(idx / D, idx % D, P)] = gsrc[(size_t)s_ext * D + idx];
     }
     for (int i = tid; i <= n_ext; i += T) {
@@ -327,6 +329,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         const int own = q * D * P + tid, oth = (1 - q) * D * P;
                         const R* ring = sm.rstep + (size_t)(set * 2 + q) * D * RP + tid;
                         R xn[D], xp[D], gp[D], xm[D], gm[D], xq[D], gn[D];
+                        [[maybe_unused]] R gq[D];          // trapezoid: the right neighbour's cache entry c_{n+1}
                         double mc[D], m1[D], m2[D];
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
@@ -340,18 +343,21 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         for (int c = 0; c < D; ++c) {
                             xm[c] = sm.xs[oth + c * P + jl]; gm[c] = gc[oth + c * P + jl];
                             xq[c] = sm.xs[oth + c * P + jr]; gn[c] = gc[own + c * P];
+                            if constexpr (TRAP) gq[c] = gc[oth + c * P + jr];
                             mc[c] = sm.cc[own + c * P]; m1[c] = sm.S1[own + c * P]; m2[c] = sm.S2[own + c * P];
                         }
                         const R logu = sm.rlogu[(size_t)(set * 2 + q) * RP + tid];
                         R kgo[NK > 0 ? NK : 1], kgn[NK > 0 ? NK : 1];
 #pragma unroll
                         for (int c = 0; c < NK; ++c) kgo[c] = sm.kg[(q * NK + c) * P + tid];
-                        Model::template increment_k<false, true>(xp, prm, prep, I0, I1, a.dt, gp, nullptr, kgn);
+                        if constexpr (TRAP) Model::half_rhs(xp, prm, prep, I0, gp);                      // c' = (dt/2) F(x'_n)
+                        else Model::template increment_k<false, true>(xp, prm, prep, I0, I1, a.dt, gp, nullptr, kgn);
                         R dL = R(0), dR = R(0);
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
-                            const R r_new = (xp[c] - xm[c]) - gm[c];
-                            const R r_old = (xn[c] - xm[c]) - gm[c];
+                            R r_new = (xp[c] - xm[c]) - gm[c];
+                            R r_old = (xn[c] - xm[c]) - gm[c];
+                            if constexpr (TRAP) { r_new -= gp[c]; r_old -= gn[c]; }
                             dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
                         }
 #pragma unroll
@@ -364,13 +370,14 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         }
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
-                            const R r_new = (xq[c] - xp[c]) - gp[c];
-                            const R r_old = (xq[c] - xn[c]) - gn[c];
+                            R r_new = (xq[c] - xp[c]) - gp[c];
+                            R r_old = (xq[c] - xn[c]) - gn[c];
+                            if constexpr (TRAP) { r_new -= gq[c]; r_old -= gq[c]; }
                             dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
                         }
                         const R dA = (has_l ? dL : R(0)) + (has_r ? dR : R(0));
                         const bool accept = logu < -dA;
-                        const bool keep_g = accept && has_r;
+                        const bool keep_g = accept && (TRAP || has_r);     // trapezoid: site M has a cache entry too
 #pragma unroll
                         for (int c = 0; c < NK; ++c) sm.kg[(q * NK + c) * P + tid] = accept ? kgn[c] : kgo[c];
                         // unconditional stores of selected values: no divergent branch in the tail of the update
@@ -406,7 +413,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         // ---------------- A4: parameter moves, in sequence; one tile site per thread ----------------
         if (a.do_params) {
             const int n = s_ext + prm_iloc;
-            const bool can_eval = prm_iloc < n_ext && n <= M - 1;
+            const bool can_eval = prm_iloc < n_ext && n <= (TRAP ? M : M - 1);
             const bool owned = n >= s && n < e && n <= M - 1;
             bool params_changed = false;
 #pragma unroll 1
@@ -432,20 +439,45 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     if (can_eval) {
                         R xn[D], gp[D];
                         lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
-                        R kk[NK > 0 ? NK : 1];
+                        if constexpr (TRAP) {
+                            Model::half_rhs(xn, pp, Model::prepare(pp, a.dt), sm.Is[prm_iloc], gp);
+                            sts_site<R, D>(ga, prm_q, prm_j, P, gp);
+                        } else {
+                            R kk[NK > 0 ? NK : 1];
 #pragma unroll
-                        for (int c = 0; c < NK; ++c) kk[c] = sm.kg[(prm_q * NK + c) * P + prm_j];
-                        Model::template increment_k<(NK > 0), false>(xn, pp, Model::prepare(pp, a.dt), sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp, kk, nullptr);
-                        sts_site<R, D>(ga, prm_q, prm_j, P, gp);
+                            for (int c = 0; c < NK; ++c) kk[c] = sm.kg[(prm_q * NK + c) * P + prm_j];
+                            Model::template increment_k<(NK > 0), false>(xn, pp, Model::prepare(pp, a.dt), sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp, kk, nullptr);
+                            sts_site<R, D>(ga, prm_q, prm_j, P, gp);
+                            if (owned) {
+                                R xq[D], gn[D];
+                                lds_site<R, D>(sm.xs, 1 - prm_q, prm_j + prm_q, P, xq);
+                                lds_site<R, D>(gc, prm_q, prm_j, P, gn);
+                                R acc = R(0);
+#pragma unroll
+                                for (int c = 0; c < D; ++c) {
+                                    const R d = xq[c] - xn[c];
+                                    const R r_new = d - gp[c], r_old = d - gn[c];
+                                    acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                                }
+                                part = (double)acc;
+                            }
+                        }
+                    }
+                    if constexpr (TRAP) {      // term n -> n+1 needs the NEIGHBOUR's new entry c'_{n+1} as well: one more barrier
+                        __syncthreads();
                         if (owned) {
-                            R xq[D], gn[D];
+                            R xn[D], xq[D], cn[D], cq[D], cpn[D], cpq[D];
+                            lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
                             lds_site<R, D>(sm.xs, 1 - prm_q, prm_j + prm_q, P, xq);
-                            lds_site<R, D>(gc, prm_q, prm_j, P, gn);
+                            lds_site<R, D>(gc, prm_q, prm_j, P, cn);
+                            lds_site<R, D>(gc, 1 - prm_q, prm_j + prm_q, P, cq);
+                            lds_site<R, D>(ga, prm_q, prm_j, P, cpn);
+                            lds_site<R, D>(ga, 1 - prm_q, prm_j + prm_q, P, cpq);
                             R acc = R(0);
 #pragma unroll
                             for (int c = 0; c < D; ++c) {
                                 const R d = xq[c] - xn[c];
-                                const R r_new = d - gp[c], r_old = d - gn[c];
+                                const R r_new = (d - cpn[c]) - cpq[c], r_old = (d - cn[c]) - cq[c];
                                 acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
                             }
                             part = (double)acc;
@@ -511,7 +543,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 const int widx = so<D>(nsite - s_ext, cw / WPV, P) * WPV + cw % WPV;
                 uint32_t payload = 0;
                 if (which == 0) payload = xs32[widx];
-                else if (nsite <= M - 1) payload = gc32[widx];
+                else if (nsite <= (TRAP ? M : M - 1)) payload = gc32[widx];
                 const int dst_cta = (int)blockIdx.x + (dir == 0 ? -1 : 1);
                 const int dst_side = dir == 0 ? 1 : 0;           // my left neighbour receives "from its right"
                 unsigned long long* box = a.hx_words + (((size_t)dst_cta * 2 + dst_side) * 2 + slot) * (size_t)kHaloWordsPerSide;
@@ -530,7 +562,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 const unsigned long long* box = a.hx_words + (((size_t)blockIdx.x * 2 + side) * 2 + slot) * (size_t)kHaloWordsPerSide;
                 const uint32_t payload = ll_wait(box + q, tag, a.fault);
                 if (which == 0) xd32[widx] = payload;
-                else if (nsite <= M - 1) gd32[widx] = payload;
+                else if (nsite <= (TRAP ? M : M - 1)) gd32[widx] = payload;
             }
             hx_count += 1ull;
             k_phase = 0;
@@ -591,7 +623,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     {
         R* gdst = cur ? gg1 : gg0;
         const R* gsrc = cur ? sm.g1 : sm.g0;
-        const int hi_g = min(e, M);
+        const int hi_g = min(e, TRAP ? M + 1 : M);
         for (int idx = (s - s_ext) * D + tid; idx < (hi_g - s_ext) * D; idx += T) gdst[(size_t)s_ext * D + idx] = gsrc[so<D>(idx / D, idx % D, P)];
     }
     if (a.accum) {

@@ -35,8 +35,8 @@ def test_cfg3_full_size_teacher_forced_in_bench_launch(P):
     assert rep["max_xprop_ulp"] <= 4.0 and rep["max_path_diff"] <= 1e-12, rep
 
 
-def _free_running_uniform(P, w, n_sweeps, seed, chains=None):
-    h = gpu_handle(w, kind=1)
+def _free_running_uniform(P, w, n_sweeps, seed, chains=None, disc=0):
+    h = gpu_handle(w, kind=1, disc=disc)
     tr = h.enable_trace()
     h.set_accum(True, 1); h.reset_moments()
     h.sweep(n_sweeps, seed=seed)
@@ -45,7 +45,7 @@ def _free_running_uniform(P, w, n_sweeps, seed, chains=None):
     dA = tr["dA"].cpu().numpy(); acc = tr["acc"].cpu().numpy()
     mx, mp, n = h.moments()
     mx = mx.cpu().numpy()
-    orcs = oracle_chains(w, kind=1)
+    orcs = oracle_chains(w, kind=1, disc=disc)
     worst = 0.0
     for c in (range(w.n_chains) if chains is None else chains):
         o = orcs[c]
@@ -70,6 +70,13 @@ def test_cfg3_full_size_free_running_bit_identical(P):
     w = make_workload(3)
     worst = _free_running_uniform(P, w, 24, seed=7)       # 24 sweeps: three halo exchanges of the tile engine
     print("cfg3 free-running, max dA error / scale:", worst)
+
+
+def test_cfg3_full_size_trapezoid_bit_identical(P):
+    # the paper's own discretisation (Eq. 7) at the benchmarked size, tile-resident engine, 148 CTAs
+    w = make_workload(3)
+    worst = _free_running_uniform(P, w, 20, seed=7, disc=1)
+    print("cfg3 trapezoid free-running, max dA error / scale:", worst)
 
 
 def test_cfg4_full_size_batched_chains_bit_identical(P):

@@ -21,20 +21,28 @@ def P():
 
 
 CASES = [
-    ("cfg0_M256_auto", 0, 256, None, False, 40),
-    ("cfg0_M257_3ctas", 0, 257, (3, 32), False, 20),
-    ("cfg2_M600_auto", 2, 600, None, True, 40),
-    ("cfg2_M601_5ctas", 2, 601, (5, 64), True, 20),
-    ("cfg2_M333_1cta", 2, 333, (1, 96), True, 20),
-    ("cfg1_M999_7ctas", 1, 999, (7, 32), False, 20),
+    # name, cfg, M, launch, with_params, n_sweeps, engine (0 automatic = tile-resident when it fits, 1 global-memory)
+    ("cfg0_M256_auto", 0, 256, None, False, 40, 0),
+    ("cfg0_M257_3ctas_global", 0, 257, (3, 32), False, 20, 1),
+    ("cfg2_M600_auto", 2, 600, None, True, 40, 0),
+    ("cfg2_M601_5ctas_global", 2, 601, (5, 64), True, 20, 1),
+    ("cfg2_M601_5ctas_tile", 2, 601, (5, 192), True, 20, 2),
+    ("cfg2_M333_1cta_global", 2, 333, (1, 96), True, 20, 1),
+    ("cfg1_M999_7ctas_global", 1, 999, (7, 32), False, 20, 1),
+    ("cfg1_M1000_auto", 1, 1000, None, False, 40, 0),
 ]
 
 
-@pytest.mark.parametrize("name,cfg,M,launch,with_params,n_sweeps", CASES, ids=[c[0] for c in CASES])
-def test_teacher_forced_parity_trapezoid(P, name, cfg, M, launch, with_params, n_sweeps):
+@pytest.mark.parametrize("name,cfg,M,launch,with_params,n_sweeps,engine", CASES, ids=[c[0] for c in CASES])
+def test_teacher_forced_parity_trapezoid(P, name, cfg, M, launch, with_params, n_sweeps, engine):
     w = make_workload(cfg, M=M)
-    h = gpu_handle(w, with_params=with_params, launch=launch, disc=TRAP)
-    assert h.get_engine()["engine"] == P.ENGINE_GLOBAL
+    h = gpu_handle(w, with_params=with_params, disc=TRAP)
+    if engine:
+        h.set_engine(engine)
+    if launch:
+        h.set_launch(*launch)
+    if engine:
+        assert h.get_engine()["engine"] == engine
     orcs = oracle_chains(w, with_params=with_params, disc=TRAP)
     rep = teacher_forced(w, h, orcs, n_sweeps, seed=20110347, do_params=with_params, disc=TRAP)
     print(name, h.get_launch(), rep)
@@ -46,10 +54,15 @@ def test_teacher_forced_parity_trapezoid(P, name, cfg, M, launch, with_params, n
     assert rep["max_path_diff"] <= 1e-12
 
 
-@pytest.mark.parametrize("cfg,M,launch", [(0, 256, None), (2, 500, (4, 64)), (1, 700, (3, 128)), (3, 4001, None)])
-def test_free_running_uniform_bit_identical_trapezoid(P, cfg, M, launch):
+@pytest.mark.parametrize("cfg,M,launch,engine", [(0, 256, None, 0), (2, 500, (4, 64), 1), (2, 500, (4, 192), 2), (1, 700, (3, 128), 1),
+                                                 (3, 4001, None, 0), (3, 4001, None, 1)])
+def test_free_running_uniform_bit_identical_trapezoid(P, cfg, M, launch, engine):
     w = make_workload(cfg, M=M)
-    h = gpu_handle(w, launch=launch, kind=1, disc=TRAP)
+    h = gpu_handle(w, kind=1, disc=TRAP)
+    if engine:
+        h.set_engine(engine)
+    if launch:
+        h.set_launch(*launch)
     o = oracle_chains(w, kind=1, disc=TRAP)[0]
     h.set_accum(True, 2); o.set_accum(True, 2)
     h.reset_moments(); o.reset_moments()
@@ -90,14 +103,12 @@ def test_edge_sizes_switching_and_engine_rule_trapezoid(P):
         h = gpu_handle(w, with_params=False, disc=TRAP)
         rep = teacher_forced(w, h, oracle_chains(w, with_params=False, disc=TRAP), 10, seed=3, do_params=False, disc=TRAP)
         assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0, (M, rep)
-    # switching the discretisation on a live handle rebuilds the cache; the TILE engine refuses the trapezoid form
+    # switching the discretisation on a live handle rebuilds the cache
     w = make_workload(2, M=300)
     h = gpu_handle(w)
     h.sweep(3, seed=1)
     h.set_discretisation(Pm.DISC_TRAPEZOID)
-    assert h.get_cache().shape == (1, 301, 4) and h.get_engine()["engine"] == Pm.ENGINE_GLOBAL
-    with pytest.raises(Pm.PimcError):
-        h.set_engine(Pm.ENGINE_TILE)
+    assert h.get_cache().shape == (1, 301, 4)
     h.sweep(3, seed=1)
     h.set_discretisation(Pm.DISC_RK4MAP)
     assert h.get_cache().shape == (1, 300, 4)
