@@ -110,7 +110,10 @@ def run_reference(args):
         return
     from oracle import OracleChain
     w = make_workload(args.config)
+    trap = args.disc == "trapezoid"
     o = OracleChain.from_workload(w, chain=0)
+    if trap:
+        o.set_discretisation(1)
     t0 = time.perf_counter(); o.sweep(1, seed=1); per = time.perf_counter() - t0
     n_per_step = max(1, int(min(args.ref_budget / (args.steps + args.warmup), 60.0) / per))
     for _ in range(args.warmup):
