@@ -436,11 +436,29 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
         // ---------------- A5: running moments and histograms ----------------
         if (a.accum && ((t - a.t_enable) % a.n_skip) == 0ull) {
             // own sites only; they were last written by this CTA (visible after the barriers above)
-            for (int idx = s * D + tid; idx < e * D; idx += T) {
-                const size_t gi = site0 * D + (size_t)idx;
-                const double d = (double)__ldcg(x + idx) - a.cx[gi];
-                a.S1x[gi] += d;
-                a.S2x[gi] += d * d;
+            // four elements per thread per pass with all loads issued before the first store (the arrays do not alias): the
+            // loop is bound by the L2/HBM round trip of its read-modify-writes, not by arithmetic
+            {
+                const R* __restrict__ xr = x;
+                const double* __restrict__ cxr = a.cx + site0 * D;
+                double* __restrict__ S1r = a.S1x + site0 * D;
+                double* __restrict__ S2r = a.S2x + site0 * D;
+                const int lo_i = s * D, hi_i = e * D;
+                int i0 = lo_i + tid;
+                for (; i0 + 3 * T < hi_i; i0 += 4 * T) {
+                    const double x0 = (double)__ldcg(xr + i0), x1 = (double)__ldcg(xr + i0 + T), x2 = (double)__ldcg(xr + i0 + 2 * T), x3 = (double)__ldcg(xr + i0 + 3 * T);
+                    const double c0 = cxr[i0], c1 = cxr[i0 + T], c2 = cxr[i0 + 2 * T], c3 = cxr[i0 + 3 * T];
+                    const double p0 = S1r[i0], p1 = S1r[i0 + T], p2 = S1r[i0 + 2 * T], p3 = S1r[i0 + 3 * T];
+                    const double q0 = S2r[i0], q1 = S2r[i0 + T], q2 = S2r[i0 + 2 * T], q3 = S2r[i0 + 3 * T];
+                    const double d0 = x0 - c0, d1 = x1 - c1, d2 = x2 - c2, d3 = x3 - c3;
+                    S1r[i0] = p0 + d0; S1r[i0 + T] = p1 + d1; S1r[i0 + 2 * T] = p2 + d2; S1r[i0 + 3 * T] = p3 + d3;
+                    S2r[i0] = q0 + d0 * d0; S2r[i0 + T] = q1 + d1 * d1; S2r[i0 + 2 * T] = q2 + d2 * d2; S2r[i0 + 3 * T] = q3 + d3 * d3;
+                }
+                for (; i0 < hi_i; i0 += T) {
+                    const double d = (double)__ldcg(xr + i0) - cxr[i0];
+                    S1r[i0] += d;
+                    S2r[i0] += d * d;
+                }
             }
             if (b == 0 && tid < NP) {
                 const size_t gi = (size_t)chain * NP + tid;
