@@ -110,6 +110,39 @@ __device__ __forceinline__ double div_series(double num, double den) {
     return fma(t, S, t);
 }
 
+// ---- single precision (the fp32 variant of config 3) -----------------------------------------------------------
+// exp(x) SATURATED to [2^-60, 2^61) (so that its square stays finite in fp32): x = k ln2 + r, |r| <= ln2/2,
+// e^r = 1 + r + r^2 Q(r) with Q of degree 5 (truncation < 2e-8 relative); k clamped in integer arithmetic.
+__device__ __forceinline__ float expf_sat(float x) {
+    constexpr float kMagic = 12582912.0f;                          // 1.5 * 2^23
+    constexpr float kLog2e = 1.44269504088896341f;
+    constexpr float kLn2Hi = 0.693145751953125f, kLn2Lo = 1.42860682030941723e-6f;   // hi has 12 trailing zero bits
+    const float t = fmaf(x, kLog2e, kMagic);
+    int k = __float_as_int(t) - __float_as_int(kMagic);
+    const float kd = t - kMagic;
+    float r = fmaf(kd, -kLn2Hi, x);
+    r = fmaf(kd, -kLn2Lo, r);
+    const float r2 = r * r;
+    const float a0 = fmaf(1.0f / 6.0f, r, 0.5f);
+    const float a1 = fmaf(1.0f / 120.0f, r, 1.0f / 24.0f);
+    const float a2 = fmaf(1.0f / 5040.0f, r, 1.0f / 720.0f);
+    const float r4 = r2 * r2;
+    const float b = fmaf(a1, r2, a0);
+    const float p = fmaf(a2, r4, b);
+    const float e = fmaf(p, r2, r);                                // e^r - 1
+    k = min(max(k, -60), 60);
+    const float s = __int_as_float((k + 127) << 23);               // 2^k
+    return fmaf(e, s, s);
+}
+// num / den for normal den: MUFU reciprocal (1 ulp) + one Newton step
+__device__ __forceinline__ float divf_fast(float num, float den) {
+    float y0;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(den));
+    const float e = fmaf(-den, y0, 1.0f);
+    const float y = fmaf(y0, e, y0);
+    return num * y;
+}
+
 // log(u) for normal positive u (here u in (0,1)): u = m 2^e, m in [sqrt(1/2), sqrt(2)); log m = 2 atanh((m-1)/(m+1)).
 __device__ __forceinline__ double log_fast(double u) {
     constexpr double kLn2Hi = 6.93147180369123816490e-01, kLn2Lo = 1.90821492927058770002e-10;   // hi has 21 trailing zero bits

@@ -39,12 +39,21 @@ template <typename R> struct HHModel {
         return div_series(num, den);
     }
     // dV/dt (Eq. 11 with the config's physical parameters): the only place the parameters enter
+    // Single precision: the same one-exponential form with branch-free fp32 exp and reciprocal (no libdevice tanhf / division);
+    // e saturates at 2^+-60 (tanh = +-1 to 1e-18).  |x| is limited by the caller's guard.
+    static __device__ __forceinline__ float gate_fast_f(float V, float a, float Va, float dVa, float tau0, float tau1) {
+        const float c1 = 2.0f / dVa, c0 = -2.0f * Va / dVa;
+        const float e = expf_sat(fmaf(V, c1, c0));
+        const float q = e + 1.0f;
+        const float den = fmaf(e, fmaf(e, tau0, 2.0f * tau0 + 4.0f * tau1), tau0);
+        const float num = fmaf(-a, q, e) * q;
+        return divf_fast(num, den);
+    }
     static __device__ __forceinline__ R rhs_V(const R x[4], const R* __restrict__ p, R inv_C, R I) {
         const R V = x[0], m = x[1], h = x[2], n = x[3];
         const R n2 = n * n;
         const R cur = I + p[0] * (m * m * m) * h * (p[3] - V) + p[1] * (n2 * n2) * (p[4] - V) + p[2] * (p[5] - V);
-        if constexpr (sizeof(R) == 8) return cur * inv_C;
-        else return cur / p[6];
+        return cur * inv_C;
     }
     // d(m,h,n)/dt (Eq. 12-14): functions of the state only, not of the parameters
     static __device__ __forceinline__ void rhs_gates(const R x[4], R Fg[3]) {
@@ -54,9 +63,9 @@ template <typename R> struct HHModel {
             Fg[1] = gate_fast(V, h, -60.0, -15.0, 1.0, 7.0);
             Fg[2] = gate_fast(V, n, -55.0, 30.0, 1.0, 5.0);
         } else {
-            Fg[0] = gate(V, m, R(-40.0), R(15.0), R(0.1), R(0.4));
-            Fg[1] = gate(V, h, R(-60.0), R(-15.0), R(1.0), R(7.0));
-            Fg[2] = gate(V, n, R(-55.0), R(30.0), R(1.0), R(5.0));
+            Fg[0] = gate_fast_f(V, m, -40.0f, 15.0f, 0.1f, 0.4f);
+            Fg[1] = gate_fast_f(V, h, -60.0f, -15.0f, 1.0f, 7.0f);
+            Fg[2] = gate_fast_f(V, n, -55.0f, 30.0f, 1.0f, 5.0f);
         }
     }
     static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R inv_C, R I, R F[4]) {
@@ -71,13 +80,14 @@ template <typename R> struct HHModel {
     struct Prep { R inv_C, hdt, dt6; };
     static __device__ __forceinline__ Prep prepare(const R* __restrict__ p, R dt) {
         Prep q;
-        q.inv_C = R(0);
         if constexpr (sizeof(R) == 8) q.inv_C = div_fast(1.0, p[6]);
+        else q.inv_C = 1.0f / p[6];
         q.hdt = R(0.5) * dt;
         q.dt6 = dt / R(6);
         return q;
     }
-    // Domain guard of the double-precision gates: a stage voltage beyond +-1e8 mV (or NaN) makes the whole increment
+    static constexpr R kVmax = sizeof(R) == 8 ? R(1e8) : R(1e6);
+    // Domain guard of the branch-free gates: a stage voltage beyond +-1e8 mV (fp32: 1e6 mV) or NaN makes the whole increment
     // NaN, i.e. the proposal is rejected; inside the guard the gates saturate exactly like tanh.
     // kg_in: stage-1 gate rates computed earlier at this same x (bit-identical to recomputing them); kg_out: receives them
     template <bool IN, bool OUT>
@@ -95,23 +105,23 @@ template <typename R> struct HHModel {
 #pragma unroll
             for (int a = 0; a < 3; ++a) kg_out[a] = k[1 + a];
         }
-        if constexpr (sizeof(R) == 8) sane = sane && fabs(x[0]) < 1e8;
+        sane = sane && fabs(x[0]) < kVmax;
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] = k[a]; xs[a] = x[a] + q.hdt * k[a]; }
         rhs(xs, p, q.inv_C, Ih, k);
-        if constexpr (sizeof(R) == 8) sane = sane && fabs(xs[0]) < 1e8;
+        sane = sane && fabs(xs[0]) < kVmax;
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + q.hdt * k[a]; }
         rhs(xs, p, q.inv_C, Ih, k);
-        if constexpr (sizeof(R) == 8) sane = sane && fabs(xs[0]) < 1e8;
+        sane = sane && fabs(xs[0]) < kVmax;
 #pragma unroll
         for (int a = 0; a < 4; ++a) { acc[a] += R(2) * k[a]; xs[a] = x[a] + dt * k[a]; }
         rhs(xs, p, q.inv_C, I1, k);
-        if constexpr (sizeof(R) == 8) sane = sane && fabs(xs[0]) < 1e8;
+        sane = sane && fabs(xs[0]) < kVmax;
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             g[a] = q.dt6 * (acc[a] + k[a]);
-            if constexpr (sizeof(R) == 8) g[a] = sane ? g[a] : __longlong_as_double(0x7FF8000000000000ll);
+            g[a] = sane ? g[a] : (R)__longlong_as_double(0x7FF8000000000000ll);
         }
     }
     static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, const Prep& q, R I0, R I1, R dt, R g[4]) {
@@ -125,11 +135,11 @@ template <typename R> struct HHModel {
         R F[4];
         rhs(x, p, q.inv_C, I, F);
         bool sane = true;
-        if constexpr (sizeof(R) == 8) sane = fabs(x[0]) < 1e8;
+        sane = fabs(x[0]) < kVmax;
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             c[a] = q.hdt * F[a];
-            if constexpr (sizeof(R) == 8) c[a] = sane ? c[a] : __longlong_as_double(0x7FF8000000000000ll);
+            c[a] = sane ? c[a] : (R)__longlong_as_double(0x7FF8000000000000ll);
         }
     }
 };
