@@ -33,6 +33,7 @@ namespace {
 
 constexpr int MODEL_LINEAR = 0;
 constexpr int MODEL_HH = 1;
+constexpr int MODEL_HH_CLASSIC = 2;   // same V equation, the classic alpha/beta rate functions
 constexpr int MAXD = 8;
 
 // ---------------------------------------------------------------------------------------
@@ -112,10 +113,28 @@ double gate_rate(const Kinetics& k, double V, double a) {
     return (a_inf - a) / tau;
 }
 
-void hh_rhs(const double* x, const double* p, double I, double* F) {
+// Classic Hodgkin-Huxley rate functions (Hodgkin & Huxley 1952, voltages shifted so that rest is -65 mV; BASELINE.json
+// config 0 says "standard HH"):  da/dt = alpha_a(V) (1 - a) - beta_a(V) a  with
+//   alpha_m = 0.1 (V+40) / (1 - exp(-(V+40)/10))    beta_m = 4 exp(-(V+65)/18)
+//   alpha_h = 0.07 exp(-(V+65)/20)                  beta_h = 1 / (1 + exp(-(V+35)/10))
+//   alpha_n = 0.01 (V+55) / (1 - exp(-(V+55)/10))   beta_n = 0.125 exp(-(V+65)/80)
+// u / (1 - exp(-u)) has a removable singularity at u = 0 (value 1); expm1 keeps it accurate nearby.
+double u_over_1mexp(double u) { return u == 0.0 ? 1.0 : u / -std::expm1(-u); }
+
+void classic_gate_rates(double V, double m, double h, double n, double* Fg) {
+    const double am = u_over_1mexp((V + 40.0) / 10.0), bm = 4.0 * std::exp(-(V + 65.0) / 18.0);          // 0.1 * 10 * u/(1-e^-u)
+    const double ah = 0.07 * std::exp(-(V + 65.0) / 20.0), bh = 1.0 / (1.0 + std::exp(-(V + 35.0) / 10.0));
+    const double an = 0.1 * u_over_1mexp((V + 55.0) / 10.0), bn = 0.125 * std::exp(-(V + 65.0) / 80.0);  // 0.01 * 10 * u/(1-e^-u)
+    Fg[0] = am * (1.0 - m) - bm * m;
+    Fg[1] = ah * (1.0 - h) - bh * h;
+    Fg[2] = an * (1.0 - n) - bn * n;
+}
+
+void hh_rhs(const double* x, const double* p, double I, double* F, int model = MODEL_HH) {
     const double V = x[0], m = x[1], h = x[2], n = x[3];
     const double gNa = p[0], gK = p[1], gL = p[2], ENa = p[3], EK = p[4], EL = p[5], C = p[6];
     F[0] = (I + gNa * (m * m * m) * h * (ENa - V) + gK * (n * n * n * n) * (EK - V) + gL * (EL - V)) / C;
+    if (model == MODEL_HH_CLASSIC) { classic_gate_rates(V, m, h, n, F + 1); return; }
     F[1] = gate_rate(KIN_M, V, m);
     F[2] = gate_rate(KIN_H, V, h);
     F[3] = gate_rate(KIN_N, V, n);
@@ -136,17 +155,17 @@ void step_increment(int model, int D, const double* x, const double* p, double I
     }
     const double Ih = 0.5 * (I0 + I1);
     double k1[4], k2[4], k3[4], k4[4], xs[4];
-    hh_rhs(x, p, I0, k1);
+    hh_rhs(x, p, I0, k1, model);
     for (int a = 0; a < 4; ++a) xs[a] = x[a] + 0.5 * dt * k1[a];
-    hh_rhs(xs, p, Ih, k2);
+    hh_rhs(xs, p, Ih, k2, model);
     for (int a = 0; a < 4; ++a) xs[a] = x[a] + 0.5 * dt * k2[a];
-    hh_rhs(xs, p, Ih, k3);
+    hh_rhs(xs, p, Ih, k3, model);
     for (int a = 0; a < 4; ++a) xs[a] = x[a] + dt * k3[a];
-    hh_rhs(xs, p, I1, k4);
+    hh_rhs(xs, p, I1, k4, model);
     for (int a = 0; a < 4; ++a) g[a] = (dt / 6.0) * (k1[a] + 2.0 * k2[a] + 2.0 * k3[a] + k4[a]);
 }
 
-int model_np(int model, int D) { return model == MODEL_HH ? 7 : D * D; }
+int model_np(int model, int D) { return (model == MODEL_HH || model == MODEL_HH_CLASSIC) ? 7 : D * D; }
 
 // Neumaier compensated accumulator (S4: parameter-move sum in index order).
 struct Neumaier {
@@ -203,7 +222,7 @@ void half_rhs(int model, int D, const double* x, const double* p, double I, doub
         return;
     }
     double F[4];
-    hh_rhs(x, p, I, F);
+    hh_rhs(x, p, I, F, model);
     for (int a = 0; a < 4; ++a) out[a] = 0.5 * dt * F[a];
 }
 
@@ -492,14 +511,14 @@ double orc_u01_from_two_words(uint32_t w0, uint32_t w1) { return u01_from_two_wo
 float orc_u01f_from_word(uint32_t w) { return u01f_from_word(w); }
 void orc_box_muller(double u1, double u2, double* z) { box_muller(u1, u2, &z[0], &z[1]); }
 int orc_model_np(int model, int D) { return model_np(model, D); }
-void orc_rhs(int model, const double* x, const double* p, double I, double* F) { if (model == MODEL_HH) hh_rhs(x, p, I, F); }
+void orc_rhs(int model, const double* x, const double* p, double I, double* F) { if (model == MODEL_HH || model == MODEL_HH_CLASSIC) hh_rhs(x, p, I, F, model); }
 void orc_step_increment(int model, int D, const double* x, const double* p, double I0, double I1, double dt,
                         double* g) { step_increment(model, D, x, p, I0, I1, dt, g); }
 
 void* orc_create(int model, int D, int L, int M, double dt, double Rm, const double* Rf, const double* p0,
                  int state_dtype, uint32_t chain_id) {
-    if (!(model == MODEL_LINEAR || model == MODEL_HH)) return nullptr;
-    if (model == MODEL_HH && D != 4) return nullptr;
+    if (!(model == MODEL_LINEAR || model == MODEL_HH || model == MODEL_HH_CLASSIC)) return nullptr;
+    if (model != MODEL_LINEAR && D != 4) return nullptr;
     if (D < 1 || D > MAXD || (model == MODEL_LINEAR && D > 4) || L < 0 || L > D || M < 1) return nullptr;
     if (!(state_dtype == 64 || state_dtype == 32)) return nullptr;
     Chain* c = new (std::nothrow) Chain();

@@ -9,6 +9,6 @@ to the method, not part of it.  Neither ``oracle/`` nor the CUDA package calls
 that integrator for anything they compute.
 """
 from .configs import (  # noqa: F401
-    MODEL_LINEAR, MODEL_HH, HH_P_TRUE, Workload, make_workload, hh_truth, linear_truth,
+    MODEL_LINEAR, MODEL_HH, MODEL_HH_CLASSIC, HH_P_TRUE, Workload, make_workload, hh_truth, linear_truth,
     linear_matrix, N_CONFIGS,
 )

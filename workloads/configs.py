@@ -12,6 +12,7 @@ import numpy as np
 
 MODEL_LINEAR = 0
 MODEL_HH = 1
+MODEL_HH_CLASSIC = 2          # classic alpha/beta rate functions
 N_CONFIGS = 5
 DATA_SEED0 = 11034887
 
@@ -23,12 +24,27 @@ HH_P_TRUE = np.array([120.0, 36.0, 0.3, 50.0, -77.0, -54.4, 1.0])
 _KIN = {"m": (-40.0, 15.0, 0.1, 0.4), "h": (-60.0, -15.0, 1.0, 7.0), "n": (-55.0, 30.0, 1.0, 5.0)}
 
 
-def _hh_rhs_batch(x, I, p):
+def _classic_rates(V):
+    """Data-synthesis only: classic Hodgkin-Huxley alpha/beta at rest = -65 mV."""
+    def vtrap(u):
+        u = np.where(np.abs(u) < 1e-9, 1e-9, u)
+        return u / -np.expm1(-u)
+    am, bm = vtrap((V + 40.0) / 10.0), 4.0 * np.exp(-(V + 65.0) / 18.0)
+    ah, bh = 0.07 * np.exp(-(V + 65.0) / 20.0), 1.0 / (1.0 + np.exp(-(V + 35.0) / 10.0))
+    an, bn = 0.1 * vtrap((V + 55.0) / 10.0), 0.125 * np.exp(-(V + 65.0) / 80.0)
+    return (am, bm), (ah, bh), (an, bn)
+
+
+def _hh_rhs_batch(x, I, p, kinetics="tanh"):
     """Data-synthesis only.  x: (..., 4) = (V, m, h, n); I: (...,); p: (7,)."""
     V, m, h, n = x[..., 0], x[..., 1], x[..., 2], x[..., 3]
     gNa, gK, gL, ENa, EK, EL, C = p
     out = np.empty_like(x)
     out[..., 0] = (I + gNa * m**3 * h * (ENa - V) + gK * n**4 * (EK - V) + gL * (EL - V)) / C
+    if kinetics == "classic":
+        for j, (al, be) in enumerate(_classic_rates(V), start=1):
+            out[..., j] = al * (1.0 - x[..., j]) - be * x[..., j]
+        return out
     for j, key in ((1, "m"), (2, "h"), (3, "n")):
         Va, dVa, t0, t1 = _KIN[key]
         th = np.tanh((V - Va) / dVa)
@@ -36,7 +52,7 @@ def _hh_rhs_batch(x, I, p):
     return out
 
 
-def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1):
+def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1, kinetics: str = "tanh"):
     """Twin-experiment data: returns I (C,M+1), x_true (C,M+1,4), y (C,M+1).
 
     Step current: 5 ms segments, segment k covers steps [k*5/dt, (k+1)*5/dt), amplitude U(0,15) uA/cm2.
@@ -54,15 +70,18 @@ def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1):
     for j, key in ((1, "m"), (2, "h"), (3, "n")):
         Va, dVa, _, _ = _KIN[key]
         x[:, 0, j] = 0.5 + 0.5 * np.tanh((V0 - Va) / dVa)
+    if kinetics == "classic":
+        for j, (al, be) in enumerate(_classic_rates(np.float64(V0)), start=1):
+            x[:, 0, j] = al / (al + be)
     p = HH_P_TRUE
     for k in range(M):
         xn = x[:, k]
         I0, I1 = I[:, k], I[:, k + 1]
         Ih = 0.5 * (I0 + I1)
-        k1 = _hh_rhs_batch(xn, I0, p)
-        k2 = _hh_rhs_batch(xn + 0.5 * dt * k1, Ih, p)
-        k3 = _hh_rhs_batch(xn + 0.5 * dt * k2, Ih, p)
-        k4 = _hh_rhs_batch(xn + dt * k3, I1, p)
+        k1 = _hh_rhs_batch(xn, I0, p, kinetics)
+        k2 = _hh_rhs_batch(xn + 0.5 * dt * k1, Ih, p, kinetics)
+        k3 = _hh_rhs_batch(xn + 0.5 * dt * k2, Ih, p, kinetics)
+        k4 = _hh_rhs_batch(xn + dt * k3, I1, p, kinetics)
         x[:, k + 1] = xn + (dt / 6.0) * (k1 + 2 * k2 + 2 * k3 + k4)
     y = x[:, :, 0] + rng.normal(0.0, 1.0, size=(n_chains, M + 1))
     return I, x, y
@@ -121,9 +140,9 @@ _WP_CFG2 = np.array([0.10, 0.03, 0.008, 0.025, 0.035, 0.5, 0.004])
 _WP_CFG3 = np.array([0.07, 0.02, 0.005, 0.018, 0.025, 0.4, 0.0026])
 
 
-def _hh_workload(name, cfg, M, dt, n_chains, w_param, n_sweeps, estimate, seed=None):
+def _hh_workload(name, cfg, M, dt, n_chains, w_param, n_sweeps, estimate, seed=None, kinetics="tanh"):
     rng = np.random.default_rng(DATA_SEED0 + cfg if seed is None else seed)
-    I, xt, y = hh_truth(M, dt, rng, n_chains)
+    I, xt, y = hh_truth(M, dt, rng, n_chains, kinetics)
     x0 = np.empty((n_chains, M + 1, 4))
     x0[:, :, 0] = y
     x0[:, :, 1:] = 0.5
@@ -137,17 +156,18 @@ def _hh_workload(name, cfg, M, dt, n_chains, w_param, n_sweeps, estimate, seed=N
         wp = np.zeros(7)
     lo = np.tile(pt - 0.5 * np.abs(pt), (n_chains, 1))
     hi = np.tile(pt + 0.5 * np.abs(pt), (n_chains, 1))
-    return Workload(name=name, model=MODEL_HH, D=4, L=1, Np=7, M=M, dt=dt, Rm=1.0,
+    return Workload(name=name + ("_classic" if kinetics == "classic" else ""), model=MODEL_HH_CLASSIC if kinetics == "classic" else MODEL_HH, D=4, L=1, Np=7, M=M, dt=dt, Rm=1.0,
                     Rf=np.array([1e2, 1e4, 1e4, 1e4]), n_chains=n_chains, p0=p0, p_true=pt.copy(),
                     lo=lo, hi=hi, w_state=np.array([0.5, 0.02, 0.02, 0.02]), w_param=wp,
                     y=y[:, :, None].copy(), I=I, x0=x0, x_true=xt, n_sweeps=n_sweeps)
 
 
 def make_workload(cfg: int, *, M: int | None = None, n_chains: int | None = None,
-                  seed: int | None = None) -> Workload:
-    """BASELINE.json `configs[cfg]`; M / n_chains may be overridden to make small parity cases."""
+                  seed: int | None = None, kinetics: str = "tanh") -> Workload:
+    """BASELINE.json `configs[cfg]`; M / n_chains may be overridden to make small parity cases.
+    kinetics = "classic" generates the Hodgkin-Huxley configs with the classic alpha/beta rate functions (model 2)."""
     if cfg == 0:
-        return _hh_workload("cfg0_hh_M256", 0, M or 256, 0.02, n_chains or 1, None, 2000, False, seed)
+        return _hh_workload("cfg0_hh_M256", 0, M or 256, 0.02, n_chains or 1, None, 2000, False, seed, kinetics)
     if cfg == 1:
         M = M or 4096
         rng = np.random.default_rng(DATA_SEED0 + 1 if seed is None else seed)
@@ -160,10 +180,10 @@ def make_workload(cfg: int, *, M: int | None = None, n_chains: int | None = None
                         w_state=np.array([0.1, 0.1]), w_param=np.zeros(4), y=y[None, :, None].copy(),
                         I=None, x0=x0, x_true=xt[None], n_sweeps=5000)
     if cfg == 2:
-        return _hh_workload("cfg2_hh_M4096_params", 2, M or 4096, 0.02, n_chains or 1, _WP_CFG2, 20000, True, seed)
+        return _hh_workload("cfg2_hh_M4096_params", 2, M or 4096, 0.02, n_chains or 1, _WP_CFG2, 20000, True, seed, kinetics)
     if cfg == 3:
-        return _hh_workload("cfg3_hh_M32768_params", 3, M or 32768, 0.01, n_chains or 1, _WP_CFG3, 10000, True, seed)
+        return _hh_workload("cfg3_hh_M32768_params", 3, M or 32768, 0.01, n_chains or 1, _WP_CFG3, 10000, True, seed, kinetics)
     if cfg == 4:
         return _hh_workload("cfg4_hh_128x8192_params", 4, M or 8192, 0.02, n_chains or 128,
-                            _WP_CFG2 / np.sqrt(2.0), 5000, True, seed)
+                            _WP_CFG2 / np.sqrt(2.0), 5000, True, seed, kinetics)
     raise ValueError(f"no config {cfg}")
