@@ -44,8 +44,12 @@ enum { PIMC_OK = 0, PIMC_EINVAL = -1, PIMC_ESTATE = -2, PIMC_ECUDA = -3, PIMC_EU
 
 /* Models.  LINEAR: D in 1..4, parameters = the D*D map matrix (row-major), g = A x - x.
  * HH: D = 4, x = (V,m,h,n), p = (gNa,gK,gL,ENa,EK,EL,C); tanh kinetics of PAPER.md:256-270 (Eq. 11-14)
- * with Table 1 shifted by -65 mV; needs the injected current I. */
-enum { PIMC_MODEL_LINEAR = 0, PIMC_MODEL_HH = 1 };
+ * with Table 1 shifted by -65 mV; needs the injected current I.
+ * HH_CLASSIC: as HH, with the classic rate functions da/dt = alpha_a(V)(1-a) - beta_a(V) a of Hodgkin & Huxley (1952),
+ * rest at -65 mV: alpha_m = 0.1(V+40)/(1-exp(-(V+40)/10)), beta_m = 4 exp(-(V+65)/18), alpha_h = 0.07 exp(-(V+65)/20),
+ * beta_h = 1/(1+exp(-(V+35)/10)), alpha_n = 0.01(V+55)/(1-exp(-(V+55)/10)), beta_n = 0.125 exp(-(V+65)/80)
+ * (BASELINE.json says "standard HH"). */
+enum { PIMC_MODEL_LINEAR = 0, PIMC_MODEL_HH = 1, PIMC_MODEL_HH_CLASSIC = 2 };
 enum { PIMC_PROPOSAL_GAUSSIAN = 0, PIMC_PROPOSAL_UNIFORM = 1 };
 /* Sweep engines (same results, different data placement).  GLOBAL: path and cache stay
  * in global memory (L2), threads stride over the tile, neighbour tiles synchronise every half-sweep with

@@ -7,7 +7,7 @@ import os
 
 import numpy as np
 
-MODEL_LINEAR, MODEL_HH = 0, 1
+MODEL_LINEAR, MODEL_HH, MODEL_HH_CLASSIC = 0, 1, 2
 PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM = 0, 1
 ENGINE_AUTO, ENGINE_GLOBAL, ENGINE_TILE = 0, 1, 2
 DISC_RK4MAP, DISC_TRAPEZOID = 0, 1

@@ -91,10 +91,10 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
 
 bool shape_ok(int model, int D, int L, int M, int C, int dtype, int* why) {
     *why = PIMC_EINVAL;
-    if (!(model == PIMC_MODEL_LINEAR || model == PIMC_MODEL_HH)) return false;
+    if (!(model == PIMC_MODEL_LINEAR || model == PIMC_MODEL_HH || model == PIMC_MODEL_HH_CLASSIC)) return false;
     if (D < 1 || L < 0 || L > D || M < 1 || C < 1 || !(dtype == 64 || dtype == 32)) return false;
     *why = PIMC_EUNSUPPORTED;
-    if (model == PIMC_MODEL_HH && D != 4) return false;
+    if (model != PIMC_MODEL_LINEAR && D != 4) return false;
     if (model == PIMC_MODEL_LINEAR && D > 4) return false;
     if ((long long)C * ((long long)M + 1) > (1ll << 31)) return false;
     return true;
@@ -145,6 +145,10 @@ template <typename F> int dispatch(int model, int D, int dtype, F&& f) {
     if (model == PIMC_MODEL_HH) {
         if (dtype == 64) return f(HHModel<double>{}, double{});
         return f(HHModel<float>{}, float{});
+    }
+    if (model == PIMC_MODEL_HH_CLASSIC) {
+        if (dtype == 64) return f(HHClassicModel<double>{}, double{});
+        return f(HHClassicModel<float>{}, float{});
     }
     switch (D * 100 + dtype) {
         case 164: return f(LinearModel<double, 1>{}, double{});
@@ -350,7 +354,7 @@ bool finite_all(const double* v, int n) {
 extern "C" {
 
 int pimc_model_np(int model, int D) {
-    if (model == PIMC_MODEL_HH) return D == 4 ? 7 : -1;
+    if (model == PIMC_MODEL_HH || model == PIMC_MODEL_HH_CLASSIC) return D == 4 ? 7 : -1;
     if (model == PIMC_MODEL_LINEAR) return (D >= 1 && D <= 4) ? D * D : -1;
     return -1;
 }
@@ -418,7 +422,7 @@ int pimc_set_data(pimc_handle* h, const void* y, const void* I) {
     if (h->L > 0 && !y) return fail(h, PIMC_EINVAL, "y is required when L > 0");
     const size_t es = h->dtype == 64 ? 8 : 4;
     if (h->L > 0) PIMC_CUDA(h, cudaMemcpyAsync(h->lay.y, y, (size_t)h->C * (h->M + 1) * h->L * es, cudaMemcpyDeviceToDevice, h->stream));
-    if (h->model == PIMC_MODEL_HH && !I) return fail(h, PIMC_EINVAL, "the HH model needs the injected current I");
+    if (h->model != PIMC_MODEL_LINEAR && !I) return fail(h, PIMC_EINVAL, "the HH model needs the injected current I");
     h->have_I = I != nullptr;
     if (I) PIMC_CUDA(h, cudaMemcpyAsync(h->lay.I, I, (size_t)h->C * (h->M + 1) * es, cudaMemcpyDeviceToDevice, h->stream));
     h->have_data = true;

@@ -110,6 +110,28 @@ __device__ __forceinline__ double div_series(double num, double den) {
     return fma(t, S, t);
 }
 
+// exp(x) - 1 for |x| <= 700, accurate near 0: same reduction as exp_fast; with k = 0 the result is the polynomial itself,
+// otherwise 2^k (1 + e) - 1 = e 2^k + (2^k - 1) with 2^k - 1 exact (|k| <= 52) or absorbed (larger |k|).
+__device__ __forceinline__ double expm1_fast(double x) {
+    constexpr double kMagic = 6755399441055744.0;
+    constexpr double kLog2e = 1.4426950408889634074;
+    constexpr double kLn2Hi = 0x1.62e42fefa39efp-1, kLn2Lo = 0x1.abc9e3b39803fp-56;
+    const double t = fma(x, kLog2e, kMagic);
+    const int k = __double2loint(t);
+    const double kd = t - kMagic;
+    double r = fma(kd, -kLn2Hi, x);
+    r = fma(kd, -kLn2Lo, r);
+    const double e = expm1_small(r);
+    const double s = __hiloint2double((k + 1023) << 20, 0);
+    return fma(e, s, s - 1.0);
+}
+// u / (1 - exp(-u)) with its removable singularity at u = 0 (value 1); |u| <= 700
+__device__ __forceinline__ double u_over_1mexp(double u) {
+    const double d = -expm1_fast(-u);
+    const double q = div_fast(u, d);
+    return u == 0.0 ? 1.0 : q;
+}
+
 // ---- single precision (the fp32 variant of config 3) -----------------------------------------------------------
 // exp(x) SATURATED to [2^-60, 2^61) (so that its square stays finite in fp32): x = k ln2 + r, |r| <= ln2/2,
 // e^r = 1 + r + r^2 Q(r) with Q of degree 5 (truncation < 2e-8 relative); k clamped in integer arithmetic.

@@ -14,7 +14,9 @@ template <> __device__ __forceinline__ double tanh_<double>(double v) { return t
 template <> __device__ __forceinline__ float tanh_<float>(float v) { return tanhf(v); }
 
 // ---------------------------------------------------------------------------------------------------
-template <typename R> struct HHModel {
+// KIN selects the gate kinetics: 0 = the paper's tanh forms, 1 = the classic alpha/beta rate functions
+// (Hodgkin & Huxley 1952, rest at -65 mV; include/pimc.h PIMC_MODEL_HH_CLASSIC).  Everything else is shared.
+template <typename R, int KIN> struct HHModelK {
     static constexpr int D = 4;
     static constexpr int NP = 7;
 
@@ -58,7 +60,27 @@ template <typename R> struct HHModel {
     // d(m,h,n)/dt (Eq. 12-14): functions of the state only, not of the parameters
     static __device__ __forceinline__ void rhs_gates(const R x[4], R Fg[3]) {
         const R V = x[0], m = x[1], h = x[2], n = x[3];
-        if constexpr (sizeof(R) == 8) {
+        if constexpr (KIN == 1) {
+            // da/dt = alpha_a (1 - a) - beta_a a; exponent arguments clamped so that nothing overflows inside the domain guard
+            if constexpr (sizeof(R) == 8) {
+                const double Vc = fmin(fmax(V, -6000.0), 6000.0);
+                const double am = u_over_1mexp((Vc + 40.0) * 0.1), bm = 4.0 * exp_fast((Vc + 65.0) * (-1.0 / 18.0));
+                const double ah = 0.07 * exp_fast((Vc + 65.0) * (-1.0 / 20.0)), bh = div_fast(1.0, 1.0 + exp_fast((Vc + 35.0) * -0.1));
+                const double an = 0.1 * u_over_1mexp((Vc + 55.0) * 0.1), bn = 0.125 * exp_fast((Vc + 65.0) * (-1.0 / 80.0));
+                Fg[0] = am * (1.0 - m) - bm * m;
+                Fg[1] = ah * (1.0 - h) - bh * h;
+                Fg[2] = an * (1.0 - n) - bn * n;
+            } else {
+                const float Vc = fminf(fmaxf(V, -700.0f), 700.0f);
+                const float um = (Vc + 40.0f) * 0.1f, un = (Vc + 55.0f) * 0.1f;
+                const float am = um == 0.0f ? 1.0f : um / -expm1f(-um), bm = 4.0f * expf(-(Vc + 65.0f) / 18.0f);
+                const float ah = 0.07f * expf(-(Vc + 65.0f) / 20.0f), bh = 1.0f / (1.0f + expf(-(Vc + 35.0f) * 0.1f));
+                const float an = un == 0.0f ? 0.1f : 0.1f * (un / -expm1f(-un)), bn = 0.125f * expf(-(Vc + 65.0f) / 80.0f);
+                Fg[0] = am * (1.0f - m) - bm * m;
+                Fg[1] = ah * (1.0f - h) - bh * h;
+                Fg[2] = an * (1.0f - n) - bn * n;
+            }
+        } else if constexpr (sizeof(R) == 8) {
             Fg[0] = gate_fast(V, m, -40.0, 15.0, 0.1, 0.4);
             Fg[1] = gate_fast(V, h, -60.0, -15.0, 1.0, 7.0);
             Fg[2] = gate_fast(V, n, -55.0, 30.0, 1.0, 5.0);
@@ -143,6 +165,9 @@ template <typename R> struct HHModel {
         }
     }
 };
+
+template <typename R> using HHModel = HHModelK<R, 0>;
+template <typename R> using HHClassicModel = HHModelK<R, 1>;
 
 // ---------------------------------------------------------------------------------------------------
 template <typename R, int D_> struct LinearModel {
