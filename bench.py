@@ -109,7 +109,7 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle import OracleChain
-    w = make_workload(args.config)
+    w = make_workload(args.config, kinetics=args.kinetics)
     trap = args.disc == "trapezoid"
     o = OracleChain.from_workload(w, chain=0)
     if trap:
@@ -162,7 +162,7 @@ def run_ours(args):
     dev_index = torch.cuda.current_device()
 
     # replicas only: every rank runs the same shape with its own data realisation and Philox key
-    w = make_workload(args.config, seed=None if rank == 0 else 11034887 + args.config + 7919 * rank)
+    w = make_workload(args.config, seed=None if rank == 0 else 11034887 + args.config + 7919 * rank, kinetics=args.kinetics)
     seed = w.chain_seed + rank
     S = args.sweeps_per_step
     h = P.Pimc.from_workload(w, dtype=args.dtype)
@@ -279,6 +279,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--kinetics", default="tanh", choices=["tanh", "classic"], help="HH gate kinetics: the paper's tanh forms (default) or the classic alpha/beta rate functions (model 2)")
     ap.add_argument("--disc", default="rk4", choices=["rk4", "trapezoid"], help="model-error discretisation: the north_star's RK4 map or the paper's trapezoid rule")
     ap.add_argument("--dtype", type=int, default=64, choices=[64, 32], help="arithmetic type of the path (config 3 is also quoted in fp32)")
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
