@@ -54,6 +54,7 @@ def lib():
             "orc_param_delta_A": (C.c_double, [C.c_void_p, C.c_int, C.c_double, dp]),
             "orc_full_action": (None, [C.c_void_p, dp, dp, dp, dp]),
             "orc_cache_len": (C.c_int, [C.c_void_p]),
+            "orc_set_update_mode": (C.c_int, [C.c_void_p, C.c_int]),
             "orc_set_discretisation": (C.c_int, [C.c_void_p, C.c_int]),
             "orc_half_rhs": (None, [C.c_int, C.c_int, dp, dp, C.c_double, C.c_double, dp]),
         }
@@ -183,6 +184,11 @@ class OracleChain:
         lib().orc_get_cache(self._h, _dp(g))
         return g
 
+    def set_update_mode(self, mode):
+        """0 = joint D-vector proposal per site (default), 1 = component-wise (D decisions per site)."""
+        assert lib().orc_set_update_mode(self._h, int(mode)) == 0
+        self.update_mode = int(mode)
+
     def set_discretisation(self, disc):
         """0 = explicit RK4 map (default), 1 = the paper's trapezoid rule (Eq. 7)."""
         assert lib().orc_set_discretisation(self._h, int(disc)) == 0
@@ -245,7 +251,8 @@ class OracleChain:
 
     def trace(self):
         M, D, Np = self.M, self.D, self.Np
-        t = dict(dA=np.empty(M + 1), S=np.empty(M + 1), logu=np.empty(M + 1), acc=np.empty(M + 1, np.uint8),
+        sh = (M + 1, D) if getattr(self, "update_mode", 0) == 1 else (M + 1,)       # per (site, component) or per site
+        t = dict(dA=np.empty(sh), S=np.empty(sh), logu=np.empty(sh), acc=np.empty(sh, np.uint8),
                  xprop=np.empty((M + 1, D)), dAp=np.empty(Np), Sp=np.empty(Np), logup=np.empty(Np),
                  accp=np.empty(Np, np.uint8), pprop=np.empty(Np))
         u8 = C.POINTER(C.c_uint8)

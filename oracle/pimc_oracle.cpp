@@ -186,6 +186,7 @@ struct Chain {
     double Rf[MAXD];
     std::vector<double> x, g, y, I, p, lo, hi, wx, wp;
     int proposal_kind = 0;                    // 0 gaussian, 1 uniform
+    int update_mode = 0;                      // 0 = joint D-vector proposal, one decision per site (Fig. 1); 1 = one component at a time, D decisions per site (NEXT-2)
     int disc = 0;                             // model-error discretisation: 0 = explicit RK4 map (north_star), 1 = trapezoid rule (Eq. 7)
     uint64_t t = 0;                           // absolute sweep index
     uint32_t chain_id = 0;
@@ -354,9 +355,9 @@ void propose_site(const Chain& c, uint64_t seed, int n, double* xp) {
     }
 }
 
-double accept_log_u_state(const Chain& c, uint64_t seed, int n) {
+double accept_log_u_state(const Chain& c, uint64_t seed, int n, int block = 0) {
     uint32_t w[4];
-    draw_words(seed, c.t, c.chain_id, (uint32_t)n, STREAM_STATE_ACCEPT, 0, w);
+    draw_words(seed, c.t, c.chain_id, (uint32_t)n, STREAM_STATE_ACCEPT, (uint32_t)block, w);
     if (c.state_dtype == 32) return (double)std::log(u01f_from_word(w[0]));
     return std::log(u01_from_two_words(w[0], w[1]));
 }
@@ -366,6 +367,30 @@ void update_site(Chain& c, uint64_t seed, int n) {
     const int D = c.D;
     double xp[MAXD], gp[MAXD], S;
     propose_site(c, seed, n, xp);
+    if (c.update_mode == 1) {
+        // Component-wise updates (PAPER.md:226-230 keeps step sizes and acceptance counters "per component of the path"):
+        // component a of site n is proposed with the SAME draw as in the joint move (x'_a = x_a + w_a z_a; x_a is untouched
+        // by the other components' decisions), judged on its own with the accept uniform of block a of the accept stream,
+        // and the next component starts from the state and cache this decision leaves.  Trace entries are per (n, a).
+        for (int a = 0; a < D; ++a) {
+            double xa[MAXD];
+            for (int b = 0; b < D; ++b) xa[b] = c.x[(size_t)n * D + b];
+            xa[a] = xp[a];
+            const double dA = site_delta_A(c, n, xa, gp, &S);
+            const double logu = accept_log_u_state(c, seed, n, a);
+            const bool accept = logu < -dA;
+            const size_t k = (size_t)n * D + a;
+            c.tr_dA[k] = dA; c.tr_S[k] = S; c.tr_logu[k] = logu; c.tr_acc[k] = accept ? 1 : 0;
+            c.tr_xprop[k] = xp[a];
+            c.prop[a] += 1;
+            if (accept) {
+                c.acc[a] += 1;
+                c.x[k] = xp[a];
+                if (n < cache_len(c)) for (int b = 0; b < D; ++b) c.g[(size_t)n * D + b] = gp[b];
+            }
+        }
+        return;
+    }
     const double dA = site_delta_A(c, n, xp, gp, &S);
     const double logu = accept_log_u_state(c, seed, n);
     const bool accept = logu < -dA;                 // G3: NaN / +inf reject, dA <= 0 always accepts
@@ -536,8 +561,8 @@ void* orc_create(int model, int D, int L, int M, double dt, double Rm, const dou
     c->cx.assign(nx, 0.0); c->S1x.assign(nx, 0.0); c->S2x.assign(nx, 0.0);
     c->cp.assign(c->Np, 0.0); c->S1p.assign(c->Np, 0.0); c->S2p.assign(c->Np, 0.0);
     c->acc.assign(D + c->Np, 0); c->prop.assign(D + c->Np, 0);
-    c->tr_dA.assign(M + 1, 0.0); c->tr_S.assign(M + 1, 0.0); c->tr_logu.assign(M + 1, 0.0);
-    c->tr_xprop.assign(nx, 0.0); c->tr_acc.assign(M + 1, 0);
+    c->tr_dA.assign(nx, 0.0); c->tr_S.assign(nx, 0.0); c->tr_logu.assign(nx, 0.0);     // (M+1) entries used by joint updates, (M+1) D by component-wise ones
+    c->tr_xprop.assign(nx, 0.0); c->tr_acc.assign(nx, 0);
     c->tr_dAp.assign(c->Np, 0.0); c->tr_Sp.assign(c->Np, 0.0); c->tr_logup.assign(c->Np, 0.0);
     c->tr_pprop.assign(c->Np, 0.0); c->tr_accp.assign(c->Np, 0);
     return c;
@@ -579,6 +604,13 @@ int orc_set_discretisation(void* h, int disc) {
     if (!(disc == 0 || disc == 1)) return -1;
     c.disc = disc;
     if (c.have_path) rebuild_cache(c);
+    return 0;
+}
+// 0 = joint proposal per site (default), 1 = component-wise
+int orc_set_update_mode(void* h, int mode) {
+    Chain& c = *(Chain*)h;
+    if (!(mode == 0 || mode == 1)) return -1;
+    c.update_mode = mode;
     return 0;
 }
 void orc_half_rhs(int model, int D, const double* x, const double* p, double I, double dt, double* out) { half_rhs(model, D, x, p, I, dt, out); }
@@ -649,10 +681,11 @@ void orc_stats(void* h, uint64_t* out) {      // (2, D+Np): accepted, proposed
 void orc_trace(void* h, double* dA, double* S, double* logu, uint8_t* acc, double* xprop, double* dAp, double* Sp,
                double* logup, uint8_t* accp, double* pprop) {
     Chain& c = *(Chain*)h;
-    if (dA) std::memcpy(dA, c.tr_dA.data(), c.tr_dA.size() * 8);
-    if (S) std::memcpy(S, c.tr_S.data(), c.tr_S.size() * 8);
-    if (logu) std::memcpy(logu, c.tr_logu.data(), c.tr_logu.size() * 8);
-    if (acc) std::memcpy(acc, c.tr_acc.data(), c.tr_acc.size());
+    const size_t nt = (size_t)(c.M + 1) * (c.update_mode == 1 ? c.D : 1);      // per site, or per (site, component)
+    if (dA) std::memcpy(dA, c.tr_dA.data(), nt * 8);
+    if (S) std::memcpy(S, c.tr_S.data(), nt * 8);
+    if (logu) std::memcpy(logu, c.tr_logu.data(), nt * 8);
+    if (acc) std::memcpy(acc, c.tr_acc.data(), nt);
     if (xprop) std::memcpy(xprop, c.tr_xprop.data(), c.tr_xprop.size() * 8);
     if (dAp) std::memcpy(dAp, c.tr_dAp.data(), c.tr_dAp.size() * 8);
     if (Sp) std::memcpy(Sp, c.tr_Sp.data(), c.tr_Sp.size() * 8);
