@@ -65,6 +65,14 @@ enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2 };
  *            c_n = (dt/2) F(x_n), n = 0..M (PAPER.md:189, 242 caches F_n).  One right-hand side per proposal instead of
  *            four.  Both engines support both discretisations. */
 enum { PIMC_DISC_RK4MAP = 0, PIMC_DISC_TRAPEZOID = 1 };
+/* How a site is updated (Fig. 1 proposes all D components together; PAPER.md:226-230 keeps step sizes and
+ * acceptance counters per component).  JOINT (default): x'_n = x_n + w o z, one decision per site.  COMPONENTWISE: for
+ * a = 0..D-1 in order, x'_{n,a} = x_{n,a} + w_a z_a (the same draw z_a as the joint move) with the other components as they
+ * stand, its own Delta-A and decision (accept uniform = words 0,1 of block a of the accept stream); D decisions and D model
+ * evaluations per site.  Runs on the GLOBAL engine (the automatic engine choice falls back to it; PIMC_EUNSUPPORTED if the
+ * TILE engine is forced).  With the debug trace on, dA_out and acc_out are (n_chains, M+1, D) and xprop_out holds the proposed
+ * value of each component. */
+enum { PIMC_UPDATE_JOINT = 0, PIMC_UPDATE_COMPONENTWISE = 1 };
 
 /* Number of parameters the model defines (HH: 7, LINEAR: D*D); negative on bad arguments. */
 int pimc_model_np(int model, int D);
@@ -102,6 +110,9 @@ int pimc_get_cache(pimc_handle* h, void* g_out);
 
 /* Select the discretisation (PIMC_DISC_*); rebuilds the cache if a path is set.  PIMC_EINVAL on an unknown value. */
 int pimc_set_discretisation(pimc_handle* h, int disc);
+
+/* Select joint or component-wise site updates (PIMC_UPDATE_*).  PIMC_EINVAL on an unknown value. */
+int pimc_set_update_mode(pimc_handle* h, int mode);
 
 /* Proposal widths (PAPER.md:188 step (a), 226): w_state host D values >= 0; w_param host Np values >= 0
  * or NULL (= all 0; a parameter with width 0 is frozen and never proposed); kind = PIMC_PROPOSAL_*. */

@@ -11,6 +11,7 @@ MODEL_LINEAR, MODEL_HH, MODEL_HH_CLASSIC = 0, 1, 2
 PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM = 0, 1
 ENGINE_AUTO, ENGINE_GLOBAL, ENGINE_TILE = 0, 1, 2
 DISC_RK4MAP, DISC_TRAPEZOID = 0, 1
+UPDATE_JOINT, UPDATE_COMPONENTWISE = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libpimc.so")
@@ -44,6 +45,7 @@ _SIGNATURES = {
     "pimc_get_launch": (C.c_int, [_vp, _ip, _ip, _ip, _ip]),
     "pimc_set_engine": (C.c_int, [_vp, C.c_int, C.c_int]),
     "pimc_set_discretisation": (C.c_int, [_vp, C.c_int]),
+    "pimc_set_update_mode": (C.c_int, [_vp, C.c_int]),
     "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
     "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
@@ -242,6 +244,12 @@ class Pimc:
         _check(lib().pimc_get_cache(self._h, _ptr(g)), self._h)
         return g
 
+    def set_update_mode(self, mode):
+        """UPDATE_JOINT (default) or UPDATE_COMPONENTWISE (D decisions per site; GLOBAL engine).  Re-enable the trace afterwards:
+        its dA / acc buffers are per (site, component) in component-wise mode."""
+        _check(lib().pimc_set_update_mode(self._h, int(mode)), self._h)
+        self.update_mode = int(mode)
+
     def set_discretisation(self, disc):
         """DISC_RK4MAP (default) or DISC_TRAPEZOID (the paper's rule, Eq. 7; GLOBAL engine)."""
         _check(lib().pimc_set_discretisation(self._h, int(disc)), self._h)
@@ -277,8 +285,9 @@ class Pimc:
 
     def enable_trace(self, params=True, xprop=True):
         t = self.torch
-        tr = dict(dA=t.zeros((self.C, self.M + 1), dtype=self.tdtype, device=self.device),
-                  acc=t.zeros((self.C, self.M + 1), dtype=t.uint8, device=self.device),
+        sh = (self.C, self.M + 1, self.D) if getattr(self, "update_mode", UPDATE_JOINT) == UPDATE_COMPONENTWISE else (self.C, self.M + 1)
+        tr = dict(dA=t.zeros(sh, dtype=self.tdtype, device=self.device),
+                  acc=t.zeros(sh, dtype=t.uint8, device=self.device),
                   xprop=t.zeros((self.C, self.M + 1, self.D), dtype=self.tdtype, device=self.device) if xprop else None,
                   dAp=t.zeros((self.C, self.Np), dtype=self.tdtype, device=self.device) if params else None,
                   accp=t.zeros((self.C, self.Np), dtype=t.uint8, device=self.device) if params else None,

@@ -110,6 +110,7 @@ struct pimc_handle {
     double wx[kMaxD], wp[kMaxNp];
     int kind = 0;
     int disc = PIMC_DISC_RK4MAP;
+    int update_mode = PIMC_UPDATE_JOINT;
     bool have_data = false, have_path = false, have_prop = false, have_I = false;
     int accum = 0;
     unsigned long long n_skip = 1, t_enable = 0, n_samples = 0, t = 0;
@@ -206,6 +207,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int sites = h->M + 1;
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
+    if (h->update_mode != PIMC_UPDATE_JOINT) return no("component-wise updates run on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
     if (T != 0 && (T % 64 != 0 || T > 512)) return no("threads_per_cta must be a multiple of 64, at most 512");
@@ -276,6 +278,7 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     if (rc != PIMC_OK) return rc;
     SweepArgs<R> a{};
     a.M = h->M; a.L = h->L; a.n_chains = h->C; a.G = ls.G; a.tile = ls.tile; a.kind = h->kind;
+    a.update_mode = h->update_mode;
     a.disc = h->disc; a.nc = h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M;
     a.dt = (R)h->dt; a.Rm = (R)h->Rm;
     for (int c = 0; c < h->D; ++c) { a.Rf[c] = (R)h->Rf[c]; a.wx[c] = (R)h->wx[c]; }
@@ -468,6 +471,15 @@ int pimc_get_cache(pimc_handle* h, void* g_out) {
         const char* src = (const char*)(cur[c] ? h->lay.g1 : h->lay.g0) + per * c;
         PIMC_CUDA(h, cudaMemcpyAsync((char*)g_out + per * c, src, per, cudaMemcpyDeviceToDevice, h->stream));
     }
+    return PIMC_OK;
+}
+
+int pimc_set_update_mode(pimc_handle* h, int mode) {
+    if (!h) return PIMC_EINVAL;
+    if (!(mode == PIMC_UPDATE_JOINT || mode == PIMC_UPDATE_COMPONENTWISE)) return fail(h, PIMC_EINVAL, "unknown update mode %d", mode);
+    if (mode == PIMC_UPDATE_COMPONENTWISE && h->engine_user == PIMC_ENGINE_TILE)
+        return fail(h, PIMC_EUNSUPPORTED, "component-wise updates run on the GLOBAL engine");
+    h->update_mode = mode;
     return PIMC_OK;
 }
 

@@ -31,6 +31,7 @@ constexpr int kMaxHistSel = 64;
 template <typename R> struct SweepArgs {
     // problem
     int M, L, n_chains, G, tile, kind;
+    int update_mode;      // 0 = joint D-vector proposal per site (Fig. 1), 1 = one component at a time, D decisions per site (GLOBAL engine)
     int disc;             // model-error discretisation: 0 = explicit RK4 map, 1 = trapezoid rule (Eq. 7)
     int nc;               // cache entries per chain: M (disc 0: g_n, n <= M-1) or M + 1 (disc 1: c_n = (dt/2) F(x_n), n <= M)
     R dt, Rm, Rf[kMaxD], wx[kMaxD];
@@ -157,22 +158,30 @@ __device__ __forceinline__ void propose_state(const SweepArgs<R>& a, unsigned lo
     }
 }
 
-template <typename R> __device__ __forceinline__ R log_accept_uniform(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n) {
-    const Words4 w = draw(a.seed, t, chain, n, kStreamStateAccept, 0);
+template <typename R> __device__ __forceinline__ R log_accept_uniform(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n, uint32_t block = 0) {
+    const Words4 w = draw(a.seed, t, chain, n, kStreamStateAccept, block);
     if constexpr (sizeof(R) == 8) return log_fast(unit_open52(w.w[0], w.w[1]));
     else return logf(unit_openf(w.w[0]));
 }
 
 // ---- one Metropolis site update: Fig. 1 (a)-(i) ----------------------------------------------------------
 template <class Model, typename R>
-__device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __restrict__ prm, unsigned long long t,
+__device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* __restrict__ prm, unsigned long long t,
                                             uint32_t chain, int n, R* __restrict__ x, R* __restrict__ g, const R* __restrict__ y,
                                             const R* __restrict__ I, bool trace, size_t chain_site0) {
     constexpr int D = Model::D;
     const int M = a.M;
-    R xn[D], xp[D], gp[D];
+    R xn[D], xfull[D], xp[D], gp[D];
     load_vec<R, D>(x, n, xn);
-    propose_state<R, D>(a, t, chain, (uint32_t)n, xn, xp);
+    propose_state<R, D>(a, t, chain, (uint32_t)n, xn, xfull);
+    // joint move: one pass with the whole proposal.  Component-wise moves: D passes; pass ai changes component ai only (same
+    // draw as the joint move), is judged with the accept uniform of block ai, and the next pass starts from what it leaves.
+    const int ncomp = a.update_mode == 1 ? D : 1;
+    unsigned accepted_mask = 0;                 // bit c: a move that changed component c was accepted
+#pragma unroll 1
+    for (int ai = 0; ai < ncomp; ++ai) {
+#pragma unroll
+    for (int c = 0; c < D; ++c) xp[c] = (a.update_mode == 1 && c != ai) ? xn[c] : xfull[c];
     R dL = R(0), dR = R(0);     // left part (term n-1 -> n and measurement n) and right part (term n -> n+1), summed separately
     if (a.disc == 1) {
         // trapezoid rule, Fig. 1 (b)-(f) as printed: c' = (dt/2) F(x'_n) enters BOTH neighbouring terms; every residual is
@@ -246,19 +255,32 @@ __device__ __forceinline__ bool update_site(const SweepArgs<R>& a, const R* __re
     }
     }
     const R dA = dL + dR;
-    const R logu = log_accept_uniform<R>(a, t, chain, (uint32_t)n);
+    const R logu = log_accept_uniform<R>(a, t, chain, (uint32_t)n, (uint32_t)ai);
     const bool accept = logu < -dA;      // NaN or +inf rejects; dA <= 0 always accepts
     if (accept) {
         store_vec<R, D>(x, n, xp);
         if (n < a.nc) store_vec<R, D>(g, n, gp);
+#pragma unroll
+        for (int c = 0; c < D; ++c) xn[c] = xp[c];
+        accepted_mask |= a.update_mode == 1 ? (1u << ai) : ((1u << D) - 1u);
     }
     if (trace) {
         const size_t gs = chain_site0 + (size_t)n;
-        if (a.tr_dA) a.tr_dA[gs] = dA;
-        if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
-        if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
+        if (a.update_mode == 1) {          // trace entries per (site, component)
+            R xa = R(0);
+#pragma unroll
+            for (int c = 0; c < D; ++c) xa = (c == ai) ? xfull[c] : xa;
+            if (a.tr_dA) a.tr_dA[gs * D + ai] = dA;
+            if (a.tr_acc) a.tr_acc[gs * D + ai] = accept ? 1 : 0;
+            if (a.tr_xprop) a.tr_xprop[gs * D + ai] = xa;
+        } else {
+            if (a.tr_dA) a.tr_dA[gs] = dA;
+            if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
+            if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
+        }
     }
-    return accept;
+    }
+    return accepted_mask;
 }
 
 // ---- the persistent sweep kernel ---------------------------------------------------------------------------
@@ -291,7 +313,9 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     if (tid == 0) s_cur = a.cur[chain];
     __syncthreads();
     int cur = s_cur;
-    unsigned int n_acc_state = 0;
+    unsigned int n_acc_comp[D];                       // accepted moves per component class (A6)
+#pragma unroll
+    for (int c = 0; c < D; ++c) n_acc_comp[c] = 0;
     unsigned long long ar_count = a.ar_epoch[chain];   // all-reduce events this chain has performed so far
 
     for (long long i = 0; i < a.n_sweeps; ++i) {
@@ -310,7 +334,11 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     __syncthreads();
                 }
                 for (int n = s + parity + 2 * tid; n < e; n += 2 * T)
-                    n_acc_state += update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0) ? 1u : 0u;
+                {
+                    const unsigned mask = update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0);
+#pragma unroll
+                    for (int c = 0; c < D; ++c) n_acc_comp[c] += (mask >> c) & 1u;
+                }
                 __syncthreads();
                 if (G > 1 && tid == 0)
                     st_release_gpu(hs_flag + b, a.hs_base + 2ull * (unsigned long long)i + (unsigned long long)parity + 1ull);
@@ -490,13 +518,16 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
 
     // ---------------- A6 + state write-back ----------------
     {
-        const double acc_total = block_sum((double)n_acc_state, red);   // exact: counts < 2^53
+        double acc_total[D];
+#pragma unroll
+        for (int c = 0; c < D; ++c) acc_total[c] = block_sum((double)n_acc_comp[c], red);   // exact: counts < 2^53
         if (tid == 0) {
             unsigned long long* cnt = a.counters + (size_t)chain * 2 * (D + NP);
-            const unsigned long long acc_u = (unsigned long long)acc_total;
             unsigned long long prop_u = 0;
             if (a.do_states) prop_u = (unsigned long long)(e - s) * (unsigned long long)a.n_sweeps;
+#pragma unroll
             for (int c = 0; c < D; ++c) {
+                const unsigned long long acc_u = (unsigned long long)acc_total[c];
                 if (acc_u) atomicAdd(cnt + c, acc_u);
                 if (prop_u) atomicAdd(cnt + (D + NP) + c, prop_u);
             }

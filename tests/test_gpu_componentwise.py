@@ -1,0 +1,111 @@
+"""GPU parity for component-wise site updates (PIMC_UPDATE_COMPONENTWISE) against the oracle's
+set_update_mode(1).  With UNIFORM proposals both sides form bit-identical proposals, so the traces compare entry by
+entry: Delta-A of every (site, component) decision within 1e-12 of its scale, identical decisions, bit-identical paths,
+per-component counters; both discretisations, several CTAs per chain, batched chains, the classic model, fp32."""
+import numpy as np
+import pytest
+
+from helpers import TOL32, TOL64, gpu_handle, oracle_chains
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+COMP = 1
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    import paper_1103_4887_b200 as P
+    assert torch.cuda.is_available()
+    P.lib()
+    return P
+
+
+def _run(P, w, launch, disc, n_sweeps, dtype=64, kind=1, with_params=True, tol=TOL64):
+    h = gpu_handle(w, dtype=dtype, with_params=with_params, launch=launch, kind=kind, disc=disc)
+    h.set_update_mode(P.UPDATE_COMPONENTWISE)
+    assert h.get_engine()["engine"] == P.ENGINE_GLOBAL
+    tr = h.enable_trace()
+    orcs = oracle_chains(w, state_dtype=dtype, with_params=with_params, kind=kind, disc=disc)
+    for o in orcs:
+        o.set_update_mode(COMP)
+    worst, n_dec = 0.0, 0
+    for t in range(n_sweeps):
+        if with_params:
+            h.sweep(1, seed=31)
+        else:
+            h.sweep_states_only(1, seed=31)
+        dA = tr["dA"].cpu().numpy().astype(np.float64); acc = tr["acc"].cpu().numpy(); xprop = tr["xprop"].cpu().numpy().astype(np.float64)
+        assert dA.shape == (w.n_chains, w.M + 1, w.D)
+        xg, pg = [a.cpu().numpy().astype(np.float64) for a in h.get_path()]
+        for c, o in enumerate(orcs):
+            o.sweep(1, seed=31, do_params=with_params)
+            ot = o.trace()
+            if dtype == 64:
+                assert np.array_equal(xprop[c], ot["xprop"]), (t, c)           # uniform proposals are bit-reproducible
+            err = np.abs(dA[c] - ot["dA"]) / np.maximum(np.maximum(np.abs(ot["dA"]), ot["S"]), 1e-300)
+            worst = max(worst, float(err.max()))
+            bad = np.argwhere(acc[c] != ot["acc"])
+            for n, a in bad:                                                    # only inside the near-tie window
+                assert abs(ot["dA"][n, a] + ot["logu"][n, a]) < (1e-9 if dtype == 64 else 1e-5 * max(1.0, ot["S"][n, a])), (t, c, n, a)
+            n_dec += acc[c].size
+            if len(bad) == 0 and dtype == 64:
+                xo, po = o.get_path()
+                assert np.array_equal(xg[c], xo) and np.array_equal(pg[c], po), (t, c)
+            else:                                                               # resync after a near-tie / in fp32
+                x, p = o.get_path()
+                import torch
+                X = np.stack([q.get_path()[0] for q in orcs]); Pp = np.stack([q.get_path()[1] for q in orcs])
+                h.set_params(torch.as_tensor(Pp, dtype=h.tdtype, device=h.device)); h.set_path(torch.as_tensor(X, dtype=h.tdtype, device=h.device))
+    assert worst <= tol, worst
+    if dtype == 64:
+        st = h.stats().cpu().numpy().astype(np.uint64)
+        for c, o in enumerate(orcs):
+            assert np.array_equal(st[c], o.stats()), c
+    return worst, n_dec
+
+
+@pytest.mark.parametrize("cfg,M,launch,disc", [(0, 256, None, 0), (2, 500, (4, 64), 0), (2, 501, (1, 96), 1), (1, 700, (3, 128), 0),
+                                               (2, 333, (5, 32), 1)])
+def test_componentwise_decisions_match_oracle(P, cfg, M, launch, disc):
+    w = make_workload(cfg, M=M)
+    worst, n = _run(P, w, launch, disc, 25, with_params=bool(np.any(w.w_param > 0)))
+    print(cfg, M, launch, disc, "max dA error / scale", worst, "decisions", n)
+
+
+def test_componentwise_batched_classic_and_fp32(P):
+    w = make_workload(4, M=300, n_chains=4, kinetics="classic")
+    _run(P, w, (1, 64), 0, 10)
+    w = make_workload(2, M=400)
+    _run(P, w, None, 0, 10, dtype=32, tol=TOL32)
+
+
+def test_componentwise_gaussian_proposals_and_engine_rule(P):
+    import paper_1103_4887_b200 as Pm
+    w = make_workload(2, M=400)
+    # Gaussian proposals: different math libraries, proposals agree to a few ulp, decisions identical except near ties
+    h = gpu_handle(w); h.set_update_mode(Pm.UPDATE_COMPONENTWISE)
+    o = oracle_chains(w)[0]; o.set_update_mode(COMP)
+    tr = h.enable_trace()
+    mism = 0
+    for t in range(30):
+        h.sweep(1, seed=8); o.sweep(1, seed=8)
+        ot = o.trace()
+        acc = tr["acc"].cpu().numpy()[0]
+        bad = np.argwhere(acc != ot["acc"])
+        for n, a in bad:
+            assert abs(ot["dA"][n, a] + ot["logu"][n, a]) < 1e-9
+            mism += 1
+        if len(bad):
+            import torch
+            x, p = o.get_path(); h.set_params(torch.as_tensor(p[None], device="cuda")); h.set_path(torch.as_tensor(x[None], device="cuda"))
+    assert mism <= 1
+    assert np.max(np.abs(h.get_path()[0].cpu().numpy()[0] - o.get_path()[0])) < 1e-10
+    # the tile-resident engine refuses component-wise updates (GLOBAL engine only in this round)
+    with pytest.raises(Pm.PimcError):
+        h.set_engine(Pm.ENGINE_TILE)
+    h2 = gpu_handle(w); h2.set_engine(Pm.ENGINE_TILE)
+    with pytest.raises(Pm.PimcError):
+        h2.set_update_mode(Pm.UPDATE_COMPONENTWISE)
+    with pytest.raises(Pm.PimcError):
+        h2.set_update_mode(5)
