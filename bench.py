@@ -34,6 +34,8 @@ W_EVAL_SLOTS = 560.0
 # trapezoid discretisation (--disc trapezoid, the paper's own rule): one right-hand side per proposal instead of four
 # (108 + Delta-A 97 + RNG 175), one per parameter-move evaluation (108 + 32)
 W_SITE_SLOTS_TRAP = 380.0
+# component-wise updates (--update componentwise): D = 4 model evaluations and decisions per site visit (4 x (433 + 67) + RNG 300)
+W_SITE_SLOTS_COMP = 2300.0
 W_EVAL_SLOTS_TRAP = 140.0
 # FP64 peak derived from unit counts and clocks: 148 SMs x 64 FP64 lanes/clk/SM x 1.965 GHz, 2 FLOP per lane-FMA.
 FP64_LANES_PER_SM_CLK = 64
@@ -87,12 +89,14 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def oracle_rate(w, budget_s, chain=0, disc=0):
+def oracle_rate(w, budget_s, chain=0, disc=0, mode=0):
     """Time the CPU oracle, as it stands, on a bounded sample of the same workload.  Returns (site-updates/s, sweeps, seconds)."""
     from oracle import OracleChain
     o = OracleChain.from_workload(w, chain=chain)
     if disc:
         o.set_discretisation(disc)
+    if mode:
+        o.set_update_mode(mode)
     t0 = time.perf_counter()
     o.sweep(2, seed=w.chain_seed)                       # warm-up + first estimate
     per = (time.perf_counter() - t0) / 2
@@ -170,6 +174,10 @@ def run_ours(args):
     if trap:
         h.set_discretisation(P.DISC_TRAPEZOID)
     w_site, w_eval = (W_SITE_SLOTS_TRAP, W_EVAL_SLOTS_TRAP) if trap else (W_SITE_SLOTS, W_EVAL_SLOTS)
+    comp = args.update == "componentwise"
+    if comp:
+        h.set_update_mode(P.UPDATE_COMPONENTWISE)
+        w_site = W_SITE_SLOTS_COMP if not trap else 4 * 205.0 + 300.0
     peak_tflops = PEAK_TFLOPS_DERIVED * (1.0 if args.dtype == 64 else 2.0)   # fp32: 128 FP32 lanes/clk/SM
     h.set_accum(True, 1)
     h.reset_moments()
@@ -240,7 +248,7 @@ def run_ours(args):
 
     # end to end through the C ABI on HOST buffers: H2D of y, I, x0, p0 + sweeps + D2H of the moments inside the timed region
     e2e = None
-    if (rank == 0 or world > 1) and not trap:     # pimc_run_host is the RK4-map convenience call
+    if (rank == 0 or world > 1) and not trap and not comp:     # pimc_run_host is the RK4-map, joint-update convenience call
         P.run_host(w, 0, max(1, S // 10), seed, dtype=args.dtype)         # warm-up (context, allocator)
         reps = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
@@ -252,14 +260,14 @@ def run_ours(args):
                "ms_per_step": s_e2e / reps * 1e3, "call": "pimc_run_host (cudaMalloc + H2D + pimc_sweep + pimc_moments + D2H + sync)"}
 
     if rank == 0:
-        cpu_rate, cpu_n, cpu_s = oracle_rate(w, args.cpu_budget, disc=1 if trap else 0)
+        cpu_rate, cpu_n, cpu_s = oracle_rate(w, args.cpu_budget, disc=1 if trap else 0, mode=1 if comp else 0)
         cpu = {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{cpu_n} full sweeps of chain 0 of {w.name} in {cpu_s:.1f} s (serial fp64 C++ -O2, {os.cpu_count()} cores present)"}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.dtype == 64 else "f32",
             "data": "synthetic",
-            "config": {"workload": w.name + ("_trapezoid" if trap else ""), "discretisation": args.disc, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
+            "config": {"workload": w.name + ("_trapezoid" if trap else ""), "discretisation": args.disc, "update": args.update, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
                        "accumulate_every": 1, "launch": shape, "l2": "flushed between timed steps (256 MiB fill)",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "sweeps_per_s": value / (w.M + 1),
@@ -280,6 +288,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--kinetics", default="tanh", choices=["tanh", "classic"], help="HH gate kinetics: the paper's tanh forms (default) or the classic alpha/beta rate functions (model 2)")
+    ap.add_argument("--update", default="joint", choices=["joint", "componentwise"], help="site update: joint D-vector proposal (default) or one component at a time (GLOBAL engine)")
     ap.add_argument("--disc", default="rk4", choices=["rk4", "trapezoid"], help="model-error discretisation: the north_star's RK4 map or the paper's trapezoid rule")
     ap.add_argument("--dtype", type=int, default=64, choices=[64, 32], help="arithmetic type of the path (config 3 is also quoted in fp32)")
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
