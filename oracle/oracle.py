@@ -55,6 +55,8 @@ def lib():
             "orc_full_action": (None, [C.c_void_p, dp, dp, dp, dp]),
             "orc_cache_len": (C.c_int, [C.c_void_p]),
             "orc_set_update_mode": (C.c_int, [C.c_void_p, C.c_int]),
+            "orc_set_annealing": (C.c_int, [C.c_void_p, C.c_double, C.c_uint64]),
+            "orc_annealing_beta": (C.c_double, [C.c_void_p]),
             "orc_set_discretisation": (C.c_int, [C.c_void_p, C.c_int]),
             "orc_half_rhs": (None, [C.c_int, C.c_int, dp, dp, C.c_double, C.c_double, dp]),
         }
@@ -183,6 +185,13 @@ class OracleChain:
         g = np.empty((lib().orc_cache_len(self._h), self.D))     # M rows (RK4 map) or M + 1 (trapezoid)
         lib().orc_get_cache(self._h, _dp(g))
         return g
+
+    def set_annealing(self, beta0, n_cool):
+        """Simulated annealing of the dynamics term from the current sweep on (Eq. 10); n_cool = 0 = off."""
+        assert lib().orc_set_annealing(self._h, float(beta0), int(n_cool)) == 0
+
+    def annealing_beta(self):
+        return lib().orc_annealing_beta(self._h)
 
     def set_update_mode(self, mode):
         """0 = joint D-vector proposal per site (default), 1 = component-wise (D decisions per site)."""

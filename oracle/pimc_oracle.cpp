@@ -183,7 +183,9 @@ struct HistSel { int site, comp; double lo, hi, width; };
 struct Chain {
     int model, D, L, M, Np, state_dtype;     // state_dtype 64 or 32 (state values rounded to float)
     double dt, Rm;
-    double Rf[MAXD];
+    double Rf[MAXD];                          // model-error weights IN EFFECT this sweep: beta * Rf0 (beta = 1 unless annealing)
+    double Rf0[MAXD];                         // the weights given at creation
+    double beta0 = 1.0; uint64_t n_cool = 0, t_anneal = 0;   // simulated annealing of the dynamics term (Eq. 10)
     std::vector<double> x, g, y, I, p, lo, hi, wx, wp;
     int proposal_kind = 0;                    // 0 gaussian, 1 uniform
     int update_mode = 0;                      // 0 = joint D-vector proposal, one decision per site (Fig. 1); 1 = one component at a time, D decisions per site (NEXT-2)
@@ -495,6 +497,20 @@ void reset_moments(Chain& c) {
     c.n_samples = 0; c.t_enable = c.t;
 }
 
+// Simulated annealing: the dynamics term A_d carries a multiplier beta that starts at beta0 < 1 and is
+// multiplied by f_beta = (1/beta0)^(1/N_cool) (Eq. 10) after each iteration until it reaches 1; the observation term does
+// not.  After k iterations beta = beta0 f_beta^k = beta0^(1 - k/N_cool), evaluated in that closed form.
+double annealing_beta(const Chain& c) {
+    if (c.n_cool == 0 || c.t < c.t_anneal) return 1.0;
+    const uint64_t k = c.t - c.t_anneal;
+    if (k >= c.n_cool) return 1.0;
+    return std::exp(std::log(c.beta0) * (1.0 - (double)k / (double)c.n_cool));
+}
+void apply_annealing(Chain& c) {
+    const double beta = annealing_beta(c);
+    for (int a = 0; a < c.D; ++a) c.Rf[a] = beta * c.Rf0[a];
+}
+
 // Test-only "truth": the full action in long double, straight from the definition.
 long double full_action(const Chain& c, const double* x, const double* p) {
     const int D = c.D;
@@ -550,7 +566,7 @@ void* orc_create(int model, int D, int L, int M, double dt, double Rm, const dou
     if (!c) return nullptr;
     c->model = model; c->D = D; c->L = L; c->M = M; c->Np = model_np(model, D); c->state_dtype = state_dtype;
     c->dt = dt; c->Rm = Rm; c->chain_id = chain_id;
-    for (int a = 0; a < D; ++a) c->Rf[a] = Rf[a];
+    for (int a = 0; a < D; ++a) c->Rf[a] = c->Rf0[a] = Rf[a];
     const size_t nx = (size_t)(M + 1) * D;
     c->x.assign(nx, 0.0); c->g.assign((size_t)(M + 1) * D, 0.0); c->y.assign((size_t)(M + 1) * (L > 0 ? L : 1), 0.0);
     c->p.assign(p0, p0 + c->Np);
@@ -606,6 +622,15 @@ int orc_set_discretisation(void* h, int disc) {
     if (c.have_path) rebuild_cache(c);
     return 0;
 }
+// Start annealing at the current sweep index: beta0 in (0, 1], n_cool iterations (0 switches it off)
+int orc_set_annealing(void* h, double beta0, uint64_t n_cool) {
+    Chain& c = *(Chain*)h;
+    if (!(beta0 > 0.0 && beta0 <= 1.0)) return -1;
+    c.beta0 = beta0; c.n_cool = n_cool; c.t_anneal = c.t;
+    apply_annealing(c);
+    return 0;
+}
+double orc_annealing_beta(void* h) { return annealing_beta(*(Chain*)h); }
 // 0 = joint proposal per site (default), 1 = component-wise
 int orc_set_update_mode(void* h, int mode) {
     Chain& c = *(Chain*)h;
@@ -630,7 +655,7 @@ void orc_set_accum(void* h, int enabled, uint64_t n_skip) {
 }
 void orc_reset_moments(void* h) { reset_moments(*(Chain*)h); }
 uint64_t orc_sweep_index(void* h) { return ((Chain*)h)->t; }
-void orc_set_sweep_index(void* h, uint64_t t) { ((Chain*)h)->t = t; }
+void orc_set_sweep_index(void* h, uint64_t t) { ((Chain*)h)->t = t; apply_annealing(*(Chain*)h); }
 
 int orc_hist_config(void* h, int n_sel, const int* site, const int* comp, const double* lo, const double* hi, int nbins) {
     Chain& c = *(Chain*)h;
@@ -648,12 +673,14 @@ int orc_sweep(void* h, uint64_t n_sweeps, uint64_t seed, int order, int do_param
     Chain& c = *(Chain*)h;
     if (!c.have_data || !c.have_path) return -2;
     for (uint64_t s = 0; s < n_sweeps; ++s) {
+        apply_annealing(c);
         half_sweep(c, seed, 0, order);
         half_sweep(c, seed, 1, order);
         if (do_params) parameter_moves(c, seed);
         if (c.accum && ((c.t - c.t_enable) % c.n_skip) == 0) accumulate(c);
         c.t += 1;
     }
+    apply_annealing(c);          // the weights in effect always belong to the current sweep index
     return 0;
 }
 
