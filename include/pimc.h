@@ -111,6 +111,13 @@ int pimc_get_cache(pimc_handle* h, void* g_out);
 /* Select the discretisation (PIMC_DISC_*); rebuilds the cache if a path is set.  PIMC_EINVAL on an unknown value. */
 int pimc_set_discretisation(pimc_handle* h, int disc);
 
+/* Simulated annealing of the dynamics term (Eq. 10): from the current sweep index on, the model-error
+ * weights Rf are multiplied by beta_k = beta0 f^k, f = (1/beta0)^(1/n_cool), k = sweeps since this call, until beta = 1
+ * (k >= n_cool); the measurement term is not scaled.  0 < beta0 <= 1; n_cool = 0 switches annealing off.  While beta < 1 the
+ * sweeps run on the GLOBAL engine (the automatic choice falls back; PIMC_EUNSUPPORTED if TILE is forced); once the
+ * schedule is over the TILE engine is used again. */
+int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool);
+
 /* Select joint or component-wise site updates (PIMC_UPDATE_*).  PIMC_EINVAL on an unknown value. */
 int pimc_set_update_mode(pimc_handle* h, int mode);
 

@@ -46,6 +46,7 @@ _SIGNATURES = {
     "pimc_set_engine": (C.c_int, [_vp, C.c_int, C.c_int]),
     "pimc_set_discretisation": (C.c_int, [_vp, C.c_int]),
     "pimc_set_update_mode": (C.c_int, [_vp, C.c_int]),
+    "pimc_set_annealing": (C.c_int, [_vp, C.c_double, C.c_longlong]),
     "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
     "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
@@ -243,6 +244,10 @@ class Pimc:
         g = self.torch.empty((self.C, rows, self.D), dtype=self.tdtype, device=self.device)
         _check(lib().pimc_get_cache(self._h, _ptr(g)), self._h)
         return g
+
+    def set_annealing(self, beta0, n_cool):
+        """Anneal the dynamics term from the current sweep on (Eq. 10); n_cool = 0 switches it off."""
+        _check(lib().pimc_set_annealing(self._h, float(beta0), int(n_cool)), self._h)
 
     def set_update_mode(self, mode):
         """UPDATE_JOINT (default) or UPDATE_COMPONENTWISE (D decisions per site; GLOBAL engine).  Re-enable the trace afterwards:

@@ -111,6 +111,7 @@ struct pimc_handle {
     int kind = 0;
     int disc = PIMC_DISC_RK4MAP;
     int update_mode = PIMC_UPDATE_JOINT;
+    double beta0 = 1.0; unsigned long long n_cool = 0, t_anneal = 0;
     bool have_data = false, have_path = false, have_prop = false, have_I = false;
     int accum = 0;
     unsigned long long n_skip = 1, t_enable = 0, n_samples = 0, t = 0;
@@ -208,6 +209,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
     if (h->update_mode != PIMC_UPDATE_JOINT) return no("component-wise updates run on the GLOBAL engine");
+    if (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool) return no("sweeps with the annealing multiplier below 1 run on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
     if (T != 0 && (T % 64 != 0 || T > 512)) return no("threads_per_cta must be a multiple of 64, at most 512");
@@ -279,6 +281,7 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     SweepArgs<R> a{};
     a.M = h->M; a.L = h->L; a.n_chains = h->C; a.G = ls.G; a.tile = ls.tile; a.kind = h->kind;
     a.update_mode = h->update_mode;
+    a.ln_beta0 = std::log(h->beta0); a.n_cool = h->n_cool; a.t_anneal = h->t_anneal;
     a.disc = h->disc; a.nc = h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M;
     a.dt = (R)h->dt; a.Rm = (R)h->Rm;
     for (int c = 0; c < h->D; ++c) { a.Rf[c] = (R)h->Rf[c]; a.wx[c] = (R)h->wx[c]; }
@@ -471,6 +474,13 @@ int pimc_get_cache(pimc_handle* h, void* g_out) {
         const char* src = (const char*)(cur[c] ? h->lay.g1 : h->lay.g0) + per * c;
         PIMC_CUDA(h, cudaMemcpyAsync((char*)g_out + per * c, src, per, cudaMemcpyDeviceToDevice, h->stream));
     }
+    return PIMC_OK;
+}
+
+int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool) {
+    if (!h) return PIMC_EINVAL;
+    if (!(beta0 > 0.0 && beta0 <= 1.0) || n_cool < 0) return fail(h, PIMC_EINVAL, "annealing needs 0 < beta0 <= 1 and n_cool >= 0");
+    h->beta0 = beta0; h->n_cool = (unsigned long long)n_cool; h->t_anneal = h->t;
     return PIMC_OK;
 }
 

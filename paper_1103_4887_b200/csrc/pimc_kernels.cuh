@@ -31,6 +31,8 @@ constexpr int kMaxHistSel = 64;
 template <typename R> struct SweepArgs {
     // problem
     int M, L, n_chains, G, tile, kind;
+    double ln_beta0;      // simulated annealing of the dynamics term (Eq. 10): beta_k = exp(ln_beta0 (1 - k/n_cool)),
+    unsigned long long n_cool, t_anneal;   //   k = t - t_anneal < n_cool, else 1; n_cool = 0 switches it off
     int update_mode;      // 0 = joint D-vector proposal per site (Fig. 1), 1 = one component at a time, D decisions per site (GLOBAL engine)
     int disc;             // model-error discretisation: 0 = explicit RK4 map, 1 = trapezoid rule (Eq. 7)
     int nc;               // cache entries per chain: M (disc 0: g_n, n <= M-1) or M + 1 (disc 1: c_n = (dt/2) F(x_n), n <= M)
@@ -74,6 +76,14 @@ template <typename R> struct SweepArgs {
     unsigned long long* ar_words;   // (2 slots, kTileMaxCtas, kArSlotWords) Delta-A partials, one 128-byte line per CTA
     int* fault;                     // set to 1 if a hand-off was never delivered
 };
+
+// ---- annealing multiplier of the model-error weights at sweep t (same closed form as the oracle; beta = 1 when off) ----
+template <typename R> __device__ __forceinline__ double anneal_beta(const SweepArgs<R>& a, unsigned long long t) {
+    if (a.n_cool == 0ull || t < a.t_anneal) return 1.0;
+    const unsigned long long k = t - a.t_anneal;
+    if (k >= a.n_cool) return 1.0;
+    return exp_fast(a.ln_beta0 * (1.0 - (double)k / (double)a.n_cool));
+}
 
 // ---- memory-model helpers ------------------------------------------------------------------------
 __device__ __forceinline__ void st_release_gpu(unsigned long long* p, unsigned long long v) {
@@ -168,7 +178,7 @@ template <typename R> __device__ __forceinline__ R log_accept_uniform(const Swee
 template <class Model, typename R>
 __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* __restrict__ prm, unsigned long long t,
                                             uint32_t chain, int n, R* __restrict__ x, R* __restrict__ g, const R* __restrict__ y,
-                                            const R* __restrict__ I, bool trace, size_t chain_site0) {
+                                            const R* __restrict__ I, bool trace, size_t chain_site0, const R* __restrict__ Rfs) {
     constexpr int D = Model::D;
     const int M = a.M;
     R xn[D], xfull[D], xp[D], gp[D];
@@ -198,7 +208,7 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
             for (int c = 0; c < D; ++c) {
                 const R r_new = ((xp[c] - xm[c]) - cm[c]) - gp[c];
                 const R r_old = ((xn[c] - xm[c]) - cm[c]) - cn[c];
-                dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                dL += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
             }
 #pragma unroll
             for (int l = 0; l < D; ++l) {
@@ -217,7 +227,7 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
             for (int c = 0; c < D; ++c) {
                 const R r_new = ((xq[c] - xp[c]) - gp[c]) - cq[c];
                 const R r_old = ((xq[c] - xn[c]) - cn[c]) - cq[c];
-                dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                dR += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
             }
         }
     } else {
@@ -229,7 +239,7 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
         for (int c = 0; c < D; ++c) {   // model-error term n-1 -> n
             const R r_new = (xp[c] - xm[c]) - gm[c];
             const R r_old = (xn[c] - xm[c]) - gm[c];
-            dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+            dL += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
         }
 #pragma unroll
         for (int l = 0; l < D; ++l) {    // measurement term n (the action sums n = 1..M); the first L components are observed
@@ -250,7 +260,7 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
         for (int c = 0; c < D; ++c) {   // model-error term n -> n+1
             const R r_new = (xq[c] - xp[c]) - gp[c];
             const R r_old = (xq[c] - xn[c]) - gn[c];
-            dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+            dR += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
         }
     }
     }
@@ -321,6 +331,12 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     for (long long i = 0; i < a.n_sweeps; ++i) {
         const unsigned long long t = a.t0 + (unsigned long long)i;
         const bool trace = (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
+        R Rfs[D];                                  // model-error weights in effect this sweep (annealing multiplier applied)
+        {
+            const double beta = anneal_beta(a, t);
+#pragma unroll
+            for (int c = 0; c < D; ++c) Rfs[c] = (R)(beta * (double)a.Rf[c]);
+        }
 
         // ---------------- A2/A3: even half-sweep, then odd half-sweep ----------------
         if (a.do_states) {
@@ -335,7 +351,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                 }
                 for (int n = s + parity + 2 * tid; n < e; n += 2 * T)
                 {
-                    const unsigned mask = update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0);
+                    const unsigned mask = update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0, Rfs);
 #pragma unroll
                     for (int c = 0; c < D; ++c) n_acc_comp[c] += (mask >> c) & 1u;
                 }
@@ -395,7 +411,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                             for (int c = 0; c < D; ++c) {
                                 const R d = xq[c] - xn[c];
                                 const R r_new = (d - cpn[c]) - cpq[c], r_old = (d - cn[c]) - cq[c];
-                                acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                                acc += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
                             }
                             part += (double)acc;
                         }
@@ -413,7 +429,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                         for (int c = 0; c < D; ++c) {
                             const R d = xq[c] - xn[c];
                             const R r_new = d - gp[c], r_old = d - gn[c];
-                            acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            acc += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
                         }
                         part += (double)acc;
                     }

@@ -42,7 +42,7 @@ def ulp_diff(a, b):
     return np.abs(a - b) / np.maximum(np.spacing(np.maximum(np.abs(a), np.abs(b))), 1e-300)
 
 
-def teacher_forced(w, h, orcs, n_sweeps, seed, tol=TOL64, tie=TIE64, do_params=True, state_dtype=64, disc=0):
+def teacher_forced(w, h, orcs, n_sweeps, seed, tol=TOL64, tie=TIE64, do_params=True, state_dtype=64, disc=0, anneal=None):
     """SURVEY.md §8(c) T1.  For every sweep: force the GPU to the oracle's state, run one sweep on both with the
     trace on, and compare per-site Delta-A (evaluated by the oracle AT THE GPU's proposals, on the path as it stood
     when the site was visited), decisions, parameter moves and the resulting path.  Returns a report dict."""
@@ -54,10 +54,14 @@ def teacher_forced(w, h, orcs, n_sweeps, seed, tol=TOL64, tie=TIE64, do_params=T
     for hc in helper:
         if disc:
             hc.set_discretisation(disc)
+        if anneal:
+            hc.set_annealing(*anneal)
     for t in range(n_sweeps):
         X = np.stack([o.get_path()[0] for o in orcs]); Pp = np.stack([o.get_path()[1] for o in orcs])
         h.set_params(to_dev(Pp, h)); h.set_path(to_dev(X, h))
         h.sweep_index = orcs[0].sweep_index
+        for hc in helper:
+            hc.sweep_index = orcs[0].sweep_index          # same annealing multiplier as the sweep under test
         if do_params:
             h.sweep(1, seed)
         else:
