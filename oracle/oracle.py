@@ -56,6 +56,8 @@ def lib():
             "orc_cache_len": (C.c_int, [C.c_void_p]),
             "orc_set_update_mode": (C.c_int, [C.c_void_p, C.c_int]),
             "orc_set_annealing": (C.c_int, [C.c_void_p, C.c_double, C.c_uint64]),
+            "orc_set_tuning": (C.c_int, [C.c_void_p, C.c_int, C.c_uint64, C.c_double, C.c_double]),
+            "orc_get_widths": (None, [C.c_void_p, dp, dp]),
             "orc_annealing_beta": (C.c_double, [C.c_void_p]),
             "orc_set_discretisation": (C.c_int, [C.c_void_p, C.c_int]),
             "orc_half_rhs": (None, [C.c_int, C.c_int, dp, dp, C.c_double, C.c_double, dp]),
@@ -185,6 +187,15 @@ class OracleChain:
         g = np.empty((lib().orc_cache_len(self._h), self.D))     # M rows (RK4 map) or M + 1 (trapezoid)
         lib().orc_get_cache(self._h, _dp(g))
         return g
+
+    def set_tuning(self, enabled, n_skip=1, f_acc=0.23, alpha=0.02):
+        """Step-size auto-tuning from the current sweep on; enabled=False freezes the step sizes."""
+        assert lib().orc_set_tuning(self._h, int(bool(enabled)), int(n_skip), float(f_acc), float(alpha)) == 0
+
+    def get_widths(self):
+        ws, wp = np.empty((self.M + 1, self.D)), np.empty(self.Np)
+        lib().orc_get_widths(self._h, _dp(ws), _dp(wp))
+        return ws, wp
 
     def set_annealing(self, beta0, n_cool):
         """Simulated annealing of the dynamics term from the current sweep on (Eq. 10); n_cool = 0 = off."""

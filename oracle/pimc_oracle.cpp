@@ -188,6 +188,11 @@ struct Chain {
     double beta0 = 1.0; uint64_t n_cool = 0, t_anneal = 0;   // simulated annealing of the dynamics term (Eq. 10)
     std::vector<double> x, g, y, I, p, lo, hi, wx, wp;
     int proposal_kind = 0;                    // 0 gaussian, 1 uniform
+    // step-size auto-tuning: one step size per path component (n, a) and per parameter, adjusted every
+    // tune_skip-th iteration from the acceptance counts of the last tune_skip iterations
+    std::vector<double> ws;                   // (M+1)*D step sizes in use (all rows = wx until tuned)
+    std::vector<uint32_t> nacc_s, nacc_p;     // accepted changes since the last adjustment, per (n, a) and per parameter
+    bool tune = false; uint64_t tune_skip = 1, t_tune = 0; double f_acc = 0.23, alpha = 0.02;
     int update_mode = 0;                      // 0 = joint D-vector proposal, one decision per site (Fig. 1); 1 = one component at a time, D decisions per site (NEXT-2)
     int disc = 0;                             // model-error discretisation: 0 = explicit RK4 map (north_star), 1 = trapezoid rule (Eq. 7)
     uint64_t t = 0;                           // absolute sweep index
@@ -323,7 +328,7 @@ void propose_site(const Chain& c, uint64_t seed, int n, double* xp) {
                 const int a = 4 * b + j;
                 if (c.proposal_kind == 1) {
                     const float u = u01f_from_word(w[j]);
-                    const float step = (float)c.wx[a] * (2.0f * u - 1.0f);
+                    const float step = (float)c.ws[(size_t)n * D + a] * (2.0f * u - 1.0f);
                     xp[a] = (double)((float)xn[a] + step);
                 }
             }
@@ -335,14 +340,14 @@ void propose_site(const Chain& c, uint64_t seed, int n, double* xp) {
                     const float z[2] = {r * std::cos(ang), r * std::sin(ang)};
                     for (int j = 0; j < 2; ++j) {
                         const int a = 4 * b + 2 * pair + j;
-                        if (a < D) xp[a] = (double)((float)xn[a] + (float)c.wx[a] * z[j]);
+                        if (a < D) xp[a] = (double)((float)xn[a] + (float)c.ws[(size_t)n * D + a] * z[j]);
                     }
                 }
             }
         } else if (c.proposal_kind == 1) {
             for (int j = 0; j < 4 && 4 * b + j < D; ++j) {
                 const int a = 4 * b + j;
-                xp[a] = xn[a] + c.wx[a] * (2.0 * u01_from_word(w[j]) - 1.0);
+                xp[a] = xn[a] + c.ws[(size_t)n * D + a] * (2.0 * u01_from_word(w[j]) - 1.0);
             }
         } else {
             for (int pair = 0; pair < 2; ++pair) {
@@ -350,7 +355,7 @@ void propose_site(const Chain& c, uint64_t seed, int n, double* xp) {
                 box_muller(u01_from_word(w[2 * pair]), u01_from_word(w[2 * pair + 1]), &z[0], &z[1]);
                 for (int j = 0; j < 2; ++j) {
                     const int a = 4 * b + 2 * pair + j;
-                    if (a < D) xp[a] = xn[a] + c.wx[a] * z[j];
+                    if (a < D) xp[a] = xn[a] + c.ws[(size_t)n * D + a] * z[j];
                 }
             }
         }
@@ -386,7 +391,7 @@ void update_site(Chain& c, uint64_t seed, int n) {
             c.tr_xprop[k] = xp[a];
             c.prop[a] += 1;
             if (accept) {
-                c.acc[a] += 1;
+                c.acc[a] += 1; c.nacc_s[k] += 1;
                 c.x[k] = xp[a];
                 if (n < cache_len(c)) for (int b = 0; b < D; ++b) c.g[(size_t)n * D + b] = gp[b];
             }
@@ -400,6 +405,7 @@ void update_site(Chain& c, uint64_t seed, int n) {
     for (int a = 0; a < D; ++a) c.tr_xprop[(size_t)n * D + a] = xp[a];
     for (int a = 0; a < D; ++a) { c.prop[a] += 1; if (accept) c.acc[a] += 1; }
     if (accept) {
+        for (int a = 0; a < D; ++a) c.nacc_s[(size_t)n * D + a] += 1;     // a joint move changes every component of the site
         for (int a = 0; a < D; ++a) c.x[(size_t)n * D + a] = xp[a];
         if (n < cache_len(c)) for (int a = 0; a < D; ++a) c.g[(size_t)n * D + a] = gp[a];
     }
@@ -465,7 +471,7 @@ void parameter_moves(Chain& c, uint64_t seed) {
         const double dA = param_delta_sum(c, pnew.data(), gnew, &S);
         const bool accept = logu < -dA;
         c.tr_dAp[l] = dA; c.tr_Sp[l] = S; c.tr_accp[l] = accept ? 1 : 0;
-        if (accept) { c.p[l] = pl; c.g.swap(gnew); c.acc[D + l] += 1; }
+        if (accept) { c.p[l] = pl; c.g.swap(gnew); c.acc[D + l] += 1; c.nacc_p[l] += 1; }
     }
 }
 
@@ -495,6 +501,23 @@ void reset_moments(Chain& c) {
     std::fill(c.S1p.begin(), c.S1p.end(), 0.0); std::fill(c.S2p.begin(), c.S2p.end(), 0.0);
     std::fill(c.hist.begin(), c.hist.end(), 0ull);
     c.n_samples = 0; c.t_enable = c.t;
+}
+
+// Step-size adjustment: Delta_i <- Delta_i [1 + alpha (N_acc,i / N_skip - f_acc)] for every path component
+// and every parameter, every N_skip-th iteration while tuning is on; N_acc,i restarts from zero.
+void maybe_tune(Chain& c) {
+    if (!c.tune) return;
+    const uint64_t k = c.t - c.t_tune + 1;               // iterations completed since tuning was switched on
+    if (k % c.tune_skip != 0) return;
+    const double ns = (double)c.tune_skip;
+    for (size_t i = 0; i < c.ws.size(); ++i) {
+        c.ws[i] = c.ws[i] * (1.0 + c.alpha * ((double)c.nacc_s[i] / ns - c.f_acc));
+        c.nacc_s[i] = 0;
+    }
+    for (int l = 0; l < c.Np; ++l) {
+        c.wp[l] = c.wp[l] * (1.0 + c.alpha * ((double)c.nacc_p[l] / ns - c.f_acc));
+        c.nacc_p[l] = 0;
+    }
 }
 
 // Simulated annealing: the dynamics term A_d carries a multiplier beta that starts at beta0 < 1 and is
@@ -574,6 +597,7 @@ void* orc_create(int model, int D, int L, int M, double dt, double Rm, const dou
     c->lo.assign(c->Np, -std::numeric_limits<double>::infinity());
     c->hi.assign(c->Np, std::numeric_limits<double>::infinity());
     c->wx.assign(D, 0.0); c->wp.assign(c->Np, 0.0);
+    c->ws.assign(nx, 0.0); c->nacc_s.assign(nx, 0); c->nacc_p.assign(c->Np, 0);
     c->cx.assign(nx, 0.0); c->S1x.assign(nx, 0.0); c->S2x.assign(nx, 0.0);
     c->cp.assign(c->Np, 0.0); c->S1p.assign(c->Np, 0.0); c->S2p.assign(c->Np, 0.0);
     c->acc.assign(D + c->Np, 0); c->prop.assign(D + c->Np, 0);
@@ -644,6 +668,25 @@ void orc_set_proposal(void* h, const double* w_state, const double* w_param, int
     c.wx.assign(w_state, w_state + c.D);
     if (w_param) c.wp.assign(w_param, w_param + c.Np); else c.wp.assign(c.Np, 0.0);
     c.proposal_kind = kind;
+    c.ws.resize((size_t)(c.M + 1) * c.D);
+    for (int n = 0; n <= c.M; ++n) for (int a = 0; a < c.D; ++a) c.ws[(size_t)n * c.D + a] = c.wx[a];
+    c.nacc_s.assign(c.ws.size(), 0); c.nacc_p.assign(c.Np, 0);
+}
+// Step-size auto-tuning from the current sweep index on; enabled = 0 freezes the step sizes as they are.
+int orc_set_tuning(void* h, int enabled, uint64_t n_skip, double f_acc, double alpha) {
+    Chain& c = *(Chain*)h;
+    if (enabled && (n_skip < 1 || !(f_acc > 0.0 && f_acc < 1.0) || !(alpha >= 0.0 && alpha < 1.0))) return -1;
+    c.tune = enabled != 0;
+    if (enabled) {
+        c.tune_skip = n_skip; c.f_acc = f_acc; c.alpha = alpha; c.t_tune = c.t;
+        std::fill(c.nacc_s.begin(), c.nacc_s.end(), 0u); std::fill(c.nacc_p.begin(), c.nacc_p.end(), 0u);
+    }
+    return 0;
+}
+void orc_get_widths(void* h, double* ws, double* wp) {
+    Chain& c = *(Chain*)h;
+    if (ws) std::memcpy(ws, c.ws.data(), c.ws.size() * 8);
+    if (wp) std::memcpy(wp, c.wp.data(), c.wp.size() * 8);
 }
 void orc_set_bounds(void* h, const double* lo, const double* hi) {
     Chain& c = *(Chain*)h; c.lo.assign(lo, lo + c.Np); c.hi.assign(hi, hi + c.Np);
@@ -678,6 +721,7 @@ int orc_sweep(void* h, uint64_t n_sweeps, uint64_t seed, int order, int do_param
         half_sweep(c, seed, 1, order);
         if (do_params) parameter_moves(c, seed);
         if (c.accum && ((c.t - c.t_enable) % c.n_skip) == 0) accumulate(c);
+        maybe_tune(c);
         c.t += 1;
     }
     apply_annealing(c);          // the weights in effect always belong to the current sweep index
