@@ -118,6 +118,17 @@ int pimc_set_discretisation(pimc_handle* h, int disc);
  * schedule is over the TILE engine is used again. */
 int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool);
 
+/* Step-size auto-tuning: from the current sweep index on, every n_skip-th sweep each step size is
+ * adjusted, Delta_i <- Delta_i [1 + alpha (N_acc,i / n_skip - f_acc)], N_acc,i = accepted changes of path component
+ * i = (n, a) (joint updates: of site n) or of parameter i over the last n_skip sweeps; one step size per (site, component)
+ * and per parameter, all starting from the widths of pimc_set_proposal.  enabled = 0 freezes the step sizes as they are
+ * (they stay per-site until the next pimc_set_proposal).  Tuning biases the chain: discard its sweeps (the paper tunes during
+ * the initialisation phase only).  Runs on the GLOBAL engine, and so do sweeps with tuned step sizes
+ * (PIMC_EUNSUPPORTED if TILE is forced).  n_skip >= 1, 0 < f_acc < 1 (paper: 0.23), 0 <= alpha < 1 (paper: 0.02). */
+int pimc_set_tuning(pimc_handle* h, int enabled, long long n_skip, double f_acc, double alpha);
+/* Copy out the step sizes in use: ws_out dev (n_chains, M+1, D) double, wp_out dev (n_chains, Np) double; either may be NULL. */
+int pimc_get_widths(pimc_handle* h, double* ws_out, double* wp_out);
+
 /* Select joint or component-wise site updates (PIMC_UPDATE_*).  PIMC_EINVAL on an unknown value. */
 int pimc_set_update_mode(pimc_handle* h, int mode);
 

@@ -47,6 +47,8 @@ _SIGNATURES = {
     "pimc_set_discretisation": (C.c_int, [_vp, C.c_int]),
     "pimc_set_update_mode": (C.c_int, [_vp, C.c_int]),
     "pimc_set_annealing": (C.c_int, [_vp, C.c_double, C.c_longlong]),
+    "pimc_set_tuning": (C.c_int, [_vp, C.c_int, C.c_longlong, C.c_double, C.c_double]),
+    "pimc_get_widths": (C.c_int, [_vp, _vp, _vp]),
     "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
     "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
@@ -244,6 +246,17 @@ class Pimc:
         g = self.torch.empty((self.C, rows, self.D), dtype=self.tdtype, device=self.device)
         _check(lib().pimc_get_cache(self._h, _ptr(g)), self._h)
         return g
+
+    def set_tuning(self, enabled, n_skip=1, f_acc=0.23, alpha=0.02):
+        """Step-size auto-tuning from the current sweep on (GLOBAL engine); enabled=False freezes the step sizes."""
+        _check(lib().pimc_set_tuning(self._h, int(bool(enabled)), int(n_skip), float(f_acc), float(alpha)), self._h)
+
+    def get_widths(self):
+        t = self.torch
+        ws = t.empty((self.C, self.M + 1, self.D), dtype=t.float64, device=self.device)
+        wp = t.empty((self.C, max(self.Np, 1)), dtype=t.float64, device=self.device)
+        _check(lib().pimc_get_widths(self._h, _ptr(ws), _ptr(wp) if self.Np else None), self._h)
+        return ws, wp[:, :self.Np]
 
     def set_annealing(self, beta0, n_cool):
         """Anneal the dynamics term from the current sweep on (Eq. 10); n_cool = 0 switches it off."""

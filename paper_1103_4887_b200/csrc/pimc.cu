@@ -43,6 +43,8 @@ struct Layout {
     unsigned long long *hs_flag, *ar_flag, *ar_epoch;
     double* ar_val;
     unsigned long long *hx_words, *hx_epoch, *ar_words;
+    double *ws, *wpd;                 // tuned step sizes (C, M+1, D), (C, Np)
+    unsigned int *nacc_s, *nacc_p;    // accepted changes since the last adjustment
     int* fault;
     size_t bytes;
 };
@@ -84,6 +86,10 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     o.hx_epoch = c.take<unsigned long long>(C);
     o.hx_words = c.take<unsigned long long>((size_t)kTileMaxCtas * 2 * 2 * kHaloWordsPerSide);
     o.ar_words = c.take<unsigned long long>((size_t)2 * kTileMaxCtas * kArSlotWords);
+    o.ws = c.take<double>(nx);
+    o.wpd = c.take<double>((size_t)C * Np);
+    o.nacc_s = c.take<unsigned int>(nx);
+    o.nacc_p = c.take<unsigned int>((size_t)C * Np);
     o.fault = c.take<int>(4);
     o.bytes = (c.off + 255) & ~(size_t)255;
     return o;
@@ -112,6 +118,8 @@ struct pimc_handle {
     int disc = PIMC_DISC_RK4MAP;
     int update_mode = PIMC_UPDATE_JOINT;
     double beta0 = 1.0; unsigned long long n_cool = 0, t_anneal = 0;
+    bool site_widths = false;         // per-(site, component) step sizes in use (step-size tuning was switched on since the last set_proposal)
+    int tune = 0; unsigned long long tune_skip = 1, t_tune = 0; double f_acc = 0.23, alpha = 0.02;
     bool have_data = false, have_path = false, have_prop = false, have_I = false;
     int accum = 0;
     unsigned long long n_skip = 1, t_enable = 0, n_samples = 0, t = 0;
@@ -209,6 +217,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
     if (h->update_mode != PIMC_UPDATE_JOINT) return no("component-wise updates run on the GLOBAL engine");
+    if (h->site_widths) return no("tuned per-site step sizes run on the GLOBAL engine");
     if (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool) return no("sweeps with the annealing multiplier below 1 run on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
@@ -281,6 +290,8 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     SweepArgs<R> a{};
     a.M = h->M; a.L = h->L; a.n_chains = h->C; a.G = ls.G; a.tile = ls.tile; a.kind = h->kind;
     a.update_mode = h->update_mode;
+    a.ws = h->site_widths ? h->lay.ws : nullptr; a.nacc_s = h->lay.nacc_s; a.wpd = h->lay.wpd; a.nacc_p = h->lay.nacc_p;
+    a.tune = h->site_widths ? h->tune : 0; a.tune_skip = h->tune_skip; a.t_tune = h->t_tune; a.f_acc = h->f_acc; a.alpha = h->alpha;
     a.ln_beta0 = std::log(h->beta0); a.n_cool = h->n_cool; a.t_anneal = h->t_anneal;
     a.disc = h->disc; a.nc = h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M;
     a.dt = (R)h->dt; a.Rm = (R)h->Rm;
@@ -477,6 +488,47 @@ int pimc_get_cache(pimc_handle* h, void* g_out) {
     return PIMC_OK;
 }
 
+int pimc_set_tuning(pimc_handle* h, int enabled, long long n_skip, double f_acc, double alpha) {
+    if (!h) return PIMC_EINVAL;
+    if (!h->have_prop) return fail(h, PIMC_ESTATE, "pimc_set_tuning before pimc_set_proposal");
+    if (!enabled) { h->tune = 0; return PIMC_OK; }                  // step sizes stay as they are
+    if (n_skip < 1 || !(f_acc > 0.0 && f_acc < 1.0) || !(alpha >= 0.0 && alpha < 1.0))
+        return fail(h, PIMC_EINVAL, "tuning needs n_skip >= 1, 0 < f_acc < 1, 0 <= alpha < 1");
+    if (h->engine_user == PIMC_ENGINE_TILE) return fail(h, PIMC_EUNSUPPORTED, "step-size tuning runs on the GLOBAL engine");
+    const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
+    if (!h->site_widths) {                                           // first time: every site starts from the uniform widths
+        std::vector<double> w(nx), wp(np);
+        for (size_t i = 0; i < nx; ++i) w[i] = h->wx[i % h->D];
+        for (size_t i = 0; i < np; ++i) wp[i] = h->wp[i % h->Np];
+        PIMC_CUDA(h, cudaMemcpyAsync(h->lay.ws, w.data(), sizeof(double) * nx, cudaMemcpyHostToDevice, h->stream));
+        if (np) PIMC_CUDA(h, cudaMemcpyAsync(h->lay.wpd, wp.data(), sizeof(double) * np, cudaMemcpyHostToDevice, h->stream));
+        PIMC_CUDA(h, cudaStreamSynchronize(h->stream));
+        h->site_widths = true;
+    }
+    PIMC_CUDA(h, cudaMemsetAsync(h->lay.nacc_s, 0, sizeof(unsigned int) * nx, h->stream));
+    if (np) PIMC_CUDA(h, cudaMemsetAsync(h->lay.nacc_p, 0, sizeof(unsigned int) * np, h->stream));
+    h->tune = 1; h->tune_skip = (unsigned long long)n_skip; h->f_acc = f_acc; h->alpha = alpha; h->t_tune = h->t;
+    return PIMC_OK;
+}
+
+int pimc_get_widths(pimc_handle* h, double* ws_out, double* wp_out) {
+    if (!h) return PIMC_EINVAL;
+    if (!h->have_prop) return fail(h, PIMC_ESTATE, "no proposal widths set");
+    const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
+    if (h->site_widths) {
+        if (ws_out) PIMC_CUDA(h, cudaMemcpyAsync(ws_out, h->lay.ws, sizeof(double) * nx, cudaMemcpyDeviceToDevice, h->stream));
+        if (wp_out && np) PIMC_CUDA(h, cudaMemcpyAsync(wp_out, h->lay.wpd, sizeof(double) * np, cudaMemcpyDeviceToDevice, h->stream));
+    } else {
+        std::vector<double> w(nx), wp(np);
+        for (size_t i = 0; i < nx; ++i) w[i] = h->wx[i % h->D];
+        for (size_t i = 0; i < np; ++i) wp[i] = h->wp[i % h->Np];
+        if (ws_out) PIMC_CUDA(h, cudaMemcpyAsync(ws_out, w.data(), sizeof(double) * nx, cudaMemcpyHostToDevice, h->stream));
+        if (wp_out && np) PIMC_CUDA(h, cudaMemcpyAsync(wp_out, wp.data(), sizeof(double) * np, cudaMemcpyHostToDevice, h->stream));
+        PIMC_CUDA(h, cudaStreamSynchronize(h->stream));
+    }
+    return PIMC_OK;
+}
+
 int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool) {
     if (!h) return PIMC_EINVAL;
     if (!(beta0 > 0.0 && beta0 <= 1.0) || n_cool < 0) return fail(h, PIMC_EINVAL, "annealing needs 0 < beta0 <= 1 and n_cool >= 0");
@@ -510,6 +562,7 @@ int pimc_set_proposal(pimc_handle* h, const double* w_state, const double* w_par
     for (int l = 0; l < h->Np; ++l) h->wp[l] = w_param ? w_param[l] : 0.0;
     h->kind = kind;
     h->have_prop = true;
+    h->site_widths = false; h->tune = 0;      // uniform step sizes again
     return PIMC_OK;
 }
 

@@ -33,6 +33,15 @@ template <typename R> struct SweepArgs {
     int M, L, n_chains, G, tile, kind;
     double ln_beta0;      // simulated annealing of the dynamics term (Eq. 10): beta_k = exp(ln_beta0 (1 - k/n_cool)),
     unsigned long long n_cool, t_anneal;   //   k = t - t_anneal < n_cool, else 1; n_cool = 0 switches it off
+    // step-size auto-tuning (GLOBAL engine): per-(site, component) and per-parameter step sizes; ws == nullptr
+    // means the uniform widths wx / wp are in use
+    double* ws;           // (C, M+1, D) state step sizes
+    unsigned int* nacc_s; // (C, M+1, D) accepted changes since the last adjustment
+    double* wpd;          // (C, Np) parameter step sizes
+    unsigned int* nacc_p; // (C, Np)
+    int tune;             // adjust every tune_skip-th sweep counted from t_tune
+    unsigned long long tune_skip, t_tune;
+    double f_acc, alpha;
     int update_mode;      // 0 = joint D-vector proposal per site (Fig. 1), 1 = one component at a time, D decisions per site (GLOBAL engine)
     int disc;             // model-error discretisation: 0 = explicit RK4 map, 1 = trapezoid rule (Eq. 7)
     int nc;               // cache entries per chain: M (disc 0: g_n, n <= M-1) or M + 1 (disc 1: c_n = (dt/2) F(x_n), n <= M)
@@ -145,11 +154,14 @@ template <typename R, int D>
 __device__ __forceinline__ void propose_state(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n,
                                               const R xn[D], R xp[D]) {
     const Words4 w = draw(a.seed, t, chain, n, kStreamStateProposal, 0);
+    R wd[D];                                         // step sizes of this site: tuned per (site, component), else the uniform ones
+#pragma unroll
+    for (int c = 0; c < D; ++c) wd[c] = a.ws ? (R)a.ws[((size_t)chain * (a.M + 1) + n) * D + c] : a.wx[c];
     if (a.kind == 1) {   // uniform: x' = x + w (2u - 1)
 #pragma unroll
         for (int c = 0; c < D; ++c) {
-            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], __dmul_rn(a.wx[c], 2.0 * unit_open(w.w[c]) - 1.0));   // no FMA: bit-reproducible
-            else xp[c] = __fadd_rn(xn[c], __fmul_rn(a.wx[c], __fsub_rn(__fmul_rn(2.0f, unit_openf(w.w[c])), 1.0f)));
+            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], __dmul_rn(wd[c], 2.0 * unit_open(w.w[c]) - 1.0));   // no FMA: bit-reproducible
+            else xp[c] = __fadd_rn(xn[c], __fmul_rn(wd[c], __fsub_rn(__fmul_rn(2.0f, unit_openf(w.w[c])), 1.0f)));
         }
     } else {             // Gaussian: Box-Muller pairs from words (0,1) and (2,3)
         R z[4];
@@ -162,8 +174,8 @@ __device__ __forceinline__ void propose_state(const SweepArgs<R>& a, unsigned lo
         }
 #pragma unroll
         for (int c = 0; c < D; ++c) {
-            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], __dmul_rn(a.wx[c], z[c]));
-            else xp[c] = __fadd_rn(xn[c], __fmul_rn(a.wx[c], z[c]));
+            if constexpr (sizeof(R) == 8) xp[c] = __dadd_rn(xn[c], __dmul_rn(wd[c], z[c]));
+            else xp[c] = __fadd_rn(xn[c], __fmul_rn(wd[c], z[c]));
         }
     }
 }
@@ -302,6 +314,8 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     __shared__ R ps[NP];          // current parameters
     __shared__ R ps_prop[NP];     // parameters with the proposed entry
     __shared__ unsigned int s_pacc[NP], s_pprop[NP];
+    __shared__ double wps[NP];            // parameter step sizes in use (every CTA of a chain keeps the same copy)
+    __shared__ unsigned int s_ntune[NP];  // accepted parameter moves since the last adjustment
     __shared__ double bcast[4];
     __shared__ int s_cur;
 
@@ -319,7 +333,11 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     const R* I = a.I ? a.I + site0 : nullptr;
     unsigned long long* hs_flag = a.hs_flag + (size_t)chain * G;
 
-    if (tid < NP) { ps[tid] = a.p[(size_t)chain * NP + tid]; s_pacc[tid] = 0; s_pprop[tid] = 0; }
+    if (tid < NP) {
+        ps[tid] = a.p[(size_t)chain * NP + tid]; s_pacc[tid] = 0; s_pprop[tid] = 0;
+        wps[tid] = a.ws ? a.wpd[(size_t)chain * NP + tid] : a.wp[tid];
+        s_ntune[tid] = a.ws ? a.nacc_p[(size_t)chain * NP + tid] : 0u;
+    }
     if (tid == 0) s_cur = a.cur[chain];
     __syncthreads();
     int cur = s_cur;
@@ -354,6 +372,10 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     const unsigned mask = update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0, Rfs);
 #pragma unroll
                     for (int c = 0; c < D; ++c) n_acc_comp[c] += (mask >> c) & 1u;
+                    if (a.ws && a.tune) {        // N_acc,i of the tuning rule: this thread is the only writer of its site
+#pragma unroll
+                        for (int c = 0; c < D; ++c) a.nacc_s[(site0 + (size_t)n) * D + c] += (mask >> c) & 1u;
+                    }
                 }
                 __syncthreads();
                 if (G > 1 && tid == 0)
@@ -364,13 +386,13 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
         // ---------------- A4: parameter moves, in sequence ----------------
         if (a.do_params) {
             for (int l = 0; l < NP; ++l) {
-                if (!(a.wp[l] > 0.0)) continue;
+                if (!(wps[l] > 0.0)) continue;
                 // one thread draws the proposal and the accept uniform; everybody needs p', log u and the bounds verdict
                 if (tid == 0) {
                     const Words4 w = draw(a.seed, t, chain, (uint32_t)l, kStreamParam, 0);
                     double step;
-                    if (a.kind == 1) step = __dmul_rn(a.wp[l], 2.0 * unit_open(w.w[0]) - 1.0);
-                    else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(a.wp[l], z0); }
+                    if (a.kind == 1) step = __dmul_rn(wps[l], 2.0 * unit_open(w.w[0]) - 1.0);
+                    else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(wps[l], z0); }
                     double pl;
                     if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)ps[l], step);
                     else pl = (double)__fadd_rn(ps[l], (float)step);
@@ -454,7 +476,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     if (accept) cur ^= 1;
                 }
                 if (tid == 0) {
-                    if (accept) ps[l] = (R)pl;
+                    if (accept) { ps[l] = (R)pl; s_ntune[l] += 1u; }
                     if (b == 0) {
                         s_pprop[l] += 1;
                         if (accept) s_pacc[l] += 1;
@@ -469,7 +491,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
             }
             if (trace && b == 0 && tid == 0) {
                 for (int l = 0; l < NP; ++l)
-                    if (!(a.wp[l] > 0.0)) {
+                    if (!(wps[l] > 0.0)) {
                         if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)__longlong_as_double(0x7FF8000000000000ll);
                         if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = 0;
                         if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = ps[l];
@@ -530,6 +552,26 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
             }
             __syncthreads();   // the next half-sweep overwrites x
         }
+
+        // ---------------- step-size adjustment, every tune_skip-th sweep while tuning ----------------
+        // Delta_i <- Delta_i [1 + alpha (N_acc,i / N_skip - f_acc)]; written without FMA contraction, so that the step sizes
+        // (and with them the proposals) stay bit-identical to the oracle's
+        if (a.ws && a.tune && ((t - a.t_tune + 1ull) % a.tune_skip) == 0ull) {
+            __syncthreads();
+            const double ns = (double)a.tune_skip;
+            for (int idx = s * D + tid; idx < e * D; idx += T) {
+                const size_t gi = site0 * D + (size_t)idx;
+                const double rate = __ddiv_rn((double)a.nacc_s[gi], ns);
+                a.ws[gi] = __dmul_rn(a.ws[gi], __dadd_rn(1.0, __dmul_rn(a.alpha, __dsub_rn(rate, a.f_acc))));
+                a.nacc_s[gi] = 0u;
+            }
+            if (tid < NP) {
+                const double rate = __ddiv_rn((double)s_ntune[tid], ns);
+                wps[tid] = __dmul_rn(wps[tid], __dadd_rn(1.0, __dmul_rn(a.alpha, __dsub_rn(rate, a.f_acc))));
+                s_ntune[tid] = 0u;
+            }
+            __syncthreads();
+        }
     }
 
     // ---------------- A6 + state write-back ----------------
@@ -552,6 +594,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     cnt[D + l] += s_pacc[l];
                     cnt[(D + NP) + D + l] += s_pprop[l];
                     a.p[(size_t)chain * NP + l] = ps[l];
+                    if (a.ws) { a.wpd[(size_t)chain * NP + l] = wps[l]; a.nacc_p[(size_t)chain * NP + l] = s_ntune[l]; }
                 }
                 a.cur[chain] = cur;
                 a.ar_epoch[chain] = ar_count;
