@@ -100,6 +100,8 @@ template <typename R> struct TileSmem {
     double *blo, *bhi;          // [kMaxNp] bounds
     double *pS1, *pS2, *pcc;    // [kMaxNp] running moments of the parameters (tile 0 of each chain)
     R *xs, *g0, *g1;            // [2*D*P]
+    R *wsx;                     // [2*D*P] step sizes of every tile site (tuned per (site, component), else the uniform widths)
+    double *wpl;                // [kMaxNp] parameter step sizes in use
     R *kg;                      // [2*NK*P] parameter-independent first-stage rates of every tile site (Model::stage1_cache)
     R *Is, *ys;                 // [E+2], [E*L]
     R *rstep, *rlogu;           // [2 sets][2 parities][D][TC], [2][2][TC]
@@ -112,9 +114,9 @@ __host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512)
 
 template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
-    size_t dbl = 3 * 2 * D * P + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
+    size_t dbl = 3 * 2 * D * P + kMaxNp + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
     const size_t RP = P - 2;
-    size_t real = 3 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
+    size_t real = 4 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
     (void)TC;
     return dbl * 8 + ((real * sizeof(R) + 15) & ~(size_t)15) + 16;
 }
@@ -128,6 +130,7 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.S2 = d; d += 2 * D * P;
     m.cc = d; d += 2 * D * P;
     m.red = d; d += 64;
+    m.wpl = d; d += kMaxNp;
     m.pdraw = d; d += 2 * kMaxNp * 2;
     m.blo = d; d += kMaxNp;
     m.bhi = d; d += kMaxNp;
@@ -140,6 +143,7 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.g0 = r; r += 2 * D * P;
     m.g1 = r; r += 2 * D * P;
     m.kg = r; r += 2 * (size_t)NK * P;
+    m.wsx = r; r += 2 * D * P;
     m.Is = r; r += E + 2;
     m.ys = r; r += E * (size_t)(L > 0 ? L : 1);
     m.rstep = r; r += 4 * (P - 2) * D;
@@ -163,14 +167,15 @@ template <typename R, int D> __device__ __forceinline__ void sts_site(R* base, i
 
 // ---- producer: proposal steps w_a z_a and log u for one site of one half-sweep (row A1) ----------------------
 template <typename R, int D>
-__device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n, R* step_out, int stride, R* logu_out) {
+__device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned long long t, uint32_t chain, uint32_t n, const R* wsite, int wstride,
+                                             R* step_out, int stride, R* logu_out) {
     const Words4 w = draw(a.seed, t, chain, n, kStreamStateProposal, 0);
     R st[4] = {R(0), R(0), R(0), R(0)};
     if (a.kind == 1) {
 #pragma unroll
         for (int c = 0; c < D; ++c) {
-            if constexpr (sizeof(R) == 8) st[c] = __dmul_rn(a.wx[c], 2.0 * unit_open(w.w[c]) - 1.0);
-            else st[c] = __fmul_rn(a.wx[c], __fsub_rn(__fmul_rn(2.0f, unit_openf(w.w[c])), 1.0f));
+            if constexpr (sizeof(R) == 8) st[c] = __dmul_rn(wsite[c * wstride], 2.0 * unit_open(w.w[c]) - 1.0);
+            else st[c] = __fmul_rn(wsite[c * wstride], __fsub_rn(__fmul_rn(2.0f, unit_openf(w.w[c])), 1.0f));
         }
     } else {
         R z[4] = {R(0), R(0), R(0), R(0)};
@@ -183,8 +188,8 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
         }
 #pragma unroll
         for (int c = 0; c < D; ++c) {
-            if constexpr (sizeof(R) == 8) st[c] = __dmul_rn(a.wx[c], z[c]);
-            else st[c] = __fmul_rn(a.wx[c], z[c]);
+            if constexpr (sizeof(R) == 8) st[c] = __dmul_rn(wsite[c * wstride], z[c]);
+            else st[c] = __fmul_rn(wsite[c * wstride], z[c]);
         }
     }
 #pragma unroll
@@ -233,6 +238,9 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         sm.Is[i] = (a.I && n <= M) ? a.I[site0 + n] : R(0);
     }
     for (int idx = tid; idx < n_ext * L; idx += T) sm.ys[idx] = a.y[(site0 + s_ext) * L + idx];
+    for (int idx = tid; idx < n_ext * D; idx += T)      // step sizes: frozen tuned values per (site, component), else the uniform ones
+        sm.wsx[so<D>(idx / D, idx % D, P)] = a.ws ? (R)a.ws[(site0 + s_ext) * D + idx] : a.wx[idx % D];
+    if (tid < NP) sm.wpl[tid] = a.ws ? a.wpd[(size_t)chain * NP + tid] : a.wp[tid];
     if (a.accum) {
         for (int idx = tid; idx < n_ext * D; idx += T) {
             const size_t gi = (site0 + s_ext) * D + idx;
@@ -265,19 +273,20 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             for (int parity = 0; parity < 2; ++parity) {
                 const int n = s_ext + 2 * j + parity;
                 if (n <= M && 2 * j + parity < n_ext)
-                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.rstep + (size_t)(set * 2 + parity) * D * RP + j, RP,
+                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.wsx + parity * D * P + j, P, sm.rstep + (size_t)(set * 2 + parity) * D * RP + j, RP,
                                        sm.rlogu + (size_t)(set * 2 + parity) * RP + j);
             }
         }
-        if (a.do_params && j < NP && a.wp[j] > 0.0) {
+        if (a.do_params && j < NP && sm.wpl[j] > 0.0) {
             const Words4 w = draw(a.seed, t, chain, (uint32_t)j, kStreamParam, 0);
             double step;
-            if (a.kind == 1) step = __dmul_rn(a.wp[j], 2.0 * unit_open(w.w[0]) - 1.0);
-            else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(a.wp[j], z0); }
+            if (a.kind == 1) step = __dmul_rn(sm.wpl[j], 2.0 * unit_open(w.w[0]) - 1.0);
+            else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(sm.wpl[j], z0); }
             sm.pdraw[(set * kMaxNp + j) * 2 + 0] = step;
             sm.pdraw[(set * kMaxNp + j) * 2 + 1] = log_fast(unit_open52(w.w[2], w.w[3]));
         }
     };
+    __syncthreads();                               // the step sizes the producers read were loaded by other threads
     if (tid >= TC) produce(0, a.t0);
     __syncthreads();
 
@@ -418,7 +427,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             bool params_changed = false;
 #pragma unroll 1
             for (int l = 0; l < NP; ++l) {
-                if (!(a.wp[l] > 0.0)) continue;
+                if (!(sm.wpl[l] > 0.0)) continue;
                 const double step = sm.pdraw[(set * kMaxNp + l) * 2 + 0], logu = sm.pdraw[(set * kMaxNp + l) * 2 + 1];
                 R pcur = R(0);
 #pragma unroll
@@ -514,7 +523,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             if (trace && b == 0 && tid == 0) {
 #pragma unroll
                 for (int l = 0; l < NP; ++l)
-                    if (!(a.wp[l] > 0.0)) {
+                    if (!(sm.wpl[l] > 0.0)) {
                         if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)__longlong_as_double(0x7FF8000000000000ll);
                         if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = 0;
                         if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = prm[l];

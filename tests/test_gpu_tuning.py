@@ -20,7 +20,7 @@ def P():
     return P
 
 
-@pytest.mark.parametrize("cfg,M,launch,mode,disc", [(2, 500, None, 0, 0), (2, 501, (4, 64), 0, 0), (2, 400, (1, 128), 1, 0), (2, 333, (3, 64), 1, 1),
+@pytest.mark.parametrize("cfg,M,launch,mode,disc", [(2, 500, None, 0, 0), (3, 4001, None, 0, 1), (2, 501, (4, 64), 0, 0), (2, 400, (1, 128), 1, 0), (2, 333, (3, 64), 1, 1),
                                                     (1, 700, (3, 128), 0, 0)])
 def test_tuned_chains_and_step_sizes_bit_identical(P, cfg, M, launch, mode, disc):
     w = make_workload(cfg, M=M)
@@ -39,8 +39,11 @@ def test_tuned_chains_and_step_sizes_bit_identical(P, cfg, M, launch, mode, disc
     assert not np.array_equal(ows, np.tile(w.w_state, (M + 1, 1)))        # they did move
     xg, pg = [a.cpu().numpy() for a in h.get_path()]
     assert np.array_equal(xg[0], o.get_path()[0]) and np.array_equal(pg[0], o.get_path()[1])
-    # freeze: the tuned step sizes stay in use, unchanged
+    # freeze: the tuned step sizes stay in use, unchanged -- and the automatic engine choice is free again (the tile-resident
+    # engine reads the frozen per-site step sizes; component-wise updates stay on the global-memory engine)
     h.set_tuning(False); o.set_tuning(False)
+    if launch is None and mode == 0:
+        assert h.get_engine()["engine"] == P.ENGINE_TILE
     h.sweep(9, seed=5); o.sweep(9, seed=5)
     assert np.array_equal(h.get_widths()[0].cpu().numpy()[0], ows)
     assert np.array_equal(h.get_path()[0].cpu().numpy()[0], o.get_path()[0])
@@ -78,6 +81,8 @@ def test_batched_chains_gaussian_proposals_and_engine_rule(P):
     assert h4.get_engine()["engine"] == Pm.ENGINE_TILE
     h4.set_tuning(True, 5)
     assert h4.get_engine()["engine"] == Pm.ENGINE_GLOBAL
+    h4.set_tuning(False)
+    assert h4.get_engine()["engine"] == Pm.ENGINE_TILE
     for bad in ((0, 0.23, 0.02), (5, 0.0, 0.02), (5, 0.23, 1.0)):
         with pytest.raises(Pm.PimcError):
             h4.set_tuning(True, *bad)
