@@ -10,5 +10,5 @@ that integrator for anything they compute.
 """
 from .configs import (  # noqa: F401
     MODEL_LINEAR, MODEL_HH, MODEL_HH_CLASSIC, HH_P_TRUE, Workload, make_workload, hh_truth, linear_truth,
-    linear_matrix, N_CONFIGS,
+    linear_matrix, N_CONFIGS, lorenz_current, PAPER_P_TRUE,
 )

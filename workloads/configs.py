@@ -52,18 +52,48 @@ def _hh_rhs_batch(x, I, p, kinetics="tanh"):
     return out
 
 
-def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1, kinetics: str = "tanh"):
+def lorenz_current(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1, ms_per_unit: float = 20.0,
+                   offset: float = 5.0, gain: float = 0.7):
+    """Chaotic stimulus for the paper-shaped workload ("a chaotic stimulus current generated from one of the
+    variables of the Lorenz model").  The paper's series is not available and its scaling is not stated: the x variable of
+    the Lorenz-63 system (sigma = 10, rho = 28, beta = 8/3), one Lorenz time unit = ms_per_unit ms, I = offset + gain * x
+    uA/cm2 (about -9 .. 19), started from a seeded point after a transient.  Returns I (C, M+1)."""
+    h = dt / ms_per_unit
+    sub = max(1, int(np.ceil(h / 0.002)))
+    hs = h / sub
+
+    def f(u):
+        return np.stack([10.0 * (u[:, 1] - u[:, 0]), u[:, 0] * (28.0 - u[:, 2]) - u[:, 1], u[:, 0] * u[:, 1] - (8.0 / 3.0) * u[:, 2]], axis=1)
+
+    def step(u):
+        k1 = f(u); k2 = f(u + 0.5 * hs * k1); k3 = f(u + 0.5 * hs * k2); k4 = f(u + hs * k3)
+        return u + (hs / 6.0) * (k1 + 2 * k2 + 2 * k3 + k4)
+
+    u = np.array([1.0, 1.0, 20.0])[None, :] + rng.normal(size=(n_chains, 3))
+    for _ in range(int(20.0 / hs)):                      # transient onto the attractor
+        u = step(u)
+    I = np.empty((n_chains, M + 1))
+    for k in range(M + 1):
+        I[:, k] = offset + gain * u[:, 0]
+        for _ in range(sub):
+            u = step(u)
+    return I
+
+
+def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1, kinetics: str = "tanh", I=None, p=None,
+             noise_sd: float = 1.0):
     """Twin-experiment data: returns I (C,M+1), x_true (C,M+1,4), y (C,M+1).
 
     Step current: 5 ms segments, segment k covers steps [k*5/dt, (k+1)*5/dt), amplitude U(0,15) uA/cm2.
     Truth: RK4 at dt with midpoint current 0.5*(I_n + I_{n+1}); x(0) = rest at -65 mV.
     Observation: V + N(0, 1 mV).
     """
-    seg = int(round(5.0 / dt))
-    nseg = M // seg + 2
-    amp = rng.uniform(0.0, 15.0, size=(n_chains, nseg))
-    idx = np.arange(M + 1) // seg
-    I = amp[:, idx]
+    if I is None:
+        seg = int(round(5.0 / dt))
+        nseg = M // seg + 2
+        amp = rng.uniform(0.0, 15.0, size=(n_chains, nseg))
+        idx = np.arange(M + 1) // seg
+        I = amp[:, idx]
     x = np.empty((n_chains, M + 1, 4))
     V0 = -65.0
     x[:, 0, 0] = V0
@@ -73,7 +103,7 @@ def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1, kin
     if kinetics == "classic":
         for j, (al, be) in enumerate(_classic_rates(np.float64(V0)), start=1):
             x[:, 0, j] = al / (al + be)
-    p = HH_P_TRUE
+    p = HH_P_TRUE if p is None else p
     for k in range(M):
         xn = x[:, k]
         I0, I1 = I[:, k], I[:, k + 1]
@@ -83,7 +113,7 @@ def hh_truth(M: int, dt: float, rng: np.random.Generator, n_chains: int = 1, kin
         k3 = _hh_rhs_batch(xn + 0.5 * dt * k2, Ih, p, kinetics)
         k4 = _hh_rhs_batch(xn + dt * k3, I1, p, kinetics)
         x[:, k + 1] = xn + (dt / 6.0) * (k1 + 2 * k2 + 2 * k3 + k4)
-    y = x[:, :, 0] + rng.normal(0.0, 1.0, size=(n_chains, M + 1))
+    y = x[:, :, 0] + rng.normal(0.0, noise_sd, size=(n_chains, M + 1))
     return I, x, y
 
 
@@ -186,4 +216,36 @@ def make_workload(cfg: int, *, M: int | None = None, n_chains: int | None = None
     if cfg == 4:
         return _hh_workload("cfg4_hh_128x8192_params", 4, M or 8192, 0.02, n_chains or 128,
                             _WP_CFG2 / np.sqrt(2.0), 5000, True, seed, kinetics)
+    if cfg == 5:
+        return _paper_workload(M or 8000, n_chains or 1, seed, kinetics)
     raise ValueError(f"no config {cfg}")
+
+
+# PAPER.md:282-284, Table 2, in this build's conventions: rest at -65 mV instead of 0 (E_Na = 115 - 65,
+# E_K = -12 - 65, E_L = 10.6 - 65) and physical parameters (gNa, gK, gL, ENa, EK, EL, C) instead of (p_1..p_7).
+PAPER_P_TRUE = np.array([120.0, 20.0, 0.3, 50.0, -77.0, -54.4, 1.0])
+
+
+def _paper_workload(M, n_chains, seed, kinetics):
+    """The paper's own experiment shape: M = 8000 steps of dt = 0.04 ms (25 kHz,
+    320 ms), Lorenz-driven current, R_d = diag(100, 1e6, 1e6, 1e6), R_o = 100, gK = 20, initial step sizes 2e-3 (V) and 1e-3
+    (gates), to be tuned.  Synthetic regeneration: the original series is not available.  Meant for the trapezoid
+    discretisation with annealing (beta0 = 0.01) and step-size tuning (f_acc = 0.23, alpha = 0.02, N_skip = 400)."""
+    dt = 0.04
+    rng = np.random.default_rng(DATA_SEED0 + 5 if seed is None else seed)
+    I = lorenz_current(M, dt, rng, n_chains)
+    pt = PAPER_P_TRUE
+    I, xt, y = hh_truth(M, dt, rng, n_chains, kinetics, I=I, p=pt, noise_sd=0.1)     # R_o = 100 <=> sd 0.1 mV
+    x0 = np.empty((n_chains, M + 1, 4))
+    x0[:, :, 0] = y
+    x0[:, :, 1:] = 0.5
+    sgn = np.where(rng.random((n_chains, 7)) < 0.5, -1.0, 1.0)
+    p0 = pt[None, :] * (1.0 + 0.2 * sgn)
+    lo = np.tile(pt - 0.5 * np.abs(pt), (n_chains, 1))
+    hi = np.tile(pt + 0.5 * np.abs(pt), (n_chains, 1))
+    return Workload(name="cfg5_paper_shape_M8000" + ("_classic" if kinetics == "classic" else ""),
+                    model=MODEL_HH_CLASSIC if kinetics == "classic" else MODEL_HH, D=4, L=1, Np=7, M=M, dt=dt, Rm=100.0,
+                    Rf=np.array([1e2, 1e6, 1e6, 1e6]), n_chains=n_chains, p0=p0, p_true=pt.copy(), lo=lo, hi=hi,
+                    w_state=np.array([2e-3, 1e-3, 1e-3, 1e-3]), w_param=1e-3 * np.abs(pt), y=y[:, :, None].copy(), I=I, x0=x0,
+                    x_true=xt, n_sweeps=1000000,
+                    extra=dict(n_init=500000, n_cool=100000, beta0=0.01, f_acc=0.23, alpha=0.02, n_skip=400, disc="trapezoid"))
