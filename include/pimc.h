@@ -69,8 +69,7 @@ enum { PIMC_DISC_RK4MAP = 0, PIMC_DISC_TRAPEZOID = 1 };
  * acceptance counters per component).  JOINT (default): x'_n = x_n + w o z, one decision per site.  COMPONENTWISE: for
  * a = 0..D-1 in order, x'_{n,a} = x_{n,a} + w_a z_a (the same draw z_a as the joint move) with the other components as they
  * stand, its own Delta-A and decision (accept uniform = words 0,1 of block a of the accept stream); D decisions and D model
- * evaluations per site.  Runs on the GLOBAL engine (the automatic engine choice falls back to it; PIMC_EUNSUPPORTED if the
- * TILE engine is forced).  With the debug trace on, dA_out and acc_out are (n_chains, M+1, D) and xprop_out holds the proposed
+ * evaluations per site.  Both engines (TILE: at most 256 threads per CTA).  With the debug trace on, dA_out and acc_out are (n_chains, M+1, D) and xprop_out holds the proposed
  * value of each component. */
 enum { PIMC_UPDATE_JOINT = 0, PIMC_UPDATE_COMPONENTWISE = 1 };
 

@@ -19,6 +19,7 @@ NVCC_FLAGS = [
     # IEEE arithmetic everywhere except FMA contraction: never --use_fast_math
     "-ftz=false", "-prec-div=true", "-prec-sqrt=true", "-fmad=true",
     "--shared", "-Xcompiler", "-fPIC",
+    # no --split-compile: parallel ptxas builds 2.4x faster but the same source then runs 5 % slower (measured)
 ]
 
 

@@ -216,13 +216,14 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int sites = h->M + 1;
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
-    if (h->update_mode != PIMC_UPDATE_JOINT) return no("component-wise updates run on the GLOBAL engine");
     if (h->site_widths && h->tune) return no("step-size tuning runs on the GLOBAL engine (frozen tuned step sizes run on both)");
     if (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool) return no("sweeps with the annealing multiplier below 1 run on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
-    if (T != 0 && (T % 64 != 0 || T > 512)) return no("threads_per_cta must be a multiple of 64, at most 512");
-    const int Tmax = T ? T : 512;
+    // the 512-thread instantiation exists for the RK4-map, joint-update kernel only (build time); the others stop at 256
+    const int Tcap = (h->disc != PIMC_DISC_RK4MAP || h->update_mode != PIMC_UPDATE_JOINT) ? 256 : 512;
+    if (T != 0 && (T % 64 != 0 || T > Tcap)) return no("threads_per_cta must be a multiple of 64, at most 512 (256 for the trapezoid rule or component-wise updates)");
+    const int Tmax = T ? T : Tcap;
     const int h_want = h->halo_user >= 0 ? h->halo_user : kTileHaloMax;
     if (G == 0) {
         if (sites <= (T ? T : 256)) G = 1;                          // whole chain in one CTA: no hand-off at all
@@ -252,9 +253,9 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
         if (hh < 2) return no("tile plus halos does not fit the CTA");
     }
     if (T == 0) T = std::max(64, (tile + 2 * hh + 63) / 64 * 64);
-    if (tile + 2 * hh > T || T > 512) return no("tile plus halos does not fit the CTA");
+    if (tile + 2 * hh > T || T > Tcap) return no("tile plus halos does not fit the CTA");
     out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1; out->engine = PIMC_ENGINE_TILE; out->h = hh;
-    out->smem = tile_smem_bytes<R>(T, h->D, h->L, h->disc == PIMC_DISC_TRAPEZOID ? 0 : Model::NK);
+    out->smem = tile_smem_bytes<R>(T, h->D, h->L, h->disc == PIMC_DISC_TRAPEZOID ? 0 : Model::NK, h->update_mode == PIMC_UPDATE_COMPONENTWISE ? h->D : 1);
     if (out->smem > 227 * 1024) return no("shared memory");
     return PIMC_OK;
 }
@@ -316,8 +317,16 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     const bool trap = h->disc == PIMC_DISC_TRAPEZOID;
     const void* fn = (const void*)sweep_kernel<Model, R>;
     if (ls.engine == PIMC_ENGINE_TILE) {
-        if (ls.T <= 256) fn = trap ? (const void*)tile_sweep_kernel<Model, R, 256, true> : (const void*)tile_sweep_kernel<Model, R, 256, false>;
-        else fn = trap ? (const void*)tile_sweep_kernel<Model, R, 512, true> : (const void*)tile_sweep_kernel<Model, R, 512, false>;
+        const bool comp = h->update_mode == PIMC_UPDATE_COMPONENTWISE;
+        const int sel = (ls.T <= 256 ? 0 : 4) + (trap ? 2 : 0) + (comp ? 1 : 0);
+        switch (sel) {
+            case 0: fn = (const void*)tile_sweep_kernel<Model, R, 256, false, false>; break;
+            case 1: fn = (const void*)tile_sweep_kernel<Model, R, 256, false, true>; break;
+            case 2: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, false>; break;
+            case 3: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, true>; break;
+            case 4: fn = (const void*)tile_sweep_kernel<Model, R, 512, false, false>; break;
+            default: return fail(h, PIMC_EUNSUPPORTED, "no 512-thread tile kernel for this discretisation / update mode");   // choose_shape_tile never offers it
+        }
     }
     if (ls.smem > 48 * 1024) PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
     void* params[] = {&a};
@@ -539,8 +548,6 @@ int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool) {
 int pimc_set_update_mode(pimc_handle* h, int mode) {
     if (!h) return PIMC_EINVAL;
     if (!(mode == PIMC_UPDATE_JOINT || mode == PIMC_UPDATE_COMPONENTWISE)) return fail(h, PIMC_EINVAL, "unknown update mode %d", mode);
-    if (mode == PIMC_UPDATE_COMPONENTWISE && h->engine_user == PIMC_ENGINE_TILE)
-        return fail(h, PIMC_EUNSUPPORTED, "component-wise updates run on the GLOBAL engine");
     h->update_mode = mode;
     return PIMC_OK;
 }

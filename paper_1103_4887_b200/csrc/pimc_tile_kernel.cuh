@@ -104,24 +104,24 @@ template <typename R> struct TileSmem {
     double *wpl;                // [kMaxNp] parameter step sizes in use
     R *kg;                      // [2*NK*P] parameter-independent first-stage rates of every tile site (Model::stage1_cache)
     R *Is, *ys;                 // [E+2], [E*L]
-    R *rstep, *rlogu;           // [2 sets][2 parities][D][TC], [2][2][TC]
-    unsigned int* cnt;          // [2]: accepted owned state updates (lo, unused)
+    R *rstep, *rlogu;           // [2 sets][2 parities][npass][D][RP], [2][2][npass][RP]
+    unsigned int* cnt;          // [4]: accepted owned state updates per component class
     int P;
 };
 
 // the pitch is a compile-time constant of the kernel instantiation (MAXT = 256 or 512), so plane offsets are immediates
 __host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512) / 2 + 2; }
 
-template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK) {
+template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK, int npass) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     size_t dbl = 3 * 2 * D * P + kMaxNp + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
     const size_t RP = P - 2;
-    size_t real = 4 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * RP * D + 4 * RP;
+    size_t real = 4 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * (size_t)npass * RP * D + 4 * (size_t)npass * RP;
     (void)TC;
     return dbl * 8 + ((real * sizeof(R) + 15) & ~(size_t)15) + 16;
 }
 
-template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L, int NK) {
+template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L, int NK, int npass) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     TileSmem<R> m;
     m.P = (int)P;
@@ -137,7 +137,7 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.pS1 = d; d += kMaxNp;
     m.pS2 = d; d += kMaxNp;
     m.pcc = d; d += kMaxNp;
-    m.cnt = reinterpret_cast<unsigned int*>(d); d += 2;
+    m.cnt = reinterpret_cast<unsigned int*>(d); d += 2;      // 2 doubles = 4 counters
     R* r = reinterpret_cast<R*>(d);
     m.xs = r; r += 2 * D * P;
     m.g0 = r; r += 2 * D * P;
@@ -146,8 +146,8 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.wsx = r; r += 2 * D * P;
     m.Is = r; r += E + 2;
     m.ys = r; r += E * (size_t)(L > 0 ? L : 1);
-    m.rstep = r; r += 4 * (P - 2) * D;
-    m.rlogu = r; r += 4 * (P - 2);
+    m.rstep = r; r += 4 * (size_t)npass * (P - 2) * D;
+    m.rlogu = r; r += 4 * (size_t)npass * (P - 2);
     (void)TC;
     return m;
 }
@@ -201,14 +201,19 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
 // ---- the kernel ----------------------------------------------------------------------------------------------
 // TRAP selects the paper's trapezoid discretisation (Eq. 7): the cache holds c_n = (dt/2) F(x_n) for n = 0..M,
 // every residual is (x_{k+1} - x_k) - c_k - c_{k+1}, the model step is ONE right-hand side, and there is no stage-1 cache.
-template <class Model, typename R, int MAXT, bool TRAP>
+// COMP selects component-wise updates (D passes per half-sweep); as a compile-time flag it leaves the joint kernel exactly as it was.
+template <class Model, typename R, int MAXT, bool TRAP, bool COMP>
 __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
     extern __shared__ __align__(16) unsigned char tile_smem_raw[];
     const int T = blockDim.x, TC = T >> 1, tid = threadIdx.x;
     constexpr int NK = TRAP ? 0 : Model::NK;
-    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK);
+    // Component-wise updates (SweepArgs::update_mode = 1) run D PASSES per half-sweep through the same site update: pass c gets a
+    // step vector that is zero except in component c and the accept uniform of block c (drawn by the producer warps), which is
+    // exactly a single-component Metropolis move; a joint sweep has one pass.
+    constexpr int npass = COMP ? D : 1;
+    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK, npass);
     constexpr int RP = MAXT / 2;                   // pitch of the random-number ring
     constexpr int P = MAXT / 2 + 2;                // == tile_pitch(T): the launcher picks MAXT = 256 for T <= 256, else 512
 
@@ -253,7 +258,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         }
     }
     if (tid < NP) { sm.blo[tid] = a.lo[(size_t)chain * NP + tid]; sm.bhi[tid] = a.hi[(size_t)chain * NP + tid]; }
-    if (tid == 0) { sm.cnt[0] = 0; }
+    if (tid < 4) { sm.cnt[tid] = 0; }
     R prm[NP];                                     // every thread keeps the (identical) parameter vector in registers
 #pragma unroll
     for (int k = 0; k < NP; ++k) prm[k] = a.p[(size_t)chain * NP + k];
@@ -261,7 +266,9 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     unsigned long long ar_count = a.ar_epoch[chain];
     unsigned long long hx_count = a.hx_epoch[chain];
     unsigned long long skip_ctr = a.skip0;         // (t - t_enable) mod n_skip, kept as a counter (no 64-bit division in the loop)
-    unsigned int n_acc_state = 0, pacc[NP], pprop[NP];
+    unsigned int n_acc_state = 0, n_acc_c[D], pacc[NP], pprop[NP];
+#pragma unroll
+    for (int c = 0; c < D; ++c) n_acc_c[c] = 0;
 #pragma unroll
     for (int k = 0; k < NP; ++k) { pacc[k] = 0; pprop[k] = 0; }
 
@@ -272,9 +279,22 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
 #pragma unroll 1
             for (int parity = 0; parity < 2; ++parity) {
                 const int n = s_ext + 2 * j + parity;
-                if (n <= M && 2 * j + parity < n_ext)
-                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.wsx + parity * D * P + j, P, sm.rstep + (size_t)(set * 2 + parity) * D * RP + j, RP,
-                                       sm.rlogu + (size_t)(set * 2 + parity) * RP + j);
+                if (n <= M && 2 * j + parity < n_ext) {
+                    R* so_step = sm.rstep + (size_t)((set * 2 + parity) * npass) * D * RP + j;
+                    R* so_logu = sm.rlogu + (size_t)((set * 2 + parity) * npass) * RP + j;
+                    produce_site<R, D>(a, t, chain, (uint32_t)n, sm.wsx + parity * D * P + j, P, so_step, RP, so_logu);
+                    if (npass > 1) {        // pass c: the joint step masked to component c, accept uniform of block c
+                        R st[D];
+#pragma unroll
+                        for (int c = 0; c < D; ++c) st[c] = so_step[c * RP];
+#pragma unroll
+                        for (int c = 0; c < D; ++c) {
+#pragma unroll
+                            for (int c2 = 0; c2 < D; ++c2) so_step[((size_t)c * D + c2) * RP] = (c2 == c) ? st[c] : R(0);
+                            if (c > 0) so_logu[(size_t)c * RP] = log_accept_uniform<R>(a, t, chain, (uint32_t)n, (uint32_t)c);
+                        }
+                    }
+                }
             }
         }
         if (a.do_params && j < NP && sm.wpl[j] > 0.0) {
@@ -324,7 +344,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             // ---------------- A2: even half-sweep, then odd half-sweep (compute warps) ----------------
             if (a.do_states) {
 #pragma unroll 1
-                for (int q = 0; q < 2; ++q) {
+                for (int hs = 0; hs < 2 * npass; ++hs) {
+                    const int q = hs >= npass ? 1 : 0, pass = hs - q * npass;
+                    const bool acc_here = acc_now && pass == npass - 1;       // the site's value is final after its last pass
+                    const unsigned acc_before = n_acc_state;
                     const int k = k_phase + q + 1;           // half-sweeps run on the current halos, this one included
                     const int iloc = 2 * tid + q, n = s_ext + iloc;
                     const bool ok = n <= M && iloc < n_ext && (edge_lo || iloc >= k) && (edge_hi || iloc < n_ext - k);
@@ -336,7 +359,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         const bool has_l = n >= 1, has_r = n <= M - 1;
                         const int jl = max(tid - 1 + q, 0), jr = tid + q;   // pair index of the left / right neighbour (plane 1 - q)
                         const int own = q * D * P + tid, oth = (1 - q) * D * P;
-                        const R* ring = sm.rstep + (size_t)(set * 2 + q) * D * RP + tid;
+                        const R* ring = sm.rstep + (size_t)(set * 2 * npass + hs) * D * RP + tid;
                         R xn[D], xp[D], gp[D], xm[D], gm[D], xq[D], gn[D];
                         [[maybe_unused]] R gq[D];          // trapezoid: the right neighbour's cache entry c_{n+1}
                         double mc[D], m1[D], m2[D];
@@ -355,7 +378,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             if constexpr (TRAP) gq[c] = gc[oth + c * P + jr];
                             mc[c] = sm.cc[own + c * P]; m1[c] = sm.S1[own + c * P]; m2[c] = sm.S2[own + c * P];
                         }
-                        const R logu = sm.rlogu[(size_t)(set * 2 + q) * RP + tid];
+                        const R logu = sm.rlogu[(size_t)(set * 2 * npass + hs) * RP + tid];
                         R kgo[NK > 0 ? NK : 1], kgn[NK > 0 ? NK : 1];
 #pragma unroll
                         for (int c = 0; c < NK; ++c) kgo[c] = sm.kg[(q * NK + c) * P + tid];
@@ -397,17 +420,31 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             gc[own + c * P] = keep_g ? gp[c] : gn[c];
                             // A5 for this site: its value is final for sweep t (parameter moves do not touch x)
                             const double d = (double)xf - mc[c];
-                            sm.S1[own + c * P] = acc_now ? m1[c] + d : m1[c];
-                            sm.S2[own + c * P] = acc_now ? m2[c] + d * d : m2[c];
+                            sm.S1[own + c * P] = acc_here ? m1[c] + d : m1[c];
+                            sm.S2[own + c * P] = acc_here ? m2[c] + d * d : m2[c];
                         }
                         const bool owned = n >= s && n < e;
                         n_acc_state += (owned && accept) ? 1u : 0u;
                         if (trace && owned) {
                             const size_t gs = site0 + (size_t)n;
-                            if (a.tr_dA) a.tr_dA[gs] = dA;
-                            if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
-                            if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
+                            if (npass > 1) {       // trace entries per (site, component)
+                                R xa = R(0);
+#pragma unroll
+                                for (int c = 0; c < D; ++c) xa = (c == pass) ? xp[c] : xa;
+                                if (a.tr_dA) a.tr_dA[gs * D + pass] = dA;
+                                if (a.tr_acc) a.tr_acc[gs * D + pass] = accept ? 1 : 0;
+                                if (a.tr_xprop) a.tr_xprop[gs * D + pass] = xa;
+                            } else {
+                                if (a.tr_dA) a.tr_dA[gs] = dA;
+                                if (a.tr_acc) a.tr_acc[gs] = accept ? 1 : 0;
+                                if (a.tr_xprop) store_vec<R, D>(a.tr_xprop, gs, xp);
+                            }
                         }
+                    }
+                    if (npass > 1) {                                          // A6 per component class (a joint move counts for all)
+                        const unsigned delta = n_acc_state - acc_before;
+#pragma unroll
+                        for (int c = 0; c < D; ++c) n_acc_c[c] += (c == pass) ? delta : 0u;
                     }
                     bar_compute(TC);
                 }
@@ -646,13 +683,17 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             a.S1p[gi] = sm.pS1[tid]; a.S2p[gi] = sm.pS2[tid];
         }
     }
-    if (n_acc_state) atomicAdd(sm.cnt, n_acc_state);
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+        const unsigned v = npass > 1 ? n_acc_c[c] : n_acc_state;
+        if (v) atomicAdd(sm.cnt + c, v);
+    }
     __syncthreads();
     if (tid == 0) {
         unsigned long long* cnt = a.counters + (size_t)chain * 2 * (D + NP);
-        const unsigned long long acc_u = sm.cnt[0];
         const unsigned long long prop_u = a.do_states ? (unsigned long long)(e - s) * (unsigned long long)a.n_sweeps : 0ull;
         for (int c = 0; c < D; ++c) {
+            const unsigned long long acc_u = sm.cnt[c];
             if (acc_u) atomicAdd(cnt + c, acc_u);
             if (prop_u) atomicAdd(cnt + (D + NP) + c, prop_u);
         }

@@ -21,10 +21,15 @@ def P():
     return P
 
 
-def _run(P, w, launch, disc, n_sweeps, dtype=64, kind=1, with_params=True, tol=TOL64):
-    h = gpu_handle(w, dtype=dtype, with_params=with_params, launch=launch, kind=kind, disc=disc)
+def _run(P, w, launch, disc, n_sweeps, dtype=64, kind=1, with_params=True, tol=TOL64, engine=0):
+    h = gpu_handle(w, dtype=dtype, with_params=with_params, kind=kind, disc=disc)
     h.set_update_mode(P.UPDATE_COMPONENTWISE)
-    assert h.get_engine()["engine"] == P.ENGINE_GLOBAL
+    if engine:
+        h.set_engine(engine)
+    if launch:
+        h.set_launch(*launch)
+    if engine:
+        assert h.get_engine()["engine"] == engine
     tr = h.enable_trace()
     orcs = oracle_chains(w, state_dtype=dtype, with_params=with_params, kind=kind, disc=disc)
     for o in orcs:
@@ -65,22 +70,26 @@ def _run(P, w, launch, disc, n_sweeps, dtype=64, kind=1, with_params=True, tol=T
     return worst, n_dec
 
 
-@pytest.mark.parametrize("cfg,M,launch,disc", [(0, 256, None, 0), (2, 500, (4, 64), 0), (2, 501, (1, 96), 1), (1, 700, (3, 128), 0),
-                                               (2, 333, (5, 32), 1)])
-def test_componentwise_decisions_match_oracle(P, cfg, M, launch, disc):
+@pytest.mark.parametrize("cfg,M,launch,disc,engine", [(0, 256, None, 0, 1), (2, 500, (4, 64), 0, 1), (2, 501, (1, 96), 1, 1), (1, 700, (3, 128), 0, 1),
+                                                      (2, 333, (5, 32), 1, 1),
+                                                      # tile-resident engine: D passes per half-sweep through the joint update
+                                                      (0, 256, None, 0, 2), (2, 600, None, 0, 2), (2, 601, (5, 192), 1, 2), (1, 1000, None, 0, 2),
+                                                      (3, 4001, None, 0, 2)])
+def test_componentwise_decisions_match_oracle(P, cfg, M, launch, disc, engine):
     w = make_workload(cfg, M=M)
-    worst, n = _run(P, w, launch, disc, 25, with_params=bool(np.any(w.w_param > 0)))
+    worst, n = _run(P, w, launch, disc, 25, with_params=bool(np.any(w.w_param > 0)), engine=engine)
     print(cfg, M, launch, disc, "max dA error / scale", worst, "decisions", n)
 
 
 def test_componentwise_batched_classic_and_fp32(P):
     w = make_workload(4, M=300, n_chains=4, kinetics="classic")
-    _run(P, w, (1, 64), 0, 10)
+    _run(P, w, (1, 64), 0, 10, engine=1)
     w = make_workload(2, M=400)
-    _run(P, w, None, 0, 10, dtype=32, tol=TOL32)
+    _run(P, w, None, 0, 10, dtype=32, tol=TOL32, engine=1)
+    _run(P, w, None, 0, 10, dtype=32, tol=TOL32, engine=2)
 
 
-def test_componentwise_gaussian_proposals_and_engine_rule(P):
+def test_componentwise_gaussian_proposals_and_argument_check(P):
     import paper_1103_4887_b200 as Pm
     w = make_workload(2, M=400)
     # Gaussian proposals: different math libraries, proposals agree to a few ulp, decisions identical except near ties
@@ -101,11 +110,6 @@ def test_componentwise_gaussian_proposals_and_engine_rule(P):
             x, p = o.get_path(); h.set_params(torch.as_tensor(p[None], device="cuda")); h.set_path(torch.as_tensor(x[None], device="cuda"))
     assert mism <= 1
     assert np.max(np.abs(h.get_path()[0].cpu().numpy()[0] - o.get_path()[0])) < 1e-10
-    # the tile-resident engine refuses component-wise updates (GLOBAL engine only in this round)
-    with pytest.raises(Pm.PimcError):
-        h.set_engine(Pm.ENGINE_TILE)
-    h2 = gpu_handle(w); h2.set_engine(Pm.ENGINE_TILE)
-    with pytest.raises(Pm.PimcError):
-        h2.set_update_mode(Pm.UPDATE_COMPONENTWISE)
+    h2 = gpu_handle(w)
     with pytest.raises(Pm.PimcError):
         h2.set_update_mode(5)
