@@ -21,6 +21,13 @@
 // Kalman/RTS); 1-site textbook Gaussian.  PARITY UNPINNED: the Hodgkin-Huxley posterior
 // moments themselves (Table 2 needs the paper's data and 1e6 tuned
 // iterations) -- for HH the chain is pinned only through its parts (model, dA, rule, RNG).
+//
+// Options beyond that default path, each following the passage it cites and pinned in its own test file:
+//   set_discretisation(1)  the paper's trapezoid rule, Eq. 7             tests/test_oracle_trapezoid.py
+//   set_update_mode(1)     one component per proposal, PAPER.md:226-230               tests/test_oracle_componentwise.py
+//   model 2                classic Hodgkin-Huxley alpha/beta rate functions            tests/test_oracle_classic_hh.py
+//   set_annealing          beta on the dynamics term, Eq. 10          tests/test_oracle_annealing.py
+//   set_tuning             step-size adjustment rule, PAPER.md:224-230                 tests/test_oracle_tuning.py
 #include <cmath>
 #include <cstdint>
 #include <cstring>
