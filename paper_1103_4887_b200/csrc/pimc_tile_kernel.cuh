@@ -581,7 +581,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             const uint32_t* gc32 = reinterpret_cast<const uint32_t*>(gc);
             // send: word w <-> (site offset o, which (0: x, 1: g), component c, half)
             for (int w = tid; w < 2 * nwords; w += T) {
-                const int dir = w / nwords, q = w % nwords;      // dir 0: to the left neighbour, 1: to the right
+                // dir 0: to the left neighbour, 1: to the right (no run-time division: nwords <= 2 T)
+                const int dir = w >= nwords ? 1 : 0, q = w - dir * nwords;
                 if ((dir == 0 && b == 0) || (dir == 1 && b == G - 1)) continue;
                 const int o = q / (2 * D * WPV), rem = q % (2 * D * WPV);
                 const int which = rem / (D * WPV), cw = rem % (D * WPV);
@@ -599,7 +600,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             uint32_t* xd32 = reinterpret_cast<uint32_t*>(sm.xs);
             uint32_t* gd32 = reinterpret_cast<uint32_t*>(cur ? sm.g1 : sm.g0);
             for (int w = tid; w < 2 * nwords; w += T) {
-                const int side = w / nwords, q = w % nwords;     // side 0: from the left neighbour, 1: from the right
+                const int side = w >= nwords ? 1 : 0, q = w - side * nwords;     // side 0: from the left neighbour, 1: from the right
                 if ((side == 0 && b == 0) || (side == 1 && b == G - 1)) continue;
                 const int o = q / (2 * D * WPV), rem = q % (2 * D * WPV);
                 const int which = rem / (D * WPV), cw = rem % (D * WPV);
