@@ -16,9 +16,27 @@
 
 using namespace pimc;
 
+// ---- translation-unit split (build time) ------------------------------------------------------------------------------
+// This one source file is compiled five times (paper_1103_4887_b200/build.py, in parallel): PIMC_PART = 0 holds the C ABI
+// and all host logic and instantiates NO sweep kernel; parts 1..4 each instantiate the kernels of one model family
+// (1: HH tanh kinetics, 2: HH classic kinetics, 3: LINEAR fp64, 4: LINEAR fp32) behind one entry point, part_entry_<k>.
+// PIMC_PART undefined = everything in one translation unit.
+#ifndef PIMC_PART
+#define PIMC_PART -1
+#endif
+#define PIMC_HAS_PART(k) (PIMC_PART == -1 || PIMC_PART == (k))
+
+namespace pimc_shared {
+#if PIMC_PART <= 0
+thread_local std::string static_error;
+#else
+extern thread_local std::string static_error;
+#endif
+}  // namespace pimc_shared
+
 namespace {
 
-thread_local std::string g_static_error;
+#define g_static_error pimc_shared::static_error
 
 struct Carve {   // bump allocator over the caller's workspace; also used to size it
     char* base;
@@ -151,29 +169,32 @@ int fail(pimc_handle* h, int code, const char* fmt, ...) {
     } while (0)
 
 // ---- model / dtype dispatch --------------------------------------------------------------------------
-template <typename F> int dispatch(int model, int D, int dtype, F&& f) {
-    if (model == PIMC_MODEL_HH) {
-        if (dtype == 64) return f(HHModel<double>{}, double{});
-        return f(HHModel<float>{}, float{});
-    }
-    if (model == PIMC_MODEL_HH_CLASSIC) {
-        if (dtype == 64) return f(HHClassicModel<double>{}, double{});
-        return f(HHClassicModel<float>{}, float{});
-    }
-    switch (D * 100 + dtype) {
-        case 164: return f(LinearModel<double, 1>{}, double{});
-        case 264: return f(LinearModel<double, 2>{}, double{});
-        case 364: return f(LinearModel<double, 3>{}, double{});
-        case 464: return f(LinearModel<double, 4>{}, double{});
-        case 132: return f(LinearModel<float, 1>{}, float{});
-        case 232: return f(LinearModel<float, 2>{}, float{});
-        case 332: return f(LinearModel<float, 3>{}, float{});
-        case 432: return f(LinearModel<float, 4>{}, float{});
-    }
+// The four operations that need a model's kernels, behind one entry point per model family (see the split above).
+enum { OP_REBUILD = 0, OP_SWEEP = 1, OP_SHAPE = 2, OP_STEP = 3 };
+}  // namespace
+namespace pimc_shared {
+struct LaunchShape { int G, T, tile; bool cooperative; int engine, h; size_t smem; };
+struct OpArgs {
+    int op;
+    pimc_handle* h;
+    long long n_sweeps; unsigned long long seed; int do_states, do_params;     // OP_SWEEP
+    LaunchShape* ls;                                                           // OP_SHAPE
+    const void *x, *p, *I0, *I1; double dt; unsigned long long n; void* g; void* stream;   // OP_STEP
+};
+int part_entry_1(int model, int D, int dtype, const OpArgs& o);   // HH, tanh kinetics
+int part_entry_2(int model, int D, int dtype, const OpArgs& o);   // HH, classic kinetics
+int part_entry_3(int model, int D, int dtype, const OpArgs& o);   // LINEAR, fp64
+int part_entry_4(int model, int D, int dtype, const OpArgs& o);   // LINEAR, fp32
+}  // namespace pimc_shared
+using pimc_shared::LaunchShape;
+using pimc_shared::OpArgs;
+namespace {
+int dispatch_op(int model, int D, int dtype, const OpArgs& o) {
+    if (model == PIMC_MODEL_HH) return pimc_shared::part_entry_1(model, D, dtype, o);
+    if (model == PIMC_MODEL_HH_CLASSIC) return pimc_shared::part_entry_2(model, D, dtype, o);
+    if (model == PIMC_MODEL_LINEAR) return dtype == 64 ? pimc_shared::part_entry_3(model, D, dtype, o) : pimc_shared::part_entry_4(model, D, dtype, o);
     return PIMC_EUNSUPPORTED;
 }
-
-struct LaunchShape { int G, T, tile; bool cooperative; int engine, h; size_t smem; };
 
 // Choose CTAs per chain, threads per CTA and the tile length (even).
 template <class Model, typename R> int choose_shape_global(pimc_handle* h, LaunchShape* out) {
@@ -281,7 +302,8 @@ template <class Model, typename R> int rebuild_cache(pimc_handle* h) {
 }
 
 int rebuild(pimc_handle* h) {
-    return dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return rebuild_cache<decltype(model), decltype(real)>(h); });
+    OpArgs o{}; o.op = OP_REBUILD; o.h = h;
+    return dispatch_op(h->model, h->D, h->dtype, o);
 }
 
 template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
@@ -343,15 +365,67 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     return PIMC_OK;
 }
 
+template <class Model, typename R> int run_op(const OpArgs& o) {
+    switch (o.op) {
+        case OP_REBUILD: return rebuild_cache<Model, R>(o.h);
+        case OP_SWEEP: return run_sweeps<Model, R>(o.h, o.n_sweeps, o.seed, o.do_states, o.do_params);
+        case OP_SHAPE: return choose_shape<Model, R>(o.h, o.ls);
+        case OP_STEP: {
+            const int threads = 128;
+            const int blocks = (int)std::min<unsigned long long>((o.n + threads - 1) / threads, 148ull * 16);
+            step_selftest_kernel<Model, R><<<blocks, threads, 0, (cudaStream_t)o.stream>>>((const R*)o.x, (const R*)o.p, (const R*)o.I0, (const R*)o.I1,
+                                                                                         (R)o.dt, o.n, (R*)o.g);
+            PIMC_CUDA(nullptr, cudaGetLastError());
+            return PIMC_OK;
+        }
+    }
+    return PIMC_EINVAL;
+}
+}  // namespace
+
+// ---- the model families: each entry point is compiled in exactly one translation unit --------------------------------
+namespace pimc_shared {
+#if PIMC_HAS_PART(1)
+int part_entry_1(int, int, int dtype, const OpArgs& o) { return dtype == 64 ? run_op<HHModel<double>, double>(o) : run_op<HHModel<float>, float>(o); }
+#endif
+#if PIMC_HAS_PART(2)
+int part_entry_2(int, int, int dtype, const OpArgs& o) { return dtype == 64 ? run_op<HHClassicModel<double>, double>(o) : run_op<HHClassicModel<float>, float>(o); }
+#endif
+#if PIMC_HAS_PART(3)
+int part_entry_3(int, int D, int, const OpArgs& o) {
+    switch (D) {
+        case 1: return run_op<LinearModel<double, 1>, double>(o);
+        case 2: return run_op<LinearModel<double, 2>, double>(o);
+        case 3: return run_op<LinearModel<double, 3>, double>(o);
+        case 4: return run_op<LinearModel<double, 4>, double>(o);
+    }
+    return PIMC_EUNSUPPORTED;
+}
+#endif
+#if PIMC_HAS_PART(4)
+int part_entry_4(int, int D, int, const OpArgs& o) {
+    switch (D) {
+        case 1: return run_op<LinearModel<float, 1>, float>(o);
+        case 2: return run_op<LinearModel<float, 2>, float>(o);
+        case 3: return run_op<LinearModel<float, 3>, float>(o);
+        case 4: return run_op<LinearModel<float, 4>, float>(o);
+    }
+    return PIMC_EUNSUPPORTED;
+}
+#endif
+}  // namespace pimc_shared
+
+#if PIMC_PART <= 0      // the C ABI and its host-side helpers: part 0 (or the single translation unit) only
+namespace {
+
 int sweep_common(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
     if (!h) return PIMC_EINVAL;
     if (n_sweeps < 0) return fail(h, PIMC_EINVAL, "n_sweeps < 0");
     if (!h->have_data || !h->have_path || !h->have_prop) return fail(h, PIMC_ESTATE, "pimc_sweep before set_data / set_path / set_proposal");
     if (n_sweeps == 0) return PIMC_OK;
     if (((h->t + (unsigned long long)n_sweeps) >> 48) != 0) return fail(h, PIMC_EINVAL, "sweep index exceeds 48 bits");
-    return dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) {
-        return run_sweeps<decltype(model), decltype(real)>(h, n_sweeps, seed, do_states, do_params);
-    });
+    OpArgs o{}; o.op = OP_SWEEP; o.h = h; o.n_sweeps = n_sweeps; o.seed = seed; o.do_states = do_states; o.do_params = do_params;
+    return dispatch_op(h->model, h->D, h->dtype, o);
 }
 
 int recentre(pimc_handle* h) {
@@ -680,7 +754,8 @@ int pimc_set_launch(pimc_handle* h, int ctas_per_chain, int threads_per_cta) {
     const int G0 = h->G_user, T0 = h->T_user;
     h->G_user = ctas_per_chain; h->T_user = threads_per_cta;
     LaunchShape ls;
-    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    OpArgs o{}; o.op = OP_SHAPE; o.h = h; o.ls = &ls;
+    const int rc = dispatch_op(h->model, h->D, h->dtype, o);
     if (rc != PIMC_OK) { h->G_user = G0; h->T_user = T0; }
     return rc;
 }
@@ -688,7 +763,8 @@ int pimc_set_launch(pimc_handle* h, int ctas_per_chain, int threads_per_cta) {
 int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, int* tile_sites, int* smem_bytes) {
     if (!h) return PIMC_EINVAL;
     LaunchShape ls;
-    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    OpArgs o{}; o.op = OP_SHAPE; o.h = h; o.ls = &ls;
+    const int rc = dispatch_op(h->model, h->D, h->dtype, o);
     if (rc != PIMC_OK) return rc;
     if (ctas_per_chain) *ctas_per_chain = ls.G;
     if (threads_per_cta) *threads_per_cta = ls.T;
@@ -704,7 +780,8 @@ int pimc_set_engine(pimc_handle* h, int engine, int halo) {
     const int e0 = h->engine_user, h0 = h->halo_user;
     h->engine_user = engine; h->halo_user = halo;
     LaunchShape ls;
-    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    OpArgs o{}; o.op = OP_SHAPE; o.h = h; o.ls = &ls;
+    const int rc = dispatch_op(h->model, h->D, h->dtype, o);
     if (rc != PIMC_OK) { h->engine_user = e0; h->halo_user = h0; }
     return rc;
 }
@@ -712,7 +789,8 @@ int pimc_set_engine(pimc_handle* h, int engine, int halo) {
 int pimc_get_engine(pimc_handle* h, int* engine, int* halo) {
     if (!h) return PIMC_EINVAL;
     LaunchShape ls;
-    const int rc = dispatch(h->model, h->D, h->dtype, [&](auto model, auto real) { return choose_shape<decltype(model), decltype(real)>(h, &ls); });
+    OpArgs o{}; o.op = OP_SHAPE; o.h = h; o.ls = &ls;
+    const int rc = dispatch_op(h->model, h->D, h->dtype, o);
     if (rc != PIMC_OK) return rc;
     if (engine) *engine = ls.engine;
     if (halo) *halo = ls.h;
@@ -804,16 +882,8 @@ int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p
     if (!x || !p || !g_out) return fail(nullptr, PIMC_EINVAL, "null argument");
     if (pimc_model_np(model, D) < 0 || !(dtype == 64 || dtype == 32)) return fail(nullptr, PIMC_EUNSUPPORTED, "unsupported model / D / dtype");
     if (n == 0) return PIMC_OK;
-    const int threads = 128;
-    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, 148ull * 16);
-    return dispatch(model, D, dtype, [&](auto m, auto real) {
-        using Model = decltype(m);
-        using R = decltype(real);
-        step_selftest_kernel<Model, R><<<blocks, threads, 0, (cudaStream_t)stream>>>((const R*)x, (const R*)p, (const R*)I0, (const R*)I1,
-                                                                                     (R)dt, n, (R*)g_out);
-        PIMC_CUDA(nullptr, cudaGetLastError());
-        return (int)PIMC_OK;
-    });
+    OpArgs o{}; o.op = OP_STEP; o.h = nullptr; o.x = x; o.p = p; o.I0 = I0; o.I1 = I1; o.dt = dt; o.n = n; o.g = g_out; o.stream = stream;
+    return dispatch_op(model, D, dtype, o);
 }
 
 int pimc_math_selftest(const double* x, unsigned long long n, double* out, void* stream) {
@@ -867,3 +937,5 @@ int pimc_destroy(pimc_handle* h) {
 }
 
 }  // extern "C"
+
+#endif  // PIMC_PART <= 0

@@ -644,7 +644,7 @@ __global__ void step_selftest_kernel(const R* __restrict__ x, const R* __restric
 }
 
 // ---- RNG self-test ------------------------------------------------------------------------------------------
-__global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, unsigned long long n, uint32_t k0, uint32_t k1,
+static __global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, unsigned long long n, uint32_t k0, uint32_t k1,
                                     uint32_t* __restrict__ out, double* __restrict__ u_prop, double* __restrict__ u_acc,
                                     double* __restrict__ z) {
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
@@ -660,7 +660,7 @@ __global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, unsigned 
 }
 
 // ---- elementary-function self-test: out (n,7) = exp, log, sqrt, sin, cos, 1/x, HH gate m-rate at (x, a = 0.3) ----
-__global__ void math_selftest_kernel(const double* __restrict__ x, unsigned long long n, double* __restrict__ out) {
+static __global__ void math_selftest_kernel(const double* __restrict__ x, unsigned long long n, double* __restrict__ out) {
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
         const double v = x[i];
         const double av = fabs(v);
@@ -677,7 +677,7 @@ __global__ void math_selftest_kernel(const double* __restrict__ x, unsigned long
 }
 
 // ---- FP64 pipe probe: 8 independent FMA chains per thread, no memory traffic ------------------------------
-__global__ void fp64_peak_kernel(double* sink, int iters, double a, double b) {
+static __global__ void fp64_peak_kernel(double* sink, int iters, double a, double b) {
     double v[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) v[i] = threadIdx.x * 1e-3 + i;
@@ -692,7 +692,7 @@ __global__ void fp64_peak_kernel(double* sink, int iters, double a, double b) {
 }
 
 // ---- moments read-out: mean = c + S1/N, var = S2/N - (S1/N)^2 ---------------------------------------------
-__global__ void moments_kernel(const double* __restrict__ cx, const double* __restrict__ S1x, const double* __restrict__ S2x,
+static __global__ void moments_kernel(const double* __restrict__ cx, const double* __restrict__ S1x, const double* __restrict__ S2x,
                                const double* __restrict__ cp, const double* __restrict__ S1p, const double* __restrict__ S2p,
                                size_t nx /* (M+1)*D */, int np, int n_chains, double N, double* __restrict__ out) {
     const size_t per_chain = 2 * nx + 2 * (size_t)np;

@@ -13,7 +13,7 @@
 
 namespace pimc {
 
-#define PIMC_COEF(name, n) __constant__ double name[n]
+#define PIMC_COEF(name, n) static __constant__ double name[n]      // one copy per translation unit
 #include "pimc_math_coef.inc"
 #undef PIMC_COEF
 
