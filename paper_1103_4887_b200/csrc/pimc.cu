@@ -340,13 +340,21 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
     const void* fn = (const void*)sweep_kernel<Model, R>;
     if (ls.engine == PIMC_ENGINE_TILE) {
         const bool comp = h->update_mode == PIMC_UPDATE_COMPONENTWISE;
+        // the stage-1 cache is only worth keeping if this launch moves a parameter (and the model has one: NK > 0)
+        bool kg = false;
+        if constexpr (Model::NK > 0) {
+            if (do_params && !trap) {
+                kg = h->site_widths;                                   // tuned parameter step sizes live on the device
+                for (int l = 0; l < h->Np; ++l) kg = kg || h->wp[l] > 0.0;
+            }
+        }
         const int sel = (ls.T <= 256 ? 0 : 4) + (trap ? 2 : 0) + (comp ? 1 : 0);
         switch (sel) {
-            case 0: fn = (const void*)tile_sweep_kernel<Model, R, 256, false, false>; break;
-            case 1: fn = (const void*)tile_sweep_kernel<Model, R, 256, false, true>; break;
-            case 2: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, false>; break;
-            case 3: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, true>; break;
-            case 4: fn = (const void*)tile_sweep_kernel<Model, R, 512, false, false>; break;
+            case 0: fn = kg ? (const void*)tile_sweep_kernel<Model, R, 256, false, false, (Model::NK > 0)> : (const void*)tile_sweep_kernel<Model, R, 256, false, false, false>; break;
+            case 1: fn = kg ? (const void*)tile_sweep_kernel<Model, R, 256, false, true, (Model::NK > 0)> : (const void*)tile_sweep_kernel<Model, R, 256, false, true, false>; break;
+            case 2: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, false, false>; break;
+            case 3: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, true, false>; break;
+            case 4: fn = kg ? (const void*)tile_sweep_kernel<Model, R, 512, false, false, (Model::NK > 0)> : (const void*)tile_sweep_kernel<Model, R, 512, false, false, false>; break;
             default: return fail(h, PIMC_EUNSUPPORTED, "no 512-thread tile kernel for this discretisation / update mode");   // choose_shape_tile never offers it
         }
     }

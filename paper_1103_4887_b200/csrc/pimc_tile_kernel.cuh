@@ -202,13 +202,15 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
 // TRAP selects the paper's trapezoid discretisation (Eq. 7): the cache holds c_n = (dt/2) F(x_n) for n = 0..M,
 // every residual is (x_{k+1} - x_k) - c_k - c_{k+1}, the model step is ONE right-hand side, and there is no stage-1 cache.
 // COMP selects component-wise updates (D passes per half-sweep); as a compile-time flag it leaves the joint kernel exactly as it was.
-template <class Model, typename R, int MAXT, bool TRAP, bool COMP>
+// KG keeps the stage-1 cache of the parameter moves up to date; launches that move no parameter (states-only sweeps, frozen
+// parameters: config 0) are compiled without it.
+template <class Model, typename R, int MAXT, bool TRAP, bool COMP, bool KG>
 __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
     extern __shared__ __align__(16) unsigned char tile_smem_raw[];
     const int T = blockDim.x, TC = T >> 1, tid = threadIdx.x;
-    constexpr int NK = TRAP ? 0 : Model::NK;
+    constexpr int NK = (TRAP || !KG) ? 0 : Model::NK;
     // Component-wise updates (SweepArgs::update_mode = 1) run D PASSES per half-sweep through the same site update: pass c gets a
     // step vector that is zero except in component c and the accept uniform of block c (drawn by the producer warps), which is
     // exactly a single-component Metropolis move; a joint sweep has one pass.
