@@ -348,15 +348,20 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
                 for (int l = 0; l < h->Np; ++l) kg = kg || h->wp[l] > 0.0;
             }
         }
+        const bool tr = h->tr_dA || h->tr_acc || h->tr_xprop || h->tr_dAp || h->tr_accp || h->tr_pprop;
+        constexpr bool HK = Model::NK > 0;
         const int sel = (ls.T <= 256 ? 0 : 4) + (trap ? 2 : 0) + (comp ? 1 : 0);
+#define PIMC_TILE(MAXT_, TRAP_, COMP_, KG_) \
+    (tr ? (const void*)tile_sweep_kernel<Model, R, MAXT_, TRAP_, COMP_, KG_, true> : (const void*)tile_sweep_kernel<Model, R, MAXT_, TRAP_, COMP_, KG_, false>)
         switch (sel) {
-            case 0: fn = kg ? (const void*)tile_sweep_kernel<Model, R, 256, false, false, (Model::NK > 0)> : (const void*)tile_sweep_kernel<Model, R, 256, false, false, false>; break;
-            case 1: fn = kg ? (const void*)tile_sweep_kernel<Model, R, 256, false, true, (Model::NK > 0)> : (const void*)tile_sweep_kernel<Model, R, 256, false, true, false>; break;
-            case 2: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, false, false>; break;
-            case 3: fn = (const void*)tile_sweep_kernel<Model, R, 256, true, true, false>; break;
-            case 4: fn = kg ? (const void*)tile_sweep_kernel<Model, R, 512, false, false, (Model::NK > 0)> : (const void*)tile_sweep_kernel<Model, R, 512, false, false, false>; break;
+            case 0: fn = kg ? PIMC_TILE(256, false, false, HK) : PIMC_TILE(256, false, false, false); break;
+            case 1: fn = kg ? PIMC_TILE(256, false, true, HK) : PIMC_TILE(256, false, true, false); break;
+            case 2: fn = PIMC_TILE(256, true, false, false); break;
+            case 3: fn = PIMC_TILE(256, true, true, false); break;
+            case 4: fn = kg ? PIMC_TILE(512, false, false, HK) : PIMC_TILE(512, false, false, false); break;
             default: return fail(h, PIMC_EUNSUPPORTED, "no 512-thread tile kernel for this discretisation / update mode");   // choose_shape_tile never offers it
         }
+#undef PIMC_TILE
     }
     if (ls.smem > 48 * 1024) PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
     void* params[] = {&a};

@@ -204,7 +204,8 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
 // COMP selects component-wise updates (D passes per half-sweep); as a compile-time flag it leaves the joint kernel exactly as it was.
 // KG keeps the stage-1 cache of the parameter moves up to date; launches that move no parameter (states-only sweeps, frozen
 // parameters: config 0) are compiled without it.
-template <class Model, typename R, int MAXT, bool TRAP, bool COMP, bool KG>
+// TR compiles the debug trace in (launches with pimc_debug_trace buffers set); production launches carry none of its code.
+template <class Model, typename R, int MAXT, bool TRAP, bool COMP, bool KG, bool TR>
 __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
@@ -338,7 +339,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     for (long long i = 0; i < a.n_sweeps; ++i) {
         const unsigned long long t = a.t0 + (unsigned long long)i;
         const int set = (int)(i & 1);
-        const bool trace = (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
+        const bool trace = TR && (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
         const bool acc_now = a.accum && skip_ctr == 0ull;
         skip_ctr = (skip_ctr + 1ull == a.n_skip) ? 0ull : skip_ctr + 1ull;
 
