@@ -55,7 +55,7 @@ enum { PIMC_PROPOSAL_GAUSSIAN = 0, PIMC_PROPOSAL_UNIFORM = 1 };
  * in global memory (L2), threads stride over the tile, neighbour tiles synchronise every half-sweep with
  * release/acquire flags; any tile length.  TILE: each CTA keeps its tile plus h halo sites in shared memory, one
  * (even, odd) site pair per compute thread, halos updated redundantly and exchanged every h half-sweeps as tagged
- * 8-byte packets; needs tile + 2h <= threads_per_cta <= 512.  AUTO: TILE when it fits, else GLOBAL. */
+ * 8-byte packets; needs tile + 2h <= threads_per_cta <= 512 and L = 1 (one observed component).  AUTO: TILE when it fits, else GLOBAL. */
 enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2 };
 /* Discretisation of the model-error term between steps n and n+1, (Rf_a/2) r_a^2:
  *  RK4MAP    (default; BASELINE north_star): r = (x_{n+1} - x_n) - g_n, g_n = the increment of one RK4 step from x_n

@@ -237,6 +237,7 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int sites = h->M + 1;
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
+    if (h->L != 1) return no("the tile engine is compiled for one observed component (L = 1)");
     if (h->site_widths && h->tune) return no("step-size tuning runs on the GLOBAL engine (frozen tuned step sizes run on both)");
     if (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool) return no("sweeps with the annealing multiplier below 1 run on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");

@@ -317,3 +317,22 @@ def test_run_host_end_to_end_matches_device_api(P):
     assert np.array_equal(out["mean_x"], mx.cpu().numpy()[:, 0]) and np.array_equal(out["var_x"], mx.cpu().numpy()[:, 1])
     assert np.array_equal(out["x"], h.get_path()[0].cpu().numpy()) and np.array_equal(out["p"], h.get_path()[1].cpu().numpy())
     assert out["h2d_bytes"] > 0 and out["d2h_bytes"] > 0
+
+
+def test_several_observed_components_run_on_the_global_engine(P):
+    # the tile-resident engine is compiled for one observed component (every BASELINE config); L >= 2 falls back
+    import paper_1103_4887_b200 as Pm
+    for D, L in ((3, 2), (4, 4), (2, 2)):
+        rng = np.random.default_rng(100 * D + L)
+        A = 0.6 * np.eye(D) + 0.1 * rng.normal(size=(D, D))
+        M = 300
+        w = Workload(name="multi_obs", model=MODEL_LINEAR, D=D, L=L, Np=D * D, M=M, dt=1.0, Rm=7.0, Rf=np.linspace(5, 9, D),
+                     n_chains=1, p0=A.ravel()[None].copy(), p_true=A.ravel(), lo=np.full((1, D * D), -5.0), hi=np.full((1, D * D), 5.0),
+                     w_state=np.full(D, 0.3), w_param=np.full(D * D, 0.02), y=rng.normal(size=(1, M + 1, max(L, 1))), I=None,
+                     x0=rng.normal(size=(1, M + 1, D)), x_true=np.zeros((1, M + 1, D)), n_sweeps=10)
+        h = gpu_handle(w)
+        assert h.get_engine()["engine"] == Pm.ENGINE_GLOBAL
+        rep = teacher_forced(w, h, oracle_chains(w), 8, seed=3)
+        assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0 and rep["max_param_rel"] <= TOL64, (D, L, rep)
+        with pytest.raises(Pm.PimcError):
+            h.set_engine(Pm.ENGINE_TILE)
