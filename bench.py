@@ -42,7 +42,7 @@ FP64_LANES_PER_SM_CLK = 64
 SM_COUNT = 148
 SM_MAX_HZ = 1.965e9
 PEAK_TFLOPS_DERIVED = SM_COUNT * FP64_LANES_PER_SM_CLK * SM_MAX_HZ * 2 / 1e12
-NCU_DRAM_BYTES_PER_LAUNCH = 5977344.0   # cfg3 full sweep launch: 5.926 MB read + 51 KB written (profiles/r01_v7_final.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 5939456.0   # cfg3 full sweep launch: 5.917 MB read + 22 KB written (profiles/r01_v8_final.md)
 
 
 def rank_info():
@@ -234,7 +234,7 @@ def run_ours(args):
     measured_peak = P.fp64_peak(150) * 2 / 1e12 if rank == 0 else None
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == 3 and args.dtype == 64 and not trap) else None,
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r01_v7_final.md (tile loaded once, written back once: independent of the sweeps per launch)",
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r01_v8_final.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
                 "peak_measured_dfma_tflops": measured_peak,
                 "frac_of_measured_dfma": (achieved_tflops / measured_peak) if measured_peak else None,
