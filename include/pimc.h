@@ -112,9 +112,9 @@ int pimc_set_discretisation(pimc_handle* h, int disc);
 
 /* Simulated annealing of the dynamics term (Eq. 10): from the current sweep index on, the model-error
  * weights Rf are multiplied by beta_k = beta0 f^k, f = (1/beta0)^(1/n_cool), k = sweeps since this call, until beta = 1
- * (k >= n_cool); the measurement term is not scaled.  0 < beta0 <= 1; n_cool = 0 switches annealing off.  While beta < 1 the
- * sweeps run on the GLOBAL engine (the automatic choice falls back; PIMC_EUNSUPPORTED if TILE is forced); once the
- * schedule is over the TILE engine is used again. */
+ * (k >= n_cool); the measurement term is not scaled.  0 < beta0 <= 1; n_cool = 0 switches annealing off.  Both engines
+ * carry the schedule (launches that contain a sweep with beta < 1 use the TILE engine's general variant, a few per cent
+ * slower than the production one; once the schedule is over the production variant is launched again). */
 int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool);
 
 /* Step-size auto-tuning: from the current sweep index on, every n_skip-th sweep each step size is

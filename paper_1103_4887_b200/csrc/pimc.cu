@@ -239,7 +239,6 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
     if (h->L != 1) return no("the tile engine is compiled for one observed component (L = 1)");
     if (h->site_widths && h->tune) return no("step-size tuning runs on the GLOBAL engine (frozen tuned step sizes run on both)");
-    if (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool) return no("sweeps with the annealing multiplier below 1 run on the GLOBAL engine");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
     // the 512-thread instantiation exists for the RK4-map, joint-update kernel only (build time); the others stop at 256
@@ -349,7 +348,9 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
                 for (int l = 0; l < h->Np; ++l) kg = kg || h->wp[l] > 0.0;
             }
         }
-        const bool tr = h->tr_dA || h->tr_acc || h->tr_xprop || h->tr_dAp || h->tr_accp || h->tr_pprop;
+        // the general variant (template flag TR): debug trace requested, or a sweep of this launch has the annealing multiplier below 1
+        const bool tr = h->tr_dA || h->tr_acc || h->tr_xprop || h->tr_dAp || h->tr_accp || h->tr_pprop ||
+                        (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool && h->t + (unsigned long long)n_sweeps > h->t_anneal);
         constexpr bool HK = Model::NK > 0;
         const int sel = (ls.T <= 256 ? 0 : 4) + (trap ? 2 : 0) + (comp ? 1 : 0);
 #define PIMC_TILE(MAXT_, TRAP_, COMP_, KG_) \

@@ -204,7 +204,8 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
 // COMP selects component-wise updates (D passes per half-sweep); as a compile-time flag it leaves the joint kernel exactly as it was.
 // KG keeps the stage-1 cache of the parameter moves up to date; launches that move no parameter (states-only sweeps, frozen
 // parameters: config 0) are compiled without it.
-// TR compiles the debug trace in (launches with pimc_debug_trace buffers set); production launches carry none of its code.
+// TR is the general variant: the debug trace (launches with pimc_debug_trace buffers set) and the annealing multiplier on R_f
+// (launches that contain a sweep with beta < 1) are compiled in; production launches carry none of that code.
 template <class Model, typename R, int MAXT, bool TRAP, bool COMP, bool KG, bool TR>
 __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
@@ -343,6 +344,15 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         const int set = (int)(i & 1);
         const bool trace = TR && (i == a.n_sweeps - 1) && (a.tr_dA || a.tr_acc || a.tr_xprop || a.tr_dAp || a.tr_accp || a.tr_pprop);
         const bool acc_now = a.accum && skip_ctr == 0ull;
+        // Annealing (reading 12a) is compiled into the TR variant only: the model-error weights of
+        // sweep t are beta(t) * R_f, rounded exactly as sweep_kernel rounds them; production launches read R_f from the arguments.
+        [[maybe_unused]] R Rfs[D];
+        if constexpr (TR) {
+            const double beta = anneal_beta(a, t);
+#pragma unroll
+            for (int c = 0; c < D; ++c) Rfs[c] = (R)(beta * (double)a.Rf[c]);
+        }
+        auto rf = [&](int c) -> R { if constexpr (TR) return Rfs[c]; else return a.Rf[c]; };
         skip_ctr = (skip_ctr + 1ull == a.n_skip) ? 0ull : skip_ctr + 1ull;
 
         if (tid < TC) {
@@ -395,7 +405,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             R r_new = (xp[c] - xm[c]) - gm[c];
                             R r_old = (xn[c] - xm[c]) - gm[c];
                             if constexpr (TRAP) { r_new -= gp[c]; r_old -= gn[c]; }
-                            dL += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            dL += R(0.5) * rf(c) * (r_new * r_new - r_old * r_old);
                         }
 #pragma unroll
                         for (int l = 0; l < D; ++l) {
@@ -410,7 +420,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             R r_new = (xq[c] - xp[c]) - gp[c];
                             R r_old = (xq[c] - xn[c]) - gn[c];
                             if constexpr (TRAP) { r_new -= gq[c]; r_old -= gq[c]; }
-                            dR += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                            dR += R(0.5) * rf(c) * (r_new * r_new - r_old * r_old);
                         }
                         const R dA = (has_l ? dL : R(0)) + (has_r ? dR : R(0));
                         const bool accept = logu < -dA;
@@ -508,7 +518,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                                 for (int c = 0; c < D; ++c) {
                                     const R d = xq[c] - xn[c];
                                     const R r_new = d - gp[c], r_old = d - gn[c];
-                                    acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                                    acc += R(0.5) * rf(c) * (r_new * r_new - r_old * r_old);
                                 }
                                 part = (double)acc;
                             }
@@ -529,7 +539,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             for (int c = 0; c < D; ++c) {
                                 const R d = xq[c] - xn[c];
                                 const R r_new = (d - cpn[c]) - cpq[c], r_old = (d - cn[c]) - cq[c];
-                                acc += R(0.5) * a.Rf[c] * (r_new * r_new - r_old * r_old);
+                                acc += R(0.5) * rf(c) * (r_new * r_new - r_old * r_old);
                             }
                             part = (double)acc;
                         }

@@ -1,5 +1,5 @@
 """GPU parity for the simulated annealing of the dynamics term (pimc_set_annealing; Eq. 10; SURVEY.md
-§8(f) NEXT-4, first half) against the oracle: teacher-forced sweeps while beta rises, on both engines and discretisations,
+§8(f) NEXT-4, first half) against the oracle: teacher-forced sweeps while beta rises, on both engines (automatic, forced global-memory, forced tile-resident) and discretisations,
 and free-running bit-identical chains through the whole cooling schedule and beyond."""
 import numpy as np
 import pytest
@@ -20,7 +20,7 @@ def P():
     return P
 
 
-@pytest.mark.parametrize("M,launch,engine,disc", [(600, None, 0, 0), (601, (5, 64), 1, 0), (600, None, 0, 1), (333, (1, 96), 1, 1)])   # engine 0: automatic
+@pytest.mark.parametrize("M,launch,engine,disc", [(600, None, 0, 0), (601, (5, 64), 1, 0), (600, None, 0, 1), (333, (1, 96), 1, 1), (2500, None, 2, 0), (1201, None, 2, 1)])   # engine 0: automatic, 1: global-memory, 2: tile-resident
 def test_teacher_forced_parity_while_annealing(P, M, launch, engine, disc):
     w = make_workload(2, M=M)
     h = gpu_handle(w, disc=disc)
@@ -37,11 +37,11 @@ def test_teacher_forced_parity_while_annealing(P, M, launch, engine, disc):
     assert rep["max_rel"] <= TOL64 and rep["mismatch_outside_window"] == 0 and rep["ties"] <= 2, rep
     assert rep["param_moves"] > 0 and rep["max_param_rel"] <= TOL64 and rep["max_path_diff"] <= 1e-12, rep
     assert orcs[0].annealing_beta() == 1.0
-    if not engine:                                   # schedule over: the automatic choice is the tile-resident engine again
+    if engine != 1:                                  # the tile-resident engine carries the schedule (its general variant) and what follows
         assert h.get_engine()["engine"] == P.ENGINE_TILE
 
 
-@pytest.mark.parametrize("cfg,M,launch,engine", [(2, 500, None, 0), (2, 500, (4, 64), 1), (3, 4001, None, 0)])
+@pytest.mark.parametrize("cfg,M,launch,engine", [(2, 500, None, 0), (2, 500, (4, 64), 1), (3, 4001, None, 0), (3, 32768, None, 2)])
 def test_free_running_through_the_cooling_schedule(P, cfg, M, launch, engine):
     w = make_workload(cfg, M=M)
     h = gpu_handle(w, kind=1)
@@ -52,8 +52,8 @@ def test_free_running_through_the_cooling_schedule(P, cfg, M, launch, engine):
     o = oracle_chains(w, kind=1)[0]
     h.sweep(3, seed=5); o.sweep(3, seed=5)               # annealing starts at the sweep index of the call
     h.set_annealing(0.02, 20); o.set_annealing(0.02, 20)
-    if not engine:                                   # while beta < 1 the automatic choice is the global-memory engine
-        assert h.get_engine()["engine"] == P.ENGINE_GLOBAL
+    if engine != 1:                                  # while beta < 1 the automatic choice stays the tile-resident engine
+        assert h.get_engine()["engine"] == P.ENGINE_TILE
     h.sweep(11, seed=5); h.sweep(19, seed=5); o.sweep(30, seed=5)     # two launches across the schedule and past its end
     xg, pg = [a.cpu().numpy() for a in h.get_path()]
     xo, po = o.get_path()
