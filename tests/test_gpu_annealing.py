@@ -67,3 +67,20 @@ def test_free_running_through_the_cooling_schedule(P, cfg, M, launch, engine):
         h.set_annealing(0.0, 10)
     with pytest.raises(Pm.PimcError):
         h.set_annealing(1.5, 10)
+
+
+@pytest.mark.parametrize("disc,update", [(0, 1), (1, 0), (1, 1)])
+def test_cooling_schedule_with_the_other_tile_kernels(P, disc, update):
+    # the general variants of the trapezoid / component-wise tile kernels carry the schedule too: bit-identical chains
+    w = make_workload(3, M=3001)
+    h = gpu_handle(w, kind=1, disc=disc)
+    h.set_engine(P.ENGINE_TILE)
+    o = oracle_chains(w, kind=1, disc=disc)[0]
+    h.set_update_mode(update); o.set_update_mode(update)
+    h.set_annealing(0.05, 14); o.set_annealing(0.05, 14)
+    h.sweep(9, seed=8); h.sweep(9, seed=8); o.sweep(18, seed=8)
+    assert h.get_engine()["engine"] == P.ENGINE_TILE
+    xg, pg = [a.cpu().numpy() for a in h.get_path()]
+    xo, po = o.get_path()
+    assert np.array_equal(xg[0], xo) and np.array_equal(pg[0], po)
+    assert np.array_equal(h.stats().cpu().numpy()[0].astype(np.uint64), o.stats())
