@@ -122,8 +122,9 @@ int pimc_set_annealing(pimc_handle* h, double beta0, long long n_cool);
  * i = (n, a) (joint updates: of site n) or of parameter i over the last n_skip sweeps; one step size per (site, component)
  * and per parameter, all starting from the widths of pimc_set_proposal.  enabled = 0 freezes the step sizes as they are
  * (they stay per-site until the next pimc_set_proposal).  Tuning biases the chain: discard its sweeps (the paper tunes during
- * the initialisation phase only).  While tuning is ON the sweeps run on the GLOBAL engine (PIMC_EUNSUPPORTED if TILE is
- * forced); frozen tuned step sizes are used by both engines.  n_skip >= 1, 0 < f_acc < 1 (paper: 0.23), 0 <= alpha < 1 (paper: 0.02). */
+ * the initialisation phase only).  Both engines tune: the GLOBAL engine adjusts inside its kernel, the TILE engine ends its
+ * launches at the adjustment sweeps and adjusts between them (a pimc_sweep call may therefore be several launches); the step
+ * sizes are the same bit for bit.  n_skip >= 1, 0 < f_acc < 1 (paper: 0.23), 0 <= alpha < 1 (paper: 0.02). */
 int pimc_set_tuning(pimc_handle* h, int enabled, long long n_skip, double f_acc, double alpha);
 /* Copy out the step sizes in use: ws_out dev (n_chains, M+1, D) double, wp_out dev (n_chains, Np) double; either may be NULL. */
 int pimc_get_widths(pimc_handle* h, double* ws_out, double* wp_out);

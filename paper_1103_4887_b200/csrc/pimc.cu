@@ -238,7 +238,6 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     const int cap_ctas = std::min(h->sm_count, kTileMaxCtas);      // one CTA per SM: the FP64 pipe is the shared resource
     auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "tile engine: %s", why); };
     if (h->L != 1) return no("the tile engine is compiled for one observed component (L = 1)");
-    if (h->site_widths && h->tune) return no("step-size tuning runs on the GLOBAL engine (frozen tuned step sizes run on both)");
     if (h->C > cap_ctas) return no("more chains than co-resident CTAs");
     int T = h->T_user, G = h->G_user;
     // the 512-thread instantiation exists for the RK4-map, joint-update kernel only (build time); the others stop at 256
@@ -306,7 +305,7 @@ int rebuild(pimc_handle* h) {
     return dispatch_op(h->model, h->D, h->dtype, o);
 }
 
-template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
+template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
     LaunchShape ls;
     int rc = choose_shape<Model, R>(h, &ls);
     if (rc != PIMC_OK) return rc;
@@ -350,7 +349,8 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
         }
         // the general variant (template flag TR): debug trace requested, or a sweep of this launch has the annealing multiplier below 1
         const bool tr = h->tr_dA || h->tr_acc || h->tr_xprop || h->tr_dAp || h->tr_accp || h->tr_pprop ||
-                        (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool && h->t + (unsigned long long)n_sweeps > h->t_anneal);
+                        (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool && h->t + (unsigned long long)n_sweeps > h->t_anneal) ||
+                        (h->site_widths && h->tune);
         constexpr bool HK = Model::NK > 0;
         const int sel = (ls.T <= 256 ? 0 : 4) + (trap ? 2 : 0) + (comp ? 1 : 0);
 #define PIMC_TILE(MAXT_, TRAP_, COMP_, KG_) \
@@ -377,6 +377,36 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
         h->n_samples += (last + k - 1) / k - (first + k - 1) / k;
     }
     h->t += (unsigned long long)n_sweeps;
+    return PIMC_OK;
+}
+
+// While the step sizes are being tuned the tile-resident engine cannot adjust them inside a launch (its producer
+// warps have drawn the next sweep's proposals already, and the halo copies of a site do not see all of its decisions), so the
+// launcher ends every launch at an adjustment sweep -- (t - t_tune + 1) % tune_skip == 0 -- and runs tune_adjust_kernel on the
+// counters the owners kept.  The global-memory engine adjusts inside its kernel; both give the oracle's step sizes bit for bit.
+template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
+    if (!(h->site_widths && h->tune) || n_sweeps <= 0) return run_sweeps_once<Model, R>(h, n_sweeps, seed, do_states, do_params);
+    LaunchShape ls;
+    int rc = choose_shape<Model, R>(h, &ls);
+    if (rc != PIMC_OK) return rc;
+    if (ls.engine != PIMC_ENGINE_TILE) return run_sweeps_once<Model, R>(h, n_sweeps, seed, do_states, do_params);
+    long long left = n_sweeps;
+    while (left > 0) {
+        const unsigned long long to_adjust = h->tune_skip - (h->t - h->t_tune) % h->tune_skip;   // up to and including the adjustment sweep
+        const long long n = (unsigned long long)left < to_adjust ? left : (long long)to_adjust;
+        rc = run_sweeps_once<Model, R>(h, n, seed, do_states, do_params);
+        if (rc != PIMC_OK) return rc;
+        if ((unsigned long long)n == to_adjust) {
+            const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
+            const int threads = 256;
+            const int blocks = (int)std::min<size_t>((nx + np + threads - 1) / threads, (size_t)h->sm_count * 8);
+            tune_adjust_kernel<<<blocks, threads, 0, h->stream>>>(h->lay.ws, h->lay.nacc_s, nx, h->lay.wpd, h->lay.nacc_p, np,
+                                                                   (double)h->tune_skip, h->f_acc, h->alpha);
+            PIMC_CUDA(h, cudaGetLastError());
+            h->launches++;
+        }
+        left -= n;
+    }
     return PIMC_OK;
 }
 
@@ -592,7 +622,6 @@ int pimc_set_tuning(pimc_handle* h, int enabled, long long n_skip, double f_acc,
     if (!enabled) { h->tune = 0; return PIMC_OK; }                  // step sizes stay as they are
     if (n_skip < 1 || !(f_acc > 0.0 && f_acc < 1.0) || !(alpha >= 0.0 && alpha < 1.0))
         return fail(h, PIMC_EINVAL, "tuning needs n_skip >= 1, 0 < f_acc < 1, 0 <= alpha < 1");
-    if (h->engine_user == PIMC_ENGINE_TILE) return fail(h, PIMC_EUNSUPPORTED, "step-size tuning runs on the GLOBAL engine");
     const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
     if (!h->site_widths) {                                           // first time: every site starts from the uniform widths
         std::vector<double> w(nx), wp(np);

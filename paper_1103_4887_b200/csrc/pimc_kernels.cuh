@@ -94,6 +94,22 @@ template <typename R> __device__ __forceinline__ double anneal_beta(const SweepA
     return exp_fast(a.ln_beta0 * (1.0 - (double)k / (double)a.n_cool));
 }
 
+// ---- step-size adjustment between two launches of the tile-resident engine ------------------
+// Delta_i <- Delta_i [1 + alpha (N_acc,i / N_skip - f_acc)] for every (chain, site, component) and every parameter, counters
+// reset: the same correctly rounded operations, in the same order, as the in-kernel adjustment of sweep_kernel.
+static __global__ void tune_adjust_kernel(double* __restrict__ ws, unsigned int* __restrict__ nacc_s, size_t n_site_widths,
+                                          double* __restrict__ wpd, unsigned int* __restrict__ nacc_p, size_t n_param_widths,
+                                          double n_skip, double f_acc, double alpha) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_site_widths + n_param_widths; i += stride) {
+        double* w = i < n_site_widths ? ws + i : wpd + (i - n_site_widths);
+        unsigned int* na = i < n_site_widths ? nacc_s + i : nacc_p + (i - n_site_widths);
+        const double rate = __ddiv_rn((double)*na, n_skip);
+        *w = __dmul_rn(*w, __dadd_rn(1.0, __dmul_rn(alpha, __dsub_rn(rate, f_acc))));
+        *na = 0u;
+    }
+}
+
 // ---- memory-model helpers ------------------------------------------------------------------------
 __device__ __forceinline__ void st_release_gpu(unsigned long long* p, unsigned long long v) {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");

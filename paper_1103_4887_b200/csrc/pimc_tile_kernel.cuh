@@ -204,8 +204,9 @@ __device__ __forceinline__ void produce_site(const SweepArgs<R>& a, unsigned lon
 // COMP selects component-wise updates (D passes per half-sweep); as a compile-time flag it leaves the joint kernel exactly as it was.
 // KG keeps the stage-1 cache of the parameter moves up to date; launches that move no parameter (states-only sweeps, frozen
 // parameters: config 0) are compiled without it.
-// TR is the general variant: the debug trace (launches with pimc_debug_trace buffers set) and the annealing multiplier on R_f
-// (launches that contain a sweep with beta < 1) are compiled in; production launches carry none of that code.
+// TR is the general variant: the debug trace (launches with pimc_debug_trace buffers set), the annealing multiplier on R_f
+// (launches that contain a sweep with beta < 1) and the accept counters of the step-size tuning (the launcher ends such launches
+// at the adjustment sweeps and runs tune_adjust_kernel between them) are compiled in; production launches carry none of that code.
 template <class Model, typename R, int MAXT, bool TRAP, bool COMP, bool KG, bool TR>
 __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
@@ -440,6 +441,16 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         }
                         const bool owned = n >= s && n < e;
                         n_acc_state += (owned && accept) ? 1u : 0u;
+                        if constexpr (TR) {      // N_acc,i of the tuning rule: the owner is the only writer of its site
+                            if (a.tune && owned && accept) {
+                                unsigned int* na = a.nacc_s + (site0 + (size_t)n) * D;
+                                if (npass > 1) na[pass] += 1u;
+                                else {
+#pragma unroll
+                                    for (int c = 0; c < D; ++c) na[c] += 1u;
+                                }
+                            }
+                        }
                         if (trace && owned) {
                             const size_t gs = site0 + (size_t)n;
                             if (npass > 1) {       // trace entries per (site, component)
@@ -719,6 +730,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 cnt[D + l] += pacc[l];
                 cnt[(D + NP) + D + l] += pprop[l];
                 a.p[(size_t)chain * NP + l] = prm[l];
+                if constexpr (TR) { if (a.tune) a.nacc_p[(size_t)chain * NP + l] += pacc[l]; }
             }
             a.cur[chain] = cur;
             a.ar_epoch[chain] = ar_count;

@@ -1,7 +1,7 @@
 """GPU parity for the step-size auto-tuning (pimc_set_tuning, second half)
 against the oracle: with uniform proposals the chains, the per-(site, component) step sizes and the parameter step sizes
-must stay bit-identical through many adjustment rounds, in both update modes, across launches and CTA splits; and the
-engine rule (tuning and tuned step sizes run on the GLOBAL engine)."""
+must stay bit-identical through many adjustment rounds, in both update modes, across launches and CTA splits, on both
+engines (the tile-resident engine ends its launches at the adjustment sweeps and adjusts between them)."""
 import numpy as np
 import pytest
 
@@ -20,17 +20,22 @@ def P():
     return P
 
 
-@pytest.mark.parametrize("cfg,M,launch,mode,disc", [(2, 500, None, 0, 0), (3, 4001, None, 0, 1), (2, 501, (4, 64), 0, 0), (2, 400, (1, 128), 1, 0), (2, 333, (3, 64), 1, 1),
-                                                    (1, 700, (3, 128), 0, 0)])
-def test_tuned_chains_and_step_sizes_bit_identical(P, cfg, M, launch, mode, disc):
+@pytest.mark.parametrize("cfg,M,launch,mode,disc,engine", [
+    (2, 500, None, 0, 0, 0), (3, 4001, None, 0, 1, 0), (2, 1500, None, 1, 0, 0), (2, 901, None, 1, 1, 2), (3, 32768, None, 0, 0, 2),     # tile-resident
+    (2, 500, None, 0, 0, 1), (3, 4001, None, 0, 1, 1), (2, 501, (4, 64), 0, 0, 0), (2, 400, (1, 128), 1, 0, 0), (2, 333, (3, 64), 1, 1, 0),
+    (1, 700, (3, 128), 0, 0, 0)])                                                                                                       # global-memory
+def test_tuned_chains_and_step_sizes_bit_identical(P, cfg, M, launch, mode, disc, engine):
     w = make_workload(cfg, M=M)
     h = gpu_handle(w, launch=launch, kind=1, disc=disc)
+    if engine:
+        h.set_engine(engine)
+    tile = launch is None and engine != 1
     o = oracle_chains(w, kind=1, disc=disc)[0]
     if mode:
         h.set_update_mode(P.UPDATE_COMPONENTWISE); o.set_update_mode(1)
     h.sweep(2, seed=5); o.sweep(2, seed=5)
     h.set_tuning(True, 4, 0.23, 0.05); o.set_tuning(True, 4, 0.23, 0.05)
-    assert h.get_engine()["engine"] == P.ENGINE_GLOBAL
+    assert h.get_engine()["engine"] == (P.ENGINE_TILE if tile else P.ENGINE_GLOBAL)
     h.sweep(7, seed=5); h.sweep(18, seed=5); o.sweep(25, seed=5)          # six adjustments, spread over two launches
     ws, wp = [a.cpu().numpy() for a in h.get_widths()]
     ows, owp = o.get_widths()
@@ -39,11 +44,9 @@ def test_tuned_chains_and_step_sizes_bit_identical(P, cfg, M, launch, mode, disc
     assert not np.array_equal(ows, np.tile(w.w_state, (M + 1, 1)))        # they did move
     xg, pg = [a.cpu().numpy() for a in h.get_path()]
     assert np.array_equal(xg[0], o.get_path()[0]) and np.array_equal(pg[0], o.get_path()[1])
-    # freeze: the tuned step sizes stay in use, unchanged -- and the automatic engine choice is free again (the tile-resident
-    # engine reads the frozen per-site step sizes; component-wise updates stay on the global-memory engine)
+    # freeze: the tuned step sizes stay in use, unchanged, on the same engine
     h.set_tuning(False); o.set_tuning(False)
-    if launch is None and mode == 0:
-        assert h.get_engine()["engine"] == P.ENGINE_TILE
+    assert h.get_engine()["engine"] == (P.ENGINE_TILE if tile else P.ENGINE_GLOBAL)
     h.sweep(9, seed=5); o.sweep(9, seed=5)
     assert np.array_equal(h.get_widths()[0].cpu().numpy()[0], ows)
     assert np.array_equal(h.get_path()[0].cpu().numpy()[0], o.get_path()[0])
@@ -72,15 +75,15 @@ def test_batched_chains_gaussian_proposals_and_engine_rule(P):
     assert np.array_equal(h2.get_widths()[0].cpu().numpy()[1], np.tile(w.w_state, (301, 1)))
     h.set_proposal(w.w_state, w.w_param)
     assert np.array_equal(h.get_widths()[0].cpu().numpy()[0], np.tile(w.w_state, (301, 1)))
-    # engine rule and argument checks
+    # engine rule (tuning does not change the choice) and argument checks
     w1 = make_workload(2, M=300)
     h3 = gpu_handle(w1); h3.set_engine(Pm.ENGINE_TILE)
-    with pytest.raises(Pm.PimcError):
-        h3.set_tuning(True, 5)
+    h3.set_tuning(True, 5)
+    assert h3.get_engine()["engine"] == Pm.ENGINE_TILE
     h4 = gpu_handle(w1)
     assert h4.get_engine()["engine"] == Pm.ENGINE_TILE
     h4.set_tuning(True, 5)
-    assert h4.get_engine()["engine"] == Pm.ENGINE_GLOBAL
+    assert h4.get_engine()["engine"] == Pm.ENGINE_TILE
     h4.set_tuning(False)
     assert h4.get_engine()["engine"] == Pm.ENGINE_TILE
     for bad in ((0, 0.23, 0.02), (5, 0.0, 0.02), (5, 0.23, 1.0)):

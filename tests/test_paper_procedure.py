@@ -35,7 +35,7 @@ def test_paper_procedure_end_to_end_matches_oracle():
         s.set_discretisation(1)                              # the paper's trapezoid rule
         s.set_annealing(0.01, 60)                            # N_cool
         s.set_tuning(True, 10, 0.23, 0.05)                   # N_skip, f_acc, alpha
-    assert h.get_engine()["engine"] == P.ENGINE_GLOBAL       # initialisation phase: annealing and tuning
+    assert h.get_engine()["engine"] == P.ENGINE_TILE         # initialisation phase (annealing and tuning): tile-resident too
     h.sweep(150, seed=9); o.sweep(150, seed=9)               # N_init
     for s in (h, o):
         s.set_tuning(False)
