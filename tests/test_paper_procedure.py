@@ -54,3 +54,15 @@ def test_paper_procedure_end_to_end_matches_oracle():
     assert n == on == 20
     assert np.allclose(mx.cpu().numpy()[0], ox, rtol=1e-13, atol=1e-13) and np.allclose(mp.cpu().numpy()[0], op, rtol=1e-13, atol=1e-15)
     assert np.array_equal(h.stats().cpu().numpy()[0].astype(np.uint64), o.stats())
+
+
+@pytest.mark.gpu
+def test_procedure_module_runs_both_phases_tile_resident():
+    # paper_1103_4887_b200.procedure: the paper's example calculation through the public binding, shortened
+    from paper_1103_4887_b200 import procedure
+    r = procedure.run(iterations=3000, n_skip=50, M=2000)
+    assert r["engine"] == {"initialisation": "tile-resident", "production": "tile-resident"} and r["fault"] == 0
+    assert r["samples"] == 1500 // 50 and r["proposed"][0] == 2001 * 3000 and r["proposed"][4] == 3000
+    assert 0.15 < r["accepted"][0] / r["proposed"][0] < 0.6          # tuned towards f_acc = 0.23 from too small a step
+    assert r["mean_step_size"][0] > 2e-3                             # and the step sizes grew on the way
+    assert all(np.isfinite(r["param_mean"])) and all(s >= 0 for s in r["param_sd"])
