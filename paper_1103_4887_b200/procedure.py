@@ -9,7 +9,7 @@
 on the synthetic stand-in for the paper's experiment (`make_workload(5)`: M = 8000, dt = 0.04 ms, Lorenz-driven current,
 trapezoid rule).  Every iteration runs in libpimc's kernels; this module only sequences the calls.
 
-    python -m paper_1103_4887_b200.procedure                      # the paper's 10^6 iterations (about half a minute on a B200)
+    python -m paper_1103_4887_b200.procedure                      # the paper's 10^6 iterations (about a quarter of a minute on a B200)
     python -m paper_1103_4887_b200.procedure --iterations 20000   # a short run
 
 prints one JSON line: seconds per phase (wall clock around a device synchronize), iterations/s, the engine each phase ran on,
