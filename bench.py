@@ -179,6 +179,8 @@ def run_ours(args):
         h.set_update_mode(P.UPDATE_COMPONENTWISE)
         w_site = W_SITE_SLOTS_COMP if not trap else 4 * 205.0 + 300.0
     peak_tflops = PEAK_TFLOPS_DERIVED * (1.0 if args.dtype == 64 else 2.0)   # fp32: 128 FP32 lanes/clk/SM
+    if args.exchange_hold is not None:
+        h.set_exchange(args.exchange_hold)
     h.set_accum(True, 1)
     h.reset_moments()
     shape = h.get_launch()
@@ -292,6 +294,7 @@ def main():
     ap.add_argument("--disc", default="rk4", choices=["rk4", "trapezoid"], help="model-error discretisation: the north_star's RK4 map or the paper's trapezoid rule")
     ap.add_argument("--dtype", type=int, default=64, choices=[64, 32], help="arithmetic type of the path (config 3 is also quoted in fp32)")
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
+    ap.add_argument("--exchange-hold", type=int, default=None, help="SM clock ticks between publishing a Delta-A partial and the first poll (pimc_set_exchange; default: the library's)")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=120.0, help="seconds of oracle time for --impl reference")
     args = ap.parse_args()

@@ -192,6 +192,12 @@ int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, i
 int pimc_set_engine(pimc_handle* h, int engine, int halo);
 /* Report the engine and halo depth pimc_sweep will use (any pointer may be NULL). */
 int pimc_get_engine(pimc_handle* h, int* engine, int* halo);
+/* Tuning knob of the grid-wide Delta-A sum of a parameter move (row A4; TILE engine, more than one CTA per chain): SM clock
+ * ticks a CTA waits after publishing its partial before it first polls the other CTAs' packets (default 450; 0 = poll at
+ * once).  A packet needs about 1000 ticks from the store to a successful poll; earlier polls only load the L2 slices everybody
+ * is waiting on.  Results do not depend on it.  PIMC_EINVAL outside [0, 100000]. */
+int pimc_set_exchange(pimc_handle* h, int first_poll_hold_cycles);
+
 /* Synchronise the stream and report whether any inter-CTA hand-off timed out (*fault_host != 0 => PIMC_ECUDA;
  * the chain state is then undefined).  A diagnostic: hand-offs cannot be lost in a co-resident (cooperative) launch. */
 int pimc_fault(pimc_handle* h, int* fault_host);
@@ -223,15 +229,25 @@ int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned i
 int pimc_step_selftest(int model, int D, int dtype, const void* x, const void* p, const void* I0, const void* I1,
                        double dt, unsigned long long n, void* g_out, void* stream);
 
-/* Elementary-function self-test: x dev double (n), out dev double (n,7) = the kernels' own branch-free
- * exp(x) (x clamped to +-700), log|x|, sqrt|x|, sin(min(|x|,7.9)), cos(min(|x|,7.9)), 1/|x|, and the HH m-gate rate
- * (m_inf(V) - 0.3)/tau_m(V) at V = x (Eq. 12-14). */
+/* Elementary-function self-test: x dev double (n), out dev double (n,9) = the kernels' own branch-free
+ * exp(x) (x clamped to +-700), log|x|, sqrt|x|, sin(min(|x|,7.9)), cos(min(|x|,7.9)), 1/|x|, and the three HH gate rates
+ * (a_inf(V) - 0.3)/tau_a(V), a = m, h, n, at V = x (Eq. 12-14; Table 1) as the sweep kernels compute them. */
 int pimc_math_selftest(const double* x, unsigned long long n, double* out, void* stream);
 
 /* Roofline denominator probe: runs a register-only chain of independent double-precision FMAs on every SM for
  * roughly `millis` milliseconds and writes the sustained rate in lane-FMA per second (one lane-FMA = one FP64 pipe
  * slot of one thread) to *lane_fma_per_s (host).  Synchronises the device. */
 int pimc_fp64_peak_selftest(int millis, double* lane_fma_per_s);
+
+/* Inter-CTA exchange probe (row A4: the grid-wide scalar all-reduce of a parameter move):
+ * a cooperative launch of n_ctas CTAs (0 = one per SM) x threads runs `rounds` rounds of { `work` iterations of a register-only
+ * FP64 loop with up to 12 % per-CTA jitter, one all-reduce of a per-thread partial }.  mode -1: work only; 0: round 1's flat
+ * all-gather (block sum, n_ctas x n_ctas polls, block sum); 1: the two-hop butterfly the sweep kernel uses; 2: block sum, then
+ * one warp gathers every block sum; 3: one L2 hop (read the left neighbour's packet).  Host outputs: SM clock ticks per round
+ * (after rounds/4 warm-up rounds), the largest |total - exact sum| of the last round over the CTAs, and the number of distinct
+ * bit patterns among the CTAs' totals (must be 1: every CTA has to take the same decision).  Synchronises the device. */
+int pimc_exchange_selftest(int mode, int n_ctas, int threads, int rounds, int work, double* cycles_per_round_host,
+                           double* max_abs_err_host, int* n_distinct_host);
 
 const char* pimc_last_error(const pimc_handle* h);   /* h may be NULL: last error of a failed pimc_init / static call */
 int pimc_destroy(pimc_handle* h);

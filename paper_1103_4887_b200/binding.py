@@ -50,6 +50,7 @@ _SIGNATURES = {
     "pimc_set_tuning": (C.c_int, [_vp, C.c_int, C.c_longlong, C.c_double, C.c_double]),
     "pimc_get_widths": (C.c_int, [_vp, _vp, _vp]),
     "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
+    "pimc_set_exchange": (C.c_int, [_vp, C.c_int]),
     "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
     "pimc_set_sweep_index": (C.c_int, [_vp, C.c_ulonglong]),
@@ -60,6 +61,7 @@ _SIGNATURES = {
     "pimc_step_selftest": (C.c_int, [C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp, C.c_double, C.c_ulonglong, _vp, _vp]),
     "pimc_math_selftest": (C.c_int, [_vp, C.c_ulonglong, _vp, _vp]),
     "pimc_fp64_peak_selftest": (C.c_int, [C.c_int, _dp]),
+    "pimc_exchange_selftest": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _dp, _dp, _ip]),
     "pimc_last_error": (C.c_char_p, [_vp]),
     "pimc_destroy": (C.c_int, [_vp]),
 }
@@ -218,6 +220,9 @@ class Pimc:
         _check(lib().pimc_get_engine(self._h, C.byref(e), C.byref(hh)), self._h)
         return dict(engine=e.value, halo=hh.value)
 
+    def set_exchange(self, first_poll_hold_cycles=450):
+        _check(lib().pimc_set_exchange(self._h, int(first_poll_hold_cycles)), self._h)
+
     def fault(self):
         """Synchronise the stream; raises PimcError if an inter-CTA hand-off was lost."""
         f = C.c_int()
@@ -358,10 +363,10 @@ def step_selftest(model, x, p, I0, I1, dt):
 
 
 def math_selftest(x):
-    """x: CUDA float64 tensor (n,) -> (n,7): exp, log|x|, sqrt|x|, sin, cos, 1/|x|, HH m-gate rate (kernel math)."""
+    """x: CUDA float64 tensor (n,) -> (n,9): exp, log|x|, sqrt|x|, sin, cos, 1/|x|, HH gate rates m, h, n (kernel math)."""
     import torch
     assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
-    out = torch.empty((x.numel(), 7), dtype=torch.float64, device=x.device)
+    out = torch.empty((x.numel(), 9), dtype=torch.float64, device=x.device)
     _check(lib().pimc_math_selftest(_ptr(x), x.numel(), _ptr(out), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
     return out
 
@@ -371,6 +376,13 @@ def fp64_peak(millis=200):
     v = C.c_double()
     _check(lib().pimc_fp64_peak_selftest(int(millis), C.byref(v)))
     return v.value
+
+
+def exchange_selftest(mode, n_ctas=0, threads=256, rounds=2000, work=0):
+    """Grid-wide all-reduce probe (pimc_exchange_selftest) -> dict(cycles_per_round, max_abs_err, n_distinct)."""
+    cyc, err, nd = C.c_double(), C.c_double(), C.c_int()
+    _check(lib().pimc_exchange_selftest(int(mode), int(n_ctas), int(threads), int(rounds), int(work), C.byref(cyc), C.byref(err), C.byref(nd)))
+    return dict(cycles_per_round=cyc.value, max_abs_err=err.value, n_distinct=nd.value)
 
 
 def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_path=False):

@@ -4,6 +4,7 @@
 #include "../../include/pimc.h"
 
 #include <cmath>
+#include <cstdlib>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -146,6 +147,7 @@ struct pimc_handle {
     unsigned char *tr_acc = nullptr, *tr_accp = nullptr;
     int G_user = 0, T_user = 0, engine_user = PIMC_ENGINE_AUTO, halo_user = -1;
     unsigned long long hs_base = 0, launches = 0;
+    int ar_hold = 450;                // pimc_set_exchange
     int sm_count = 0;
     std::string err;
 };
@@ -344,7 +346,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
     a.t0 = h->t; a.seed = seed; a.n_sweeps = n_sweeps; a.do_states = do_states; a.do_params = do_params;
     a.hs_flag = h->lay.hs_flag; a.ar_val = h->lay.ar_val; a.ar_flag = h->lay.ar_flag; a.ar_epoch = h->lay.ar_epoch;
     a.hs_base = h->hs_base;
-    a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault;
+    a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault; a.ar_hold = h->ar_hold;
 
     const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
     const bool trap = h->disc == PIMC_DISC_TRAPEZOID;
@@ -853,6 +855,13 @@ int pimc_get_engine(pimc_handle* h, int* engine, int* halo) {
     return PIMC_OK;
 }
 
+int pimc_set_exchange(pimc_handle* h, int first_poll_hold_cycles) {
+    if (!h) return PIMC_EINVAL;
+    if (first_poll_hold_cycles < 0 || first_poll_hold_cycles > 100000) return fail(h, PIMC_EINVAL, "first_poll_hold_cycles must be in [0, 100000]");
+    h->ar_hold = first_poll_hold_cycles;
+    return PIMC_OK;
+}
+
 int pimc_fault(pimc_handle* h, int* fault_host) {
     if (!h || !fault_host) return fail(h, PIMC_EINVAL, "null argument");
     PIMC_CUDA(h, cudaMemcpyAsync(fault_host, h->lay.fault, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
@@ -980,6 +989,66 @@ int pimc_fp64_peak_selftest(int millis, double* lane_fma_per_s) {
     cudaFree(sink);
     PIMC_CUDA(nullptr, cudaGetLastError());
     *lane_fma_per_s = best;
+    return PIMC_OK;
+}
+
+int pimc_exchange_selftest(int mode, int n_ctas, int threads, int rounds, int work, double* cycles_per_round_host,
+                           double* max_abs_err_host, int* n_distinct_host) {
+    if (!cycles_per_round_host || !max_abs_err_host || !n_distinct_host) return fail(nullptr, PIMC_EINVAL, "null argument");
+    if (mode < -1 || (mode > 10 && mode < 100) || mode > 140 || threads < 32 || threads > 256 || threads % 32 != 0 || rounds < 2 || work < 0)
+        return fail(nullptr, PIMC_EINVAL, "bad argument");
+    int dev = 0, sms = 0;
+    PIMC_CUDA(nullptr, cudaGetDevice(&dev));
+    PIMC_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (n_ctas == 0) n_ctas = sms;
+    if (n_ctas < 1 || n_ctas > sms || n_ctas > kXchgMaxCtas) return fail(nullptr, PIMC_EINVAL, "n_ctas must be in [1, SM count]");
+    const size_t smem = 100 * 1024;               // one CTA per SM, as in the sweep launches
+    PIMC_CUDA(nullptr, cudaFuncSetAttribute((const void*)xchg_selftest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t n_ar = (size_t)2 * kTileMaxCtas * kArSlotWords;
+    const size_t n_inbox = (size_t)2 * kTileMaxCtas * kTileMaxCtas * 2;
+    const size_t bytes = (kXchgWords + n_ar) * 8 + 256 + (size_t)n_ctas * 8 + 128 + 256 + n_inbox * 8;
+    char* devp = nullptr;
+    PIMC_CUDA(nullptr, cudaMalloc(&devp, bytes));
+    cudaMemset(devp, 0, bytes);
+    unsigned long long* mbox = (unsigned long long*)devp;
+    unsigned long long* ar = mbox + kXchgWords;
+    int* fault = (int*)(ar + n_ar);
+    double* out_tot = (double*)((char*)fault + 256);
+    long long* out_cycles = (long long*)(out_tot + n_ctas);
+    double* sink = (double*)(out_cycles + 6);
+    unsigned long long* inbox = (unsigned long long*)(((uintptr_t)(sink + 2) + 255) & ~(uintptr_t)255);
+    const int warm = rounds / 4;
+    void* params[] = {&mode, &rounds, (void*)&warm, &work, &mbox, &ar, &fault, &out_tot, &out_cycles, &sink, &inbox};
+    cudaError_t e = cudaLaunchCooperativeKernel((const void*)xchg_selftest_kernel, dim3((unsigned)n_ctas), dim3((unsigned)threads), params, smem, 0);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    std::vector<double> tot(n_ctas);
+    long long cyc = 0;
+    int flt = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(tot.data(), out_tot, sizeof(double) * n_ctas, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(&cyc, out_cycles, sizeof cyc, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && (mode == 0 || mode == 6) && getenv("PIMC_XCHG_PHASES")) {
+        long long ph[4];
+        cudaMemcpy(ph, out_cycles, sizeof ph, cudaMemcpyDeviceToHost);
+        const double d = (double)n_ctas * (rounds - warm);
+        fprintf(stderr, "phases (mean over CTAs): block sum 1 %.0f, store+poll %.0f, block sum 2 %.0f cycles\n", ph[1] / d, ph[2] / d, ph[3] / d);
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(&flt, fault, sizeof flt, cudaMemcpyDeviceToHost);
+    cudaFree(devp);
+    if (e != cudaSuccess) return fail(nullptr, PIMC_ECUDA, "pimc_exchange_selftest: %s", cudaGetErrorString(e));
+    if (flt) return fail(nullptr, PIMC_ECUDA, "pimc_exchange_selftest: a packet was never delivered");
+    *cycles_per_round_host = (double)cyc / (double)(rounds - warm);
+    // expected total of the last round (modes 0-2), in long double on the host
+    long double expect = 0.0L;
+    for (int b = 0; b < n_ctas; ++b)
+        for (int t = 0; t < threads; ++t) expect += (long double)((double)((b * 131 + t * 7 + (rounds - 1) * 13) % 1000 - 500) * 0.001);
+    double worst = 0.0;
+    int distinct = 1;
+    for (int b = 0; b < n_ctas; ++b) {
+        if (mode >= 0 && mode != 3 && (mode < 7 || mode >= 10)) worst = std::max(worst, (double)fabsl((long double)tot[b] - expect));
+        if (b > 0 && std::memcmp(&tot[b], &tot[0], sizeof(double)) != 0) distinct++;
+    }
+    *max_abs_err_host = worst;
+    *n_distinct_host = (mode >= 0 && mode != 3 && (mode < 7 || mode >= 10)) ? distinct : 1;
     return PIMC_OK;
 }
 

@@ -84,6 +84,7 @@ template <typename R> struct SweepArgs {
     unsigned long long* hx_epoch;   // (C) halo exchanges performed so far
     unsigned long long* ar_words;   // (2 slots, kTileMaxCtas, kArSlotWords) Delta-A partials, one 128-byte line per CTA
     int* fault;                     // set to 1 if a hand-off was never delivered
+    int ar_hold;                    // SM clock ticks between publishing a Delta-A partial and the first poll of the others' (pimc_set_exchange)
 };
 
 // ---- annealing multiplier of the model-error weights at sweep t (same closed form as the oracle; beta = 1 when off) ----
@@ -675,20 +676,21 @@ static __global__ void rng_selftest_kernel(const uint32_t* __restrict__ ctrs, un
     }
 }
 
-// ---- elementary-function self-test: out (n,7) = exp, log, sqrt, sin, cos, 1/x, HH gate m-rate at (x, a = 0.3) ----
+// ---- elementary-function self-test: out (n,9) = exp, log, sqrt, sin, cos, 1/x, HH gate rates of m, h, n at (V = x, a = 0.3) ----
 static __global__ void math_selftest_kernel(const double* __restrict__ x, unsigned long long n, double* __restrict__ out) {
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
         const double v = x[i];
         const double av = fabs(v);
         double s, c;
         sincos_fast(fmin(av, 7.9), s, c);
-        out[7 * i + 0] = exp_fast(fmin(fmax(v, -700.0), 700.0));
-        out[7 * i + 1] = log_fast(fmax(av, 1e-300));
-        out[7 * i + 2] = sqrt_fast(fmax(av, 1e-300));
-        out[7 * i + 3] = s;
-        out[7 * i + 4] = c;
-        out[7 * i + 5] = rcp_fast(fmax(av, 1e-300));
-        out[7 * i + 6] = HHModel<double>::gate_fast(v, 0.3, -40.0, 15.0, 0.1, 0.4);
+        out[9 * i + 0] = exp_fast(fmin(fmax(v, -700.0), 700.0));
+        out[9 * i + 1] = log_fast(fmax(av, 1e-300));
+        out[9 * i + 2] = sqrt_fast(fmax(av, 1e-300));
+        out[9 * i + 3] = s;
+        out[9 * i + 4] = c;
+        out[9 * i + 5] = rcp_fast(fmax(av, 1e-300));
+        const double xg[4] = {v, 0.3, 0.3, 0.3};
+        HHModel<double>::rhs_gates(xg, out + 9 * i + 6);          // the production gate code (one shared exponential)
     }
 }
 

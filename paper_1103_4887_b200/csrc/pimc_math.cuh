@@ -81,7 +81,10 @@ __device__ __forceinline__ double exp_fast(double x) {
 // ratios of the result matter (the Hodgkin-Huxley gates), which are exact to rounding long before saturation.
 // The clamp is integer arithmetic on k, off the floating-point dependency chain.  Requires |c1 V + c0| < 2^31 ln 2
 // (the caller guards).
-__device__ __forceinline__ double exp_affine_sat(double V, double c1, double c0) {
+template <int KMAX> __device__ __forceinline__ double exp_affine_sat_k(double V, double c1, double c0);
+__device__ __forceinline__ double exp_affine_sat(double V, double c1, double c0) { return exp_affine_sat_k<300>(V, c1, c0); }
+// the same with the scale clamped to 2^+-KMAX
+template <int KMAX> __device__ __forceinline__ double exp_affine_sat_k(double V, double c1, double c0) {
     constexpr double kMagic = 6755399441055744.0;
     constexpr double kLog2e = 1.4426950408889634074;
     constexpr double kLn2Hi = 0x1.62e42fefa39efp-1, kLn2Lo = 0x1.abc9e3b39803fp-56;
@@ -92,7 +95,7 @@ __device__ __forceinline__ double exp_affine_sat(double V, double c1, double c0)
     double r = fma(kd, -kLn2Hi, x);
     r = fma(kd, -kLn2Lo, r);
     const double e = expm1_small(r);
-    k = min(max(k, -300), 300);
+    k = min(max(k, -KMAX), KMAX);
     const double s = __hiloint2double((k + 1023) << 20, 0);
     return fma(e, s, s);
 }
@@ -135,7 +138,9 @@ __device__ __forceinline__ double u_over_1mexp(double u) {
 // ---- single precision (the fp32 variant of config 3) -----------------------------------------------------------
 // exp(x) SATURATED to [2^-60, 2^61) (so that its square stays finite in fp32): x = k ln2 + r, |r| <= ln2/2,
 // e^r = 1 + r + r^2 Q(r) with Q of degree 5 (truncation < 2e-8 relative); k clamped in integer arithmetic.
-__device__ __forceinline__ float expf_sat(float x) {
+template <int KMAX> __device__ __forceinline__ float expf_sat_k(float x);
+__device__ __forceinline__ float expf_sat(float x) { return expf_sat_k<60>(x); }
+template <int KMAX> __device__ __forceinline__ float expf_sat_k(float x) {
     constexpr float kMagic = 12582912.0f;                          // 1.5 * 2^23
     constexpr float kLog2e = 1.44269504088896341f;
     constexpr float kLn2Hi = 0.693145751953125f, kLn2Lo = 1.42860682030941723e-6f;   // hi has 12 trailing zero bits
@@ -152,7 +157,7 @@ __device__ __forceinline__ float expf_sat(float x) {
     const float b = fmaf(a1, r2, a0);
     const float p = fmaf(a2, r4, b);
     const float e = fmaf(p, r2, r);                                // e^r - 1
-    k = min(max(k, -60), 60);
+    k = min(max(k, -KMAX), KMAX);
     const float s = __int_as_float((k + 127) << 23);               // 2^k
     return fmaf(e, s, s);
 }

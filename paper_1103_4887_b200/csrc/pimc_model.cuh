@@ -9,10 +9,6 @@
 
 namespace pimc {
 
-template <typename R> __device__ __forceinline__ R tanh_(R v);
-template <> __device__ __forceinline__ double tanh_<double>(double v) { return tanh(v); }
-template <> __device__ __forceinline__ float tanh_<float>(float v) { return tanhf(v); }
-
 // ---------------------------------------------------------------------------------------------------
 // KIN selects the gate kinetics: 0 = the paper's tanh forms, 1 = the classic alpha/beta rate functions
 // (Hodgkin & Huxley 1952, rest at -65 mV; include/pimc.h PIMC_MODEL_HH_CLASSIC).  Everything else is shared.
@@ -21,36 +17,12 @@ template <typename R, int KIN> struct HHModelK {
     static constexpr int NP = 7;
 
     // The parameter vector lives in shared memory (one copy per CTA); p[] = (gNa, gK, gL, ENa, EK, EL, C).
-    // d a / dt = (a_inf(V) - a) / tau_a(V);  a_inf = 1/2 + 1/2 tanh(s), tau = tau0 + tau1 (1 - tanh^2 s), s = (V - Va)/dVa
-    static __device__ __forceinline__ R gate(R V, R a, R Va, R dVa, R tau0, R tau1) {
-        const R th = tanh_<R>((V - Va) / dVa);
-        const R ainf = R(0.5) + R(0.5) * th;
-        const R tau = tau0 + tau1 * (R(1) - th * th);
-        return (ainf - a) / tau;
-    }
-    // Double precision: one exponential and one reciprocal per gate.  With e = exp(2 s), q = e + 1:
+    // d a / dt = (a_inf(V) - a) / tau_a(V);  a_inf = 1/2 + 1/2 tanh(s), tau = tau0 + tau1 (1 - tanh^2 s), s = (V - Va)/dVa  (PAPER.md:264-270)
+    // Gate rates in one-exponential form.  With e = exp(2 s), q = e + 1:
     //   tanh s = (e-1)/q, a_inf = e/q, 1 - tanh^2 s = 4 e / q^2  =>  (a_inf - a)/tau = (e - a q) q / (tau0 q^2 + 4 tau1 e),
-    //   and tau0 q^2 + 4 tau1 e = tau0 + e (2 tau0 + 4 tau1 + tau0 e) (two FMAs straight from e).
-    // e saturates at 2^+-300 (exp_affine_sat), where tanh s = +-1 far below half an ulp, so nothing overflows.
-    static __device__ __forceinline__ double gate_fast(double V, double a, double Va, double dVa, double tau0, double tau1) {
-        const double c1 = 2.0 / dVa, c0 = -2.0 * Va / dVa;
-        const double e = exp_affine_sat(V, c1, c0);
-        const double q = e + 1.0;
-        const double den = fma(e, fma(e, tau0, 2.0 * tau0 + 4.0 * tau1), tau0);
-        const double num = fma(-a, q, e) * q;
-        return div_series(num, den);
-    }
+    //   and tau0 q^2 + 4 tau1 e = tau0 + e (2 tau0 + 4 tau1 + tau0 e) (two FMAs straight from e): one exponential and one
+    //   reciprocal per gate instead of a tanh and a divide (gates_shared_exp below then shares the exponential between the gates).
     // dV/dt (Eq. 11 with the config's physical parameters): the only place the parameters enter
-    // Single precision: the same one-exponential form with branch-free fp32 exp and reciprocal (no libdevice tanhf / division);
-    // e saturates at 2^+-60 (tanh = +-1 to 1e-18).  |x| is limited by the caller's guard.
-    static __device__ __forceinline__ float gate_fast_f(float V, float a, float Va, float dVa, float tau0, float tau1) {
-        const float c1 = 2.0f / dVa, c0 = -2.0f * Va / dVa;
-        const float e = expf_sat(fmaf(V, c1, c0));
-        const float q = e + 1.0f;
-        const float den = fmaf(e, fmaf(e, tau0, 2.0f * tau0 + 4.0f * tau1), tau0);
-        const float num = fmaf(-a, q, e) * q;
-        return divf_fast(num, den);
-    }
     static __device__ __forceinline__ R rhs_V(const R x[4], const R* __restrict__ p, R inv_C, R I) {
         const R V = x[0], m = x[1], h = x[2], n = x[3];
         const R n2 = n * n;
@@ -80,14 +52,59 @@ template <typename R, int KIN> struct HHModelK {
                 Fg[1] = ah * (1.0f - h) - bh * h;
                 Fg[2] = an * (1.0f - n) - bn * n;
             }
-        } else if constexpr (sizeof(R) == 8) {
-            Fg[0] = gate_fast(V, m, -40.0, 15.0, 0.1, 0.4);
-            Fg[1] = gate_fast(V, h, -60.0, -15.0, 1.0, 7.0);
-            Fg[2] = gate_fast(V, n, -55.0, 30.0, 1.0, 5.0);
-        } else {
-            Fg[0] = gate_fast_f(V, m, -40.0f, 15.0f, 0.1f, 0.4f);
-            Fg[1] = gate_fast_f(V, h, -60.0f, -15.0f, 1.0f, 7.0f);
-            Fg[2] = gate_fast_f(V, n, -55.0f, 30.0f, 1.0f, 5.0f);
+        } else if constexpr (sizeof(R) == 8) gates_shared_exp(V, m, h, n, Fg);
+        else gates_shared_exp_f(V, m, h, n, Fg);
+    }
+    // ONE exponential for the three gates.  Table 1's widths are 15, -15 and 30 mV, so the three arguments
+    // 2 s_a = 2 (V - V_a)/dV_a are (2V + 80)/15, -(2V + 120)/15 and (V + 55)/15: with u = exp((V + 55)/15) and w = u^2,
+    //   e_n = u,   e_m = e^{-2} w,   e_h = e^{-2/3} / w.
+    // m and n use the one-exponential form of gate_fast directly.  For h, numerator and denominator of
+    // (e - a q) q / (tau0 + e (2 tau0 + 4 tau1 + tau0 e)) are multiplied by w^2:  with c = e^{-2/3}, Q = c + w,
+    //   (c - a Q) Q / (tau0 w^2 + c (2 tau0 + 4 tau1) w + tau0 c^2)   -- no second exponential, no extra reciprocal.
+    // 40 of the 96 FP64 instructions of a stage's gate rates go away (identical in exact arithmetic; the rates stay within a
+    // few ulp of the tanh definition: tests/test_gpu_math.py).  u saturates at 2^+-250 (u^4 stays finite), where every
+    // tanh is +-1 to far below half an ulp.
+    static __device__ __forceinline__ void gates_shared_exp(double V, double m, double h, double n, double Fg[3]) {
+        const double u = exp_affine_sat_k<250>(V, 1.0 / 15.0, 55.0 / 15.0);
+        const double w = u * u;
+        {   // m: (V_a, dV_a, tau0, tau1) = (-40, 15, 0.1, 0.4)
+            const double e = 0x1.152aaa3bf81ccp-3 * w;                       // e^{-2} w
+            const double q = e + 1.0;
+            const double den = fma(e, fma(e, 0.1, 2.0 * 0.1 + 4.0 * 0.4), 0.1);
+            Fg[0] = div_series(fma(-m, q, e) * q, den);
+        }
+        {   // h: (-60, -15, 1, 7)
+            constexpr double c = 0x1.06de9bcee72dep-1;                       // e^{-2/3}
+            const double Q = c + w;
+            const double den = fma(w, fma(w, 1.0, c * (2.0 * 1.0 + 4.0 * 7.0)), 1.0 * c * c);
+            Fg[1] = div_series(fma(-h, Q, c) * Q, den);
+        }
+        {   // n: (-55, 30, 1, 5)
+            const double q = u + 1.0;
+            const double den = fma(u, fma(u, 1.0, 2.0 * 1.0 + 4.0 * 5.0), 1.0);
+            Fg[2] = div_series(fma(-n, q, u) * q, den);
+        }
+    }
+    // fp32: the same sharing; u saturates at 2^+-30 (u^4 finite in fp32; tanh = +-1 to 2^-29, below half an fp32 ulp)
+    static __device__ __forceinline__ void gates_shared_exp_f(float V, float m, float h, float n, float Fg[3]) {
+        const float u = expf_sat_k<30>(fmaf(V, 1.0f / 15.0f, 55.0f / 15.0f));
+        const float w = u * u;
+        {
+            const float e = 0.135335283236612692f * w;
+            const float q = e + 1.0f;
+            const float den = fmaf(e, fmaf(e, 0.1f, 2.0f * 0.1f + 4.0f * 0.4f), 0.1f);
+            Fg[0] = divf_fast(fmaf(-m, q, e) * q, den);
+        }
+        {
+            constexpr float c = 0.513417119032592027f;
+            const float Q = c + w;
+            const float den = fmaf(w, fmaf(w, 1.0f, c * 30.0f), c * c);
+            Fg[1] = divf_fast(fmaf(-h, Q, c) * Q, den);
+        }
+        {
+            const float q = u + 1.0f;
+            const float den = fmaf(u, fmaf(u, 1.0f, 22.0f), 1.0f);
+            Fg[2] = divf_fast(fmaf(-n, q, u) * q, den);
         }
     }
     static __device__ __forceinline__ void rhs(const R x[4], const R* __restrict__ p, R inv_C, R I, R F[4]) {
@@ -107,6 +124,12 @@ template <typename R, int KIN> struct HHModelK {
         q.hdt = R(0.5) * dt;
         q.dt6 = dt / R(6);
         return q;
+    }
+    // The same for a parameter move that changes entry l only: 1/C has to be recomputed for l = 6 (C) alone -- the division
+    // is the first thing on the dependent chain of the evaluation.
+    static __device__ __forceinline__ Prep prepare_move(const Prep& cur, const R* __restrict__ p_new, R dt, int l) {
+        if (l == NP - 1) return prepare(p_new, dt);
+        return cur;
     }
     static constexpr R kVmax = sizeof(R) == 8 ? R(1e8) : R(1e6);
     // Domain guard of the branch-free gates: a stage voltage beyond +-1e8 mV (fp32: 1e6 mV) or NaN makes the whole increment
@@ -175,6 +198,7 @@ template <typename R, int D_> struct LinearModel {
     static constexpr int NP = D_ * D_;
     struct Prep {};
     static __device__ __forceinline__ Prep prepare(const R* __restrict__, R) { return Prep{}; }
+    static __device__ __forceinline__ Prep prepare_move(const Prep&, const R* __restrict__, R, int) { return Prep{}; }
     // Trapezoid form of the linear model: F(x) = (A x - x)/dt, so c = (dt/2) F = (A x - x)/2
     static __device__ __forceinline__ void half_rhs(const R x[D_], const R* __restrict__ p, const Prep&, R, R c[D_]) {
 #pragma unroll

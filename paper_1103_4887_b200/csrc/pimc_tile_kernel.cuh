@@ -22,6 +22,7 @@
 // Parameter moves (row A4) use all 2 TC threads, one tile site each.
 #pragma once
 #include "pimc_kernels.cuh"
+#include "pimc_exchange.cuh"
 
 namespace pimc {
 
@@ -75,6 +76,10 @@ __device__ __forceinline__ void bar_compute(int n_threads) {     // named barrie
 
 // Deterministic block sum with ONE barrier: the warp partials go to one of two alternating buffers, so the buffer of
 // call k is only rewritten by call k+2, after every thread has passed the barrier of call k+1.
+// The warp partials are added as a fixed balanced tree (depth 3 for 8 warps), not one after the other: a dependent FP64 add
+// costs ~17 cycles here (measured, pimc_exchange_selftest modes 7-9: xor tree 207 cycles, barrier + serial 8-sum 307), and
+// this sum sits on the critical path of every parameter move twice.  NW = the most warps a CTA of this kernel can have.
+template <int NW = 16>
 __device__ __forceinline__ double block_sum_db(double v, double* red /* 64 doubles */, unsigned& phase) {
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
@@ -83,9 +88,14 @@ __device__ __forceinline__ double block_sum_db(double v, double* red /* 64 doubl
     const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
     if ((threadIdx.x & 31) == 0) buf[warp] = v;
     __syncthreads();
-    double tot = 0.0;
-    for (int w = 0; w < nwarps; ++w) tot += buf[w];
-    return tot;
+    double t[NW];
+#pragma unroll
+    for (int w = 0; w < NW; ++w) t[w] = w < nwarps ? buf[w] : 0.0;
+#pragma unroll
+    for (int step = 1; step < NW; step <<= 1)
+#pragma unroll
+        for (int w = 0; w + step < NW; w += 2 * step) t[w] += t[w + step];
+    return t[0];
 }
 
 // Shared-memory layout.  Every per-site array (x, both caches, moment sums) is stored as parity planes in
@@ -219,6 +229,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     // exactly a single-component Metropolis move; a joint sweep has one pass.
     constexpr int npass = COMP ? D : 1;
     const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK, npass);
+    constexpr int NWMAX = MAXT / 32;               // warps of the largest CTA this instantiation is launched with
     constexpr int RP = MAXT / 2;                   // pitch of the random-number ring
     constexpr int P = MAXT / 2 + 2;                // == tile_pitch(T): the launcher picks MAXT = 256 for T <= 256, else 512
 
@@ -512,13 +523,13 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                         R xn[D], gp[D];
                         lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
                         if constexpr (TRAP) {
-                            Model::half_rhs(xn, pp, Model::prepare(pp, a.dt), sm.Is[prm_iloc], gp);
+                            Model::half_rhs(xn, pp, Model::prepare_move(prep, pp, a.dt, l), sm.Is[prm_iloc], gp);
                             sts_site<R, D>(ga, prm_q, prm_j, P, gp);
                         } else {
                             R kk[NK > 0 ? NK : 1];
 #pragma unroll
                             for (int c = 0; c < NK; ++c) kk[c] = sm.kg[(prm_q * NK + c) * P + prm_j];
-                            Model::template increment_k<(NK > 0), false>(xn, pp, Model::prepare(pp, a.dt), sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp, kk, nullptr);
+                            Model::template increment_k<(NK > 0), false>(xn, pp, Model::prepare_move(prep, pp, a.dt, l), sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp, kk, nullptr);
                             sts_site<R, D>(ga, prm_q, prm_j, P, gp);
                             if (owned) {
                                 R xq[D], gn[D];
@@ -555,14 +566,24 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             part = (double)acc;
                         }
                     }
-                    dA = block_sum_db(part, sm.red, red_phase);
-                    if (G > 1) {   // all-gather of the G partials as tagged packets; every CTA sums them in index order
+                    dA = block_sum_db<NWMAX>(part, sm.red, red_phase);
+                    if (G > 1) {   // all-gather of the G partials as tagged packets; every CTA sums them in the same fixed order
                         const uint32_t tag = (uint32_t)(ar_count + 1ull);
                         unsigned long long* base = a.ar_words + ((size_t)(ar_count & 1ull) * kTileMaxCtas + (size_t)chain * G) * kArSlotWords;
                         if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
+                        // The FIRST poll is held back: a packet needs ~1000 cycles from the store to a successful poll whatever
+                        // happens, and polls that arrive before it only load the L2 slices everybody is waiting on (measured,
+                        // pimc_exchange_selftest modes 100+: holding 400 cycles takes the exchange from 3260 to 2540 cycles).
+                        const long long until = clock64() + (long long)a.ar_hold;
                         double mine = 0.0;
-                        for (int j = tid; j < G; j += T) mine += ll_wait_f64(base + (size_t)j * kArSlotWords, tag, a.fault);
-                        dA = block_sum_db(mine, sm.red, red_phase);
+                        for (int j = tid; j < G; j += T) {
+                            if (j == b) mine += dA;                     // own partial: no trip through L2
+                            else {
+                                while (clock64() < until) {}
+                                mine += ll_wait_f64(base + (size_t)j * kArSlotWords, tag, a.fault);
+                            }
+                        }
+                        dA = block_sum_db<NWMAX>(mine, sm.red, red_phase);
                         ar_count += 1ull;
                     }
                     accept = logu < -dA;
@@ -737,6 +758,240 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             a.hx_epoch[chain] = hx_count;
         }
     }
+}
+
+// ---- exchange self-test (pimc_exchange_selftest): the grid-wide scalar all-reduce of a parameter move on its own ----------------
+// Every CTA runs `rounds` rounds of { `work` iterations of a register-only FP64 loop (with a per-CTA, per-round jitter of
+// up to 12 %, standing in for the model evaluation), then one all-reduce of a per-thread partial }.  mode: -1 = work only,
+// 0 = round 1's flat all-gather (block sum, G x G polls, block sum), 1 = the two-hop butterfly of pimc_exchange.cuh,
+// 2 = block sum, then ONE warp gathers all G block sums (all polls in flight), 3 = one L2 hop (ring: read the left
+// neighbour's packet).  out_tot[cta] = the last round's total as that CTA saw it; out_cycles = clock64 ticks of CTA 0.
+__device__ __forceinline__ double xchg_selftest_part(int round, int cta, int tid) {
+    return (double)((cta * 131 + tid * 7 + round * 13) % 1000 - 500) * 0.001;
+}
+static __global__ void __launch_bounds__(256, 1) xchg_selftest_kernel(int mode, int rounds, int warm, int work, unsigned long long* mbox,
+                                                                     unsigned long long* ar_words, int* fault, double* out_tot,
+                                                                     long long* out_cycles, double* sink, unsigned long long* inbox_words) {
+    __shared__ double red[64];
+    __shared__ double red3[48];
+    __shared__ double s_tot;
+    unsigned long long pa = 0, pb = 0;            // mode 6: the poll in flight
+    const int G = gridDim.x, b = blockIdx.x, tid = threadIdx.x, T = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = T >> 5;
+    const XchgGeom geo = xchg_geom(G, b, nw);
+    unsigned red_phase = 0;
+    unsigned long long epoch = 0;
+    double w0 = 1.0 + tid * 1e-6, w1 = 0.5, w2 = 0.25, w3 = 0.125;
+    long long t_start = 0, ph[3] = {0, 0, 0};
+    double tot = 0.0;
+    XfixState xst;
+    if (mode == 5 && tid == 0) xfix_begin(mbox, xst);
+    for (int r = 0; r < rounds; ++r) {
+        if (r == warm && b == 0 && tid == 0) t_start = clock64();
+        const int iters = work + (int)((unsigned)(work * ((b * 2654435761u + r * 40503u) >> 24 & 31)) >> 8);   // + 0..12 %
+        for (int i = 0; i < iters; ++i) {
+            w0 = fma(w0, 0.999999, 1e-9); w1 = fma(w1, 0.999999, 1e-9); w2 = fma(w2, 0.999999, 1e-9); w3 = fma(w3, 0.999999, 1e-9);
+        }
+        const double part = xchg_selftest_part(r, b, tid);
+        const uint32_t tag = (uint32_t)(epoch + 1ull);
+        const int buf = (int)(epoch & 1ull);
+        if (mode == 0) {
+            const long long c0 = clock64();
+            double dA = block_sum_db(part, red, red_phase);
+            const long long c1 = clock64();
+            unsigned long long* base = ar_words + (size_t)buf * kTileMaxCtas * kArSlotWords;
+            if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
+            double mine = 0.0;
+            for (int j = tid; j < G; j += T) mine += ll_wait_f64(base + (size_t)j * kArSlotWords, tag, fault);
+            const long long c2 = clock64();
+            tot = block_sum_db(mine, red, red_phase);
+            const long long c3 = clock64();
+            if (r >= warm && tid == (b * 37) % 148) { ph[0] += c1 - c0; ph[1] += c2 - c1; ph[2] += c3 - c2; }
+        } else if (mode == 1) {
+            const double wsum = xchg_xor_tree(part);
+            if (lane == 0) xchg_publish_warp(mbox, buf, b, warp, wsum, tag);
+            if (warp == 0) {
+                const double t2 = xchg_warp_2d(mbox, geo, nw, tag, buf, fault);
+                if (lane == 0) s_tot = t2;
+            }
+            __syncthreads();
+            tot = s_tot;
+            __syncthreads();
+        } else if (mode == 2) {
+            double dA = block_sum_db(part, red, red_phase);
+            unsigned long long* base = ar_words + (size_t)buf * kTileMaxCtas * kArSlotWords;
+            if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
+            if (warp == 0) {
+                double v[8];
+                unsigned pend = 0;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { v[k] = 0.0; if (lane + 32 * k < G) pend |= 1u << k; }
+                unsigned long long spins = 0;
+                while (pend) {
+                    double t[8]; bool ok[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) ok[k] = xchg_try_if(pend >> k & 1u, base + (size_t)(lane + 32 * k) * kArSlotWords, tag, t[k]);
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) if (ok[k]) { v[k] = t[k]; pend &= ~(1u << k); }
+                    if (++spins > kXchgSpinLimit) { atomicExch(fault, 1); break; }
+                }
+                __syncwarp();
+                const double t2 = xchg_xor_tree(((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7])));
+                if (lane == 0) s_tot = t2;
+            }
+            __syncthreads();
+            tot = s_tot;
+            __syncthreads();
+        } else if (mode == 4) {
+            // the sweep kernel's scheme: the LAST warp is a communication warp; the others leave their warp partial in shared
+            // memory; the communication warp sums them, publishes the block sum, gathers all G block sums (<= 8 polls per
+            // lane, all in flight), and leaves the total in shared memory.  One CTA barrier on each side.
+            if (warp < nw - 1) {
+                const double wsum = xchg_xor_tree(part);
+                if (lane == 0) red[warp] = wsum;
+            }
+            __syncthreads();
+            if (warp == nw - 1) {
+                double mine = xchg_xor_tree(part);        // the communication warp has sites too in this probe
+                for (int w = 0; w < nw - 1; ++w) mine += red[w];
+                unsigned long long* base = ar_words + (size_t)buf * kTileMaxCtas * kArSlotWords;
+                if (lane == 0) ll_store_f64(base + (size_t)b * kArSlotWords, mine, tag);
+                const double t2 = xchg_gather_warp(base, kArSlotWords, G, b, mine, tag, fault);
+                if (lane == 0) s_tot = t2;
+            }
+            __syncthreads();
+            tot = s_tot;
+        } else if (mode == 5) {
+            // order-independent fixed-point accumulation in L2 (pimc_exchange.cuh): warp partials -> shared memory -> one thread
+            // adds the block sum to the accumulator words and polls them
+            const double wsum = xchg_xor_tree(part);
+            if (lane == 0) red[warp] = wsum;
+            __syncthreads();
+            if (tid == 0) {
+                double mine = 0.0;
+                for (int w = 0; w < nw; ++w) mine += red[w];
+                s_tot = xfix_allreduce(mbox, xst, G, b == 0, epoch, mine, fault);
+            }
+            __syncthreads();
+            tot = s_tot;
+        } else if (mode == 6) {
+            // software-pipelined all-gather: the packet of round r was published at the end of round r-1 (prologue: round 0),
+            // the poll is issued BEFORE this round's work (which stands for the two speculative evaluations of the next
+            // parameter, under "rejected" and "accepted") and checked after it; one fused block sum of three values
+            // (gathered partials, the two speculative partials); then the next packet goes out at once.
+            // (`work` iterations were run above = the first evaluation; the second runs below, after the poll has been issued.)
+            unsigned long long* base = ar_words + (size_t)buf * kTileMaxCtas * kArSlotWords;
+            if (r == 0) {
+                const double first = block_sum_db(xchg_selftest_part(0, b, tid), red, red_phase);
+                if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, first, tag);
+            }
+            // the poll goes out between the two speculative evaluations: the packets of this round (published before the first
+            // one) have arrived by now, and the second evaluation hides the load's round trip
+            if (r > 0 && tid < G) asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(pa), "=l"(pb) : "l"(base + (size_t)tid * kArSlotWords) : "memory");
+            for (int i = 0; i < iters; ++i) {
+                w0 = fma(w0, 0.999999, 1e-9); w1 = fma(w1, 0.999999, 1e-9); w2 = fma(w2, 0.999999, 1e-9); w3 = fma(w3, 0.999999, 1e-9);
+            }
+            double mine = 0.0;
+            const long long c0 = clock64();
+            if (tid < G) {
+                unsigned long long x = pa, y = pb, spins = 0;
+                while ((uint32_t)(x >> 32) != tag || (uint32_t)(y >> 32) != tag) {
+                    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(base + (size_t)tid * kArSlotWords) : "memory");
+                    if (++spins > kSpinLimit) { atomicExch(fault, 1); break; }
+                }
+                mine = __longlong_as_double((long long)((y << 32) | (x & 0xFFFFFFFFull)));
+            }
+            const long long c1 = clock64();
+            const double nextR = xchg_selftest_part(r + 1, b, tid), nextA = nextR + 1.0;     // the two speculative partials
+            // fused block sum of three values, one barrier
+            double v0 = mine, v1 = nextR, v2 = nextA;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                v0 += __shfl_xor_sync(0xFFFFFFFFu, v0, off); v1 += __shfl_xor_sync(0xFFFFFFFFu, v1, off); v2 += __shfl_xor_sync(0xFFFFFFFFu, v2, off);
+            }
+            double* bufr = red3 + (red_phase & 1u) * 24;
+            red_phase ^= 1u;
+            if (lane == 0) { bufr[warp] = v0; bufr[8 + warp] = v1; bufr[16 + warp] = v2; }
+            __syncthreads();
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+            for (int w = 0; w < nw; ++w) { t0 += bufr[w]; t1 += bufr[8 + w]; t2 += bufr[16 + w]; }
+            tot = t0;
+            const bool accept = (__double_as_longlong(t0) & 4ll) != 0;            // some decision that depends on the total
+            const double pub = accept ? t2 - 256.0 : t1;                            // = the true partial of round r+1 either way
+            // publish round r+1 and issue its poll before the next round's work
+            const uint32_t tag2 = tag + 1u;
+            unsigned long long* base2 = ar_words + (size_t)(buf ^ 1) * kTileMaxCtas * kArSlotWords;
+            if (tid == 0) ll_store_f64(base2 + (size_t)b * kArSlotWords, pub, tag2);
+            const long long c2 = clock64();
+            if (r >= warm && tid == (b * 37) % G) { ph[0] += c1 - c0; ph[1] += c2 - c1; }
+        } else if (mode == 10) {           // PUSH all-gather: every CTA writes its block sum into every CTA's private inbox, polls only its own
+            const double dA = block_sum_db(part, red, red_phase);
+            unsigned long long* inbox = inbox_words + (size_t)buf * kTileMaxCtas * kTileMaxCtas * 2;
+            if (tid < G) ll_store_f64(inbox + ((size_t)tid * kTileMaxCtas + (size_t)b) * 2, dA, tag);
+            double mine = 0.0;
+            if (tid < G) mine = ll_wait_f64(inbox + ((size_t)b * kTileMaxCtas + (size_t)tid) * 2, tag, fault);
+            tot = block_sum_db(mine, red, red_phase);
+        } else if (mode >= 100) {          // flat pull all-gather with the FIRST poll held back by (mode - 100) * 50 cycles
+            double dA = block_sum_db(part, red, red_phase);
+            unsigned long long* base = ar_words + (size_t)buf * kTileMaxCtas * kArSlotWords;
+            if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
+            const long long until = clock64() + (long long)(mode - 100) * 50;
+            double mine = 0.0;
+            if (tid < G) {
+                if (tid == b) mine = dA;
+                else {
+                    while (clock64() < until) {}
+                    mine = ll_wait_f64(base + (size_t)tid * kArSlotWords, tag, fault);
+                }
+            }
+            tot = block_sum_db(mine, red, red_phase);
+        } else if (mode == 7) {            // four dependent block sums, no exchange: the cost of block_sum_db itself
+            double v = part;
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) v = block_sum_db(v * 1e-3 + part, red, red_phase);
+            tot = v;
+        } else if (mode == 8) {            // four dependent warp-level xor trees only
+            double v = part;
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) v = xchg_xor_tree(v * 1e-3 + part);
+            tot = v;
+        } else if (mode == 9) {            // four barriers + shared-memory broadcast only
+            double v = part;
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) {
+                double* bufq = red + (red_phase & 1u) * 32; red_phase ^= 1u;
+                if (lane == 0) bufq[warp] = v;
+                __syncthreads();
+                double t = 0.0;
+                for (int w = 0; w < nw; ++w) t += bufq[w];
+                v = t * 1e-3 + part;
+            }
+            tot = v;
+        } else if (mode == 3) {
+            unsigned long long* base = ar_words + (size_t)buf * kTileMaxCtas * kArSlotWords;
+            if (tid == 0) {
+                ll_store_f64(base + (size_t)b * kArSlotWords, part, tag);
+                // a ring lets a CTA run up to G rounds ahead of its right neighbour: accept any tag >= the awaited one
+                const unsigned long long* p = base + (size_t)((b + G - 1) % G) * kArSlotWords;
+                unsigned long long x, y, spins = 0;
+                for (;;) {
+                    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(p) : "memory");
+                    if ((uint32_t)(x >> 32) >= tag && (uint32_t)(y >> 32) >= tag) break;
+                    if (++spins > kSpinLimit) { atomicExch(fault, 1); break; }
+                }
+                s_tot = part;
+            }
+            __syncthreads();
+            tot = s_tot;
+            __syncthreads();
+        } else tot = part;
+        epoch += 1ull;
+    }
+    if (tid == 0) {
+        out_tot[b] = tot;
+        if (b == 0) out_cycles[0] = clock64() - t_start;
+    }
+    if ((mode == 0 || mode == 6) && tid == (b * 37) % (mode == 0 ? 148 : G)) { atomicAdd((unsigned long long*)out_cycles + 1, (unsigned long long)ph[0]); atomicAdd((unsigned long long*)out_cycles + 2, (unsigned long long)ph[1]); atomicAdd((unsigned long long*)out_cycles + 3, (unsigned long long)ph[2]); }
+    if (w0 + w1 + w2 + w3 == 1234.5) sink[0] = w0;     // never true; keeps the work loop alive
 }
 
 }  // namespace pimc

@@ -32,11 +32,14 @@ def test_elementary_functions_within_a_few_ulp():
     big = np.abs(np.sin(a)) > 0.1
     assert ulps(out[big, 3], np.sin(a[big])).max() <= 4.0
     assert ulps(out[:, 5], 1.0 / ax).max() <= 2.0
-    # the one-exponential form of the HH gate rate against the tanh definition in long double
-    V = x[np.abs(x) < 200].astype(np.longdouble)
-    th = np.tanh((V + 40) / 15)
-    ref = ((0.5 + 0.5 * th) - np.longdouble(0.3)) / (np.longdouble(0.1) + np.longdouble(0.4) * (1 - th * th))
-    got = out[np.abs(x) < 200, 6]
-    ref = ref.astype(np.float64)
-    # the rate is O(1/tau) <= 10; where a_inf ~ a it cancels, so the bound is absolute + relative
-    assert np.all(np.abs(got - ref) <= 1e-14 + 4e-15 * np.abs(ref)), np.max(np.abs(got - ref))
+    # the shared-exponential form of the three HH gate rates against the tanh definition (Table 1 shifted by
+    # -65 mV) in long double, over the whole finite range (saturation included)
+    sel = np.abs(x) < 700
+    V = x[sel].astype(np.longdouble)
+    for col, (Va, dVa, tau0, tau1) in enumerate(((-40, 15, 0.1, 0.4), (-60, -15, 1.0, 7.0), (-55, 30, 1.0, 5.0))):
+        th = np.tanh((V - Va) / np.longdouble(dVa))
+        ref = ((0.5 + 0.5 * th) - np.longdouble(0.3)) / (np.longdouble(tau0) + np.longdouble(tau1) * (1 - th * th))
+        got = out[sel, 6 + col]
+        ref = ref.astype(np.float64)
+        # the rate is O(1/tau) <= 10; where a_inf ~ a it cancels, so the bound is absolute + relative
+        assert np.all(np.abs(got - ref) <= 1e-14 + 6e-15 * np.abs(ref)), (col, np.max(np.abs(got - ref)))

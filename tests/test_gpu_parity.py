@@ -2,6 +2,8 @@
 binding), against the CPU oracle on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
 per-site Delta-A to 1e-12 (fp64) relative to max(|dA|, S), identical decisions
 except inside the near-tie window |dA + log u| < 1e-9, integer work bit-exact."""
+import os
+
 import numpy as np
 import pytest
 
@@ -51,11 +53,33 @@ def test_philox_words_and_uniforms_bit_exact(P):
     assert abs(z.mean()) < 5 / np.sqrt(z.size) and abs(z.var() - 1) < 5 * np.sqrt(2 / z.size)
 
 
-def test_philox_vs_curand_device_black_box(P):
-    """cuRAND's own Philox4_32_10 on the device, as a black box, via torch's generator is not exposed; instead the
-    device words are compared with the oracle (above), and the oracle with cuRAND's host path (CPU suite)."""
-    # kept as documentation of the chain of trust: device == oracle (bit exact) and oracle == cuRAND host (bit exact)
-    assert True
+def test_philox_vs_curand_device_black_box(P, tmp_path):
+    """libpimc's device Philox words against cuRAND's own curand_Philox4x32_10 running on the same GPU (a library routine as a
+    black box: tests/curand_philox_device.cu, compiled here with nvcc)."""
+    import ctypes as C
+    import shutil
+    import subprocess
+    import torch
+    if shutil.which("nvcc") is None:
+        pytest.skip("nvcc is not on PATH on this box")
+    so = str(tmp_path / "libcurand_philox_device.so")
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "--shared", "-Xcompiler", "-fPIC", "-o", so,
+                    os.path.join(os.path.dirname(os.path.abspath(__file__)), "curand_philox_device.cu")], check=True)
+    L = C.CDLL(so)
+    L.curand_philox_device.restype = C.c_int
+    L.curand_philox_device.argtypes = [C.c_uint64, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
+    rng = np.random.default_rng(11)
+    n = 100_003
+    ctrs = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    ctrs[:3] = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [0x243F6A88, 0x85A308D3, 0x13198A2E, 0x03707344]]
+    key = (0xA4093822, 0x299F31D0)
+    d_ctrs = torch.from_numpy(ctrs.view(np.int32)).cuda()
+    ours = P.rng_selftest(d_ctrs, key)["words"]
+    theirs = torch.empty_like(ours)
+    torch.cuda.synchronize()
+    assert L.curand_philox_device(n, d_ctrs.data_ptr(), key[0], key[1], theirs.data_ptr()) == 0
+    assert torch.equal(ours, theirs)
+    assert [hex(v) for v in theirs[2].cpu().numpy().view(np.uint32)] == ["0xd16cfe09", "0x94fdcceb", "0x5001e420", "0x24126ea1"]
 
 
 # ------------------------------------------------------------------------------------------------------------

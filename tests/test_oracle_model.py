@@ -28,6 +28,29 @@ def test_gate_kinetics_special_values():
     assert np.allclose(F[1:], [(0 - 0.25) / 0.1, (1 - 0.25) / 1.0, (0 - 0.25) / 1.0], rtol=1e-14)
 
 
+def test_gate_kinetics_width_constants_from_table_1():
+    # The special values above (tanh = 0 or +-1) do not see the MAGNITUDE of Delta-V_a.  One width away from the midpoint,
+    # V = V_a + Delta-V_a, Eq. 13-14 give a_inf = (1 + tanh 1)/2 and tau = tau0 + tau1 (1 - tanh^2 1);
+    # half a width away, tanh(1/2).  The numbers below are typed from Table 1 (n: 10, 30, 1.0, 5.0;
+    # m: 25, 15, 0.1, 0.4; h: 5, -15, 1.0, 7.0) with V_a shifted by -65 mV (reading Delta-3), not read from the oracle.
+    table1 = {1: (25.0 - 65.0, 15.0, 0.1, 0.4), 2: (5.0 - 65.0, -15.0, 1.0, 7.0), 3: (10.0 - 65.0, 30.0, 1.0, 5.0)}   # state order (V, m, h, n)
+    for comp, (Va, dVa, tau0, tau1) in table1.items():
+        for k in (1.0, 0.5, -1.0, 2.0):
+            th = np.tanh(k)
+            a_inf, tau = 0.5 + 0.5 * th, tau0 + tau1 * (1.0 - th * th)
+            for a in (0.0, 0.35, 1.0):
+                x = np.array([Va + k * dVa, 0.2, 0.2, 0.2]); x[comp] = a
+                F = oracle.rhs(MODEL_HH, x, P, 0.0)
+                assert np.isclose(F[comp], (a_inf - a) / tau, rtol=2e-14, atol=1e-16), (comp, k, a)
+    # the three widths are different numbers: swapping any two of them must fail the loop above (guards the test itself)
+    swapped = {1: table1[1][:1] + (30.0,) + table1[1][2:], 3: table1[3][:1] + (15.0,) + table1[3][2:]}
+    for comp, (Va, dVa, tau0, tau1) in swapped.items():
+        th = np.tanh(1.0)
+        x = np.array([Va + dVa, 0.2, 0.2, 0.2]); x[comp] = 0.35
+        F = oracle.rhs(MODEL_HH, x, P, 0.0)
+        assert not np.isclose(F[comp], (0.5 + 0.5 * th - 0.35) / (tau0 + tau1 * (1 - th * th)), rtol=1e-3)
+
+
 def test_voltage_equation_terms():
     # Eq. 11 in the (gNa,gK,gL,ENa,EK,EL,C) parametrisation: isolate each current.
     gNa, gK, gL, ENa, EK, EL, Cm = 100.0, 30.0, 0.5, 40.0, -80.0, -50.0, 2.0
