@@ -27,14 +27,27 @@ from workloads import make_workload  # noqa: E402
 METRIC = "Metropolis site-updates/sec and sweeps/sec (HH, M=32768, fp64) vs FP64 roofline"
 UNIT = "site-updates/s"
 
-# Algorithmic work per unit, fixed once (SURVEY.md §8(d) "Algorithmic work"): FP64 pipe slots
-# (1 slot = one FMA/ADD/MUL lane-operation = 2 FLOP at peak) per joint site-update and per parameter-move model evaluation.
-W_SITE_SLOTS = 800.0
-W_EVAL_SLOTS = 560.0
-# trapezoid discretisation (--disc trapezoid, the paper's own rule): one right-hand side per proposal instead of four
-# (108 + Delta-A 97 + RNG 175), one per parameter-move evaluation (108 + 32)
+# ---- work model (one slot = one FP64-pipe lane operation = 2 FLOP at peak) -----------------------------
+# (1) ORACLE-COUNTED algorithmic work: what a straightforward evaluation of the paper's formulas needs per joint site update and
+#     per parameter-move model evaluation.  Written by `python -m oracle.count_work` (an instrumented restatement of the oracle's
+#     arithmetic, validated bit for bit against it; libm calls costed by a stated table) into oracle/work_constants.json;
+#     tests/test_work_model.py keeps these literals equal to that file.
+W_SITE_ORACLE = 869.0
+W_EVAL_ORACLE = 666.0
+# (2) EXECUTED FP64-pipe thread instructions of the production kernels per OWNED unit, counted by ncu (source page, DFMA + DMUL +
+#     DADD + DSETP, predicated-on threads; profiles/r02_work_counts.md).  They include the redundant halo updates and the
+#     producers' random-number arithmetic, so executed x rate / peak is the lane-level FP64 pipe utilisation: it cannot
+#     flatter.  The kernels execute FEWER operations than (1) (one shared exponential per RK4 stage instead of three tanh, one
+#     reciprocal series instead of two divides per gate, cached first-stage gate rates in parameter moves), so the useful
+#     fraction credits min((1), (2) / redundancy).
+EXEC_FP64 = {   # (model family, dtype, discretisation) -> (per owned site update, per owned parameter-move evaluation)
+    ("hh", 64, "rk4"): (596.5, 304.6),
+}
+HALO_REDUNDANCY_CFG3 = 254.0 / 222.0            # computed / owned sites per tile at the cfg3 launch (h = 16 halo sites each side)
+# ncu sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed of the same kernels, same launches (profiles/r02_*.md)
+NCU_PIPE_FP64_ACTIVE = {"full_sweep": 0.300, "a2_only": 0.437, "a4_only": 0.265, "source": "profiles/r02_work_counts.md"}
+# trapezoid discretisation / component-wise updates: estimated slots (no oracle count yet), used for the non-headline variants only
 W_SITE_SLOTS_TRAP = 380.0
-# component-wise updates (--update componentwise): D = 4 model evaluations and decisions per site visit (4 x (433 + 67) + RNG 300)
 W_SITE_SLOTS_COMP = 2300.0
 W_EVAL_SLOTS_TRAP = 140.0
 # FP64 peak derived from unit counts and clocks: 148 SMs x 64 FP64 lanes/clk/SM x 1.965 GHz, 2 FLOP per lane-FMA.
@@ -42,7 +55,7 @@ FP64_LANES_PER_SM_CLK = 64
 SM_COUNT = 148
 SM_MAX_HZ = 1.965e9
 PEAK_TFLOPS_DERIVED = SM_COUNT * FP64_LANES_PER_SM_CLK * SM_MAX_HZ * 2 / 1e12
-NCU_DRAM_BYTES_PER_LAUNCH = 5939456.0   # cfg3 full sweep launch: 5.917 MB read + 22 KB written (profiles/r01_v8_final.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 5999616.0   # cfg3 full sweep launch: 5.930 MB read + 70 KB written (profiles/r02_work_counts.md)
 
 
 def rank_info():
@@ -105,6 +118,63 @@ def oracle_rate(w, budget_s, chain=0, disc=0, mode=0):
     o.sweep(n, seed=w.chain_seed)
     dt = time.perf_counter() - t0
     return (w.M + 1) * n / dt, n, dt
+
+
+def oracle_rate_all_cores(w, budget_s, per_sweep_s):
+    """The oracle on every host core at once, one independent chain per core ("an all-cores rate with one
+    independent chain per core").  ctypes releases the GIL inside orc_sweep, so plain threads run in parallel."""
+    from oracle import OracleChain
+    cores = os.cpu_count() or 1
+    chains = [OracleChain.from_workload(w, chain=0) for _ in range(cores)]
+    n = max(1, int(budget_s / max(per_sweep_s, 1e-6)))
+    ths = [threading.Thread(target=lambda o=o, k=k: o.sweep(n, seed=w.chain_seed + 1000 + k)) for k, o in enumerate(chains)]
+    t0 = time.perf_counter()
+    for t in ths:
+        t.start()
+    for t in ths:
+        t.join()
+    dt = time.perf_counter() - t0
+    return (w.M + 1) * n * cores / dt, cores, n, dt
+
+
+OTHER_CONFIGS = [   # (config, dtype, sweeps per step): every BASELINE.json config besides the headline one, and its fp32 variant
+    (0, 64, 2000), (1, 64, 1000), (2, 64, 1000), (4, 64, 20), (3, 32, 1000),
+]
+
+
+def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=None):
+    """One extra line of the "other_configs" block: the same timed protocol as the headline (3 warm-up steps, L2 flushed before
+    every step, CUDA events on the launching stream), full sweeps with accumulation every sweep, oracle on one core beside it."""
+    w = w or make_workload(cfg)
+    h = P.Pimc.from_workload(w, dtype=dtype)
+    h.set_accum(True, 1)
+    h.reset_moments()
+    stream = torch.cuda.current_stream()
+    seed = w.chain_seed
+
+    def one():
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream); h.sweep(S, seed); e1.record(stream)
+        return e0, e1
+    for _ in range(3):
+        one()
+    torch.cuda.synchronize()
+    n0 = h.launch_count
+    evs = [one() for _ in range(steps)]
+    torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+    fault = h.fault()
+    units = float(w.n_chains) * (w.M + 1) * S
+    out = {"workload": w.name, "dtype": "f64" if dtype == 64 else "f32", "value": units / (ms * 1e-3), "unit": UNIT,
+           "chain_sweeps_per_s": w.n_chains * S / (ms * 1e-3), "ms_per_step": ms, "sweeps_per_step": S, "steps": steps,
+           "params_moved": int(np.count_nonzero(w.w_param)), "engine": {1: "GLOBAL", 2: "TILE"}[h.get_engine()["engine"]],
+           "launch": h.get_launch(), "gpu_launches": int(h.launch_count - n0), "fault": int(fault)}
+    if cpu_budget > 0 and dtype == 64:
+        r, n, dt = oracle_rate(w, cpu_budget)
+        out["oracle_1core"] = {"value": r, "unit": UNIT, "sample": f"{n} full sweeps of chain 0 in {dt:.1f} s"}
+    del h
+    return out
 
 
 def run_reference(args):
@@ -173,11 +243,13 @@ def run_ours(args):
     trap = args.disc == "trapezoid"
     if trap:
         h.set_discretisation(P.DISC_TRAPEZOID)
-    w_site, w_eval = (W_SITE_SLOTS_TRAP, W_EVAL_SLOTS_TRAP) if trap else (W_SITE_SLOTS, W_EVAL_SLOTS)
+    w_site, w_eval = (W_SITE_SLOTS_TRAP, W_EVAL_SLOTS_TRAP) if trap else (W_SITE_ORACLE, W_EVAL_ORACLE)
     comp = args.update == "componentwise"
     if comp:
         h.set_update_mode(P.UPDATE_COMPONENTWISE)
         w_site = W_SITE_SLOTS_COMP if not trap else 4 * 205.0 + 300.0
+    headline = args.config == 3 and args.kinetics == "tanh" and not trap and not comp
+    exec_counts = EXEC_FP64.get(("hh", args.dtype, args.disc)) if headline else None
     peak_tflops = PEAK_TFLOPS_DERIVED * (1.0 if args.dtype == 64 else 2.0)   # fp32: 128 FP32 lanes/clk/SM
     if args.exchange_hold is not None:
         h.set_exchange(args.exchange_hold)
@@ -220,51 +292,95 @@ def run_ours(args):
     value = tot_units / tot_s
     ms_per_step = tot_s / args.steps * 1e3
 
-    # rows A2 and A4 on their own (same launch shape, same data), for the breakdown the north_star asks for
+    # rows A2 and A4 on their own (same launch shape, same data), for the breakdown the north_star asks for; same statistic
+    # (mean over the timed launches) as the headline
     def rate(fn, units, reps=3):
         fn(max(1, S // 10), seed); torch.cuda.synchronize()
         ms = []
         for _ in range(reps):
             a, b = one_step(fn); torch.cuda.synchronize(); ms.append(a.elapsed_time(b))
-        return units / (min(ms) * 1e-3), min(ms)
+        return units / (float(np.mean(ms)) * 1e-3), float(np.mean(ms))
     a2_rate, a2_ms = rate(h.sweep_states_only, units_per_step)
     a4_rate, a4_ms = (rate(h.sweep_params_only, evals_per_step) if n_active else (0.0, 0.0))
 
-    # roofline of the dominant (only) kernel of the step: the persistent sweep kernel
-    slots_per_launch = units_per_step * w_site + evals_per_step * w_eval
-    achieved_tflops = 2.0 * slots_per_launch / (float(np.mean(step_ms)) * 1e-3) / 1e12
+    # roofline of the dominant (only) kernel of the step: the persistent sweep kernel.
+    #   frac              = EXECUTED FP64 lane operations (ncu-counted per owned unit, redundant halo work included) / time / peak:
+    #                       the lane-level FP64 pipe utilisation; ~ ncu's sm__pipe_fp64_cycles_active (warp level) x active lanes
+    #   frac_owned        = the same without the redundant halo updates (/ computed-per-owned sites)
+    #   frac_oracle_work  = oracle-counted algorithmic work / time / peak (a plain evaluation of the paper's formulas would need
+    #                       this many operations; the kernels need fewer, so this one may exceed the pipe utilisation)
+    step_s = float(np.mean(step_ms)) * 1e-3
+    tfl = lambda slots, seconds: 2.0 * slots / seconds / 1e12
+    oracle_tflops = tfl(units_per_step * w_site + evals_per_step * w_eval, step_s)
+    if exec_counts:
+        achieved_tflops = tfl(units_per_step * exec_counts[0] + evals_per_step * exec_counts[1], step_s)
+        red = HALO_REDUNDANCY_CFG3
+        a2_frac, a4_frac = tfl(a2_rate * exec_counts[0], 1.0) / peak_tflops, tfl(a4_rate * exec_counts[1], 1.0) / peak_tflops
+        useful_site, useful_eval = min(w_site, exec_counts[0] / red), min(w_eval, exec_counts[1] / red)
+        frac_useful = tfl(units_per_step * useful_site + evals_per_step * useful_eval, step_s) / peak_tflops
+    else:           # variants without an ncu count: the (estimated or oracle-counted) work model only
+        achieved_tflops, red = oracle_tflops, None
+        a2_frac, a4_frac = tfl(a2_rate * w_site, 1.0) / peak_tflops, tfl(a4_rate * w_eval, 1.0) / peak_tflops
+        frac_useful = None
     measured_peak = P.fp64_peak(150) * 2 / 1e12 if rank == 0 else None
+    tile = bool(shape.get("smem_bytes", 0))
+    model_name = {0: "LinearModel", 1: "HHModelK<0>", 2: "HHModelK<1>"}[w.model]
+    rtype = "double" if args.dtype == 64 else "float"
+    kernel = (f"pimc::tile_sweep_kernel<{model_name},{rtype},MAXT={256 if shape['threads_per_cta'] <= 256 else 512},TRAP={int(trap)},COMP={int(comp)},KG={int(n_active > 0 and not trap)},TR=0>"
+              if tile else f"pimc::sweep_kernel<{model_name},{rtype}>")
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved_tflops / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == 3 and args.dtype == 64 and not trap) else None,
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r01_v8_final.md (tile loaded once, written back once: independent of the sweeps per launch)",
+                "frac": achieved_tflops / peak_tflops,
+                "frac_definition": ("executed FP64 lane operations (ncu-counted per owned unit, redundant halo updates and RNG included) x units / CUDA-event time / peak"
+                                    if exec_counts else "work-model slots x units / CUDA-event time / peak (no ncu count for this variant)"),
+                "frac_owned": (achieved_tflops / peak_tflops / red) if red else None,
+                "frac_useful": frac_useful,
+                "frac_oracle_work": oracle_tflops / peak_tflops,
+                "halo_redundancy": red,
+                "pipe_fp64_active_ncu": NCU_PIPE_FP64_ACTIVE if exec_counts else None,
+                "target": "north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2), judged on pipe_fp64_active_ncu.a2_only: NOT reached",
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (headline and args.dtype == 64) else None,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r02_work_counts.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
                 "peak_measured_dfma_tflops": measured_peak,
                 "frac_of_measured_dfma": (achieved_tflops / measured_peak) if measured_peak else None,
-                "kernel": "pimc::tile_sweep_kernel<HHModel<double>,double,256>" if shape.get("smem_bytes", 0) else "pimc::sweep_kernel<HHModel<double>,double>",
-                "work_model": {"slots_per_site_update": w_site, "slots_per_param_eval": w_eval,
+                "kernel": kernel,
+                "work_model": {"oracle_slots_per_site_update": w_site, "oracle_slots_per_param_eval": w_eval,
+                               "executed_fp64_per_owned_site_update": exec_counts[0] if exec_counts else None,
+                               "executed_fp64_per_owned_param_eval": exec_counts[1] if exec_counts else None,
                                "site_updates_per_launch": units_per_step, "param_evals_per_launch": evals_per_step},
-                "a2_only": {"site_updates_per_s": a2_rate, "ms_per_launch": a2_ms,
-                            "frac": 2 * a2_rate * w_site / 1e12 / peak_tflops},
-                "a4_only": {"param_evals_per_s": a4_rate, "ms_per_launch": a4_ms,
-                            "frac": 2 * a4_rate * w_eval / 1e12 / peak_tflops}}
+                "a2_only": {"site_updates_per_s": a2_rate, "ms_per_launch": a2_ms, "frac": a2_frac,
+                            "frac_oracle_work": tfl(a2_rate * w_site, 1.0) / peak_tflops},
+                "a4_only": {"param_evals_per_s": a4_rate, "ms_per_launch": a4_ms, "frac": a4_frac,
+                            "frac_oracle_work": tfl(a4_rate * w_eval, 1.0) / peak_tflops}}
 
     # end to end through the C ABI on HOST buffers: H2D of y, I, x0, p0 + sweeps + D2H of the moments inside the timed region
     e2e = None
     if (rank == 0 or world > 1) and not trap and not comp:     # pimc_run_host is the RK4-map, joint-update convenience call
-        P.run_host(w, 0, max(1, S // 10), seed, dtype=args.dtype)         # warm-up (context, allocator)
+        scratch = P.run_host_scratch(w, dtype=args.dtype)                   # device scratch owned by the caller: no cudaMalloc in the timed calls
+        P.run_host(w, 0, max(1, S // 10), seed, dtype=args.dtype, scratch=scratch)         # warm-up
         reps = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
         for _ in range(reps):
-            out = P.run_host(w, 0, S, seed, dtype=args.dtype)
+            out = P.run_host(w, 0, S, seed, dtype=args.dtype, scratch=scratch)
         dt_e2e = time.perf_counter() - t0
         s_e2e, u_e2e = reduce_over_ranks(dt_e2e, units_per_step * reps, world, dist)
         e2e = {"value": u_e2e / s_e2e, "unit": UNIT, "h2d_bytes_per_step": out["h2d_bytes"], "d2h_bytes_per_step": out["d2h_bytes"],
-               "ms_per_step": s_e2e / reps * 1e3, "call": "pimc_run_host (cudaMalloc + H2D + pimc_sweep + pimc_moments + D2H + sync)"}
+               "ms_per_step": s_e2e / reps * 1e3, "call": "pimc_run_host_ws on HOST buffers (H2D of y, I, x0, p0 + pimc_init + cache build + pimc_sweep + pimc_moments + D2H + fault check + sync; device scratch provided by the caller)"}
 
     if rank == 0:
         cpu_rate, cpu_n, cpu_s = oracle_rate(w, args.cpu_budget, disc=1 if trap else 0, mode=1 if comp else 0)
         cpu = {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{cpu_n} full sweeps of chain 0 of {w.name} in {cpu_s:.1f} s (serial fp64 C++ -O2, {os.cpu_count()} cores present)"}
+        other = None
+        if headline and args.dtype == 64 and world == 1 and not args.no_other_configs:
+            # the rest of BASELINE.json's workloads (north_star: "Report throughput on the synthetic workloads below at 1 GPU"),
+            # after the timed region of the headline; and the oracle on all host cores (one independent chain per core)
+            other = []
+            for cfg, dt_, S_ in OTHER_CONFIGS:
+                other.append(measure_other_config(P, torch, flush, cfg, dt_, S_, 3, min(args.cpu_budget, 2.0), w=w if cfg == 3 else None))
+            ar, cores, an, adt = oracle_rate_all_cores(w, min(args.cpu_budget, 8.0), cpu_s / max(cpu_n, 1))
+            cpu["all_cores"] = {"value": ar, "unit": UNIT, "cores": cores,
+                                "sample": f"{cores} independent chains of {w.name}, one per core (threads), {an} full sweeps each in {adt:.1f} s"}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.dtype == 64 else "f32",
@@ -274,7 +390,7 @@ def run_ours(args):
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "sweeps_per_s": value / (w.M + 1),
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "other_configs": other,
             "wall_s_timed_region": t_wall, "speedup_vs_oracle_1core": value / cpu_rate,
         }
         print(json.dumps(line))
@@ -290,10 +406,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--kinetics", default="tanh", choices=["tanh", "classic"], help="HH gate kinetics: the paper's tanh forms (default) or the classic alpha/beta rate functions (model 2)")
-    ap.add_argument("--update", default="joint", choices=["joint", "componentwise"], help="site update: joint D-vector proposal (default) or one component at a time (GLOBAL engine)")
+    ap.add_argument("--update", default="joint", choices=["joint", "componentwise"], help="site update: joint D-vector proposal (default) or one component at a time (both engines)")
     ap.add_argument("--disc", default="rk4", choices=["rk4", "trapezoid"], help="model-error discretisation: the north_star's RK4 map or the paper's trapezoid rule")
     ap.add_argument("--dtype", type=int, default=64, choices=[64, 32], help="arithmetic type of the path (config 3 is also quoted in fp32)")
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the other_configs block (cfg0, 1, 2, 4 and cfg3-fp32 after the headline)")
     ap.add_argument("--exchange-hold", type=int, default=None, help="SM clock ticks between publishing a Delta-A partial and the first poll (pimc_set_exchange; default: the library's)")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=120.0, help="seconds of oracle time for --impl reference")

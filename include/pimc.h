@@ -18,15 +18,17 @@
  * (seed; site-or-parameter, sweep, chain, stream) so results do not depend on the launch shape.
  *
  * Conventions
- *  - Every function returns PIMC_OK or a negative error; the first error message is kept and can be
+ *  - Every function returns PIMC_OK or a negative error; the message of the latest failure can be
  *    read with pimc_last_error().  No C++ exception crosses this boundary.
+ *  - Caller-provided device arrays (x, y, I, p, outputs, trace buffers) must be 32-byte aligned: PIMC_EINVAL otherwise.
  *  - "dev" pointers are CUDA device pointers owned by the caller; "host" pointers are ordinary host
  *    memory.  The library copies what it needs into the caller-provided workspace during the call
  *    (asynchronously on `stream`), so inputs may be freed once the stream has passed the call.
  *  - Arrays are row-major and contiguous.  Element type of x, y, I, p, trace arrays = `dtype`
  *    (64: double, 32: float).  Moments are always double, counters unsigned 64-bit.
- *  - All work is enqueued on the `stream` given to pimc_init (a cudaStream_t cast to void*; NULL =
- *    the legacy default stream).  Nothing synchronises the host except where stated.
+ *  - All work is enqueued on the ONE `stream` given to pimc_init (a cudaStream_t cast to void*; NULL =
+ *    the legacy default stream), for the lifetime of the handle.  Arrays produced or consumed on another stream must be
+ *    ordered against it by the caller (event or synchronize).  Nothing synchronises the host except where stated.
  *  - There is no CPU fallback: without a CUDA device every compute call returns PIMC_ECUDA.
  */
 #ifndef PIMC_H
@@ -152,7 +154,8 @@ int pimc_reset_moments(pimc_handle* h);
 int pimc_sweep(pimc_handle* h, long long n_sweeps, unsigned long long seed);
 
 /* Only the state half-sweeps (rows A2/A3) or only the parameter moves (PAPER.md:199,
- * 209; row A4) of pimc_sweep -- for measuring the two separately.  Same RNG counters as pimc_sweep. */
+ * 209; row A4) of pimc_sweep -- for measuring the two separately.  Same RNG counters as pimc_sweep.  PIMC_ESTATE while
+ * step-size tuning is on (the rule needs the acceptance of PROPOSED moves of both classes). */
 int pimc_sweep_states_only(pimc_handle* h, long long n_sweeps, unsigned long long seed);
 int pimc_sweep_params_only(pimc_handle* h, long long n_sweeps, unsigned long long seed);
 
@@ -202,6 +205,8 @@ int pimc_set_exchange(pimc_handle* h, int first_poll_hold_cycles);
  * the chain state is then undefined).  A diagnostic: hand-offs cannot be lost in a co-resident (cooperative) launch. */
 int pimc_fault(pimc_handle* h, int* fault_host);
 
+/* The absolute sweep index (part of every RNG counter).  Setting it below the sweep at which accumulation, step-size tuning or
+ * annealing was switched on is refused (PIMC_ESTATE): their schedules count sweeps from those origins. */
 unsigned long long pimc_sweep_index(const pimc_handle* h);
 int pimc_set_sweep_index(pimc_handle* h, unsigned long long t);
 
@@ -216,6 +221,16 @@ int pimc_run_host(int model, int D, int L, int M, double dt, double Rm, const do
                   const void* y, const void* I, const void* x0, const void* p0, const double* w_state,
                   const double* w_param, const double* lo, const double* hi, int proposal_kind, long long n_burn,
                   long long n_sweeps, unsigned long long seed, double* moments_out, void* x_out, void* p_out);
+
+/* The same with a caller-provided device scratch buffer (256-byte aligned, at least pimc_run_host_workspace_bytes(); NULL =
+ * allocate as pimc_run_host does), so that repeated calls do not pay cudaMalloc / cudaFree.  Both calls end with the check of
+ * pimc_fault: a lost inter-CTA hand-off returns PIMC_ECUDA instead of a result. */
+size_t pimc_run_host_workspace_bytes(int model, int D, int L, int M, int n_chains, int dtype);
+int pimc_run_host_ws(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype,
+                     const void* y, const void* I, const void* x0, const void* p0, const double* w_state,
+                     const double* w_param, const double* lo, const double* hi, int proposal_kind, long long n_burn,
+                     long long n_sweeps, unsigned long long seed, double* moments_out, void* x_out, void* p_out,
+                     void* dev_scratch, size_t dev_scratch_bytes);
 
 /* RNG self-test entry (rows A1 / pin P4): fills out (dev u32, n*4) with Philox4x32-10(ctr[i], key), ctrs
  * dev u32 (n,4); and the library's transforms: u_prop dev double n*4 = (w+0.5)2^-32 per word, u_acc dev

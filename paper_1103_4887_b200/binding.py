@@ -57,6 +57,9 @@ _SIGNATURES = {
     "pimc_launch_count": (C.c_ulonglong, [_vp]),
     "pimc_run_host": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _vp, _vp, _vp,
                                 _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp]),
+    "pimc_run_host_workspace_bytes": (C.c_size_t, [C.c_int] * 6),
+    "pimc_run_host_ws": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _vp, _vp, _vp,
+                                   _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp, _vp, C.c_size_t]),
     "pimc_rng_selftest": (C.c_int, [_vp, C.c_ulonglong, C.c_uint, C.c_uint, _vp, _vp, _vp, _vp, _vp]),
     "pimc_step_selftest": (C.c_int, [C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp, C.c_double, C.c_ulonglong, _vp, _vp]),
     "pimc_math_selftest": (C.c_int, [_vp, C.c_ulonglong, _vp, _vp]),
@@ -116,7 +119,12 @@ def _ptr(t):
 
 
 class Pimc:
-    """One handle = n_chains independent Markov chains of the same shape, resident on the current CUDA device."""
+    """One handle = n_chains independent Markov chains of the same shape, resident on the current CUDA device.
+
+    Stream contract: the handle is bound for life to ONE stream -- `stream` if given, else the torch stream that is current
+    when the handle is created (include/pimc.h "Conventions").  Every call of this class enqueues on that stream, whatever
+    torch stream is current at the time; tensors produced or consumed under another stream must be ordered against it by the
+    caller (`handle.stream.wait_stream(other)` / `other.wait_stream(handle.stream)`)."""
 
     def __init__(self, model, D, L, M, dt, Rm, Rf, p0, n_chains=1, dtype=64, stream=None):
         import torch
@@ -141,6 +149,11 @@ class Pimc:
                                C.c_void_p(self._ws.data_ptr() + off), nbytes, C.c_void_p(self._stream.cuda_stream)))
         self._h = h
         self._keep = {}
+
+    @property
+    def stream(self):
+        """The torch stream all of this handle's work is enqueued on."""
+        return self._stream
 
     @classmethod
     def from_workload(cls, w, dtype=64, with_params=True, device_arrays=None):
@@ -230,8 +243,12 @@ class Pimc:
         return f.value
 
     # ---- the hot path ----
-    def sweep(self, n_sweeps, seed):
+    def sweep(self, n_sweeps, seed, check_fault=False):
+        """n_sweeps full sweeps (asynchronous on the handle's stream).  check_fault=True synchronises the stream afterwards and
+        raises PimcError if an inter-CTA hand-off was lost (pimc_fault): use it where a hung or torn launch must not pass."""
         _check(lib().pimc_sweep(self._h, int(n_sweeps), int(seed)), self._h)
+        if check_fault:
+            self.fault()
 
     def sweep_states_only(self, n_sweeps, seed):
         _check(lib().pimc_sweep_states_only(self._h, int(n_sweeps), int(seed)), self._h)
@@ -253,7 +270,7 @@ class Pimc:
         return g
 
     def set_tuning(self, enabled, n_skip=1, f_acc=0.23, alpha=0.02):
-        """Step-size auto-tuning from the current sweep on (GLOBAL engine); enabled=False freezes the step sizes."""
+        """Step-size auto-tuning from the current sweep on (both engines); enabled=False freezes the step sizes."""
         _check(lib().pimc_set_tuning(self._h, int(bool(enabled)), int(n_skip), float(f_acc), float(alpha)), self._h)
 
     def get_widths(self):
@@ -268,13 +285,13 @@ class Pimc:
         _check(lib().pimc_set_annealing(self._h, float(beta0), int(n_cool)), self._h)
 
     def set_update_mode(self, mode):
-        """UPDATE_JOINT (default) or UPDATE_COMPONENTWISE (D decisions per site; GLOBAL engine).  Re-enable the trace afterwards:
+        """UPDATE_JOINT (default) or UPDATE_COMPONENTWISE (D decisions per site; both engines).  Re-enable the trace afterwards:
         its dA / acc buffers are per (site, component) in component-wise mode."""
         _check(lib().pimc_set_update_mode(self._h, int(mode)), self._h)
         self.update_mode = int(mode)
 
     def set_discretisation(self, disc):
-        """DISC_RK4MAP (default) or DISC_TRAPEZOID (the paper's rule, Eq. 7; GLOBAL engine)."""
+        """DISC_RK4MAP (default) or DISC_TRAPEZOID (the paper's rule, Eq. 7; both engines)."""
         _check(lib().pimc_set_discretisation(self._h, int(disc)), self._h)
         self.disc = int(disc)
 
@@ -385,8 +402,16 @@ def exchange_selftest(mode, n_ctas=0, threads=256, rounds=2000, work=0):
     return dict(cycles_per_round=cyc.value, max_abs_err=err.value, n_distinct=nd.value)
 
 
-def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_path=False):
-    """End-to-end call on HOST numpy buffers (pimc_run_host): H2D, sweeps, moments, D2H inside the call."""
+def run_host_scratch(w, dtype=64):
+    """A device scratch tensor for run_host(..., scratch=...) (pimc_run_host_workspace_bytes), so repeated calls skip cudaMalloc."""
+    import torch
+    n = lib().pimc_run_host_workspace_bytes(w.model, w.D, w.L, w.M, w.n_chains, dtype)
+    t = torch.empty(n + 256, dtype=torch.uint8, device="cuda")
+    return t
+
+
+def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_path=False, scratch=None):
+    """End-to-end call on HOST numpy buffers (pimc_run_host / pimc_run_host_ws): H2D, sweeps, moments, D2H inside the call."""
     npd = np.float64 if dtype == 64 else np.float32
     y = np.ascontiguousarray(w.y, dtype=npd)
     I = None if w.I is None else np.ascontiguousarray(w.I, dtype=npd)
@@ -402,8 +427,13 @@ def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_p
     xo = np.empty_like(x0) if want_path else None
     po = np.empty_like(p0) if want_path else None
     vp = lambda a: None if a is None else C.c_void_p(a.ctypes.data)
-    _check(lib().pimc_run_host(w.model, w.D, w.L, w.M, float(w.dt), float(w.Rm), rf, w.n_chains, dtype, vp(y), vp(I), vp(x0), vp(p0),
-                               ws, wp, lo, hi, kind, int(n_burn), int(n_sweeps), int(seed), mom.ctypes.data_as(_dp), vp(xo), vp(po)))
+    sp, sn = None, 0
+    if scratch is not None:
+        off = (-scratch.data_ptr()) % 256
+        sp, sn = C.c_void_p(scratch.data_ptr() + off), scratch.numel() - off
+    _check(lib().pimc_run_host_ws(w.model, w.D, w.L, w.M, float(w.dt), float(w.Rm), rf, w.n_chains, dtype, vp(y), vp(I), vp(x0), vp(p0),
+                                  ws, wp, lo, hi, kind, int(n_burn), int(n_sweeps), int(seed), mom.ctypes.data_as(_dp), vp(xo), vp(po),
+                                  sp, sn))
     mx = mom[:, : 2 * nx].reshape(w.n_chains, 2, w.M + 1, w.D)
     mp = mom[:, 2 * nx:].reshape(w.n_chains, 2, w.Np)
     bytes_in = y.nbytes + (0 if I is None else I.nbytes) + x0.nbytes + p0.nbytes

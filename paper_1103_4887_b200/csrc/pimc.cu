@@ -154,13 +154,22 @@ struct pimc_handle {
 
 namespace {
 
+// SM count of the current device (grid sizing of the helper kernels); 148 on B200, never assumed
+int sm_count_now() {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return 1;
+    return sms;
+}
+// caller-provided device arrays must be 32-byte aligned (SURVEY.md §8(b) conventions: vectorised loads)
+bool aligned32(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) == 0; }
+
 int fail(pimc_handle* h, int code, const char* fmt, ...) {
     char buf[512];
     va_list ap;
     va_start(ap, fmt);
     vsnprintf(buf, sizeof buf, fmt, ap);
     va_end(ap);
-    if (h) { if (h->err.empty()) h->err = buf; }
+    if (h) h->err = buf;                 // the message of the LATEST failure (pimc_last_error)
     else g_static_error = buf;
     return code;
 }
@@ -304,7 +313,7 @@ template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape*
 template <class Model, typename R> int rebuild_cache(pimc_handle* h) {
     const size_t total = (size_t)h->C * (h->M + 1);
     const int threads = 128;
-    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, 148 * 16);
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 16);
     // after a rebuild, buffer 0 is current
     build_cache_kernel<Model, R><<<blocks, threads, 0, h->stream>>>((const R*)h->lay.x, h->have_I ? (const R*)h->lay.I : nullptr,
                                                                      (const R*)h->lay.p, (R*)h->lay.g0, h->M, h->C, (R)h->dt, h->disc);
@@ -431,7 +440,7 @@ template <class Model, typename R> int run_op(const OpArgs& o) {
         case OP_SHAPE: return choose_shape<Model, R>(o.h, o.ls);
         case OP_STEP: {
             const int threads = 128;
-            const int blocks = (int)std::min<unsigned long long>((o.n + threads - 1) / threads, 148ull * 16);
+            const int blocks = (int)std::min<unsigned long long>((o.n + threads - 1) / threads, (unsigned long long)sm_count_now() * 16);
             step_selftest_kernel<Model, R><<<blocks, threads, 0, (cudaStream_t)o.stream>>>((const R*)o.x, (const R*)o.p, (const R*)o.I0, (const R*)o.I1,
                                                                                          (R)o.dt, o.n, (R*)o.g);
             PIMC_CUDA(nullptr, cudaGetLastError());
@@ -482,6 +491,10 @@ int sweep_common(pimc_handle* h, long long n_sweeps, unsigned long long seed, in
     if (n_sweeps < 0) return fail(h, PIMC_EINVAL, "n_sweeps < 0");
     if (!h->have_data || !h->have_path || !h->have_prop) return fail(h, PIMC_ESTATE, "pimc_sweep before set_data / set_path / set_proposal");
     if (n_sweeps == 0) return PIMC_OK;
+    // The tuning rule turns the acceptance rate of the last N_skip PROPOSED moves into a step size; a sweep
+    // that proposes only one class would shrink the other class's step sizes with no proposals behind it.
+    if (h->site_widths && h->tune && !(do_states && do_params))
+        return fail(h, PIMC_ESTATE, "step-size tuning needs full sweeps: pimc_sweep_states_only / _params_only are refused while it is on");
     if (((h->t + (unsigned long long)n_sweeps) >> 48) != 0) return fail(h, PIMC_EINVAL, "sweep index exceeds 48 bits");
     OpArgs o{}; o.op = OP_SWEEP; o.h = h; o.n_sweeps = n_sweeps; o.seed = seed; o.do_states = do_states; o.do_params = do_params;
     return dispatch_op(h->model, h->D, h->dtype, o);
@@ -490,7 +503,7 @@ int sweep_common(pimc_handle* h, long long n_sweeps, unsigned long long seed, in
 int recentre(pimc_handle* h) {
     const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
     const int threads = 256;
-    const int bx = (int)std::min<size_t>((nx + threads - 1) / threads, 148 * 8), bp = (int)((np + threads - 1) / threads);
+    const int bx = (int)std::min<size_t>((nx + threads - 1) / threads, (size_t)h->sm_count * 8), bp = (int)((np + threads - 1) / threads);
     if (h->dtype == 64) {
         widen_kernel<double><<<bx, threads, 0, h->stream>>>((const double*)h->lay.x, h->lay.cx, nx);
         if (np) widen_kernel<double><<<bp, threads, 0, h->stream>>>((const double*)h->lay.p, h->lay.cp, np);
@@ -579,6 +592,7 @@ int pimc_init(pimc_handle** out, int model, int D, int L, int M, double dt, doub
 int pimc_set_data(pimc_handle* h, const void* y, const void* I) {
     if (!h) return PIMC_EINVAL;
     if (h->L > 0 && !y) return fail(h, PIMC_EINVAL, "y is required when L > 0");
+    if (!aligned32(y) || !aligned32(I)) return fail(h, PIMC_EINVAL, "y and I must be 32-byte aligned device pointers");
     const size_t es = h->dtype == 64 ? 8 : 4;
     if (h->L > 0) PIMC_CUDA(h, cudaMemcpyAsync(h->lay.y, y, (size_t)h->C * (h->M + 1) * h->L * es, cudaMemcpyDeviceToDevice, h->stream));
     if (h->model != PIMC_MODEL_LINEAR && !I) return fail(h, PIMC_EINVAL, "the HH model needs the injected current I");
@@ -591,6 +605,7 @@ int pimc_set_data(pimc_handle* h, const void* y, const void* I) {
 
 int pimc_set_path(pimc_handle* h, const void* x) {
     if (!h || !x) return fail(h, PIMC_EINVAL, "null argument");
+    if (!aligned32(x)) return fail(h, PIMC_EINVAL, "x must be a 32-byte aligned device pointer");
     if (!h->have_data) return fail(h, PIMC_ESTATE, "pimc_set_path before pimc_set_data");
     const size_t es = h->dtype == 64 ? 8 : 4;
     PIMC_CUDA(h, cudaMemcpyAsync(h->lay.x, x, (size_t)h->C * (h->M + 1) * h->D * es, cudaMemcpyDeviceToDevice, h->stream));
@@ -600,6 +615,7 @@ int pimc_set_path(pimc_handle* h, const void* x) {
 
 int pimc_set_params(pimc_handle* h, const void* p) {
     if (!h || !p) return fail(h, PIMC_EINVAL, "null argument");
+    if (!aligned32(p)) return fail(h, PIMC_EINVAL, "p must be a 32-byte aligned device pointer");
     const size_t es = h->dtype == 64 ? 8 : 4;
     PIMC_CUDA(h, cudaMemcpyAsync(h->lay.p, p, (size_t)h->C * h->Np * es, cudaMemcpyDeviceToDevice, h->stream));
     if (h->have_path) return rebuild(h);
@@ -608,6 +624,7 @@ int pimc_set_params(pimc_handle* h, const void* p) {
 
 int pimc_get_path(pimc_handle* h, void* x_out, void* p_out) {
     if (!h) return PIMC_EINVAL;
+    if (!aligned32(x_out) || !aligned32(p_out)) return fail(h, PIMC_EINVAL, "x_out and p_out must be 32-byte aligned device pointers");
     const size_t es = h->dtype == 64 ? 8 : 4;
     if (x_out) PIMC_CUDA(h, cudaMemcpyAsync(x_out, h->lay.x, (size_t)h->C * (h->M + 1) * h->D * es, cudaMemcpyDeviceToDevice, h->stream));
     if (p_out) PIMC_CUDA(h, cudaMemcpyAsync(p_out, h->lay.p, (size_t)h->C * h->Np * es, cudaMemcpyDeviceToDevice, h->stream));
@@ -746,10 +763,11 @@ int pimc_sweep_params_only(pimc_handle* h, long long n_sweeps, unsigned long lon
 
 int pimc_moments(pimc_handle* h, double* out, unsigned long long* n_samples_host) {
     if (!h || !out) return fail(h, PIMC_EINVAL, "null argument");
+    if (!aligned32(out)) return fail(h, PIMC_EINVAL, "out must be a 32-byte aligned device pointer");
     const size_t nx = (size_t)(h->M + 1) * h->D;
     const size_t total = (size_t)h->C * (nx + h->Np);
     const int threads = 256;
-    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, 148 * 8);
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 8);
     moments_kernel<<<blocks, threads, 0, h->stream>>>(h->lay.cx, h->lay.S1x, h->lay.S2x, h->lay.cp, h->lay.S1p, h->lay.S2p, nx, h->Np,
                                                       h->C, (double)h->n_samples, out);
     h->launches++;
@@ -800,6 +818,8 @@ int pimc_hist(pimc_handle* h, unsigned long long* counts_out) {
 int pimc_debug_trace(pimc_handle* h, void* dA_out, unsigned char* acc_out, void* xprop_out, void* dA_param, unsigned char* acc_param,
                      void* pprop_out) {
     if (!h) return PIMC_EINVAL;
+    if (!aligned32(dA_out) || !aligned32(xprop_out) || !aligned32(dA_param) || !aligned32(pprop_out))
+        return fail(h, PIMC_EINVAL, "trace arrays must be 32-byte aligned device pointers");
     h->tr_dA = dA_out; h->tr_acc = acc_out; h->tr_xprop = xprop_out; h->tr_dAp = dA_param; h->tr_accp = acc_param; h->tr_pprop = pprop_out;
     return PIMC_OK;
 }
@@ -874,28 +894,68 @@ unsigned long long pimc_sweep_index(const pimc_handle* h) { return h ? h->t : 0;
 int pimc_set_sweep_index(pimc_handle* h, unsigned long long t) {
     if (!h) return PIMC_EINVAL;
     if ((t >> 48) != 0) return fail(h, PIMC_EINVAL, "sweep index exceeds 48 bits");
+    // The accumulation, tuning and annealing schedules count sweeps from the index at which they were switched on: moving the
+    // index below one of those origins would wrap the unsigned differences (sample count, adjustment sweeps, beta) silently.
+    if (h->accum && t < h->t_enable) return fail(h, PIMC_ESTATE, "sweep index below the sweep at which accumulation was enabled (disable or reset first)");
+    if (h->site_widths && h->tune && t < h->t_tune) return fail(h, PIMC_ESTATE, "sweep index below the sweep at which step-size tuning was enabled");
+    if (h->n_cool != 0 && t < h->t_anneal) return fail(h, PIMC_ESTATE, "sweep index below the sweep at which annealing was enabled");
     h->t = t;
     return PIMC_OK;
 }
 unsigned long long pimc_launch_count(const pimc_handle* h) { return h ? h->launches : 0; }
 
+// layout of the device scratch of pimc_run_host: staging copies of x, y, I, p, the moments read-out, then the handle's workspace
+namespace {
+struct HostRunLayout { size_t o_x, o_y, o_I, o_p, o_m, o_ws, ws, total, nx, ny, nI, nmom; };
+HostRunLayout host_run_layout(int model, int D, int L, int M, int n_chains, int dtype) {
+    HostRunLayout q{};
+    const int Np = pimc_model_np(model, D);
+    const size_t es = dtype == 64 ? 8 : 4;
+    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    q.nx = (size_t)n_chains * (M + 1) * D; q.ny = (size_t)n_chains * (M + 1) * (L > 0 ? L : 1); q.nI = (size_t)n_chains * (M + 1);
+    q.nmom = (size_t)n_chains * (2 * (size_t)(M + 1) * D + 2 * (size_t)Np);
+    q.ws = pimc_workspace_bytes(model, D, L, M, n_chains, dtype);
+    q.o_x = 0; q.o_y = q.o_x + up(q.nx * es); q.o_I = q.o_y + up(q.ny * es); q.o_p = q.o_I + up(q.nI * es);
+    q.o_m = q.o_p + up((size_t)n_chains * Np * es); q.o_ws = q.o_m + up(q.nmom * 8);
+    q.total = q.o_ws + q.ws;
+    return q;
+}
+}  // namespace
+
+size_t pimc_run_host_workspace_bytes(int model, int D, int L, int M, int n_chains, int dtype) {
+    int why;
+    if (!shape_ok(model, D, L, M, n_chains, dtype, &why)) return 0;
+    return host_run_layout(model, D, L, M, n_chains, dtype).total;
+}
+
 int pimc_run_host(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype, const void* y,
                   const void* I, const void* x0, const void* p0, const double* w_state, const double* w_param, const double* lo,
                   const double* hi, int proposal_kind, long long n_burn, long long n_sweeps, unsigned long long seed, double* moments_out,
                   void* x_out, void* p_out) {
+    return pimc_run_host_ws(model, D, L, M, dt, Rm, Rf, n_chains, dtype, y, I, x0, p0, w_state, w_param, lo, hi, proposal_kind, n_burn,
+                            n_sweeps, seed, moments_out, x_out, p_out, nullptr, 0);
+}
+
+int pimc_run_host_ws(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype, const void* y,
+                     const void* I, const void* x0, const void* p0, const double* w_state, const double* w_param, const double* lo,
+                     const double* hi, int proposal_kind, long long n_burn, long long n_sweeps, unsigned long long seed, double* moments_out,
+                     void* x_out, void* p_out, void* dev_scratch, size_t dev_scratch_bytes) {
     int why;
     if (!shape_ok(model, D, L, M, n_chains, dtype, &why)) return fail(nullptr, why, "bad or unsupported shape");
     if (!x0 || !p0 || !w_state || !moments_out || (L > 0 && !y)) return fail(nullptr, PIMC_EINVAL, "null argument");
     const int Np = pimc_model_np(model, D);
     const size_t es = dtype == 64 ? 8 : 4;
-    const size_t nx = (size_t)n_chains * (M + 1) * D, ny = (size_t)n_chains * (M + 1) * (L > 0 ? L : 1), nI = (size_t)n_chains * (M + 1);
-    const size_t nmom = (size_t)n_chains * (2 * (size_t)(M + 1) * D + 2 * (size_t)Np);
-    const size_t ws = pimc_workspace_bytes(model, D, L, M, n_chains, dtype);
+    const HostRunLayout q = host_run_layout(model, D, L, M, n_chains, dtype);
+    const size_t nx = q.nx, ny = q.ny, nI = q.nI, nmom = q.nmom, ws = q.ws, o_x = q.o_x, o_y = q.o_y, o_I = q.o_I, o_p = q.o_p, o_m = q.o_m, o_ws = q.o_ws;
     char* dev = nullptr;
-    const size_t o_x = 0, o_y = o_x + ((nx * es + 255) & ~(size_t)255), o_I = o_y + ((ny * es + 255) & ~(size_t)255),
-                 o_p = o_I + ((nI * es + 255) & ~(size_t)255), o_m = o_p + (((size_t)n_chains * Np * es + 255) & ~(size_t)255),
-                 o_ws = o_m + ((nmom * 8 + 255) & ~(size_t)255);
-    if (cudaMalloc(&dev, o_ws + ws) != cudaSuccess) return fail(nullptr, PIMC_ENOMEM, "cudaMalloc of %zu bytes failed", o_ws + ws);
+    const bool own = dev_scratch == nullptr;
+    if (own) {
+        if (cudaMalloc(&dev, q.total) != cudaSuccess) return fail(nullptr, PIMC_ENOMEM, "cudaMalloc of %zu bytes failed", q.total);
+    } else {
+        if (((uintptr_t)dev_scratch & 255) != 0 || dev_scratch_bytes < q.total)
+            return fail(nullptr, PIMC_EINVAL, "device scratch must be 256-byte aligned and at least %zu bytes", q.total);
+        dev = (char*)dev_scratch;
+    }
     pimc_handle* h = nullptr;
     int rc = PIMC_OK;
     cudaError_t e = cudaSuccess;
@@ -922,12 +982,16 @@ int pimc_run_host(int model, int D, int L, int M, double dt, double Rm, const do
             if (x_out && (e = cudaMemcpyAsync(x_out, dev + o_x, nx * es, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) break;
             if (p_out && (e = cudaMemcpyAsync(p_out, dev + o_p, (size_t)n_chains * Np * es, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) break;
         }
+        if (rc == PIMC_OK) {                       // a lost hand-off must not pass for a result
+            int flt = 0;
+            if ((rc = pimc_fault(h, &flt)) != PIMC_OK) break;
+        }
         e = cudaStreamSynchronize(0);
     } while (0);
     if (rc != PIMC_OK && h) g_static_error = h->err;
     if (e != cudaSuccess) { rc = fail(nullptr, PIMC_ECUDA, "pimc_run_host: %s", cudaGetErrorString(e)); }
     if (h) pimc_destroy(h);
-    cudaFree(dev);
+    if (own) cudaFree(dev);
     return rc;
 }
 
@@ -936,7 +1000,7 @@ int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned i
     if (!ctrs) return fail(nullptr, PIMC_EINVAL, "null argument");
     if (n == 0) return PIMC_OK;
     const int threads = 256;
-    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, 148ull * 8);
+    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, (unsigned long long)sm_count_now() * 8);
     rng_selftest_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(ctrs, n, key0, key1, out, u_prop, u_acc, z);
     PIMC_CUDA(nullptr, cudaGetLastError());
     return PIMC_OK;
@@ -955,7 +1019,7 @@ int pimc_math_selftest(const double* x, unsigned long long n, double* out, void*
     if (!x || !out) return fail(nullptr, PIMC_EINVAL, "null argument");
     if (n == 0) return PIMC_OK;
     const int threads = 256;
-    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, 148ull * 8);
+    const int blocks = (int)std::min<unsigned long long>((n + threads - 1) / threads, (unsigned long long)sm_count_now() * 8);
     math_selftest_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(x, n, out);
     PIMC_CUDA(nullptr, cudaGetLastError());
     return PIMC_OK;

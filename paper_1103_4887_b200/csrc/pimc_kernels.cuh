@@ -120,6 +120,17 @@ __device__ __forceinline__ unsigned long long ld_acquire_gpu(const unsigned long
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
+// Poll a monotonically increasing counter until it reaches `need`.  Gives up (and raises the fault flag, pimc_fault) after
+// kWaitSpinLimit polls, or soon after another CTA has given up: a safety net against hangs -- in a co-resident (cooperative)
+// launch a hand-off cannot be lost.
+constexpr unsigned long long kWaitSpinLimit = 20ull * 1000 * 1000;
+__device__ __forceinline__ void wait_counter_ge(const unsigned long long* p, unsigned long long need, int* fault) {
+    unsigned long long spins = 0;
+    while (ld_acquire_gpu(p) < need) {
+        if (++spins > kWaitSpinLimit) { atomicExch(fault, 1); break; }
+        if ((spins & 0xFFFFull) == 0 && *reinterpret_cast<volatile int*>(fault) != 0) break;
+    }
+}
 // Path and cache values may have been written by a neighbour CTA: read them from L2, never from a stale L1 line.
 template <typename R, int D> __device__ __forceinline__ void load_vec(const R* base, size_t site, R out[D]) {
     const R* q = base + site * D;
@@ -379,8 +390,8 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                 if (G > 1) {
                     if (tid == 0) {
                         const unsigned long long need = a.hs_base + 2ull * (unsigned long long)i + (unsigned long long)parity;
-                        if (parity == 0 && b > 0) while (ld_acquire_gpu(hs_flag + b - 1) < need) {}
-                        if (parity == 1 && b < G - 1) while (ld_acquire_gpu(hs_flag + b + 1) < need) {}
+                        if (parity == 0 && b > 0) wait_counter_ge(hs_flag + b - 1, need, a.fault);
+                        if (parity == 1 && b < G - 1) wait_counter_ge(hs_flag + b + 1, need, a.fault);
                     }
                     __syncthreads();
                 }
@@ -483,7 +494,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                         }
                         double mine = 0.0;
                         for (int j = tid; j < G; j += T) {
-                            while (ld_acquire_gpu(flg + j) < ar_count + 1ull) {}
+                            wait_counter_ge(flg + j, ar_count + 1ull, a.fault);
                             mine += __ldcg(val + j);
                         }
                         dA = block_sum(mine, red);

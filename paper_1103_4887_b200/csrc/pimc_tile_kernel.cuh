@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     const bool edge_lo = s_ext == 0, edge_hi = e_ext == M + 1;
 
     R* const gx = a.x + site0 * D;
-    R* const gg0 = a.g[0] + (size_t)chain * a.nc * D;     // this engine runs the RK4-map discretisation only: nc == M
+    R* const gg0 = a.g[0] + (size_t)chain * a.nc * D;     // nc = M (RK4 map) or M + 1 (trapezoid rule) cache entries per chain
     R* const gg1 = a.g[1] + (size_t)chain * a.nc * D;
     int cur = a.cur[chain];
 
@@ -604,6 +604,9 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 }
             }
             if (params_changed) prep = Model::prepare(prm, a.dt);
+            // The producer warps overwrite this sweep's pdraw set while drawing sweep t + 2 (next pass of the loop).  A move that
+            // is out of bounds reads pdraw and meets no barrier afterwards, so order those reads before the next produce().
+            __syncthreads();
             if (trace && b == 0 && tid == 0) {
 #pragma unroll
                 for (int l = 0; l < NP; ++l)
@@ -936,11 +939,11 @@ static __global__ void __launch_bounds__(256, 1) xchg_selftest_kernel(int mode, 
             if (tid == 0) ll_store_f64(base + (size_t)b * kArSlotWords, dA, tag);
             const long long until = clock64() + (long long)(mode - 100) * 50;
             double mine = 0.0;
-            if (tid < G) {
-                if (tid == b) mine = dA;
+            for (int j = tid; j < G; j += T) {           // exactly the loop of tile_sweep_kernel's parameter moves
+                if (j == b) mine += dA;
                 else {
                     while (clock64() < until) {}
-                    mine = ll_wait_f64(base + (size_t)tid * kArSlotWords, tag, fault);
+                    mine += ll_wait_f64(base + (size_t)j * kArSlotWords, tag, fault);
                 }
             }
             tot = block_sum_db(mine, red, red_phase);

@@ -23,16 +23,23 @@ import time
 
 
 def run(iterations=1_000_000, n_init=None, n_cool=None, n_skip=400, beta0=0.01, f_acc=0.23, alpha=0.02, seed=1103, dtype=64,
-        M=None, chunk=20_000):
+        M=None, chunk=20_000, workload=None):
+    """workload: any object with the fields of workloads.Workload (the caller's own data); None = the synthetic stand-in for the
+    paper's experiment from the repository's `workloads` module (needs the repository root on sys.path)."""
     import torch
-    from workloads import make_workload
     from . import binding as B
+    if workload is None:
+        try:
+            from workloads import make_workload
+        except ImportError as e:
+            raise ImportError("procedure.run() without `workload=` uses the repository's synthetic workload generator: put the "
+                              "repository root on sys.path or pass your own workload object") from e
 
     if not torch.cuda.is_available():
         raise RuntimeError("paper_1103_4887_b200.procedure needs a CUDA device (libpimc has no CPU path)")
     n_init = iterations // 2 if n_init is None else n_init            # PAPER.md:282: the first half is excluded
     n_cool = iterations // 10 if n_cool is None else n_cool           # PAPER.md:282: N_cool = 10^5 of 10^6
-    w = make_workload(5) if M is None else make_workload(5, M=M)
+    w = workload if workload is not None else (make_workload(5) if M is None else make_workload(5, M=M))
     h = B.Pimc.from_workload(w, dtype=dtype)
     h.set_discretisation(B.DISC_TRAPEZOID)
     h.set_proposal(w.w_state, w.w_param)                              # PAPER.md:282 initial step sizes

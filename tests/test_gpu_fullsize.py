@@ -79,6 +79,58 @@ def test_cfg3_full_size_free_running_bit_identical(P):
     print("cfg3 free-running, max dA error / scale:", worst)
 
 
+def test_cfg3_full_size_production_variant_bit_identical(P):
+    # The instantiation bench.py times: no debug trace, no annealing, no tuning (template flag TR = 0), stage-1 cache on,
+    # automatic launch (148 CTAs x 256 threads), moments every sweep -- 40 sweeps in ONE launch, i.e. across five halo
+    # exchanges and 280 grid-wide parameter all-reduces, then path, parameters, counters, histograms bit for bit and the
+    # moments to 1e-13 against the oracle (uniform proposals: bit-reproducible draws).
+    w = make_workload(3)
+    n_sweeps, seed = 40, 20110348
+    h = gpu_handle(w, kind=1)
+    shape = h.get_launch()
+    assert shape["ctas_per_chain"] >= 100 and shape["threads_per_cta"] == 256, shape
+    sites = [0, 1, 221, 222, 16383, 32767, 32768, -1, -1]
+    comps = [0, 1, 2, 3, 0, 1, 0, 0, 6]
+    lo = [-100, 0, 0, 0, -100, 0, -100, 60, 0.5]
+    hi = [60, 1, 1, 1, 60, 1, 60, 180, 1.5]
+    h.hist_config(sites, comps, lo, hi, 16)
+    h.set_accum(True, 1); h.reset_moments()
+    n0 = h.launch_count
+    h.sweep(n_sweeps, seed=seed)
+    assert h.launch_count - n0 == 1
+    assert h.fault() == 0
+    xg, pg = [a.cpu().numpy() for a in h.get_path()]
+    o = oracle_chains(w, kind=1)[0]
+    o.hist_config(sites, comps, lo, hi, 16)
+    o.set_accum(True, 1); o.reset_moments()
+    o.sweep(n_sweeps, seed=seed)
+    xo, po = o.get_path()
+    assert np.array_equal(xg[0], xo), np.abs(xg[0] - xo).max()
+    assert np.array_equal(pg[0], po)
+    assert np.array_equal(h.stats().cpu().numpy().astype(np.uint64)[0], o.stats())
+    assert np.array_equal(h.hist().cpu().numpy()[0], o.hist())
+    mx, mp, n = h.moments()
+    ox, op, on = o.moments()
+    assert n == on == n_sweeps
+    assert np.allclose(mx.cpu().numpy()[0], ox, rtol=1e-13, atol=1e-13) and np.allclose(mp.cpu().numpy()[0], op, rtol=1e-13, atol=1e-13)
+    assert int(o.stats()[0, 4:].sum()) > 50          # parameter moves were accepted along the way (the caches flipped)
+
+
+def test_cfg3_full_size_fp32_teacher_forced_in_bench_launch(P):
+    # the fp32 variant of config 3 at the benchmarked size and launch: per-site Delta-A within 1e-5 (relative to max(|dA|, S))
+    # of the fp64 oracle evaluated on the same fp32 states at the GPU's own fp32 proposals; proposals within a few FLOAT ulp
+    w = make_workload(3)
+    h = gpu_handle(w, dtype=32)
+    shape = h.get_launch()
+    assert shape["ctas_per_chain"] >= 100, shape
+    rep = teacher_forced(w, h, oracle_chains(w, state_dtype=32), 2, seed=5, tol=TOL32, state_dtype=32)
+    print("cfg3 fp32 full size", shape, rep)
+    assert rep["sites"] == 2 * (w.M + 1)
+    assert rep["max_rel"] <= TOL32 and rep["mismatch_outside_window"] == 0, rep
+    assert rep["param_moves"] > 0 and rep["max_param_rel"] <= 10 * TOL32, rep
+    assert rep["max_xprop_ulp"] <= 8.0 * 2.0**29, rep        # helpers.ulp_diff counts fp64 ulps: 8 float ulps of the operands' scale
+
+
 def test_cfg3_full_size_trapezoid_bit_identical(P):
     # the paper's own discretisation (Eq. 7) at the benchmarked size, tile-resident engine, 148 CTAs
     w = make_workload(3)
@@ -108,6 +160,7 @@ def test_fp32_teacher_forced_parity(P, cfg, M, launch, with_params):
     assert rep["mismatch_outside_window"] == 0, rep
     if with_params:
         assert rep["param_moves"] > 0 and rep["max_param_rel"] <= 10 * TOL32, rep
+    assert rep["max_xprop_ulp"] <= 8.0 * 2.0**29, rep            # 8 float ulps (the helper counts fp64 ulps)
 
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])

@@ -332,6 +332,63 @@ def test_c_abi_argument_errors_on_device(P):
     assert L.pimc_init(C.byref(hh), 1, 3, 1, 32, 0.02, 1.0, rf, p0, 1, 64, C.c_void_p(ws.data_ptr()), 1 << 20, None) == -4
 
 
+def test_boundary_robustness_alignment_schedules_and_fault_path(P):
+    import ctypes as C
+    import torch
+    w = make_workload(2, M=200)
+    h = gpu_handle(w)
+    L = P.lib()
+    # caller arrays must be 32-byte aligned (SURVEY.md 8(b) conventions): a view that starts 8 bytes in is refused
+    x = torch.zeros((w.M + 1) * w.D + 4, dtype=torch.float64, device="cuda")
+    assert x.data_ptr() % 32 == 0
+    assert L.pimc_set_path(h._h, C.c_void_p(x.data_ptr() + 8)) == -1 and b"aligned" in L.pimc_last_error(h._h)
+    assert L.pimc_get_path(h._h, C.c_void_p(x.data_ptr() + 8), None) == -1
+    assert L.pimc_set_data(h._h, C.c_void_p(x.data_ptr() + 16), C.c_void_p(x.data_ptr())) == -1
+    assert L.pimc_moments(h._h, C.c_void_p(x.data_ptr() + 8), None) == -1
+    assert L.pimc_debug_trace(h._h, C.c_void_p(x.data_ptr() + 24), None, None, None, None, None) == -1
+    # the error string is the LATEST failure's, not the first one's
+    assert L.pimc_set_accum(h._h, 1, 0) == -1 and b"n_skip" in L.pimc_last_error(h._h)
+    assert L.pimc_sweep(h._h, -1, 0) == -1 and b"n_sweeps" in L.pimc_last_error(h._h)
+    # schedules count sweeps from the index at which they were switched on: the index may not be moved below it
+    h.sweep(5, seed=1)
+    h.set_accum(True, 2); h.reset_moments()
+    assert h.sweep_index == 5
+    assert L.pimc_set_sweep_index(h._h, 3) == -2
+    h.sweep_index = 9                                   # forward is fine
+    h.set_accum(False, 1)
+    h.sweep_index = 3                                   # and backwards once nothing counts from an origin
+    # step-size tuning needs full sweeps
+    h.set_tuning(True, 5, 0.23, 0.02)
+    assert L.pimc_sweep_states_only(h._h, 1, 1) == -2 and L.pimc_sweep_params_only(h._h, 1, 1) == -2
+    assert b"tuning" in L.pimc_last_error(h._h)
+    h.sweep(10, seed=1, check_fault=True)               # the checked path: synchronises and raises on a lost hand-off
+    h.set_tuning(False)
+    h.sweep_states_only(1, seed=1)
+    # exchange knob: results do not depend on it
+    h1, h2 = gpu_handle(w, kind=1), gpu_handle(w, kind=1)
+    h2.set_exchange(0)
+    assert L.pimc_set_exchange(h2._h, -1) == -1
+    h1.sweep(12, seed=3); h2.sweep(12, seed=3)
+    assert torch.equal(h1.get_path()[0], h2.get_path()[0]) and torch.equal(h1.get_path()[1], h2.get_path()[1])
+
+
+def test_run_host_with_caller_scratch(P):
+    w = make_workload(2, M=200)
+    scratch = P.run_host_scratch(w)
+    a = P.run_host(w, n_burn=5, n_sweeps=20, seed=6, want_path=True)
+    b = P.run_host(w, n_burn=5, n_sweeps=20, seed=6, want_path=True, scratch=scratch)
+    c = P.run_host(w, n_burn=5, n_sweeps=20, seed=6, want_path=True, scratch=scratch)      # reuse
+    for k in ("mean_x", "var_x", "mean_p", "var_p", "x", "p"):
+        assert np.array_equal(a[k], b[k]) and np.array_equal(a[k], c[k]), k
+    import ctypes as C
+    import torch
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(P.PimcError):
+        P.run_host(w, n_burn=0, n_sweeps=1, seed=6, scratch=small)
+    assert P.lib().pimc_run_host_workspace_bytes(w.model, w.D, w.L, w.M, 1, 64) > P.lib().pimc_workspace_bytes(w.model, w.D, w.L, w.M, 1, 64)
+    assert P.lib().pimc_run_host_workspace_bytes(9, 4, 1, 10, 1, 64) == 0
+
+
 def test_run_host_end_to_end_matches_device_api(P):
     w = make_workload(2, M=200)
     out = P.run_host(w, n_burn=10, n_sweeps=40, seed=6, want_path=True)
