@@ -60,6 +60,11 @@ def lib():
             "orc_get_widths": (None, [C.c_void_p, dp, dp]),
             "orc_annealing_beta": (C.c_double, [C.c_void_p]),
             "orc_set_discretisation": (C.c_int, [C.c_void_p, C.c_int]),
+            "orc_param_trace_enable": (None, [C.c_void_p, C.c_int]),
+            "orc_param_trace": (C.c_uint64, [C.c_void_p, dp, C.c_uint64]),
+            "orc_residuals": (None, [C.c_void_p, dp, dp]),
+            "orc_residual_stats_enable": (None, [C.c_void_p, C.c_int]),
+            "orc_residual_stats": (C.c_uint64, [C.c_void_p, dp]),
             "orc_half_rhs": (None, [C.c_int, C.c_int, dp, dp, C.c_double, C.c_double, dp]),
         }
         for name, (res, args) in sig.items():
@@ -263,6 +268,33 @@ class OracleChain:
         mx = out[: 2 * nx].reshape(2, self.M + 1, self.D)
         mp = out[2 * nx:].reshape(2, self.Np)
         return mx, mp, n
+
+    def param_trace_enable(self, on=True):
+        """Record the parameters at every accumulated sweep (Fig. 4); cleared by reset_moments()."""
+        lib().orc_param_trace_enable(self._h, int(bool(on)))
+
+    def param_trace(self):
+        n = lib().orc_param_trace(self._h, None, 0)
+        out = np.empty((n, self.Np))
+        lib().orc_param_trace(self._h, _dp(out), n)
+        return out
+
+    def residuals(self):
+        """Model errors eps (M, D) and observation errors delta (M+1, L) of the current path."""
+        eps, delta = np.empty((self.M, self.D)), np.empty((self.M + 1, max(self.L, 1)))[:, : self.L].copy()
+        lib().orc_residuals(self._h, _dp(eps), _dp(delta))
+        return eps, delta
+
+    def residual_stats_enable(self, on=True):
+        lib().orc_residual_stats_enable(self._h, int(bool(on)))
+
+    def residual_stats(self):
+        """(mean eps, var eps) (M, D) each, (mean delta, var delta) (M+1, L) each, sample count."""
+        ne, nd = self.M * self.D, (self.M + 1) * self.L
+        out = np.empty(2 * ne + 2 * nd)
+        n = lib().orc_residual_stats(self._h, _dp(out))
+        return (out[:ne].reshape(self.M, self.D), out[ne:2 * ne].reshape(self.M, self.D),
+                out[2 * ne:2 * ne + nd].reshape(self.M + 1, self.L), out[2 * ne + nd:].reshape(self.M + 1, self.L), n)
 
     def stats(self):
         out = np.zeros((2, self.D + self.Np), np.uint64)

@@ -208,6 +208,10 @@ struct Chain {
     // S5 accumulators
     bool accum = false; uint64_t n_skip = 1, t_enable = 0, n_samples = 0;
     std::vector<double> cx, cp, S1x, S2x, S1p, S2p;
+    // optional record of the parameters at every accumulated sweep (Fig. 4: "the evolution of one of the parameters")
+    bool ptrace_on = false; std::vector<double> ptrace;
+    // optional running sums of the model errors eps_n and observation errors delta_n of the accumulated paths
+    bool resid_on = false; std::vector<double> E1, E2, D1, D2;
     // A6 counters: accepted / proposed, per component class and per parameter
     std::vector<uint64_t> acc, prop;
     // histograms
@@ -482,6 +486,29 @@ void parameter_moves(Chain& c, uint64_t seed) {
     }
 }
 
+// Model errors and observation errors of the current path ("look at the model errors, eps_n, and the observation
+// errors, delta_n ... functions of the path"), in the discretisation in use:
+//   eps_{n,a}   = (x_{n+1,a} - x_{n,a}) - g_{n,a}                      n = 0..M-1   (RK4 map; trapezoid: ... - c_n - c_{n+1})
+//   delta_{n,l} = y_{n,l} - x_{n,l}                                     n = 1..M     (delta_0 = 0: y_0 is not in the action)
+// so that A(X) = sum (Rm/2) delta^2 + sum (Rf_a/2) eps^2 exactly as the action is defined (pinned that way in the tests).
+void residuals(const Chain& c, double* eps /* M*D */, double* delta /* (M+1)*L */) {
+    const int D = c.D, M = c.M, L = c.L;
+    for (int n = 0; n < M; ++n)
+        for (int a = 0; a < D; ++a) {
+            double r = (c.x[(size_t)(n + 1) * D + a] - c.x[(size_t)n * D + a]) - c.g[(size_t)n * D + a];
+            if (c.disc == 1) r -= c.g[(size_t)(n + 1) * D + a];
+            eps[(size_t)n * D + a] = r;
+        }
+    for (int n = 0; n <= M; ++n)
+        for (int l = 0; l < L; ++l) delta[(size_t)n * L + l] = n >= 1 ? c.y[(size_t)n * L + l] - c.x[(size_t)n * D + l] : 0.0;
+}
+void accumulate_residuals(Chain& c) {
+    std::vector<double> eps((size_t)c.M * c.D), del((size_t)(c.M + 1) * c.L);
+    residuals(c, eps.data(), del.data());
+    for (size_t i = 0; i < eps.size(); ++i) { c.E1[i] += eps[i]; c.E2[i] += eps[i] * eps[i]; }
+    for (size_t i = 0; i < del.size(); ++i) { c.D1[i] += del[i]; c.D2[i] += del[i] * del[i]; }
+}
+
 // S5. Running moments about the reference point c (values at the last reset) + histograms.
 void accumulate(Chain& c) {
     const size_t nx = (size_t)(c.M + 1) * c.D;
@@ -499,10 +526,15 @@ void accumulate(Chain& c) {
             bins[1 + b] += 1;
         }
     }
+    if (c.ptrace_on) c.ptrace.insert(c.ptrace.end(), c.p.begin(), c.p.end());
+    if (c.resid_on) accumulate_residuals(c);
     c.n_samples += 1;
 }
 
 void reset_moments(Chain& c) {
+    c.ptrace.clear();
+    std::fill(c.E1.begin(), c.E1.end(), 0.0); std::fill(c.E2.begin(), c.E2.end(), 0.0);
+    std::fill(c.D1.begin(), c.D1.end(), 0.0); std::fill(c.D2.begin(), c.D2.end(), 0.0);
     c.cx = c.x; c.cp = c.p;
     std::fill(c.S1x.begin(), c.S1x.end(), 0.0); std::fill(c.S2x.begin(), c.S2x.end(), 0.0);
     std::fill(c.S1p.begin(), c.S1p.end(), 0.0); std::fill(c.S2p.begin(), c.S2p.end(), 0.0);
@@ -736,6 +768,32 @@ int orc_sweep(void* h, uint64_t n_sweeps, uint64_t seed, int order, int do_param
 }
 
 // S6 outputs: out = mean,var of x as (2, M+1, D), then mean,var of p as (2, Np).  Population variance.
+// Record the parameters at every accumulated sweep from now on (cleared by orc_reset_moments).
+void orc_param_trace_enable(void* h, int on) { Chain& c = *(Chain*)h; c.ptrace_on = on != 0; if (!on) c.ptrace.clear(); }
+// out: (n_records, Np); returns the number of records held.
+uint64_t orc_param_trace(void* h, double* out, uint64_t max_records) {
+    Chain& c = *(Chain*)h;
+    const uint64_t n = c.Np ? c.ptrace.size() / c.Np : 0, k = n < max_records ? n : max_records;
+    if (out) std::memcpy(out, c.ptrace.data(), k * c.Np * sizeof(double));
+    return n;
+}
+// eps (M, D), delta (M+1, L) of the current path
+void orc_residuals(void* h, double* eps, double* delta) { residuals(*(Chain*)h, eps, delta); }
+// Running means and variances of eps and delta over the accumulated sweeps (population form, like the moments)
+void orc_residual_stats_enable(void* h, int on) {
+    Chain& c = *(Chain*)h; c.resid_on = on != 0;
+    c.E1.assign((size_t)c.M * c.D, 0.0); c.E2 = c.E1; c.D1.assign((size_t)(c.M + 1) * c.L, 0.0); c.D2 = c.D1;
+}
+// out: mean eps (M, D), var eps (M, D), mean delta (M+1, L), var delta (M+1, L)
+uint64_t orc_residual_stats(void* h, double* out) {
+    Chain& c = *(Chain*)h;
+    const size_t ne = (size_t)c.M * c.D, nd = (size_t)(c.M + 1) * c.L;
+    const double N = (double)c.n_samples;
+    for (size_t i = 0; i < ne; ++i) { const double m = c.n_samples ? c.E1[i] / N : 0.0; out[i] = m; out[ne + i] = c.n_samples ? c.E2[i] / N - m * m : 0.0; }
+    for (size_t i = 0; i < nd; ++i) { const double m = c.n_samples ? c.D1[i] / N : 0.0; out[2 * ne + i] = m; out[2 * ne + nd + i] = c.n_samples ? c.D2[i] / N - m * m : 0.0; }
+    return c.n_samples;
+}
+
 uint64_t orc_moments(void* h, double* out) {
     Chain& c = *(Chain*)h;
     const size_t nx = (size_t)(c.M + 1) * c.D;

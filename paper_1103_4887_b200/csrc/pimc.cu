@@ -218,7 +218,7 @@ template <class Model, typename R> int choose_shape_global(pimc_handle* h, Launc
         if (h->C >= h->sm_count / 2) G = 1;
         else {
             if (T == 0) T = 128;
-            PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R>, T, 0));
+            PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R, false>, T, 0));
             const int cap = per_sm > 0 ? h->sm_count : 0;    // one CTA per SM: the FP64 pipe is the shared resource
             G = (sites + 2 * T - 1) / (2 * T);
             if (G > cap / h->C) G = cap / h->C;
@@ -234,7 +234,7 @@ template <class Model, typename R> int choose_shape_global(pimc_handle* h, Launc
     out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1;
     out->engine = PIMC_ENGINE_GLOBAL; out->h = 0; out->smem = 0;
     if (G > 1) {
-        PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R>, T, 0));
+        PIMC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_kernel<Model, R, false>, T, 0));
         if ((long long)G * h->C > (long long)per_sm * h->sm_count)
             return fail(h, PIMC_EINVAL, "grid of %d CTAs is not co-resident (capacity %d)", G * h->C, per_sm * h->sm_count);
     }
@@ -359,7 +359,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
 
     const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
     const bool trap = h->disc == PIMC_DISC_TRAPEZOID;
-    const void* fn = (const void*)sweep_kernel<Model, R>;
+    const void* fn = ls.G == 1 ? (const void*)sweep_kernel<Model, R, true> : (const void*)sweep_kernel<Model, R, false>;
     if (ls.engine == PIMC_ENGINE_TILE) {
         const bool comp = h->update_mode == PIMC_UPDATE_COMPONENTWISE;
         // the stage-1 cache is only worth keeping if this launch moves a parameter (and the model has one: NK > 0)

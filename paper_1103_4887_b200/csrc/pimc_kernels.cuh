@@ -132,9 +132,22 @@ __device__ __forceinline__ void wait_counter_ge(const unsigned long long* p, uns
     }
 }
 // Path and cache values may have been written by a neighbour CTA: read them from L2, never from a stale L1 line.
-template <typename R, int D> __device__ __forceinline__ void load_vec(const R* base, size_t site, R out[D]) {
+// CG = false (one CTA per chain: nobody else writes this chain) uses ordinary L1-cached loads, which the prefetches of the
+// sweep loops can serve.
+template <typename R, int D, bool CG = true> __device__ __forceinline__ void load_vec(const R* base, size_t site, R out[D]) {
     const R* q = base + site * D;
-    if constexpr (D == 4 && sizeof(R) == 8) {
+    if constexpr (!CG) {
+        if constexpr (D == 4 && sizeof(R) == 8) {
+            const double2 a = reinterpret_cast<const double2*>(q)[0], b = reinterpret_cast<const double2*>(q)[1];
+            out[0] = a.x; out[1] = a.y; out[2] = b.x; out[3] = b.y;
+        } else if constexpr (D == 4 && sizeof(R) == 4) {
+            const float4 a = reinterpret_cast<const float4*>(q)[0];
+            out[0] = a.x; out[1] = a.y; out[2] = a.z; out[3] = a.w;
+        } else {
+#pragma unroll
+            for (int a = 0; a < D; ++a) out[a] = q[a];
+        }
+    } else if constexpr (D == 4 && sizeof(R) == 8) {
         const double2 a = __ldcg(reinterpret_cast<const double2*>(q));
         const double2 b = __ldcg(reinterpret_cast<const double2*>(q) + 1);
         out[0] = a.x; out[1] = a.y; out[2] = b.x; out[3] = b.y;
@@ -149,6 +162,7 @@ template <typename R, int D> __device__ __forceinline__ void load_vec(const R* b
         for (int a = 0; a < D; ++a) out[a] = __ldcg(q + a);
     }
 }
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 template <typename R, int D> __device__ __forceinline__ void store_vec(R* base, size_t site, const R v[D]) {
     R* q = base + site * D;
     if constexpr (D == 4 && sizeof(R) == 8) {
@@ -215,14 +229,15 @@ template <typename R> __device__ __forceinline__ R log_accept_uniform(const Swee
 }
 
 // ---- one Metropolis site update: Fig. 1 (a)-(i) ----------------------------------------------------------
-template <class Model, typename R>
+template <class Model, typename R, bool CG = true>
 __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* __restrict__ prm, unsigned long long t,
                                             uint32_t chain, int n, R* __restrict__ x, R* __restrict__ g, const R* __restrict__ y,
-                                            const R* __restrict__ I, bool trace, size_t chain_site0, const R* __restrict__ Rfs) {
+                                            const R* __restrict__ I, bool trace, size_t chain_site0, const R* __restrict__ Rfs,
+                                            const typename Model::Prep& prep) {
     constexpr int D = Model::D;
     const int M = a.M;
     R xn[D], xfull[D], xp[D], gp[D];
-    load_vec<R, D>(x, n, xn);
+    load_vec<R, D, CG>(x, n, xn);
     propose_state<R, D>(a, t, chain, (uint32_t)n, xn, xfull);
     // joint move: one pass with the whole proposal.  Component-wise moves: D passes; pass ai changes component ai only (same
     // draw as the joint move), is judged with the accept uniform of block ai, and the next pass starts from what it leaves.
@@ -237,13 +252,13 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
         // trapezoid rule, Fig. 1 (b)-(f) as printed: c' = (dt/2) F(x'_n) enters BOTH neighbouring terms; every residual is
         // (x_{k+1} - x_k) - c_k - c_{k+1}
         R cn[D];
-        load_vec<R, D>(g, n, cn);
+        load_vec<R, D, CG>(g, n, cn);
         const R I0 = I ? __ldg(I + n) : R(0);
-        Model::half_rhs(xp, prm, Model::prepare(prm, a.dt), I0, gp);
+        Model::half_rhs(xp, prm, prep, I0, gp);
         if (n >= 1) {
             R xm[D], cm[D];
-            load_vec<R, D>(x, n - 1, xm);
-            load_vec<R, D>(g, n - 1, cm);
+            load_vec<R, D, CG>(x, n - 1, xm);
+            load_vec<R, D, CG>(g, n - 1, cm);
 #pragma unroll
             for (int c = 0; c < D; ++c) {
                 const R r_new = ((xp[c] - xm[c]) - cm[c]) - gp[c];
@@ -261,8 +276,8 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
         }
         if (n <= M - 1) {
             R xq[D], cq[D];
-            load_vec<R, D>(x, n + 1, xq);
-            load_vec<R, D>(g, n + 1, cq);
+            load_vec<R, D, CG>(x, n + 1, xq);
+            load_vec<R, D, CG>(g, n + 1, cq);
 #pragma unroll
             for (int c = 0; c < D; ++c) {
                 const R r_new = ((xq[c] - xp[c]) - gp[c]) - cq[c];
@@ -273,8 +288,8 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
     } else {
     if (n >= 1) {
         R xm[D], gm[D];
-        load_vec<R, D>(x, n - 1, xm);
-        load_vec<R, D>(g, n - 1, gm);
+        load_vec<R, D, CG>(x, n - 1, xm);
+        load_vec<R, D, CG>(g, n - 1, gm);
 #pragma unroll
         for (int c = 0; c < D; ++c) {   // model-error term n-1 -> n
             const R r_new = (xp[c] - xm[c]) - gm[c];
@@ -292,10 +307,10 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
     }
     if (n <= M - 1) {
         R xq[D], gn[D];
-        load_vec<R, D>(x, n + 1, xq);
-        load_vec<R, D>(g, n, gn);
+        load_vec<R, D, CG>(x, n + 1, xq);
+        load_vec<R, D, CG>(g, n, gn);
         const R I0 = I ? __ldg(I + n) : R(0), I1 = I ? __ldg(I + n + 1) : R(0);
-        Model::increment(xp, prm, I0, I1, a.dt, gp);
+        Model::increment(xp, prm, prep, I0, I1, a.dt, gp);
 #pragma unroll
         for (int c = 0; c < D; ++c) {   // model-error term n -> n+1
             const R r_new = (xq[c] - xp[c]) - gp[c];
@@ -334,8 +349,13 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
 }
 
 // ---- the persistent sweep kernel ---------------------------------------------------------------------------
-template <class Model, typename R>
+// SOLO = one CTA per chain (G == 1, batched chains): no other CTA ever writes this chain's arrays, so the loops use L1-cached
+// loads and prefetch the lines of their NEXT pass (same thread, T sites further on) before working on the current one -- the
+// profile of config 4 (profiles/r02_cfg4.md) had `long_scoreboard` on top: 21 % of all samples sat on the first uses of the
+// loads of a parameter-move pass.
+template <class Model, typename R, bool SOLO = false>
 __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a) {
+    constexpr bool CG = !SOLO;
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
     __shared__ double red[32];
@@ -385,6 +405,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
         }
 
         // ---------------- A2/A3: even half-sweep, then odd half-sweep ----------------
+        const typename Model::Prep prep = Model::prepare(ps, a.dt);      // 1/C, dt/2, dt/6: once per sweep, not once per site
         if (a.do_states) {
             for (int parity = 0; parity < 2; ++parity) {
                 if (G > 1) {
@@ -397,7 +418,15 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                 }
                 for (int n = s + parity + 2 * tid; n < e; n += 2 * T)
                 {
-                    const unsigned mask = update_site<Model, R>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0, Rfs);
+                    if constexpr (SOLO) {        // next pass of this thread: sites n' - 1 .. n' + 1 and their cache entries
+                        const int np = n + 2 * T;
+                        if (np < e) {
+                            const R* gq = cur ? g_b : g_a;
+                            prefetch_l1(x + (size_t)(np - 1) * D); prefetch_l1(x + (size_t)np * D); prefetch_l1(x + (size_t)min(np + 1, M) * D);
+                            prefetch_l1(gq + (size_t)(np - 1) * D); prefetch_l1(gq + (size_t)min(np, a.nc - 1) * D);
+                        }
+                    }
+                    const unsigned mask = update_site<Model, R, CG>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0, Rfs, prep);
 #pragma unroll
                     for (int c = 0; c < D; ++c) n_acc_comp[c] += (mask >> c) & 1u;
                     if (a.ws && a.tune) {        // N_acc,i of the tuning rule: this thread is the only writer of its site
@@ -448,10 +477,10 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                         const typename Model::Prep pq = Model::prepare(ps_prop, a.dt);
                         for (int n = s + tid; n < e_fwd; n += T) {
                             R xn[D], xq[D], cn[D], cq[D], cpn[D], cpq[D];
-                            load_vec<R, D>(x, n, xn);
-                            load_vec<R, D>(x, n + 1, xq);
-                            load_vec<R, D>(gcur, n, cn);
-                            load_vec<R, D>(gcur, n + 1, cq);
+                            load_vec<R, D, CG>(x, n, xn);
+                            load_vec<R, D, CG>(x, n + 1, xq);
+                            load_vec<R, D, CG>(gcur, n, cn);
+                            load_vec<R, D, CG>(gcur, n + 1, cq);
                             Model::half_rhs(xn, ps_prop, pq, I ? __ldg(I + n) : R(0), cpn);
                             Model::half_rhs(xq, ps_prop, pq, I ? __ldg(I + n + 1) : R(0), cpq);
                             store_vec<R, D>(galt, n, cpn);
@@ -465,14 +494,19 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                             }
                             part += (double)acc;
                         }
-                    } else
+                    } else {
+                    const typename Model::Prep pq = Model::prepare(ps_prop, a.dt);
                     for (int n = s + tid; n < e_fwd; n += T) {
+                        if constexpr (SOLO) {    // x_{n'+1} is the next lane's x_{n'}: one prefetch per array covers the warp's lines
+                            const int np = n + T;
+                            if (np < e_fwd) { prefetch_l1(x + (size_t)np * D); prefetch_l1(gcur + (size_t)np * D); if (I) prefetch_l1(I + np); }
+                        }
                         R xn[D], xq[D], gn[D], gp[D];
-                        load_vec<R, D>(x, n, xn);
-                        load_vec<R, D>(x, n + 1, xq);
-                        load_vec<R, D>(gcur, n, gn);
+                        load_vec<R, D, CG>(x, n, xn);
+                        load_vec<R, D, CG>(x, n + 1, xq);
+                        load_vec<R, D, CG>(gcur, n, gn);
                         const R I0 = I ? __ldg(I + n) : R(0), I1 = I ? __ldg(I + n + 1) : R(0);
-                        Model::increment(xn, ps_prop, I0, I1, a.dt, gp);
+                        Model::increment(xn, ps_prop, pq, I0, I1, a.dt, gp);
                         store_vec<R, D>(galt, n, gp);
                         R acc = R(0);
 #pragma unroll
@@ -482,6 +516,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                             acc += R(0.5) * Rfs[c] * (r_new * r_new - r_old * r_old);
                         }
                         part += (double)acc;
+                    }
                     }
                     dA = block_sum(part, red);
                     if (G > 1) {   // all-gather of the G partials, summed in index order by every CTA
