@@ -195,6 +195,25 @@ int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, i
 int pimc_set_engine(pimc_handle* h, int engine, int halo);
 /* Report the engine and halo depth pimc_sweep will use (any pointer may be NULL). */
 int pimc_get_engine(pimc_handle* h, int* engine, int* halo);
+/* Optional record of the parameters (Fig. 4 "the evolution of one of the parameters as the MC path update
+ * procedure runs"): from now on every ACCUMULATED sweep (pimc_set_accum) writes the chain's parameter vector to record number
+ * n_samples of out, dev (n_chains, capacity, Np) of `dtype` elements, owned by the caller; records beyond capacity are dropped;
+ * pimc_reset_moments restarts at record 0; out = NULL switches it off.  Written inside the sweep kernels (no extra launch). */
+int pimc_param_trace(pimc_handle* h, void* out, long long capacity);
+
+/* Model errors and observation errors of the CURRENT path: eps_out dev (n_chains, M, D),
+ * eps_{n,a} = (x_{n+1,a} - x_{n,a}) - g_{n,a} (PIMC_DISC_TRAPEZOID: x_{n+1} - x_n - c_n - c_{n+1}); delta_out dev
+ * (n_chains, M+1, L), delta_{n,l} = y_{n,l} - x_{n,l} for n >= 1 and 0 for n = 0 -- the terms of the action, so that
+ * A = sum (Rm/2) delta^2 + sum (Rf_a/2) eps^2.  `dtype` elements; either pointer may be NULL. */
+int pimc_residuals(pimc_handle* h, void* eps_out, void* delta_out);
+/* Running statistics of eps_n and delta_n over the accumulated sweeps ("the means should be zero, the variances should come out as
+ * specified by R_o and R_d").  acc: dev double, n_chains x [M*D + M*D + (M+1)*L + (M+1)*L], owned by the caller,
+ * zeroed here and by pimc_reset_moments; NULL switches it off.  While it is on, pimc_sweep ends a launch at every accumulated
+ * sweep and runs one small kernel on that path (a diagnostic: one extra launch per sample).  pimc_residual_stats: out dev double,
+ * same layout = mean eps, var eps, mean delta, var delta (population form, sample count = that of pimc_moments). */
+int pimc_set_residual_stats(pimc_handle* h, double* acc);
+int pimc_residual_stats(pimc_handle* h, double* out);
+
 /* Tuning knob of the grid-wide Delta-A sum of a parameter move (row A4; TILE engine, more than one CTA per chain): SM clock
  * ticks a CTA waits after publishing its partial before it first polls the other CTAs' packets (default 450; 0 = poll at
  * once).  A packet needs about 1000 ticks from the store to a successful poll; earlier polls only load the L2 slices everybody

@@ -51,6 +51,10 @@ _SIGNATURES = {
     "pimc_get_widths": (C.c_int, [_vp, _vp, _vp]),
     "pimc_get_engine": (C.c_int, [_vp, _ip, _ip]),
     "pimc_set_exchange": (C.c_int, [_vp, C.c_int]),
+    "pimc_param_trace": (C.c_int, [_vp, _vp, C.c_longlong]),
+    "pimc_residuals": (C.c_int, [_vp, _vp, _vp]),
+    "pimc_set_residual_stats": (C.c_int, [_vp, _vp]),
+    "pimc_residual_stats": (C.c_int, [_vp, _vp]),
     "pimc_fault": (C.c_int, [_vp, _ip]),
     "pimc_sweep_index": (C.c_ulonglong, [_vp]),
     "pimc_set_sweep_index": (C.c_int, [_vp, C.c_ulonglong]),
@@ -232,6 +236,44 @@ class Pimc:
         e, hh = C.c_int(), C.c_int()
         _check(lib().pimc_get_engine(self._h, C.byref(e), C.byref(hh)), self._h)
         return dict(engine=e.value, halo=hh.value)
+
+    def param_trace(self, capacity):
+        """Record the parameters at every accumulated sweep (Fig. 4) -> device tensor (C, capacity, Np); 0 = off."""
+        if not capacity:
+            _check(lib().pimc_param_trace(self._h, None, 0), self._h)
+            self._keep.pop("ptrace", None)
+            return None
+        buf = self.torch.full((self.C, int(capacity), self.Np), float("nan"), dtype=self.tdtype, device=self.device)
+        self.torch.cuda.current_stream().synchronize()
+        _check(lib().pimc_param_trace(self._h, _ptr(buf), int(capacity)), self._h)
+        self._keep["ptrace"] = buf
+        return buf
+
+    def residuals(self):
+        """Model errors eps (C, M, D) and observation errors delta (C, M+1, L) of the current path."""
+        eps = self.torch.empty((self.C, self.M, self.D), dtype=self.tdtype, device=self.device)
+        delta = self.torch.empty((self.C, self.M + 1, self.L), dtype=self.tdtype, device=self.device)
+        _check(lib().pimc_residuals(self._h, _ptr(eps), _ptr(delta)), self._h)
+        return eps, delta
+
+    def set_residual_stats(self, enabled=True):
+        if not enabled:
+            _check(lib().pimc_set_residual_stats(self._h, None), self._h)
+            self._keep.pop("resid", None)
+            return
+        n = 2 * self.M * self.D + 2 * (self.M + 1) * self.L
+        buf = self.torch.zeros((self.C, n), dtype=self.torch.float64, device=self.device)
+        self.torch.cuda.current_stream().synchronize()
+        _check(lib().pimc_set_residual_stats(self._h, _ptr(buf)), self._h)
+        self._keep["resid"] = buf
+
+    def residual_stats(self):
+        """(mean eps, var eps) (C, M, D), (mean delta, var delta) (C, M+1, L) over the accumulated sweeps."""
+        ne, nd = self.M * self.D, (self.M + 1) * self.L
+        out = self.torch.empty((self.C, 2 * ne + 2 * nd), dtype=self.torch.float64, device=self.device)
+        _check(lib().pimc_residual_stats(self._h, _ptr(out)), self._h)
+        sh_e, sh_d = (self.C, self.M, self.D), (self.C, self.M + 1, self.L)
+        return (out[:, :ne].reshape(sh_e), out[:, ne:2 * ne].reshape(sh_e), out[:, 2 * ne:2 * ne + nd].reshape(sh_d), out[:, 2 * ne + nd:].reshape(sh_d))
 
     def set_exchange(self, first_poll_hold_cycles=450):
         _check(lib().pimc_set_exchange(self._h, int(first_poll_hold_cycles)), self._h)

@@ -148,6 +148,8 @@ struct pimc_handle {
     int G_user = 0, T_user = 0, engine_user = PIMC_ENGINE_AUTO, halo_user = -1;
     unsigned long long hs_base = 0, launches = 0;
     int ar_hold = 450;                // pimc_set_exchange
+    void* ptrace = nullptr; long long ptrace_cap = 0;      // pimc_param_trace
+    double* resid_acc = nullptr;                           // pimc_set_residual_stats
     int sm_count = 0;
     std::string err;
 };
@@ -356,6 +358,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
     a.hs_flag = h->lay.hs_flag; a.ar_val = h->lay.ar_val; a.ar_flag = h->lay.ar_flag; a.ar_epoch = h->lay.ar_epoch;
     a.hs_base = h->hs_base;
     a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault; a.ar_hold = h->ar_hold;
+    a.ptrace = (R*)h->ptrace; a.ptrace_cap = h->ptrace_cap; a.ptrace_n0 = h->n_samples;
 
     const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
     const bool trap = h->disc == PIMC_DISC_TRAPEZOID;
@@ -407,19 +410,43 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
 // warps have drawn the next sweep's proposals already, and the halo copies of a site do not see all of its decisions), so the
 // launcher ends every launch at an adjustment sweep -- (t - t_tune + 1) % tune_skip == 0 -- and runs tune_adjust_kernel on the
 // counters the owners kept.  The global-memory engine adjusts inside its kernel; both give the oracle's step sizes bit for bit.
+template <typename R> int accumulate_residuals(pimc_handle* h) {
+    const size_t total = (size_t)h->C * (h->M + 1);
+    const int threads = 256;
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 8);
+    residual_kernel<R><<<blocks, threads, 0, h->stream>>>((const R*)h->lay.x, (const R*)h->lay.g0, (const R*)h->lay.g1, h->lay.cur, (const R*)h->lay.y,
+                                                          h->M, h->D, h->L, h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M, h->disc, h->C,
+                                                          nullptr, nullptr, h->resid_acc);
+    h->launches++;
+    PIMC_CUDA(h, cudaGetLastError());
+    return PIMC_OK;
+}
+
+// A pimc_sweep call is ONE launch unless something has to happen between two sweeps on the host's side of the kernel:
+//  * step-size tuning on the tile-resident engine: every launch ends at an adjustment sweep, tune_adjust_kernel runs in between;
+//  * residual statistics (pimc_set_residual_stats): every launch ends at an accumulated sweep, residual_kernel adds that path's
+//    eps_n, delta_n to the running sums (a diagnostic: one extra launch per sample, nothing added to the sweep kernels).
 template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sweeps, unsigned long long seed, int do_states, int do_params) {
-    if (!(h->site_widths && h->tune) || n_sweeps <= 0) return run_sweeps_once<Model, R>(h, n_sweeps, seed, do_states, do_params);
+    const bool want_tune = h->site_widths && h->tune, want_res = h->resid_acc != nullptr && h->accum;
+    if (!(want_tune || want_res) || n_sweeps <= 0) return run_sweeps_once<Model, R>(h, n_sweeps, seed, do_states, do_params);
     LaunchShape ls;
     int rc = choose_shape<Model, R>(h, &ls);
     if (rc != PIMC_OK) return rc;
-    if (ls.engine != PIMC_ENGINE_TILE) return run_sweeps_once<Model, R>(h, n_sweeps, seed, do_states, do_params);
+    const bool split_tune = want_tune && ls.engine == PIMC_ENGINE_TILE;
+    if (!split_tune && !want_res) return run_sweeps_once<Model, R>(h, n_sweeps, seed, do_states, do_params);
     long long left = n_sweeps;
     while (left > 0) {
-        const unsigned long long to_adjust = h->tune_skip - (h->t - h->t_tune) % h->tune_skip;   // up to and including the adjustment sweep
-        const long long n = (unsigned long long)left < to_adjust ? left : (long long)to_adjust;
+        unsigned long long to_adjust = ~0ull, to_acc = ~0ull;
+        if (split_tune) to_adjust = h->tune_skip - (h->t - h->t_tune) % h->tune_skip;   // up to and including the adjustment sweep
+        if (want_res) {                                                                // up to and including the next accumulated sweep
+            const unsigned long long r = (h->t - h->t_enable) % h->n_skip;
+            to_acc = (r == 0 ? 0ull : h->n_skip - r) + 1ull;
+        }
+        const unsigned long long stop = std::min(to_adjust, to_acc);
+        const long long n = (unsigned long long)left < stop ? left : (long long)stop;
         rc = run_sweeps_once<Model, R>(h, n, seed, do_states, do_params);
         if (rc != PIMC_OK) return rc;
-        if ((unsigned long long)n == to_adjust) {
+        if (split_tune && (unsigned long long)n == to_adjust) {
             const size_t nx = (size_t)h->C * (h->M + 1) * h->D, np = (size_t)h->C * h->Np;
             const int threads = 256;
             const int blocks = (int)std::min<size_t>((nx + np + threads - 1) / threads, (size_t)h->sm_count * 8);
@@ -427,6 +454,10 @@ template <class Model, typename R> int run_sweeps(pimc_handle* h, long long n_sw
                                                                    (double)h->tune_skip, h->f_acc, h->alpha);
             PIMC_CUDA(h, cudaGetLastError());
             h->launches++;
+        }
+        if (want_res && (unsigned long long)n == to_acc) {
+            rc = accumulate_residuals<R>(h);
+            if (rc != PIMC_OK) return rc;
         }
         left -= n;
     }
@@ -752,6 +783,7 @@ int pimc_reset_moments(pimc_handle* h) {
         PIMC_CUDA(h, cudaMemsetAsync(h->lay.S2p, 0, sizeof(double) * np, h->stream));
     }
     if (h->n_sel) PIMC_CUDA(h, cudaMemsetAsync(h->lay.hist, 0, sizeof(unsigned long long) * (size_t)h->C * h->n_sel * (h->nbins + 2), h->stream));
+    if (h->resid_acc) PIMC_CUDA(h, cudaMemsetAsync(h->resid_acc, 0, sizeof(double) * (size_t)h->C * (2 * (size_t)h->M * h->D + 2 * (size_t)(h->M + 1) * h->L), h->stream));
     h->n_samples = 0;
     h->t_enable = h->t;
     return recentre(h);
@@ -872,6 +904,55 @@ int pimc_get_engine(pimc_handle* h, int* engine, int* halo) {
     if (rc != PIMC_OK) return rc;
     if (engine) *engine = ls.engine;
     if (halo) *halo = ls.h;
+    return PIMC_OK;
+}
+
+int pimc_param_trace(pimc_handle* h, void* out, long long capacity) {
+    if (!h) return PIMC_EINVAL;
+    if (out && (capacity < 1 || !aligned32(out))) return fail(h, PIMC_EINVAL, "parameter record needs capacity >= 1 and a 32-byte aligned device pointer");
+    if (out && h->Np == 0) return fail(h, PIMC_EUNSUPPORTED, "the model has no parameters");
+    h->ptrace = out; h->ptrace_cap = out ? capacity : 0;
+    return PIMC_OK;
+}
+
+int pimc_residuals(pimc_handle* h, void* eps_out, void* delta_out) {
+    if (!h) return PIMC_EINVAL;
+    if (!h->have_path) return fail(h, PIMC_ESTATE, "no path set");
+    if (!aligned32(eps_out) || !aligned32(delta_out)) return fail(h, PIMC_EINVAL, "outputs must be 32-byte aligned device pointers");
+    const size_t total = (size_t)h->C * (h->M + 1);
+    const int threads = 256;
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 8);
+    const int nc = h->disc == PIMC_DISC_TRAPEZOID ? h->M + 1 : h->M;
+    if (h->dtype == 64)
+        residual_kernel<double><<<blocks, threads, 0, h->stream>>>((const double*)h->lay.x, (const double*)h->lay.g0, (const double*)h->lay.g1, h->lay.cur,
+                                                                   (const double*)h->lay.y, h->M, h->D, h->L, nc, h->disc, h->C, (double*)eps_out, (double*)delta_out, nullptr);
+    else
+        residual_kernel<float><<<blocks, threads, 0, h->stream>>>((const float*)h->lay.x, (const float*)h->lay.g0, (const float*)h->lay.g1, h->lay.cur,
+                                                                  (const float*)h->lay.y, h->M, h->D, h->L, nc, h->disc, h->C, (float*)eps_out, (float*)delta_out, nullptr);
+    h->launches++;
+    PIMC_CUDA(h, cudaGetLastError());
+    return PIMC_OK;
+}
+
+int pimc_set_residual_stats(pimc_handle* h, double* acc) {
+    if (!h) return PIMC_EINVAL;
+    if (!aligned32(acc)) return fail(h, PIMC_EINVAL, "acc must be a 32-byte aligned device pointer");
+    h->resid_acc = acc;
+    if (acc) PIMC_CUDA(h, cudaMemsetAsync(acc, 0, sizeof(double) * (size_t)h->C * (2 * (size_t)h->M * h->D + 2 * (size_t)(h->M + 1) * h->L), h->stream));
+    return PIMC_OK;
+}
+
+int pimc_residual_stats(pimc_handle* h, double* out) {
+    if (!h || !out) return fail(h, PIMC_EINVAL, "null argument");
+    if (!h->resid_acc) return fail(h, PIMC_ESTATE, "residual statistics are not enabled");
+    if (!aligned32(out)) return fail(h, PIMC_EINVAL, "out must be a 32-byte aligned device pointer");
+    const size_t ne = (size_t)h->M * h->D, nd = (size_t)(h->M + 1) * h->L;
+    const size_t total = (size_t)h->C * (ne + nd);
+    const int threads = 256;
+    const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 8);
+    residual_stats_kernel<<<blocks, threads, 0, h->stream>>>(h->resid_acc, ne, nd, h->C, (double)h->n_samples, out);
+    h->launches++;
+    PIMC_CUDA(h, cudaGetLastError());
     return PIMC_OK;
 }
 

@@ -84,6 +84,10 @@ template <typename R> struct SweepArgs {
     unsigned long long* hx_epoch;   // (C) halo exchanges performed so far
     unsigned long long* ar_words;   // (2 slots, kTileMaxCtas, kArSlotWords) Delta-A partials, one 128-byte line per CTA
     int* fault;                     // set to 1 if a hand-off was never delivered
+    // optional record of the parameters at every accumulated sweep (pimc_param_trace; Fig. 4)
+    R* ptrace;                      // (C, ptrace_cap, Np) or nullptr
+    long long ptrace_cap;
+    unsigned long long ptrace_n0;   // records written before this launch (= samples accumulated so far)
     int ar_hold;                    // SM clock ticks between publishing a Delta-A partial and the first poll of the others' (pimc_set_exchange)
 };
 
@@ -393,6 +397,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
 #pragma unroll
     for (int c = 0; c < D; ++c) n_acc_comp[c] = 0;
     unsigned long long ar_count = a.ar_epoch[chain];   // all-reduce events this chain has performed so far
+    unsigned long long n_rec = 0;                      // sweeps accumulated by this launch so far
 
     for (long long i = 0; i < a.n_sweeps; ++i) {
         const unsigned long long t = a.t0 + (unsigned long long)i;
@@ -594,7 +599,10 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                 const double d = (double)ps[tid] - a.cp[gi];
                 a.S1p[gi] += d;
                 a.S2p[gi] += d * d;
+                const unsigned long long rec = a.ptrace_n0 + n_rec;
+                if (a.ptrace && rec < (unsigned long long)a.ptrace_cap) a.ptrace[((size_t)chain * a.ptrace_cap + rec) * NP + tid] = ps[tid];
             }
+            n_rec += 1ull;
             for (int sel = tid; sel < a.n_sel; sel += T) {
                 const int site = a.hsite[sel], comp = a.hcomp[sel];
                 const bool mine = site < 0 ? (b == 0) : (site >= s && site < e);
@@ -776,6 +784,58 @@ static __global__ void moments_kernel(const double* __restrict__ cx, const doubl
         const double m1 = N > 0.0 ? s1 / N : 0.0;
         out[o_mean] = c + m1;
         out[o_var] = N > 0.0 ? s2 / N - m1 * m1 : 0.0;
+    }
+}
+
+// ---- model errors eps_n and observation errors delta_n of the current path ------------------------------------
+// eps_{n,a} = (x_{n+1,a} - x_{n,a}) - g_{n,a} (trapezoid: ... - c_n - c_{n+1}), n < M; delta_{n,l} = y_{n,l} - x_{n,l}, n >= 1, delta_0 = 0:
+// the terms of the action as the sweep kernels form them.  Writes them out (eps_out / delta_out, either may be null) and/or adds
+// them and their squares to the running sums acc = per chain [E1 (M,D), E2 (M,D), D1 (M+1,L), D2 (M+1,L)] (no FMA contraction:
+// the sums are the oracle's bit for bit when the residuals are).
+template <typename R>
+__global__ void residual_kernel(const R* __restrict__ x, const R* __restrict__ g0, const R* __restrict__ g1, const int* __restrict__ cur,
+                                const R* __restrict__ y, int M, int D, int L, int nc, int disc, int n_chains,
+                                R* __restrict__ eps_out, R* __restrict__ delta_out, double* __restrict__ acc) {
+    const size_t per_chain = (size_t)(M + 1);
+    const size_t ne = (size_t)M * D, nd = (size_t)(M + 1) * L;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (size_t)n_chains * per_chain; idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t chain = idx / per_chain;
+        const int n = (int)(idx % per_chain);
+        const R* xc = x + chain * per_chain * D;
+        const R* gc = (cur[chain] ? g1 : g0) + chain * (size_t)nc * D;
+        double* a_c = acc ? acc + chain * (2 * ne + 2 * nd) : nullptr;
+        if (n < M) {
+            for (int a = 0; a < D; ++a) {
+                R r = (xc[(size_t)(n + 1) * D + a] - xc[(size_t)n * D + a]) - gc[(size_t)n * D + a];
+                if (disc == 1) r -= gc[(size_t)(n + 1) * D + a];
+                if (eps_out) eps_out[chain * ne + (size_t)n * D + a] = r;
+                if (a_c) {
+                    const double rd = (double)r;
+                    a_c[(size_t)n * D + a] = __dadd_rn(a_c[(size_t)n * D + a], rd);
+                    a_c[ne + (size_t)n * D + a] = __dadd_rn(a_c[ne + (size_t)n * D + a], __dmul_rn(rd, rd));
+                }
+            }
+        }
+        for (int l = 0; l < L; ++l) {
+            const R d = n >= 1 ? y[(chain * per_chain + n) * L + l] - xc[(size_t)n * D + l] : R(0);
+            if (delta_out) delta_out[chain * nd + (size_t)n * L + l] = d;
+            if (a_c) {
+                const double dd = (double)d;
+                a_c[2 * ne + (size_t)n * L + l] = __dadd_rn(a_c[2 * ne + (size_t)n * L + l], dd);
+                a_c[2 * ne + nd + (size_t)n * L + l] = __dadd_rn(a_c[2 * ne + nd + (size_t)n * L + l], __dmul_rn(dd, dd));
+            }
+        }
+    }
+}
+// read-out of the running residual sums: mean = S1/N, var = S2/N - mean^2, same layout as acc
+static __global__ void residual_stats_kernel(const double* __restrict__ acc, size_t ne, size_t nd, int n_chains, double N, double* __restrict__ out) {
+    const size_t per = 2 * ne + 2 * nd;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (size_t)n_chains * (ne + nd); idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t chain = idx / (ne + nd), r = idx % (ne + nd);
+        const size_t o1 = r < ne ? r : 2 * ne + (r - ne), o2 = r < ne ? ne + r : 2 * ne + nd + (r - ne);
+        const double m = N > 0.0 ? acc[chain * per + o1] / N : 0.0;
+        out[chain * per + o1] = m;
+        out[chain * per + o2] = N > 0.0 ? acc[chain * per + o2] / N - m * m : 0.0;
     }
 }
 

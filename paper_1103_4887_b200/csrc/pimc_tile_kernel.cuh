@@ -283,6 +283,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
 
     unsigned long long ar_count = a.ar_epoch[chain];
     unsigned long long hx_count = a.hx_epoch[chain];
+    unsigned long long n_rec = 0;                  // sweeps accumulated by this launch so far
     unsigned long long skip_ctr = a.skip0;         // (t - t_enable) mod n_skip, kept as a counter (no 64-bit division in the loop)
     unsigned int n_acc_state = 0, n_acc_c[D], pacc[NP], pprop[NP];
 #pragma unroll
@@ -685,7 +686,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 const double d = pv - sm.pcc[tid];
                 sm.pS1[tid] += d;
                 sm.pS2[tid] += d * d;
+                const unsigned long long rec = a.ptrace_n0 + n_rec;       // optional record of the parameters (pimc_param_trace)
+                if (a.ptrace && b == 0 && rec < (unsigned long long)a.ptrace_cap) a.ptrace[((size_t)chain * a.ptrace_cap + rec) * NP + tid] = (R)pv;
             }
+            n_rec += 1ull;
             if (a.n_sel > 0) {
                 for (int sel = tid; sel < a.n_sel; sel += T) {
                     const int site = a.hsite[sel], comp = a.hcomp[sel];
