@@ -40,12 +40,14 @@ W_EVAL_ORACLE = 666.0
 #     flatter.  The kernels execute FEWER operations than (1) (one shared exponential per RK4 stage instead of three tanh, one
 #     reciprocal series instead of two divides per gate, cached first-stage gate rates in parameter moves), so the useful
 #     fraction credits min((1), (2) / redundancy).
-EXEC_FP64 = {   # (model family, dtype, discretisation) -> (per owned site update, per owned parameter-move evaluation)
-    ("hh", 64, "rk4"): (596.5, 304.6),
+EXEC_FP64_COMPUTED = {   # engine -> (per COMPUTED site update, per COMPUTED parameter-move evaluation); HH tanh kinetics, fp64, RK4 map, joint updates
+    "tile": (519.9, 268.2),      # tile_sweep_kernel, profiles/r02_work_counts.md: 594.8 and 306.8 per OWNED unit at cfg3 / (254 / 222)
+    "global": (521.0, 339.0),    # sweep_kernel (one CTA per chain, no halos, no stage-1 cache), profiles/r02_cfg4.md: launch total minus
+                                 # 521 per site update, over the evaluations
 }
-HALO_REDUNDANCY_CFG3 = 254.0 / 222.0            # computed / owned sites per tile at the cfg3 launch (h = 16 halo sites each side)
-# ncu sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed of the same kernels, same launches (profiles/r02_*.md)
-NCU_PIPE_FP64_ACTIVE = {"full_sweep": 0.300, "a2_only": 0.437, "a4_only": 0.265, "source": "profiles/r02_work_counts.md"}
+# ncu sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed of the same kernels, same launches
+NCU_PIPE_FP64_ACTIVE = {3: {"full_sweep": 0.302, "a2_only": 0.438, "a4_only": 0.267, "source": "profiles/r02_final.md"},
+                        4: {"full_sweep": 0.509, "source": "profiles/r02_cfg4.md"}}
 # trapezoid discretisation / component-wise updates: estimated slots (no oracle count yet), used for the non-headline variants only
 W_SITE_SLOTS_TRAP = 380.0
 W_SITE_SLOTS_COMP = 2300.0
@@ -55,7 +57,7 @@ FP64_LANES_PER_SM_CLK = 64
 SM_COUNT = 148
 SM_MAX_HZ = 1.965e9
 PEAK_TFLOPS_DERIVED = SM_COUNT * FP64_LANES_PER_SM_CLK * SM_MAX_HZ * 2 / 1e12
-NCU_DRAM_BYTES_PER_LAUNCH = 5999616.0   # cfg3 full sweep launch: 5.930 MB read + 70 KB written (profiles/r02_work_counts.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 5917440.0   # cfg3 full sweep launch: 5.907 MB read + 10 KB written (profiles/r02_work_counts.md)
 
 
 def rank_info():
@@ -249,13 +251,21 @@ def run_ours(args):
         h.set_update_mode(P.UPDATE_COMPONENTWISE)
         w_site = W_SITE_SLOTS_COMP if not trap else 4 * 205.0 + 300.0
     headline = args.config == 3 and args.kinetics == "tanh" and not trap and not comp
-    exec_counts = EXEC_FP64.get(("hh", args.dtype, args.disc)) if headline else None
     peak_tflops = PEAK_TFLOPS_DERIVED * (1.0 if args.dtype == 64 else 2.0)   # fp32: 128 FP32 lanes/clk/SM
     if args.exchange_hold is not None:
         h.set_exchange(args.exchange_hold)
     h.set_accum(True, 1)
     h.reset_moments()
     shape = h.get_launch()
+    eng = h.get_engine()
+    # executed-instruction counts exist for the HH tanh / fp64 / RK4-map / joint-update kernels; redundancy = computed / owned sites
+    # of an interior tile (tile-resident engine with more than one tile per chain: h halo sites on each side are updated redundantly)
+    exec_counts, red = None, None
+    if w.model == 1 and args.dtype == 64 and not trap and not comp:
+        tile_engine = eng["engine"] == P.ENGINE_TILE
+        red = (shape["tile_sites"] + 2.0 * eng["halo"]) / shape["tile_sites"] if (tile_engine and shape["ctas_per_chain"] > 1) else 1.0
+        per = EXEC_FP64_COMPUTED["tile" if tile_engine else "global"]
+        exec_counts = (per[0] * red, per[1] * red)
     units_per_step = float(w.n_chains) * (w.M + 1) * S
     n_active = int(np.count_nonzero(w.w_param))
     evals_per_step = float(w.n_chains) * w.M * S * n_active
@@ -314,12 +324,11 @@ def run_ours(args):
     oracle_tflops = tfl(units_per_step * w_site + evals_per_step * w_eval, step_s)
     if exec_counts:
         achieved_tflops = tfl(units_per_step * exec_counts[0] + evals_per_step * exec_counts[1], step_s)
-        red = HALO_REDUNDANCY_CFG3
         a2_frac, a4_frac = tfl(a2_rate * exec_counts[0], 1.0) / peak_tflops, tfl(a4_rate * exec_counts[1], 1.0) / peak_tflops
         useful_site, useful_eval = min(w_site, exec_counts[0] / red), min(w_eval, exec_counts[1] / red)
         frac_useful = tfl(units_per_step * useful_site + evals_per_step * useful_eval, step_s) / peak_tflops
     else:           # variants without an ncu count: the (estimated or oracle-counted) work model only
-        achieved_tflops, red = oracle_tflops, None
+        achieved_tflops = oracle_tflops
         a2_frac, a4_frac = tfl(a2_rate * w_site, 1.0) / peak_tflops, tfl(a4_rate * w_eval, 1.0) / peak_tflops
         frac_useful = None
     measured_peak = P.fp64_peak(150) * 2 / 1e12 if rank == 0 else None
@@ -336,8 +345,8 @@ def run_ours(args):
                 "frac_useful": frac_useful,
                 "frac_oracle_work": oracle_tflops / peak_tflops,
                 "halo_redundancy": red,
-                "pipe_fp64_active_ncu": NCU_PIPE_FP64_ACTIVE if exec_counts else None,
-                "target": "north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2), judged on pipe_fp64_active_ncu.a2_only: NOT reached",
+                "pipe_fp64_active_ncu": NCU_PIPE_FP64_ACTIVE.get(args.config) if exec_counts else None,
+                "target": "north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2) of config 3, judged on pipe_fp64_active_ncu.a2_only (43.8 %): NOT reached",
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (headline and args.dtype == 64) else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r02_work_counts.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
