@@ -52,7 +52,7 @@ struct Carve {   // bump allocator over the caller's workspace; also used to siz
 };
 
 struct Layout {
-    void *x, *g0, *g1, *y, *I, *p;
+    void *x, *g0, *g1, *y, *I, *p, *kg;
     int* cur;
     double *lo, *hi, *cx, *S1x, *S2x, *cp, *S1p, *S2p;
     unsigned long long* counters;
@@ -79,6 +79,7 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     o.x = c.take<char>(nx * es);
     o.g0 = c.take<char>(ng * es);
     o.g1 = c.take<char>(ng * es);
+    o.kg = c.take<char>((size_t)C * (M + 1) * 3 * es);          // first-stage gate rates (NK <= 3 values per site)
     o.y = c.take<char>((size_t)C * (M + 1) * (L > 0 ? L : 1) * es);
     o.I = c.take<char>((size_t)C * (M + 1) * es);
     o.p = c.take<char>((size_t)C * Np * es);
@@ -148,6 +149,7 @@ struct pimc_handle {
     int G_user = 0, T_user = 0, engine_user = PIMC_ENGINE_AUTO, halo_user = -1;
     unsigned long long hs_base = 0, launches = 0;
     int ar_hold = 450;                // pimc_set_exchange
+    bool kg_valid = false;            // the global first-stage gate-rate array matches the path (GLOBAL engine keeps it current, TILE does not)
     void* ptrace = nullptr; long long ptrace_cap = 0;      // pimc_param_trace
     double* resid_acc = nullptr;                           // pimc_set_residual_stats
     int sm_count = 0;
@@ -318,10 +320,11 @@ template <class Model, typename R> int rebuild_cache(pimc_handle* h) {
     const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 16);
     // after a rebuild, buffer 0 is current
     build_cache_kernel<Model, R><<<blocks, threads, 0, h->stream>>>((const R*)h->lay.x, h->have_I ? (const R*)h->lay.I : nullptr,
-                                                                     (const R*)h->lay.p, (R*)h->lay.g0, h->M, h->C, (R)h->dt, h->disc);
+                                                                     (const R*)h->lay.p, (R*)h->lay.g0, h->M, h->C, (R)h->dt, h->disc, (R*)h->lay.kg);
     h->launches++;
     PIMC_CUDA(h, cudaGetLastError());
     PIMC_CUDA(h, cudaMemsetAsync(h->lay.cur, 0, sizeof(int) * h->C, h->stream));
+    h->kg_valid = h->disc == PIMC_DISC_RK4MAP;
     return PIMC_OK;
 }
 
@@ -344,7 +347,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
     a.dt = (R)h->dt; a.Rm = (R)h->Rm;
     for (int c = 0; c < h->D; ++c) { a.Rf[c] = (R)h->Rf[c]; a.wx[c] = (R)h->wx[c]; }
     for (int l = 0; l < h->Np; ++l) a.wp[l] = h->wp[l];
-    a.x = (R*)h->lay.x; a.g[0] = (R*)h->lay.g0; a.g[1] = (R*)h->lay.g1;
+    a.x = (R*)h->lay.x; a.g[0] = (R*)h->lay.g0; a.g[1] = (R*)h->lay.g1; a.kg = (R*)h->lay.kg;
     a.y = (const R*)h->lay.y; a.I = h->have_I ? (const R*)h->lay.I : nullptr;
     a.p = (R*)h->lay.p; a.cur = h->lay.cur; a.lo = h->lay.lo; a.hi = h->lay.hi;
     a.accum = h->accum; a.n_skip = h->n_skip; a.t_enable = h->t_enable; a.skip0 = h->accum ? (h->t - h->t_enable) % h->n_skip : 0ull;
@@ -390,6 +393,18 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
             default: return fail(h, PIMC_EUNSUPPORTED, "no 512-thread tile kernel for this discretisation / update mode");   // choose_shape_tile never offers it
         }
 #undef PIMC_TILE
+    }
+    if constexpr (Model::NK > 0) {
+        if (ls.engine == PIMC_ENGINE_GLOBAL && !trap && !h->kg_valid) {      // the previous launches ran tile-resident: refresh the stage-1 rates
+            const size_t total = (size_t)h->C * h->M;
+            const int threads = 128;
+            const int blocks = (int)std::min<size_t>((total + threads - 1) / threads, (size_t)h->sm_count * 16);
+            build_stage1_kernel<Model, R><<<blocks, threads, 0, h->stream>>>((const R*)h->lay.x, h->M, h->C, (R*)h->lay.kg);
+            h->launches++;
+            PIMC_CUDA(h, cudaGetLastError());
+            h->kg_valid = true;
+        }
+        if (ls.engine == PIMC_ENGINE_TILE && do_states) h->kg_valid = false;
     }
     if (ls.smem > 48 * 1024) PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
     void* params[] = {&a};

@@ -50,6 +50,8 @@ template <typename R> struct SweepArgs {
     // device state (per chain, chains concatenated)
     R* x;                 // (C, M+1, D)
     R* g[2];              // (C, nc, D) x 2: step caches (ping-pong)
+    R* kg;                // (C, M, NK): parameter-independent first-stage gate rates of every site (Model::stage1_cache; RK4 map only),
+                          //   kept current by the site updates and reused by the seven parameter moves of a sweep (GLOBAL engine)
     const R* y;           // (C, M+1, L)
     const R* I;           // (C, M+1) or nullptr
     R* p;                 // (C, Np)
@@ -237,8 +239,10 @@ template <class Model, typename R, bool CG = true>
 __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* __restrict__ prm, unsigned long long t,
                                             uint32_t chain, int n, R* __restrict__ x, R* __restrict__ g, const R* __restrict__ y,
                                             const R* __restrict__ I, bool trace, size_t chain_site0, const R* __restrict__ Rfs,
-                                            const typename Model::Prep& prep) {
+                                            const typename Model::Prep& prep, R* __restrict__ kg) {
     constexpr int D = Model::D;
+    constexpr int NK = Model::NK;
+    R kgn[NK > 0 ? NK : 1];
     const int M = a.M;
     R xn[D], xfull[D], xp[D], gp[D];
     load_vec<R, D, CG>(x, n, xn);
@@ -314,7 +318,7 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
         load_vec<R, D, CG>(x, n + 1, xq);
         load_vec<R, D, CG>(g, n, gn);
         const R I0 = I ? __ldg(I + n) : R(0), I1 = I ? __ldg(I + n + 1) : R(0);
-        Model::increment(xp, prm, prep, I0, I1, a.dt, gp);
+        Model::template increment_k<false, (NK > 0)>(xp, prm, prep, I0, I1, a.dt, gp, nullptr, kgn);
 #pragma unroll
         for (int c = 0; c < D; ++c) {   // model-error term n -> n+1
             const R r_new = (xq[c] - xp[c]) - gp[c];
@@ -329,6 +333,12 @@ __device__ __forceinline__ unsigned update_site(const SweepArgs<R>& a, const R* 
     if (accept) {
         store_vec<R, D>(x, n, xp);
         if (n < a.nc) store_vec<R, D>(g, n, gp);
+        if constexpr (NK > 0) {
+            if (a.disc == 0 && n < a.M) {
+#pragma unroll
+                for (int c = 0; c < NK; ++c) kg[(size_t)n * NK + c] = kgn[c];
+            }
+        }
 #pragma unroll
         for (int c = 0; c < D; ++c) xn[c] = xp[c];
         accepted_mask |= a.update_mode == 1 ? (1u << ai) : ((1u << D) - 1u);
@@ -383,6 +393,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
     R* const g_b = a.g[1] + (size_t)chain * a.nc * D;
     const R* y = a.y + site0 * a.L;
     const R* I = a.I ? a.I + site0 : nullptr;
+    R* const kgc = a.kg + (size_t)chain * M * (Model::NK > 0 ? Model::NK : 1);
     unsigned long long* hs_flag = a.hs_flag + (size_t)chain * G;
 
     if (tid < NP) {
@@ -431,7 +442,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                             prefetch_l1(gq + (size_t)(np - 1) * D); prefetch_l1(gq + (size_t)min(np, a.nc - 1) * D);
                         }
                     }
-                    const unsigned mask = update_site<Model, R, CG>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0, Rfs, prep);
+                    const unsigned mask = update_site<Model, R, CG>(a, ps, t, chain, n, x, cur ? g_b : g_a, y, I, trace, site0, Rfs, prep, kgc);
 #pragma unroll
                     for (int c = 0; c < D; ++c) n_acc_comp[c] += (mask >> c) & 1u;
                     if (a.ws && a.tune) {        // N_acc,i of the tuning rule: this thread is the only writer of its site
@@ -504,14 +515,20 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
                     for (int n = s + tid; n < e_fwd; n += T) {
                         if constexpr (SOLO) {    // x_{n'+1} is the next lane's x_{n'}: one prefetch per array covers the warp's lines
                             const int np = n + T;
-                            if (np < e_fwd) { prefetch_l1(x + (size_t)np * D); prefetch_l1(gcur + (size_t)np * D); if (I) prefetch_l1(I + np); }
+                            if (np < e_fwd) { prefetch_l1(x + (size_t)np * D); prefetch_l1(gcur + (size_t)np * D); prefetch_l1(kgc + (size_t)np * Model::NK); if (I) prefetch_l1(I + np); }
                         }
                         R xn[D], xq[D], gn[D], gp[D];
                         load_vec<R, D, CG>(x, n, xn);
                         load_vec<R, D, CG>(x, n + 1, xq);
                         load_vec<R, D, CG>(gcur, n, gn);
                         const R I0 = I ? __ldg(I + n) : R(0), I1 = I ? __ldg(I + n + 1) : R(0);
-                        Model::increment(xn, ps_prop, pq, I0, I1, a.dt, gp);
+                        constexpr int NK = Model::NK;
+                        R kk[NK > 0 ? NK : 1];
+                        if constexpr (NK > 0) {
+#pragma unroll
+                            for (int c = 0; c < NK; ++c) kk[c] = CG ? __ldcg(kgc + (size_t)n * NK + c) : kgc[(size_t)n * NK + c];
+                        }
+                        Model::template increment_k<(NK > 0), false>(xn, ps_prop, pq, I0, I1, a.dt, gp, kk, nullptr);
                         store_vec<R, D>(galt, n, gp);
                         R acc = R(0);
 #pragma unroll
@@ -677,7 +694,7 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
 // ---- A0: (re)build the step cache of every chain ---------------------------------------------------------
 template <class Model, typename R>
 __global__ void build_cache_kernel(const R* __restrict__ x, const R* __restrict__ I, const R* __restrict__ p, R* __restrict__ g,
-                                   int M, int n_chains, R dt, int disc) {
+                                   int M, int n_chains, R dt, int disc, R* __restrict__ kg) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
     const int nc = disc == 1 ? M + 1 : M;          // entries per chain
@@ -691,9 +708,38 @@ __global__ void build_cache_kernel(const R* __restrict__ x, const R* __restrict_
         for (int c = 0; c < D; ++c) xn[c] = x[(chain * (M + 1) + n) * D + c];
         const R I0 = I ? I[chain * (M + 1) + n] : R(0), I1 = (I && n < M) ? I[chain * (M + 1) + n + 1] : R(0);
         if (disc == 1) Model::half_rhs(xn, prm, Model::prepare(prm, dt), I0, gn);
-        else Model::increment(xn, prm, I0, I1, dt, gn);
+        else {
+            constexpr int NK = Model::NK;
+            R kk[NK > 0 ? NK : 1];
+            Model::template increment_k<false, (NK > 0)>(xn, prm, Model::prepare(prm, dt), I0, I1, dt, gn, nullptr, kk);
+            if constexpr (NK > 0) {
+#pragma unroll
+                for (int c = 0; c < NK; ++c) kg[(chain * M + n) * NK + c] = kk[c];
+            }
+        }
 #pragma unroll
         for (int c = 0; c < D; ++c) g[(chain * nc + n) * D + c] = gn[c];
+    }
+}
+
+// ---- first-stage gate rates of every site from the current path (after launches of the tile-resident engine, which keeps its own copy
+// in shared memory and does not write this array back) ----
+template <class Model, typename R>
+__global__ void build_stage1_kernel(const R* __restrict__ x, int M, int n_chains, R* __restrict__ kg) {
+    constexpr int D = Model::D;
+    constexpr int NK = Model::NK;
+    if constexpr (NK > 0) {
+        const size_t total = (size_t)n_chains * M;
+        for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+            const size_t chain = idx / M;
+            const int n = (int)(idx % M);
+            R xn[D], kk[NK];
+#pragma unroll
+            for (int c = 0; c < D; ++c) xn[c] = x[(chain * (M + 1) + n) * D + c];
+            Model::stage1_cache(xn, kk);
+#pragma unroll
+            for (int c = 0; c < NK; ++c) kg[idx * NK + c] = kk[c];
+        }
     }
 }
 
