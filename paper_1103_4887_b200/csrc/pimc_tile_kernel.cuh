@@ -110,6 +110,9 @@ template <typename R> struct TileSmem {
     double *blo, *bhi;          // [kMaxNp] bounds
     double *pS1, *pS2, *pcc;    // [kMaxNp] running moments of the parameters (tile 0 of each chain)
     R *xs, *g0, *g1;            // [2*D*P]
+    double *s_pl;               // [kMaxNp] this sweep's proposed parameter values p'_l = p_l + step_l (posted once per sweep)
+    int *s_in;                  // [kMaxNp] 0 = frozen, 1 = proposal out of bounds (rejected unevaluated), 2 = to be evaluated
+    unsigned int *s_pacc, *s_pprop;   // [kMaxNp] accepted / proposed parameter moves of this launch
     R *wsx;                     // [2*D*P] step sizes of every tile site (tuned per (site, component), else the uniform widths)
     double *wpl;                // [kMaxNp] parameter step sizes in use
     R *kg;                      // [2*NK*P] parameter-independent first-stage rates of every tile site (Model::stage1_cache)
@@ -124,7 +127,7 @@ __host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512)
 
 template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK, int npass) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
-    size_t dbl = 3 * 2 * D * P + kMaxNp + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2;
+    size_t dbl = 3 * 2 * D * P + kMaxNp + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2 + kMaxNp + 3 * kMaxNp / 2;
     const size_t RP = P - 2;
     size_t real = 4 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * (size_t)npass * RP * D + 4 * (size_t)npass * RP;
     (void)TC;
@@ -148,6 +151,10 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.pS2 = d; d += kMaxNp;
     m.pcc = d; d += kMaxNp;
     m.cnt = reinterpret_cast<unsigned int*>(d); d += 2;      // 2 doubles = 4 counters
+    m.s_pl = d; d += kMaxNp;
+    m.s_in = reinterpret_cast<int*>(d); d += kMaxNp / 2;
+    m.s_pacc = reinterpret_cast<unsigned int*>(d); d += kMaxNp / 2;
+    m.s_pprop = reinterpret_cast<unsigned int*>(d); d += kMaxNp / 2;
     R* r = reinterpret_cast<R*>(d);
     m.xs = r; r += 2 * D * P;
     m.g0 = r; r += 2 * D * P;
@@ -285,11 +292,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     unsigned long long hx_count = a.hx_epoch[chain];
     unsigned long long n_rec = 0;                  // sweeps accumulated by this launch so far
     unsigned long long skip_ctr = a.skip0;         // (t - t_enable) mod n_skip, kept as a counter (no 64-bit division in the loop)
-    unsigned int n_acc_state = 0, n_acc_c[D], pacc[NP], pprop[NP];
+    unsigned int n_acc_state = 0, n_acc_c[D];
 #pragma unroll
     for (int c = 0; c < D; ++c) n_acc_c[c] = 0;
-#pragma unroll
-    for (int k = 0; k < NP; ++k) { pacc[k] = 0; pprop[k] = 0; }
+    if (tid < NP) { sm.s_pacc[tid] = 0u; sm.s_pprop[tid] = 0u; }      // parameter-move counters live in shared memory (thread 0 counts)
 
     // ---- producers: fill RNG set `set` for sweep t ----
     auto produce = [&](int set, unsigned long long t) {
@@ -492,6 +498,21 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             if (i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull);
         }
         if (a.do_states) k_phase += 2;               // every thread keeps the count: the hand-off below is CTA-uniform
+        // The proposals of this sweep's parameter moves, p'_l = p_l + step_l, do not depend on the decisions of the other parameters:
+        // threads 0..NP-1 post them and the bounds verdicts once, so that a move starts with three independent shared-memory reads
+        // instead of a register-array select chain, an add and two compares on its critical path.
+        if (a.do_params && tid < NP) {
+            R pcur = R(0);
+#pragma unroll
+            for (int k = 0; k < NP; ++k) pcur = (k == tid) ? prm[k] : pcur;
+            const bool live = sm.wpl[tid] > 0.0;
+            const double step = live ? sm.pdraw[(set * kMaxNp + tid) * 2 + 0] : 0.0;
+            double pl;
+            if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)pcur, step);
+            else pl = (double)__fadd_rn(pcur, (float)step);
+            sm.s_pl[tid] = pl;
+            sm.s_in[tid] = !live ? 0 : ((pl >= sm.blo[tid] && pl <= sm.bhi[tid]) ? 2 : 1);
+        }
         __syncthreads();
 
         // ---------------- A4: parameter moves, in sequence; one tile site per thread ----------------
@@ -502,15 +523,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             bool params_changed = false;
 #pragma unroll 1
             for (int l = 0; l < NP; ++l) {
-                if (!(sm.wpl[l] > 0.0)) continue;
-                const double step = sm.pdraw[(set * kMaxNp + l) * 2 + 0], logu = sm.pdraw[(set * kMaxNp + l) * 2 + 1];
-                R pcur = R(0);
-#pragma unroll
-                for (int k = 0; k < NP; ++k) pcur = (k == l) ? prm[k] : pcur;
-                double pl;
-                if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)pcur, step);
-                else pl = (double)__fadd_rn(pcur, (float)step);
-                const bool inside = pl >= sm.blo[l] && pl <= sm.bhi[l];
+                const int st = sm.s_in[l];
+                if (st == 0) continue;
+                const double pl = sm.s_pl[l], logu = sm.pdraw[(set * kMaxNp + l) * 2 + 1];
+                const bool inside = st == 2;
                 bool accept = false;
                 double dA = __longlong_as_double(0x7FF8000000000000ll);
                 if (inside) {
@@ -592,12 +608,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     params_changed = params_changed || accept;
                 }
 #pragma unroll
-                for (int k = 0; k < NP; ++k) {
-                    if (k == l) {
-                        pprop[k] += 1;
-                        if (accept) { prm[k] = (R)pl; pacc[k] += 1; }
-                    }
-                }
+                for (int k = 0; k < NP; ++k) prm[k] = (k == l && accept) ? (R)pl : prm[k];
+                if (tid == 0) { sm.s_pprop[l] += 1u; if (accept) sm.s_pacc[l] += 1u; }
                 if (trace && b == 0 && tid == 0) {
                     if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)dA;
                     if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = accept ? 1 : 0;
@@ -755,10 +767,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         if (b == 0) {
 #pragma unroll
             for (int l = 0; l < NP; ++l) {
-                cnt[D + l] += pacc[l];
-                cnt[(D + NP) + D + l] += pprop[l];
+                cnt[D + l] += sm.s_pacc[l];
+                cnt[(D + NP) + D + l] += sm.s_pprop[l];
                 a.p[(size_t)chain * NP + l] = prm[l];
-                if constexpr (TR) { if (a.tune) a.nacc_p[(size_t)chain * NP + l] += pacc[l]; }
+                if constexpr (TR) { if (a.tune) a.nacc_p[(size_t)chain * NP + l] += sm.s_pacc[l]; }
             }
             a.cur[chain] = cur;
             a.ar_epoch[chain] = ar_count;
