@@ -41,13 +41,13 @@ W_EVAL_ORACLE = 666.0
 #     reciprocal series instead of two divides per gate, cached first-stage gate rates in parameter moves), so the useful
 #     fraction credits min((1), (2) / redundancy).
 EXEC_FP64_COMPUTED = {   # engine -> (per COMPUTED site update, per COMPUTED parameter-move evaluation); HH tanh kinetics, fp64, RK4 map, joint updates
-    "tile": (519.9, 268.2),      # tile_sweep_kernel, profiles/r02_work_counts.md: 594.8 and 306.8 per OWNED unit at cfg3 / (254 / 222)
-    "global": (521.0, 339.0),    # sweep_kernel (one CTA per chain, no halos, no stage-1 cache), profiles/r02_cfg4.md: launch total minus
+    "tile": (520.1, 264.9),      # tile_sweep_kernel, profiles/r02_work_counts.md: 595.0 and 303.1 per OWNED unit at cfg3 / (254 / 222)
+    "global": (521.0, 285.0),    # sweep_kernel (one CTA per chain, no halos, stage-1 rates cached in global memory), profiles/r02_cfg4.md: launch total minus
                                  # 521 per site update, over the evaluations
 }
 # ncu sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed of the same kernels, same launches
-NCU_PIPE_FP64_ACTIVE = {3: {"full_sweep": 0.302, "a2_only": 0.438, "a4_only": 0.267, "source": "profiles/r02_final.md"},
-                        4: {"full_sweep": 0.509, "source": "profiles/r02_cfg4.md"}}
+NCU_PIPE_FP64_ACTIVE = {3: {"full_sweep": 0.310, "a2_only": 0.427, "a4_only": 0.274, "source": "profiles/r02_final.md"},
+                        4: {"full_sweep": 0.453, "source": "profiles/r02_cfg4.md"}}
 # trapezoid discretisation / component-wise updates: estimated slots (no oracle count yet), used for the non-headline variants only
 W_SITE_SLOTS_TRAP = 380.0
 W_SITE_SLOTS_COMP = 2300.0
@@ -57,7 +57,7 @@ FP64_LANES_PER_SM_CLK = 64
 SM_COUNT = 148
 SM_MAX_HZ = 1.965e9
 PEAK_TFLOPS_DERIVED = SM_COUNT * FP64_LANES_PER_SM_CLK * SM_MAX_HZ * 2 / 1e12
-NCU_DRAM_BYTES_PER_LAUNCH = 5917440.0   # cfg3 full sweep launch: 5.907 MB read + 10 KB written (profiles/r02_work_counts.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 5918464.0   # cfg3 full sweep launch: 5.904 MB read + 14 KB written (profiles/r02_work_counts.md)
 
 
 def rank_info():
@@ -346,7 +346,7 @@ def run_ours(args):
                 "frac_oracle_work": oracle_tflops / peak_tflops,
                 "halo_redundancy": red,
                 "pipe_fp64_active_ncu": NCU_PIPE_FP64_ACTIVE.get(args.config) if exec_counts else None,
-                "target": "north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2) of config 3, judged on pipe_fp64_active_ncu.a2_only (43.8 %): NOT reached",
+                "target": "north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2) of config 3, judged on pipe_fp64_active_ncu.a2_only (42.7 %): NOT reached",
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (headline and args.dtype == 64) else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r02_work_counts.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
