@@ -521,6 +521,22 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             const bool can_eval = prm_iloc < n_ext && n <= (TRAP ? M : M - 1);
             const bool owned = n >= s && n < e && n <= M - 1;
             bool params_changed = false;
+            // RK4 map: this thread's site, its right neighbour, the first-stage rates and the currents do not change during the parameter
+            // moves, and the current cache entry changes only when THIS thread's own proposal of it is accepted: all of it is read once
+            // per sweep, so a move starts without a shared-memory round trip on its critical path
+            [[maybe_unused]] R hx[D], hq[D], hg[D], hk[NK > 0 ? NK : 1], hI0 = R(0), hI1 = R(0);
+            if constexpr (!TRAP) {
+                if (can_eval) {
+                    lds_site<R, D>(sm.xs, prm_q, prm_j, P, hx);
+#pragma unroll
+                    for (int c = 0; c < NK; ++c) hk[c] = sm.kg[(prm_q * NK + c) * P + prm_j];
+                    hI0 = sm.Is[prm_iloc]; hI1 = sm.Is[prm_iloc + 1];
+                    if (owned) {
+                        lds_site<R, D>(sm.xs, 1 - prm_q, prm_j + prm_q, P, hq);
+                        lds_site<R, D>(cur ? sm.g1 : sm.g0, prm_q, prm_j, P, hg);
+                    }
+                }
+            }
 #pragma unroll 1
             for (int l = 0; l < NP; ++l) {
                 const int st = sm.s_in[l];
@@ -536,27 +552,25 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     R* gc = cur ? sm.g1 : sm.g0;
                     R* ga = cur ? sm.g0 : sm.g1;
                     double part = 0.0;
+                    [[maybe_unused]] R gp_keep[D];
                     if (can_eval) {
-                        R xn[D], gp[D];
-                        lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
                         if constexpr (TRAP) {
+                            R xn[D], gp[D];
+                            lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
                             Model::half_rhs(xn, pp, Model::prepare_move(prep, pp, a.dt, l), sm.Is[prm_iloc], gp);
                             sts_site<R, D>(ga, prm_q, prm_j, P, gp);
                         } else {
-                            R kk[NK > 0 ? NK : 1];
-#pragma unroll
-                            for (int c = 0; c < NK; ++c) kk[c] = sm.kg[(prm_q * NK + c) * P + prm_j];
-                            Model::template increment_k<(NK > 0), false>(xn, pp, Model::prepare_move(prep, pp, a.dt, l), sm.Is[prm_iloc], sm.Is[prm_iloc + 1], a.dt, gp, kk, nullptr);
+                            R gp[D];
+                            Model::template increment_k<(NK > 0), false>(hx, pp, Model::prepare_move(prep, pp, a.dt, l), hI0, hI1, a.dt, gp, hk, nullptr);
                             sts_site<R, D>(ga, prm_q, prm_j, P, gp);
+#pragma unroll
+                            for (int c = 0; c < D; ++c) gp_keep[c] = gp[c];
                             if (owned) {
-                                R xq[D], gn[D];
-                                lds_site<R, D>(sm.xs, 1 - prm_q, prm_j + prm_q, P, xq);
-                                lds_site<R, D>(gc, prm_q, prm_j, P, gn);
                                 R acc = R(0);
 #pragma unroll
                                 for (int c = 0; c < D; ++c) {
-                                    const R d = xq[c] - xn[c];
-                                    const R r_new = d - gp[c], r_old = d - gn[c];
+                                    const R d = hq[c] - hx[c];
+                                    const R r_new = d - gp[c], r_old = d - hg[c];
                                     acc += R(0.5) * rf(c) * (r_new * r_new - r_old * r_old);
                                 }
                                 part = (double)acc;
@@ -605,6 +619,10 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     }
                     accept = logu < -dA;
                     if (accept) cur ^= 1;
+                    if constexpr (!TRAP) {      // the accepted move's entry is this site's current cache entry from now on
+#pragma unroll
+                        for (int c = 0; c < D; ++c) hg[c] = accept ? gp_keep[c] : hg[c];
+                    }
                     params_changed = params_changed || accept;
                 }
 #pragma unroll
