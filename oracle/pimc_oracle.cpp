@@ -18,7 +18,9 @@
 // host code path; RK4 order-4 convergence; local dA vs brute-force A(X')-A(X) in long
 // double; antisymmetry, telescoping, cache coherence, order independence; the linear
 // model's stationary distribution vs the closed-form Gaussian posterior (banded solve and
-// Kalman/RTS); 1-site textbook Gaussian.  PARITY UNPINNED: the Hodgkin-Huxley posterior
+// Kalman/RTS); 1-site textbook Gaussian; the gate kinetics' widths one and half a width from the
+// midpoint with Table 1's numbers typed from PAPER.md:288-294 (tests/test_oracle_model.py); the
+// fp32-state branches against exact rational arithmetic (tests/test_oracle_fp32_state.py).  PARITY UNPINNED: the Hodgkin-Huxley posterior
 // moments themselves (Table 2 needs the paper's data and 1e6 tuned
 // iterations) -- for HH the chain is pinned only through its parts (model, dA, rule, RNG).
 //
@@ -28,6 +30,10 @@
 //   model 2                classic Hodgkin-Huxley alpha/beta rate functions            tests/test_oracle_classic_hh.py
 //   set_annealing          beta on the dynamics term, Eq. 10          tests/test_oracle_annealing.py
 //   set_tuning             step-size adjustment rule, PAPER.md:224-230                 tests/test_oracle_tuning.py
+//   param_trace            record of the parameters at every accumulated sweep, Fig. 4   tests/test_oracle_diagnostics.py
+//   residuals / residual_stats   model and observation errors eps_n, delta_n, PAPER.md:331             tests/test_oracle_diagnostics.py
+// oracle/count_work.py restates this file's arithmetic on a counting number type (validated bit for bit against it) to count
+// the algorithmic work per unit that bench.py's roofline credits (tests/test_work_model.py).
 #include <cmath>
 #include <cstdint>
 #include <cstring>
