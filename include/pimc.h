@@ -57,8 +57,14 @@ enum { PIMC_PROPOSAL_GAUSSIAN = 0, PIMC_PROPOSAL_UNIFORM = 1 };
  * in global memory (L2), threads stride over the tile, neighbour tiles synchronise every half-sweep with
  * release/acquire flags; any tile length.  TILE: each CTA keeps its tile plus h halo sites in shared memory, one
  * (even, odd) site pair per compute thread, halos updated redundantly and exchanged every h half-sweeps as tagged
- * 8-byte packets; needs tile + 2h <= threads_per_cta <= 512 and L = 1 (one observed component).  AUTO: TILE when it fits, else GLOBAL. */
-enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2 };
+ * 8-byte packets; needs tile + 2h <= threads_per_cta <= 512 and L = 1 (one observed component).
+ * TILE_MC (many chains, PAPER.md:240-242 shared-memory tiles; BASELINE.json config 4 "one CTA-group per chain"): every CTA hosts 2-4
+ * independent groups of 128 threads (threads_per_cta = 256, 384 or 512), each with one (chain, tile) pair of at most 256 sites
+ * incl. halos resident in shared memory, so that one chain's exchange latency is hidden by the other chains' arithmetic; chains
+ * that do not fit at once run in waves (one launch per wave, each running all sweeps of the call).  Hodgkin-Huxley models,
+ * RK4-map discretisation, joint updates, L = 1, uniform step sizes, no debug trace, no annealing; halo default 8.
+ * AUTO: TILE when it fits; else TILE_MC for two or more chains when it fits; else GLOBAL. */
+enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2, PIMC_ENGINE_TILE_MC = 3 };
 /* Discretisation of the model-error term between steps n and n+1, (Rf_a/2) r_a^2:
  *  RK4MAP    (default; BASELINE north_star): r = (x_{n+1} - x_n) - g_n, g_n = the increment of one RK4 step from x_n
  *            (LINEAR: g = A x - x); the cache holds g_n, n = 0..M-1.

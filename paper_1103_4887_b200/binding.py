@@ -9,7 +9,7 @@ import numpy as np
 
 MODEL_LINEAR, MODEL_HH, MODEL_HH_CLASSIC = 0, 1, 2
 PROPOSAL_GAUSSIAN, PROPOSAL_UNIFORM = 0, 1
-ENGINE_AUTO, ENGINE_GLOBAL, ENGINE_TILE = 0, 1, 2
+ENGINE_AUTO, ENGINE_GLOBAL, ENGINE_TILE, ENGINE_TILE_MC = 0, 1, 2, 3
 DISC_RK4MAP, DISC_TRAPEZOID = 0, 1
 UPDATE_JOINT, UPDATE_COMPONENTWISE = 0, 1
 

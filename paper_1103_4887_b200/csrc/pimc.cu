@@ -14,6 +14,7 @@
 
 #include "pimc_kernels.cuh"
 #include "pimc_tile_kernel.cuh"
+#include "pimc_tilemc_kernel.cuh"
 
 using namespace pimc;
 
@@ -62,6 +63,7 @@ struct Layout {
     unsigned long long *hs_flag, *ar_flag, *ar_epoch;
     double* ar_val;
     unsigned long long *hx_words, *hx_epoch, *ar_words;
+    unsigned long long *mc_hx_words, *mc_ar_words;     // mailboxes of the many-chain tile-resident engine
     double *ws, *wpd;                 // tuned step sizes (C, M+1, D), (C, Np)
     unsigned int *nacc_s, *nacc_p;    // accepted changes since the last adjustment
     int* fault;
@@ -106,6 +108,8 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     o.hx_epoch = c.take<unsigned long long>(C);
     o.hx_words = c.take<unsigned long long>((size_t)kTileMaxCtas * 2 * 2 * kHaloWordsPerSide);
     o.ar_words = c.take<unsigned long long>((size_t)2 * kTileMaxCtas * kArSlotWords);
+    o.mc_hx_words = c.take<unsigned long long>((size_t)kMcMaxSlots * 2 * 2 * kHaloWordsPerSide);
+    o.mc_ar_words = c.take<unsigned long long>((size_t)2 * kMcMaxSlots * kArSlotWords);
     o.ws = c.take<double>(nx);
     o.wpd = c.take<double>((size_t)C * Np);
     o.nacc_s = c.take<unsigned int>(nx);
@@ -149,6 +153,7 @@ struct pimc_handle {
     int G_user = 0, T_user = 0, engine_user = PIMC_ENGINE_AUTO, halo_user = -1;
     unsigned long long hs_base = 0, launches = 0;
     int ar_hold = 450;                // pimc_set_exchange
+    unsigned long long mc_tag = 1;    // next unused tag of the many-chain engine's mailboxes (every launch takes a private range)
     bool kg_valid = false;            // the global first-stage gate-rate array matches the path (GLOBAL engine keeps it current, TILE does not)
     void* ptrace = nullptr; long long ptrace_cap = 0;      // pimc_param_trace
     double* resid_acc = nullptr;                           // pimc_set_residual_stats
@@ -188,7 +193,7 @@ int fail(pimc_handle* h, int code, const char* fmt, ...) {
 enum { OP_REBUILD = 0, OP_SWEEP = 1, OP_SHAPE = 2, OP_STEP = 3 };
 }  // namespace
 namespace pimc_shared {
-struct LaunchShape { int G, T, tile; bool cooperative; int engine, h; size_t smem; };
+struct LaunchShape { int G, T, tile; bool cooperative; int engine, h; size_t smem; int cpw, waves; };   // cpw: chains per wave (TILE_MC)
 struct OpArgs {
     int op;
     pimc_handle* h;
@@ -307,10 +312,62 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     return PIMC_OK;
 }
 
+// Many-chain tile-resident engine (pimc_tilemc_kernel.cuh): every CTA hosts NGRP groups of 128 threads, each with one
+// (chain, tile) pair of at most 256 sites incl. halos; chains that do not fit at once run in waves of `cpw` chains.
+template <class Model, typename R> int choose_shape_mc(pimc_handle* h, LaunchShape* out, bool quiet) {
+    auto no = [&](const char* why) { return quiet ? (int)PIMC_EUNSUPPORTED : fail(h, PIMC_EUNSUPPORTED, "many-chain tile engine: %s", why); };
+    if constexpr (!Model::kTileMc) return no("not compiled for this model");
+    else {
+        if (h->L != 1) return no("compiled for one observed component (L = 1)");
+        if (h->disc != PIMC_DISC_RK4MAP || h->update_mode != PIMC_UPDATE_JOINT) return no("RK4-map discretisation with joint updates only");
+        if (h->site_widths) return no("per-site step sizes (step-size tuning) are not supported");
+        if (h->tr_dA || h->tr_acc || h->tr_xprop || h->tr_dAp || h->tr_accp || h->tr_pprop) return no("the debug trace is not supported");
+        if (h->n_cool != 0 && h->t < h->t_anneal + h->n_cool) return no("annealing is not supported");
+        const int sites = h->M + 1;
+        int T = h->T_user ? h->T_user : 4 * kMcGroup;
+        if (T != 2 * kMcGroup && T != 3 * kMcGroup && T != 4 * kMcGroup) return no("threads_per_cta must be 256, 384 or 512 (2, 3 or 4 groups of 128)");
+        const int NG = T / kMcGroup;
+        int hh = h->halo_user >= 0 ? h->halo_user : 8, G = h->G_user, tile = 0;
+        if (G == 0 && sites <= kMcTileMax) G = 1;
+        if (G == 1) { tile = sites + (sites & 1); hh = 0; }
+        else {
+            if (hh < 2) return no("halo depth must be at least 2 with more than one tile per chain");
+            const int cap = kMcTileMax - 2 * hh;
+            if (G == 0) G = (sites + cap - 1) / cap;
+            tile = (sites + G - 1) / G;
+            tile += tile & 1;
+            for (;;) {                                                  // the last tile must hold at least the h sites it sends
+                G = (sites + tile - 1) / tile;
+                const int last = sites - (G - 1) * tile;
+                if (G == 1 || last >= hh) break;
+                tile += 2;
+            }
+            if (G == 1) hh = 0;
+        }
+        if (tile + 2 * hh > kMcTileMax) return no("tile plus halos exceeds 256 sites");
+        const int slots = std::min(h->sm_count * NG, kMcMaxSlots);
+        int cpw = std::min(slots / G, h->C);
+        if (cpw < 1) return no("a chain does not fit the co-resident groups");
+        const int waves = (h->C + cpw - 1) / cpw;
+        cpw = (h->C + waves - 1) / waves;                               // even waves
+        out->G = G; out->T = T; out->tile = tile; out->cooperative = true; out->engine = PIMC_ENGINE_TILE_MC; out->h = hh;
+        out->smem = (size_t)NG * mc_group_bytes<R>(h->D, Model::NK);
+        out->cpw = cpw; out->waves = waves;
+        if (out->smem > 227 * 1024) return no("shared memory");
+        return PIMC_OK;
+    }
+}
+
+// AUTO: the tile-resident engine when the problem fits it; several chains that do not: the many-chain tile-resident engine;
+// everything else: the global-memory engine.
 template <class Model, typename R> int choose_shape(pimc_handle* h, LaunchShape* out) {
+    out->cpw = h->C; out->waves = 1;
     if (h->engine_user == PIMC_ENGINE_GLOBAL) return choose_shape_global<Model, R>(h, out);
     if (h->engine_user == PIMC_ENGINE_TILE) return choose_shape_tile<Model, R>(h, out, false);
+    if (h->engine_user == PIMC_ENGINE_TILE_MC) return choose_shape_mc<Model, R>(h, out, false);
     if (choose_shape_tile<Model, R>(h, out, true) == PIMC_OK) return PIMC_OK;
+    if (h->C >= 2 && h->G_user == 0 && h->T_user == 0 && choose_shape_mc<Model, R>(h, out, true) == PIMC_OK) return PIMC_OK;
+    out->cpw = h->C; out->waves = 1;
     return choose_shape_global<Model, R>(h, out);
 }
 
@@ -362,6 +419,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
     a.hs_base = h->hs_base;
     a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault; a.ar_hold = h->ar_hold;
     a.ptrace = (R*)h->ptrace; a.ptrace_cap = h->ptrace_cap; a.ptrace_n0 = h->n_samples;
+    a.mc_hx_words = h->lay.mc_hx_words; a.mc_ar_words = h->lay.mc_ar_words; a.mc_chain0 = 0; a.mc_nchains = h->C; a.mc_tag0 = 0;
 
     const dim3 grid((unsigned)(ls.G * h->C)), block((unsigned)ls.T);
     const bool trap = h->disc == PIMC_DISC_TRAPEZOID;
@@ -404,13 +462,43 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
             PIMC_CUDA(h, cudaGetLastError());
             h->kg_valid = true;
         }
-        if (ls.engine == PIMC_ENGINE_TILE && do_states) h->kg_valid = false;
+        if (ls.engine != PIMC_ENGINE_GLOBAL && do_states) h->kg_valid = false;
     }
+    if constexpr (Model::kTileMc) {
+        if (ls.engine == PIMC_ENGINE_TILE_MC) {
+            // one launch per wave of ls.cpw chains, each running all n_sweeps on its chains; every launch gets a private tag range
+            const int NG = ls.T / kMcGroup;
+            fn = NG == 4 ? (const void*)tilemc_sweep_kernel<Model, R, 4> : NG == 3 ? (const void*)tilemc_sweep_kernel<Model, R, 3> : (const void*)tilemc_sweep_kernel<Model, R, 2>;
+            PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
+            const unsigned long long span = (unsigned long long)n_sweeps * (unsigned long long)(Model::NP + 1) + 4ull;
+            if (span >= (1ull << 31)) return fail(h, PIMC_EINVAL, "too many sweeps for one call of the many-chain tile engine");
+            for (int w = 0; w < ls.waves; ++w) {
+                if ((h->mc_tag & 0xFFFFFFFFull) + span >= (1ull << 32)) {   // the 32-bit tags would wrap inside this launch: start a new epoch
+                    PIMC_CUDA(h, cudaMemsetAsync(h->lay.mc_hx_words, 0, sizeof(unsigned long long) * (size_t)kMcMaxSlots * 2 * 2 * kHaloWordsPerSide, h->stream));
+                    PIMC_CUDA(h, cudaMemsetAsync(h->lay.mc_ar_words, 0, sizeof(unsigned long long) * (size_t)2 * kMcMaxSlots * kArSlotWords, h->stream));
+                    h->mc_tag = (h->mc_tag | 0xFFFFFFFFull) + 2ull;          // low word = 1: tag 0 (fresh memory) is never awaited
+                }
+                a.mc_chain0 = w * ls.cpw;
+                a.mc_nchains = std::min(ls.cpw, h->C - a.mc_chain0);
+                a.mc_tag0 = (unsigned int)(h->mc_tag & 0xFFFFFFFFull);
+                h->mc_tag += span;
+                const int groups = a.mc_nchains * ls.G;
+                const dim3 mc_grid((unsigned)std::min(h->sm_count, groups));
+                void* mc_params[] = {&a};
+                PIMC_CUDA(h, cudaLaunchCooperativeKernel(fn, mc_grid, block, mc_params, ls.smem, h->stream));
+                h->launches++;
+            }
+        }
+    }
+    if (ls.engine == PIMC_ENGINE_TILE_MC) {
+        if constexpr (!Model::kTileMc) return fail(h, PIMC_EUNSUPPORTED, "many-chain tile engine: not compiled for this model");
+    } else {
     if (ls.smem > 48 * 1024) PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
     void* params[] = {&a};
     if (ls.cooperative) PIMC_CUDA(h, cudaLaunchCooperativeKernel(fn, grid, block, params, ls.smem, h->stream));
     else PIMC_CUDA(h, cudaLaunchKernel(fn, grid, block, params, ls.smem, h->stream));
     h->launches++;
+    }
     if (do_states && ls.engine == PIMC_ENGINE_GLOBAL) h->hs_base += 2ull * (unsigned long long)n_sweeps;
     if (h->accum) {   // host bookkeeping of the sample count: sweeps t in [t0, t0+n) with (t - t_enable) % n_skip == 0
         const unsigned long long first = h->t - h->t_enable, last = first + (unsigned long long)n_sweeps;   // [first, last)
@@ -900,7 +988,7 @@ int pimc_get_launch(pimc_handle* h, int* ctas_per_chain, int* threads_per_cta, i
 
 int pimc_set_engine(pimc_handle* h, int engine, int halo) {
     if (!h) return PIMC_EINVAL;
-    if (engine < PIMC_ENGINE_AUTO || engine > PIMC_ENGINE_TILE) return fail(h, PIMC_EINVAL, "unknown engine");
+    if (engine < PIMC_ENGINE_AUTO || engine > PIMC_ENGINE_TILE_MC) return fail(h, PIMC_EINVAL, "unknown engine");
     if (halo < -1 || halo > kTileHaloMax || (halo > 0 && (halo & 1))) return fail(h, PIMC_EINVAL, "halo must be -1 (automatic) or an even number in [0,%d]", kTileHaloMax);
     const int e0 = h->engine_user, h0 = h->halo_user;
     h->engine_user = engine; h->halo_user = halo;

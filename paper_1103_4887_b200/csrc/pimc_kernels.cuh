@@ -91,6 +91,12 @@ template <typename R> struct SweepArgs {
     long long ptrace_cap;
     unsigned long long ptrace_n0;   // records written before this launch (= samples accumulated so far)
     int ar_hold;                    // SM clock ticks between publishing a Delta-A partial and the first poll of the others' (pimc_set_exchange)
+    // many-chain tile-resident engine (pimc_tilemc_kernel.cuh): the chains [mc_chain0, mc_chain0 + mc_nchains) of this wave, the
+    // first tag of this launch's private tag range, and the per-(chain, tile) mailboxes
+    int mc_chain0, mc_nchains;
+    unsigned int mc_tag0;
+    unsigned long long* mc_hx_words;   // (kMcMaxSlots, 2 sides, 2 buffers, kHaloWordsPerSide)
+    unsigned long long* mc_ar_words;   // (2 buffers, kMcMaxSlots, kArSlotWords)
 };
 
 // ---- annealing multiplier of the model-error weights at sweep t (same closed form as the oracle; beta = 1 when off) ----

@@ -15,6 +15,7 @@ namespace pimc {
 template <typename R, int KIN> struct HHModelK {
     static constexpr int D = 4;
     static constexpr int NP = 7;
+    static constexpr bool kTileMc = true;          // the many-chain tile-resident engine is compiled for this family
 
     // The parameter vector lives in shared memory (one copy per CTA); p[] = (gNa, gK, gL, ENa, EK, EL, C).
     // d a / dt = (a_inf(V) - a) / tau_a(V);  a_inf = 1/2 + 1/2 tanh(s), tau = tau0 + tau1 (1 - tanh^2 s), s = (V - Va)/dVa
@@ -196,6 +197,7 @@ template <typename R> using HHClassicModel = HHModelK<R, 1>;
 template <typename R, int D_> struct LinearModel {
     static constexpr int D = D_;
     static constexpr int NP = D_ * D_;
+    static constexpr bool kTileMc = false;
     struct Prep {};
     static __device__ __forceinline__ Prep prepare(const R* __restrict__, R) { return Prep{}; }
     static __device__ __forceinline__ Prep prepare_move(const Prep&, const R* __restrict__, R, int) { return Prep{}; }
