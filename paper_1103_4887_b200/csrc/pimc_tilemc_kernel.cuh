@@ -82,7 +82,9 @@ template <typename R> __device__ __forceinline__ McSmem<R> mc_carve(unsigned cha
     return m;
 }
 
-template <class Model, typename R, int NGRP>
+// ILP2: a parameter move evaluates the thread's two tile sites in ONE branch-free block (sites beyond the tile compute on
+// whatever the shared memory holds and are masked out of the sum), so that the compiler can interleave the two dependent chains.
+template <class Model, typename R, int NGRP, bool ILP2>
 __global__ void __launch_bounds__(NGRP * kMcGroup, 1) tilemc_sweep_kernel(const SweepArgs<R> a) {
     constexpr int D = Model::D;
     constexpr int NP = Model::NP;
@@ -216,6 +218,12 @@ __global__ void __launch_bounds__(NGRP * kMcGroup, 1) tilemc_sweep_kernel(const 
                     const int jl = max(j - 1 + q, 0), jr = j + q;     // pair index of the left / right neighbour (plane 1 - q)
                     const int own = q * D * P + j, oth = (1 - q) * D * P;
                     R xn[D], xp[D], gp[D], kgn[NKA];
+                    double mcc[D];                                   // moment centres: loaded before the model step, used after it
+                    if (acc_now) {
+                        const double* ccp = a.cx + (site0 + (size_t)n) * D;
+#pragma unroll
+                        for (int c = 0; c < D; ++c) mcc[c] = __ldg(ccp + c);
+                    }
 #pragma unroll
                     for (int c = 0; c < D; ++c) {
                         xn[c] = sm.xs[own + c * P];
@@ -256,10 +264,9 @@ __global__ void __launch_bounds__(NGRP * kMcGroup, 1) tilemc_sweep_kernel(const 
                         for (int c = 0; c < NK; ++c) sm.kg[(q * NK + c) * P + j] = kgn[c];
                     }
                     if (acc_now) {       // A5 for this site: its value is final for sweep t (parameter moves do not touch x)
-                        const double* ccp = a.cx + (site0 + (size_t)n) * D;
 #pragma unroll
                         for (int c = 0; c < D; ++c) {
-                            const double d = (double)(accept ? xp[c] : xn[c]) - __ldg(ccp + c);
+                            const double d = (double)(accept ? xp[c] : xn[c]) - mcc[c];
                             sm.S1[own + c * P] += d;
                             sm.S2[own + c * P] += d * d;
                         }
@@ -288,6 +295,30 @@ __global__ void __launch_bounds__(NGRP * kMcGroup, 1) tilemc_sweep_kernel(const 
                     const R* gc = cur ? sm.g1 : sm.g0;
                     R* ga = cur ? sm.g0 : sm.g1;
                     double part = 0.0;
+                    if constexpr (ILP2) {
+                        R x0[D], x1[D], gp0[D], gp1[D], k0[NKA], k1[NKA];
+                        lds_site<R, D>(sm.xs, 0, j, P, x0);
+                        lds_site<R, D>(sm.xs, 1, j, P, x1);
+#pragma unroll
+                        for (int c = 0; c < NK; ++c) { k0[c] = sm.kg[c * P + j]; k1[c] = sm.kg[(NK + c) * P + j]; }
+                        const R I0 = sm.Is[2 * j], I1 = sm.Is[2 * j + 1], I2 = sm.Is[2 * j + 2];
+                        Model::template increment_k<(NK > 0), false>(x0, pp, pq, I0, I1, a.dt, gp0, k0, nullptr);
+                        Model::template increment_k<(NK > 0), false>(x1, pp, pq, I1, I2, a.dt, gp1, k1, nullptr);
+                        sts_site<R, D>(ga, 0, j, P, gp0);
+                        sts_site<R, D>(ga, 1, j, P, gp1);
+                        const int n0 = s_ext + 2 * j, n1 = n0 + 1;
+                        const bool own0 = 2 * j < n_ext && n0 <= M - 1 && n0 >= s && n0 < e, own1 = 2 * j + 1 < n_ext && n1 <= M - 1 && n1 >= s && n1 < e;
+                        R acc0 = R(0), acc1 = R(0);
+#pragma unroll
+                        for (int c = 0; c < D; ++c) {
+                            const R d0 = x1[c] - x0[c], d1 = sm.xs[c * P + j + 1] - x1[c];
+                            const R rn0 = d0 - gp0[c], ro0 = d0 - gc[c * P + j];
+                            const R rn1 = d1 - gp1[c], ro1 = d1 - gc[(D + c) * P + j];
+                            acc0 += R(0.5) * a.Rf[c] * (rn0 * rn0 - ro0 * ro0);
+                            acc1 += R(0.5) * a.Rf[c] * (rn1 * rn1 - ro1 * ro1);
+                        }
+                        part = (own0 ? (double)acc0 : 0.0) + (own1 ? (double)acc1 : 0.0);
+                    } else {
 #pragma unroll 1
                     for (int q = 0; q < 2; ++q) {
                         const int iloc = 2 * j + q, n = s_ext + iloc;
@@ -309,6 +340,7 @@ __global__ void __launch_bounds__(NGRP * kMcGroup, 1) tilemc_sweep_kernel(const 
                                 part += (double)acc;
                             }
                         }
+                    }
                     }
                     double dA = group_sum(part, sm.red, red_phase, grp, j);
                     if (G > 1) {   // all-gather of the chain's G partials as tagged packets; every group sums them in the same fixed order
