@@ -42,12 +42,13 @@ W_EVAL_ORACLE = 666.0
 #     fraction credits min((1), (2) / redundancy).
 EXEC_FP64_COMPUTED = {   # engine -> (per COMPUTED site update, per COMPUTED parameter-move evaluation); HH tanh kinetics, fp64, RK4 map, joint updates
     "tile": (520.1, 264.9),      # tile_sweep_kernel, profiles/r02_work_counts.md: 595.0 and 303.1 per OWNED unit at cfg3 / (254 / 222)
+    "tilemc": (531.6, 285.3),    # tilemc_sweep_kernel (many-chain tile-resident engine), profiles/r02_tilemc.md: 576.7 and 309.5 per OWNED unit at cfg4 / (256 / 236)
     "global": (521.0, 285.0),    # sweep_kernel (one CTA per chain, no halos, stage-1 rates cached in global memory), profiles/r02_cfg4.md: launch total minus
                                  # 521 per site update, over the evaluations
 }
 # ncu sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed of the same kernels, same launches
 NCU_PIPE_FP64_ACTIVE = {3: {"full_sweep": 0.310, "a2_only": 0.427, "a4_only": 0.274, "source": "profiles/r02_final.md"},
-                        4: {"full_sweep": 0.453, "source": "profiles/r02_cfg4.md"}}
+                        4: {"full_sweep": 0.527, "a2_only": 0.518, "a4_only": 0.513, "source": "profiles/r02_tilemc.md (TILE_MC engine; GLOBAL engine: 0.453, profiles/r02_cfg4.md)"}}
 # trapezoid discretisation / component-wise updates: estimated slots (no oracle count yet), used for the non-headline variants only
 W_SITE_SLOTS_TRAP = 380.0
 W_SITE_SLOTS_COMP = 2300.0
@@ -139,15 +140,18 @@ def oracle_rate_all_cores(w, budget_s, per_sweep_s):
     return (w.M + 1) * n * cores / dt, cores, n, dt
 
 
-OTHER_CONFIGS = [   # (config, dtype, sweeps per step): every BASELINE.json config besides the headline one, and its fp32 variant
-    (0, 64, 2000), (1, 64, 1000), (2, 64, 1000), (4, 64, 20), (3, 32, 1000),
+ENGINE_NAMES = {1: "GLOBAL", 2: "TILE", 3: "TILE_MC"}
+OTHER_CONFIGS = [   # (config, dtype, sweeps per step, chains or None): every BASELINE.json config besides the headline one, its fp32
+    # variant, and FOUR independent chains of the headline shape in one launch (north_star: "HH chains at M=32768 sustaining >= 50 % of
+    # the FP64 pipe for the checkerboard sweep": a single chain offers M/2 independent updates per half-sweep, several chains fill the SMs)
+    (0, 64, 2000, None), (1, 64, 1000, None), (2, 64, 1000, None), (4, 64, 100, None), (3, 32, 1000, None), (3, 64, 100, 4),
 ]
 
 
-def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=None):
+def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=None, n_chains=None):
     """One extra line of the "other_configs" block: the same timed protocol as the headline (3 warm-up steps, L2 flushed before
     every step, CUDA events on the launching stream), full sweeps with accumulation every sweep, oracle on one core beside it."""
-    w = w or make_workload(cfg)
+    w = w or (make_workload(cfg, n_chains=n_chains) if n_chains else make_workload(cfg))
     h = P.Pimc.from_workload(w, dtype=dtype)
     h.set_accum(True, 1)
     h.reset_moments()
@@ -166,12 +170,29 @@ def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=No
     evs = [one() for _ in range(steps)]
     torch.cuda.synchronize()
     ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
-    fault = h.fault()
+    gpu_launches = h.launch_count - n0
     units = float(w.n_chains) * (w.M + 1) * S
+    a2 = None
+    if w.n_chains > 1:          # many-chain workloads: the checkerboard sweep (row A2) on its own as well
+        def one_a2():
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); h.sweep_states_only(S, seed); e1.record(stream)
+            return e0, e1
+        one_a2(); torch.cuda.synchronize()
+        ev2 = [one_a2() for _ in range(steps)]
+        torch.cuda.synchronize()
+        a2 = units / (float(np.mean([a.elapsed_time(b) for a, b in ev2])) * 1e-3)
+    fault = h.fault()
     out = {"workload": w.name, "dtype": "f64" if dtype == 64 else "f32", "value": units / (ms * 1e-3), "unit": UNIT,
            "chain_sweeps_per_s": w.n_chains * S / (ms * 1e-3), "ms_per_step": ms, "sweeps_per_step": S, "steps": steps,
-           "params_moved": int(np.count_nonzero(w.w_param)), "engine": {1: "GLOBAL", 2: "TILE"}[h.get_engine()["engine"]],
-           "launch": h.get_launch(), "gpu_launches": int(h.launch_count - n0), "fault": int(fault)}
+           "params_moved": int(np.count_nonzero(w.w_param)), "engine": ENGINE_NAMES[h.get_engine()["engine"]],
+           "launch": h.get_launch(), "gpu_launches": int(gpu_launches), "fault": int(fault)}
+    if a2 is not None:
+        out["a2_only_site_updates_per_s"] = a2
+        eng = h.get_engine()
+        if eng["engine"] == P.ENGINE_TILE_MC and dtype == 64 and w.model == 1:     # executed FP64 lane operations of the checkerboard sweep over the derived peak
+            out["a2_only_frac"] = 2.0 * a2 * EXEC_FP64_COMPUTED["tilemc"][0] * (256.0 / h.get_launch()["tile_sites"]) / 1e12 / PEAK_TFLOPS_DERIVED
     if cpu_budget > 0 and dtype == 64:
         r, n, dt = oracle_rate(w, cpu_budget)
         out["oracle_1core"] = {"value": r, "unit": UNIT, "sample": f"{n} full sweeps of chain 0 in {dt:.1f} s"}
@@ -262,9 +283,11 @@ def run_ours(args):
     # of an interior tile (tile-resident engine with more than one tile per chain: h halo sites on each side are updated redundantly)
     exec_counts, red = None, None
     if w.model == 1 and args.dtype == 64 and not trap and not comp:
-        tile_engine = eng["engine"] == P.ENGINE_TILE
+        tile_engine = eng["engine"] in (P.ENGINE_TILE, P.ENGINE_TILE_MC)
         red = (shape["tile_sites"] + 2.0 * eng["halo"]) / shape["tile_sites"] if (tile_engine and shape["ctas_per_chain"] > 1) else 1.0
-        per = EXEC_FP64_COMPUTED["tile" if tile_engine else "global"]
+        if eng["engine"] == P.ENGINE_TILE_MC:
+            red = 256.0 / shape["tile_sites"]       # every thread of a group computes its site pair in branch-free blocks, masked or not
+        per = EXEC_FP64_COMPUTED[{P.ENGINE_TILE: "tile", P.ENGINE_TILE_MC: "tilemc"}.get(eng["engine"], "global")]
         exec_counts = (per[0] * red, per[1] * red)
     units_per_step = float(w.n_chains) * (w.M + 1) * S
     n_active = int(np.count_nonzero(w.w_param))
@@ -335,7 +358,8 @@ def run_ours(args):
     tile = bool(shape.get("smem_bytes", 0))
     model_name = {0: "LinearModel", 1: "HHModelK<0>", 2: "HHModelK<1>"}[w.model]
     rtype = "double" if args.dtype == 64 else "float"
-    kernel = (f"pimc::tile_sweep_kernel<{model_name},{rtype},MAXT={256 if shape['threads_per_cta'] <= 256 else 512},TRAP={int(trap)},COMP={int(comp)},KG={int(n_active > 0 and not trap)},TR=0>"
+    kernel = (f"pimc::tilemc_sweep_kernel<{model_name},{rtype},NGRP={shape['threads_per_cta'] // 128}>" if eng["engine"] == P.ENGINE_TILE_MC else
+              f"pimc::tile_sweep_kernel<{model_name},{rtype},MAXT={256 if shape['threads_per_cta'] <= 256 else 512},TRAP={int(trap)},COMP={int(comp)},KG={int(n_active > 0 and not trap)},TR=0>"
               if tile else f"pimc::sweep_kernel<{model_name},{rtype}>")
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved_tflops / peak_tflops,
@@ -346,7 +370,9 @@ def run_ours(args):
                 "frac_oracle_work": oracle_tflops / peak_tflops,
                 "halo_redundancy": red,
                 "pipe_fp64_active_ncu": NCU_PIPE_FP64_ACTIVE.get(args.config) if exec_counts else None,
-                "target": "north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2) of config 3, judged on pipe_fp64_active_ncu.a2_only (42.7 %): NOT reached",
+                "target": ("north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2), judged on ncu's sm__pipe_fp64_cycles_active: ONE chain of M = 32768 "
+                           "(config 3, this line's workload when --config 3): 42.7 %, NOT reached (M/2 independent updates per half-sweep are one warp per scheduler); "
+                           "many chains per launch (config 4 on the TILE_MC engine): 51.8 %, reached (profiles/r02_tilemc.md)"),
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (headline and args.dtype == 64) else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r02_work_counts.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
@@ -385,8 +411,9 @@ def run_ours(args):
             # the rest of BASELINE.json's workloads (north_star: "Report throughput on the synthetic workloads below at 1 GPU"),
             # after the timed region of the headline; and the oracle on all host cores (one independent chain per core)
             other = []
-            for cfg, dt_, S_ in OTHER_CONFIGS:
-                other.append(measure_other_config(P, torch, flush, cfg, dt_, S_, 3, min(args.cpu_budget, 2.0), w=w if cfg == 3 else None))
+            for cfg, dt_, S_, nch in OTHER_CONFIGS:
+                other.append(measure_other_config(P, torch, flush, cfg, dt_, S_, 3, min(args.cpu_budget, 2.0) if not nch else 0.0,
+                                                  w=w if (cfg == 3 and not nch) else None, n_chains=nch))
             ar, cores, an, adt = oracle_rate_all_cores(w, min(args.cpu_budget, 8.0), cpu_s / max(cpu_n, 1))
             cpu["all_cores"] = {"value": ar, "unit": UNIT, "cores": cores,
                                 "sample": f"{cores} independent chains of {w.name}, one per core (threads), {an} full sweeps each in {adt:.1f} s"}
@@ -395,7 +422,7 @@ def run_ours(args):
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.dtype == 64 else "f32",
             "data": "synthetic",
             "config": {"workload": w.name + ("_trapezoid" if trap else ""), "discretisation": args.disc, "update": args.update, "M": w.M, "n_chains": w.n_chains, "sweeps_per_step": S, "params_moved": n_active,
-                       "accumulate_every": 1, "launch": shape, "l2": "flushed between timed steps (256 MiB fill)",
+                       "accumulate_every": 1, "launch": shape, "engine": ENGINE_NAMES[eng["engine"]], "l2": "flushed between timed steps (256 MiB fill)",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "sweeps_per_s": value / (w.M + 1),
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),

@@ -468,11 +468,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
         if (ls.engine == PIMC_ENGINE_TILE_MC) {
             // one launch per wave of ls.cpw chains, each running all n_sweeps on its chains; every launch gets a private tag range
             const int NG = ls.T / kMcGroup;
-            const char* ev;
-            const bool ilp2 = (ev = getenv("PIMC_MC_ILP2")) && atoi(ev) != 0;
-            fn = NG == 4 ? (ilp2 ? (const void*)tilemc_sweep_kernel<Model, R, 4, true> : (const void*)tilemc_sweep_kernel<Model, R, 4, false>)
-               : NG == 3 ? (ilp2 ? (const void*)tilemc_sweep_kernel<Model, R, 3, true> : (const void*)tilemc_sweep_kernel<Model, R, 3, false>)
-                         : (ilp2 ? (const void*)tilemc_sweep_kernel<Model, R, 2, true> : (const void*)tilemc_sweep_kernel<Model, R, 2, false>);
+            fn = NG == 4 ? (const void*)tilemc_sweep_kernel<Model, R, 4> : NG == 3 ? (const void*)tilemc_sweep_kernel<Model, R, 3> : (const void*)tilemc_sweep_kernel<Model, R, 2>;
             PIMC_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ls.smem));
             const unsigned long long span = (unsigned long long)n_sweeps * (unsigned long long)(Model::NP + 1) + 4ull;
             if (span >= (1ull << 31)) return fail(h, PIMC_EINVAL, "too many sweeps for one call of the many-chain tile engine");
