@@ -257,6 +257,24 @@ int pimc_run_host_ws(int model, int D, int L, int M, double dt, double Rm, const
                      long long n_sweeps, unsigned long long seed, double* moments_out, void* x_out, void* p_out,
                      void* dev_scratch, size_t dev_scratch_bytes);
 
+/* The same for callers that may not call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): ALL device memory of the call -- staging copies of y, I, x0, p0, the moments, and the library's workspace (caches,
+ * mailboxes, counters) -- is taken from ONE file-scope `static __device__` array of pimc_static_scratch_bytes() = 32 MiB inside
+ * libpimc.so (every GPU that loads the library holds it until the process exits).  The call performs no cudaMalloc, cudaFree
+ * or allocating library routine.  Arguments, results and error behaviour are those of pimc_run_host (HOST buffers in and out,
+ * default stream, synchronises before returning).  Limits: pimc_run_host_workspace_bytes(shape) must not exceed
+ * pimc_static_scratch_bytes(), else PIMC_EUNSUPPORTED with the two sizes in pimc_last_error(NULL) -- enough for one chain of
+ * M = 32768 in fp64 (30.6 MiB; the headline workload) or any smaller single chain, not for 16 chains of M = 8192 (68 MiB).
+ * The array is shared by every call on a device and keeps the last call's contents: each call clears the part it uses before
+ * use (what must start at zero: epochs, mailbox tags, counters, moment sums), so calls one after the other are independent,
+ * but two calls of this process that overlap on the same GPU (e.g. from two host threads) race on it -- serialise them
+ * (other processes have their own copy of the array).  One address per device, looked up once with that device current. */
+size_t pimc_static_scratch_bytes(void);
+int pimc_run_host_static(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype,
+                         const void* y, const void* I, const void* x0, const void* p0, const double* w_state,
+                         const double* w_param, const double* lo, const double* hi, int proposal_kind, long long n_burn,
+                         long long n_sweeps, unsigned long long seed, double* moments_out, void* x_out, void* p_out);
+
 /* RNG self-test entry (rows A1 / pin P4): fills out (dev u32, n*4) with Philox4x32-10(ctr[i], key), ctrs
  * dev u32 (n,4); and the library's transforms: u_prop dev double n*4 = (w+0.5)2^-32 per word, u_acc dev
  * double n = ((w1:w0 >> 12)+0.5)2^-52, z dev double n*4 = Box-Muller pairs (words 0,1) and (2,3).  Any

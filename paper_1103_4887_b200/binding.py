@@ -64,6 +64,9 @@ _SIGNATURES = {
     "pimc_run_host_workspace_bytes": (C.c_size_t, [C.c_int] * 6),
     "pimc_run_host_ws": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _vp, _vp, _vp,
                                    _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp, _vp, C.c_size_t]),
+    "pimc_static_scratch_bytes": (C.c_size_t, []),
+    "pimc_run_host_static": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _vp, _vp, _vp,
+                                       _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp]),
     "pimc_rng_selftest": (C.c_int, [_vp, C.c_ulonglong, C.c_uint, C.c_uint, _vp, _vp, _vp, _vp, _vp]),
     "pimc_step_selftest": (C.c_int, [C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp, C.c_double, C.c_ulonglong, _vp, _vp]),
     "pimc_math_selftest": (C.c_int, [_vp, C.c_ulonglong, _vp, _vp]),
@@ -452,8 +455,14 @@ def run_host_scratch(w, dtype=64):
     return t
 
 
-def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_path=False, scratch=None):
-    """End-to-end call on HOST numpy buffers (pimc_run_host / pimc_run_host_ws): H2D, sweeps, moments, D2H inside the call."""
+def static_scratch_bytes():
+    """Size of the library's static device scratch array (pimc_static_scratch_bytes): the limit of run_host(..., static=True)."""
+    return int(lib().pimc_static_scratch_bytes())
+
+
+def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_path=False, scratch=None, static=False):
+    """End-to-end call on HOST numpy buffers (pimc_run_host / pimc_run_host_ws): H2D, sweeps, moments, D2H inside the call.
+    static=True: pimc_run_host_static -- all device memory from the library's static array, no cudaMalloc anywhere."""
     npd = np.float64 if dtype == 64 else np.float32
     y = np.ascontiguousarray(w.y, dtype=npd)
     I = None if w.I is None else np.ascontiguousarray(w.I, dtype=npd)
@@ -473,9 +482,13 @@ def run_host(w, n_burn, n_sweeps, seed, dtype=64, kind=PROPOSAL_GAUSSIAN, want_p
     if scratch is not None:
         off = (-scratch.data_ptr()) % 256
         sp, sn = C.c_void_p(scratch.data_ptr() + off), scratch.numel() - off
-    _check(lib().pimc_run_host_ws(w.model, w.D, w.L, w.M, float(w.dt), float(w.Rm), rf, w.n_chains, dtype, vp(y), vp(I), vp(x0), vp(p0),
-                                  ws, wp, lo, hi, kind, int(n_burn), int(n_sweeps), int(seed), mom.ctypes.data_as(_dp), vp(xo), vp(po),
-                                  sp, sn))
+    if static:
+        _check(lib().pimc_run_host_static(w.model, w.D, w.L, w.M, float(w.dt), float(w.Rm), rf, w.n_chains, dtype, vp(y), vp(I), vp(x0), vp(p0),
+                                          ws, wp, lo, hi, kind, int(n_burn), int(n_sweeps), int(seed), mom.ctypes.data_as(_dp), vp(xo), vp(po)))
+    else:
+        _check(lib().pimc_run_host_ws(w.model, w.D, w.L, w.M, float(w.dt), float(w.Rm), rf, w.n_chains, dtype, vp(y), vp(I), vp(x0), vp(p0),
+                                      ws, wp, lo, hi, kind, int(n_burn), int(n_sweeps), int(seed), mom.ctypes.data_as(_dp), vp(xo), vp(po),
+                                      sp, sn))
     mx = mom[:, : 2 * nx].reshape(w.n_chains, 2, w.M + 1, w.D)
     mp = mom[:, 2 * nx:].reshape(w.n_chains, 2, w.Np)
     bytes_in = y.nbytes + (0 if I is None else I.nbytes) + x0.nbytes + p0.nbytes

@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -657,6 +658,37 @@ bool finite_all(const double* v, int n) {
 
 }  // namespace
 
+// ---- device scratch of the no-allocation entry point (pimc_run_host_static) -------------------------------------------------
+// A file-scope device array: every GPU that loads libpimc.so holds these 32 MiB until the process exits.  In HOST code the
+// name g_static_scratch is only a stand-in for the symbol, NOT a device address (a kernel handed it would fault, or use the
+// wrong memory where the GPU can reach host memory): the address on a device comes from cudaGetSymbolAddress with that device
+// current, looked up once per device below.  Zero-initialised at load, after that it keeps the last call's contents.
+constexpr size_t kStaticScratchBytes = (size_t)32 << 20;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+void* g_static_addr[kStaticMaxDevices];       // device address of g_static_scratch on device d; nullptr = not looked up yet
+
+int static_scratch_address(void** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, PIMC_ECUDA, "cudaGetDevice: %s (libpimc has no CPU fallback)", cudaGetErrorString(e));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, PIMC_EUNSUPPORTED, "device ordinal %d beyond the %d this entry point keeps addresses for", dev, kStaticMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_static_scratch);      // device `dev` is current
+        if (e != cudaSuccess || !ptr) return fail(nullptr, PIMC_ECUDA, "cudaGetSymbolAddress(g_static_scratch) on device %d: %s", dev, cudaGetErrorString(e));
+        if (((uintptr_t)ptr & 255) != 0) return fail(nullptr, PIMC_ECUDA, "static scratch is not 256-byte aligned on device %d", dev);
+        g_static_addr[dev] = ptr;
+    }
+    *out = g_static_addr[dev];
+    return PIMC_OK;
+}
+}  // namespace
+
 extern "C" {
 
 int pimc_model_np(int model, int D) {
@@ -1177,6 +1209,28 @@ int pimc_run_host_ws(int model, int D, int L, int M, double dt, double Rm, const
     if (h) pimc_destroy(h);
     if (own) cudaFree(dev);
     return rc;
+}
+
+size_t pimc_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+// pimc_run_host with ALL device memory taken from the static array above: no cudaMalloc, no cudaFree, no allocating library
+// routine anywhere on the path (pimc_run_host_ws with a caller buffer never allocates device memory; pimc_init clears the
+// workspace it carves -- epochs, mailbox tags, counters, moment sums must start at zero -- with a cudaMemsetAsync on the stream).
+int pimc_run_host_static(int model, int D, int L, int M, double dt, double Rm, const double* Rf, int n_chains, int dtype, const void* y,
+                         const void* I, const void* x0, const void* p0, const double* w_state, const double* w_param, const double* lo,
+                         const double* hi, int proposal_kind, long long n_burn, long long n_sweeps, unsigned long long seed,
+                         double* moments_out, void* x_out, void* p_out) {
+    int why;
+    if (!shape_ok(model, D, L, M, n_chains, dtype, &why)) return fail(nullptr, why, "bad or unsupported shape");
+    const size_t need = host_run_layout(model, D, L, M, n_chains, dtype).total;
+    if (need > kStaticScratchBytes)
+        return fail(nullptr, PIMC_EUNSUPPORTED, "pimc_run_host_static: this shape needs %zu bytes of device scratch, the static array holds %zu "
+                    "(pimc_static_scratch_bytes); use pimc_run_host_ws with a buffer of your own", need, kStaticScratchBytes);
+    void* scratch = nullptr;
+    const int rc = static_scratch_address(&scratch);
+    if (rc != PIMC_OK) return rc;
+    return pimc_run_host_ws(model, D, L, M, dt, Rm, Rf, n_chains, dtype, y, I, x0, p0, w_state, w_param, lo, hi, proposal_kind, n_burn,
+                            n_sweeps, seed, moments_out, x_out, p_out, scratch, kStaticScratchBytes);
 }
 
 int pimc_rng_selftest(const unsigned int* ctrs, unsigned long long n, unsigned int key0, unsigned int key1, unsigned int* out,
