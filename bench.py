@@ -42,7 +42,7 @@ W_EVAL_ORACLE = 666.0
 #     fraction credits min((1), (2) / redundancy).
 EXEC_FP64_COMPUTED = {   # engine -> (per COMPUTED site update, per COMPUTED parameter-move evaluation); HH tanh kinetics, fp64, RK4 map, joint updates
     "tile": (520.1, 264.9),      # tile_sweep_kernel, profiles/r02_work_counts.md: 595.0 and 303.1 per OWNED unit at cfg3 / (254 / 222)
-    "tilemc": (531.6, 285.3),    # tilemc_sweep_kernel (many-chain tile-resident engine), profiles/r02_tilemc.md: 576.7 and 309.5 per OWNED unit at cfg4 / (256 / 236)
+    "tilemc": (502.4, 255.4),    # tilemc_sweep_kernel (many-chain tile-resident engine), profiles/r02_tilemc.md: 545 and 277 per OWNED unit at cfg4 / (256 / 236)
     "global": (521.0, 285.0),    # sweep_kernel (one CTA per chain, no halos, stage-1 rates cached in global memory), profiles/r02_cfg4.md: launch total minus
                                  # 521 per site update, over the evaluations
 }
