@@ -65,6 +65,7 @@ struct Layout {
     double* ar_val;
     unsigned long long *hx_words, *hx_epoch, *ar_words;
     unsigned long long *mc_hx_words, *mc_ar_words;     // mailboxes of the many-chain tile-resident engine
+    unsigned long long *st_words;                      // mailboxes of the sufficient-statistics exchange (trapezoid parameter moves)
     double *ws, *wpd;                 // tuned step sizes (C, M+1, D), (C, Np)
     unsigned int *nacc_s, *nacc_p;    // accepted changes since the last adjustment
     int* fault;
@@ -111,6 +112,7 @@ Layout carve(char* base, int D, int L, int M, int Np, int C, int dtype) {
     o.ar_words = c.take<unsigned long long>((size_t)2 * kTileMaxCtas * kArSlotWords);
     o.mc_hx_words = c.take<unsigned long long>((size_t)kMcMaxSlots * 2 * 2 * kHaloWordsPerSide);
     o.mc_ar_words = c.take<unsigned long long>((size_t)2 * kMcMaxSlots * kArSlotWords);
+    o.st_words = c.take<unsigned long long>((size_t)2 * kTileMaxCtas * 2 * kStatSlots * 2);
     o.ws = c.take<double>(nx);
     o.wpd = c.take<double>((size_t)C * Np);
     o.nacc_s = c.take<unsigned int>(nx);
@@ -308,7 +310,8 @@ template <class Model, typename R> int choose_shape_tile(pimc_handle* h, LaunchS
     }
     if (tile + 2 * hh > T || T > Tcap) return no("tile plus halos does not fit the CTA");
     out->G = G; out->T = T; out->tile = tile; out->cooperative = G > 1; out->engine = PIMC_ENGINE_TILE; out->h = hh;
-    out->smem = tile_smem_bytes<R>(T, h->D, h->L, h->disc == PIMC_DISC_TRAPEZOID ? 0 : Model::NK, h->update_mode == PIMC_UPDATE_COMPONENTWISE ? h->D : 1);
+    out->smem = tile_smem_bytes<R>(T, h->D, h->L, h->disc == PIMC_DISC_TRAPEZOID ? 0 : Model::NK, h->update_mode == PIMC_UPDATE_COMPONENTWISE ? h->D : 1,
+                                   h->disc == PIMC_DISC_TRAPEZOID && Model::NTH > 0);
     if (out->smem > 227 * 1024) return no("shared memory");
     return PIMC_OK;
 }
@@ -418,7 +421,7 @@ template <class Model, typename R> int run_sweeps_once(pimc_handle* h, long long
     a.t0 = h->t; a.seed = seed; a.n_sweeps = n_sweeps; a.do_states = do_states; a.do_params = do_params;
     a.hs_flag = h->lay.hs_flag; a.ar_val = h->lay.ar_val; a.ar_flag = h->lay.ar_flag; a.ar_epoch = h->lay.ar_epoch;
     a.hs_base = h->hs_base;
-    a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault; a.ar_hold = h->ar_hold;
+    a.h = ls.h; a.hx_words = h->lay.hx_words; a.hx_epoch = h->lay.hx_epoch; a.ar_words = h->lay.ar_words; a.fault = h->lay.fault; a.ar_hold = h->ar_hold; a.st_words = h->lay.st_words;
     a.ptrace = (R*)h->ptrace; a.ptrace_cap = h->ptrace_cap; a.ptrace_n0 = h->n_samples;
     a.mc_hx_words = h->lay.mc_hx_words; a.mc_ar_words = h->lay.mc_ar_words; a.mc_chain0 = 0; a.mc_nchains = h->C; a.mc_tag0 = 0;
 

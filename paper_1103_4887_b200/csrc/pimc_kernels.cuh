@@ -91,6 +91,8 @@ template <typename R> struct SweepArgs {
     long long ptrace_cap;
     unsigned long long ptrace_n0;   // records written before this launch (= samples accumulated so far)
     int ar_hold;                    // SM clock ticks between publishing a Delta-A partial and the first poll of the others' (pimc_set_exchange)
+    unsigned long long* st_words;   // (2 slots, kTileMaxCtas, 2 {partials, totals}, kStatSlots) 16-byte tagged packets: sufficient statistics of the
+                                    //   trapezoid parameter moves (tile engine)
     // many-chain tile-resident engine (pimc_tilemc_kernel.cuh): the chains [mc_chain0, mc_chain0 + mc_nchains) of this wave, the
     // first tag of this launch's private tag range, and the per-(chain, tile) mailboxes
     int mc_chain0, mc_nchains;

@@ -176,6 +176,28 @@ template <typename R, int KIN> struct HHModelK {
     static __device__ __forceinline__ void increment(const R x[4], const R* __restrict__ p, R I0, R I1, R dt, R g[4]) {
         increment(x, p, prepare(p, dt), I0, I1, dt, g);
     }
+    // The parameters enter dV/dt LINEARLY through NTH monomials (Eq. 11; the gate equations hold none):
+    //   (dt/2) F_V(x, p; I) = theta(p) . phi(x, I),  theta = (1, gNa, gNa ENa, gK, gK EK, gL, gL EL) / C,
+    //                                                phi = (dt/2) (I, -m^3 h V, m^3 h, -n^4 V, n^4, -V, 1).
+    // With the trapezoid rule (Eq. 7) every V residual is d_n - theta . (phi_n + phi_{n+1}), so the action is a
+    // quadratic form in theta whose coefficients are sums over the path that do NOT depend on p: one reduction of those sums
+    // per sweep decides all parameter moves (pimc_tile_kernel.cuh, "sufficient statistics").  Always in double.
+    static constexpr int NTH = 7;
+    // which monomials a move of parameter l changes (bit j = theta_j); a move of C (l = 6) changes 1/C and with it all of them
+    static __host__ __device__ constexpr unsigned theta_mask(int l) {
+        return l == 0 ? 0x06u : l == 1 ? 0x18u : l == 2 ? 0x60u : l == 3 ? 0x04u : l == 4 ? 0x10u : l == 5 ? 0x40u : 0x7Fu;
+    }
+    static __device__ __forceinline__ double theta_pre(const R* __restrict__ p) { return 1.0 / (double)p[6]; }
+    static __device__ __forceinline__ void theta(const R* __restrict__ p, double th[7]) { theta_from(p, theta_pre(p), th); }
+    static __device__ __forceinline__ void theta_from(const R* __restrict__ p, double ic, double th[7]) {
+        th[0] = ic; th[1] = (double)p[0] * ic; th[2] = (double)p[0] * (double)p[3] * ic; th[3] = (double)p[1] * ic;
+        th[4] = (double)p[1] * (double)p[4] * ic; th[5] = (double)p[2] * ic; th[6] = (double)p[2] * (double)p[5] * ic;
+    }
+    static __device__ __forceinline__ void regressors(const R x[4], R I, double hdt, double ph[7]) {
+        const double V = x[0], m = x[1], h = x[2], n = x[3];
+        const double m3h = m * m * m * h, n2 = n * n, n4 = n2 * n2;
+        ph[0] = hdt * (double)I; ph[1] = -hdt * m3h * V; ph[2] = hdt * m3h; ph[3] = -hdt * n4 * V; ph[4] = hdt * n4; ph[5] = -hdt * V; ph[6] = hdt;
+    }
     // Trapezoid discretisation (Eq. 7): the cached quantity is c = (dt/2) F(x, p; I)
     static __device__ __forceinline__ void half_rhs(const R x[4], const R* __restrict__ p, const Prep& q, R I, R c[4]) {
         R F[4];
@@ -212,6 +234,13 @@ template <typename R, int D_> struct LinearModel {
         }
     }
     static constexpr int NK = 0;                   // nothing parameter-independent worth caching
+    static constexpr int NTH = 0;                  // no sufficient-statistics form of the parameter moves (tile engine keeps the per-move evaluation)
+    static __host__ __device__ constexpr unsigned theta_mask(int) { return 0u; }
+    static __device__ __forceinline__ double theta_pre(const R*) { return 0.0; }
+    static __device__ __forceinline__ void theta_from(const R*, double, double*) {}
+    static __device__ __forceinline__ R rhs_V(const R*, const R*, R, R) { return R(0); }
+    static __device__ __forceinline__ void theta(const R*, double*) {}
+    static __device__ __forceinline__ void regressors(const R*, R, double, double*) {}
     static __device__ __forceinline__ void stage1_cache(const R*, R*) {}
     template <bool IN, bool OUT>
     static __device__ __forceinline__ void increment_k(const R x[D_], const R* __restrict__ p, const Prep&, R I0, R I1, R dt, R g[D_], const R*, R*) {

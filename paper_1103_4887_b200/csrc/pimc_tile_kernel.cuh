@@ -23,6 +23,7 @@
 #pragma once
 #include "pimc_kernels.cuh"
 #include "pimc_exchange.cuh"
+#include <type_traits>
 
 namespace pimc {
 
@@ -31,6 +32,19 @@ constexpr int kTileMaxCtas = 256;                                  // inbox slot
 constexpr int kArSlotWords = 16;                                   // one 128-byte line per CTA: slots sharing a line serialise in L2 (measured 2x slower)
 constexpr int kHaloWordsPerSide = kTileHaloMax * 2 * kMaxD * 2;    // h sites x (x, g) x D values x 2 words
 constexpr unsigned long long kSpinLimit = 20ull * 1000 * 1000;    // polls before a hand-off is declared lost
+// Sufficient statistics of the trapezoid parameter moves (Model::NTH = 7 monomials): the 28 entries of the symmetric matrix
+// Q = sum psi psi^T and the 7 entries of b = sum d psi; product v of the table below is psi[kStatJ[v]] * (kStatK[v] < 7 ? psi[kStatK[v]] : d).
+constexpr int kStatN = 35;
+constexpr int kStatSlots = 40;                                     // packets per mailbox record (35 used)
+constexpr int kStatCols = 36;                                      // product columns of the in-CTA reduction (35 used)
+__device__ const signed char kStatJ[kStatCols] = {0, 0, 0, 0, 0, 0, 0, 1, 1, 1, 1, 1, 1, 2, 2, 2, 2, 2, 3, 3, 3, 3, 4, 4, 4, 5, 5, 6, 0, 1, 2, 3, 4, 5, 6, 0};
+__device__ const signed char kStatK[kStatCols] = {0, 1, 2, 3, 4, 5, 6, 1, 2, 3, 4, 5, 6, 2, 3, 4, 5, 6, 3, 4, 5, 6, 4, 5, 6, 5, 6, 6, 7, 7, 7, 7, 7, 7, 7, 7};
+// entry (j, k), j <= k, of Q in that order
+__host__ __device__ constexpr int stat_q(int j, int k) { return j * 7 - j * (j - 1) / 2 + (k - j); }
+__host__ __device__ constexpr int stat_qs(int j, int k) { return j <= k ? stat_q(j, k) : stat_q(k, j); }
+template <int N, class F> __device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (N > 0) { static_for<N - 1>(f); f(std::integral_constant<int, N - 1>{}); }
+}
 
 // ---- 8-byte tagged packets ---------------------------------------------------------------------------------
 __device__ __forceinline__ void ll_store(unsigned long long* p, uint32_t payload, uint32_t tag) {
@@ -119,22 +133,28 @@ template <typename R> struct TileSmem {
     R *Is, *ys;                 // [E+2], [E*L]
     R *rstep, *rlogu;           // [2 sets][2 parities][npass][D][RP], [2][2][npass][RP]
     unsigned int* cnt;          // [4]: accepted owned state updates per component class
+    // sufficient statistics of the trapezoid parameter moves (allocated only for those launches)
+    double *st_psi;             // [T][8]: psi_0..6 and d of every thread's site (zero for sites that own no term)
+    double *st_part;            // [8 warps][8 x 8]: every warp's Psi^T Psi over its 32 sites
+    double *st_red;             // [max(T, 72)] packets polled by a reducer of several statistics; then the decided parameters
+    double *st_tot;             // [kStatSlots] this CTA's partials, then the grid-wide totals
     int P;
 };
 
 // the pitch is a compile-time constant of the kernel instantiation (MAXT = 256 or 512), so plane offsets are immediates
 __host__ __device__ inline int tile_pitch(int T) { return (T <= 256 ? 256 : 512) / 2 + 2; }
 
-template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK, int npass) {
+template <typename R> __host__ __device__ inline size_t tile_smem_bytes(int T, int D, int L, int NK, int npass, bool stat = false) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     size_t dbl = 3 * 2 * D * P + kMaxNp + 64 + 2 * kMaxNp * 2 + 2 * kMaxNp + 3 * kMaxNp + 2 + kMaxNp + 3 * kMaxNp / 2;
+    if (stat) dbl += (size_t)T * 8 + 8 * 64 + (size_t)(T > 72 ? T : 72) + kStatSlots;
     const size_t RP = P - 2;
     size_t real = 4 * 2 * D * P + 2 * (size_t)NK * P + (E + 2) + E * (size_t)(L > 0 ? L : 1) + 4 * (size_t)npass * RP * D + 4 * (size_t)npass * RP;
     (void)TC;
     return dbl * 8 + ((real * sizeof(R) + 15) & ~(size_t)15) + 16;
 }
 
-template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L, int NK, int npass) {
+template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned char* base, int T, int D, int L, int NK, int npass, bool stat = false) {
     const size_t E = (size_t)T, TC = (size_t)T / 2, P = (size_t)tile_pitch(T);
     TileSmem<R> m;
     m.P = (int)P;
@@ -155,6 +175,13 @@ template <typename R> __device__ __forceinline__ TileSmem<R> tile_carve(unsigned
     m.s_in = reinterpret_cast<int*>(d); d += kMaxNp / 2;
     m.s_pacc = reinterpret_cast<unsigned int*>(d); d += kMaxNp / 2;
     m.s_pprop = reinterpret_cast<unsigned int*>(d); d += kMaxNp / 2;
+    m.st_psi = m.st_part = m.st_red = m.st_tot = nullptr;
+    if (stat) {
+        m.st_psi = d; d += (size_t)T * 8;
+        m.st_part = d; d += 8 * 64;
+        m.st_red = d; d += (size_t)(T > 72 ? T : 72);
+        m.st_tot = d; d += kStatSlots;
+    }
     R* r = reinterpret_cast<R*>(d);
     m.xs = r; r += 2 * D * P;
     m.g0 = r; r += 2 * D * P;
@@ -235,7 +262,8 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     // step vector that is zero except in component c and the accept uniform of block c (drawn by the producer warps), which is
     // exactly a single-component Metropolis move; a joint sweep has one pass.
     constexpr int npass = COMP ? D : 1;
-    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK, npass);
+    constexpr bool STAT = TRAP && Model::NTH > 0;  // parameter moves decided from one reduction of sufficient statistics per sweep
+    const TileSmem<R> sm = tile_carve<R>(tile_smem_raw, T, D, a.L, NK, npass, STAT);
     constexpr int NWMAX = MAXT / 32;               // warps of the largest CTA this instantiation is launched with
     constexpr int RP = MAXT / 2;                   // pitch of the random-number ring
     constexpr int P = MAXT / 2 + 2;                // == tile_pitch(T): the launcher picks MAXT = 256 for T <= 256, else 512
@@ -494,28 +522,234 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 }
             }
         } else {
+            // The proposals of this sweep's parameter moves, p'_l = p_l + step_l, do not depend on the state sweep or on the decisions
+            // of the other parameters: producer threads 0..NP-1 post them and the bounds verdicts at once (every thread keeps the
+            // parameter vector), so that neither the compute warps after their half-sweeps nor a move has them on its critical path.
+            const int pj = tid - TC;
+            if (a.do_params && pj < NP) {
+                R pcur = R(0);
+#pragma unroll
+                for (int k = 0; k < NP; ++k) pcur = (k == pj) ? prm[k] : pcur;
+                const bool live = sm.wpl[pj] > 0.0;
+                const double step = live ? sm.pdraw[(set * kMaxNp + pj) * 2 + 0] : 0.0;
+                double pl;
+                if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)pcur, step);
+                else pl = (double)__fadd_rn(pcur, (float)step);
+                sm.s_pl[pj] = pl;
+                sm.s_in[pj] = !live ? 0 : ((pl >= sm.blo[pj] && pl <= sm.bhi[pj]) ? 2 : 1);
+            }
             // ---------------- A1: proposals and uniforms of the next sweep (producer warps) ----------------
-            if (i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull);
+            // (trapezoid rule with parameter moves: a half-sweep is ONE field evaluation, shorter than the drawing of a sweep's random
+            //  numbers, so there the producers draw while the compute warps wait for the statistics exchange and decide the moves)
+            if (i + 1 < a.n_sweeps && !(STAT && a.do_params)) produce(set ^ 1, t + 1ull);
         }
         if (a.do_states) k_phase += 2;               // every thread keeps the count: the hand-off below is CTA-uniform
-        // The proposals of this sweep's parameter moves, p'_l = p_l + step_l, do not depend on the decisions of the other parameters:
-        // threads 0..NP-1 post them and the bounds verdicts once, so that a move starts with three independent shared-memory reads
-        // instead of a register-array select chain, an add and two compares on its critical path.
-        if (a.do_params && tid < NP) {
-            R pcur = R(0);
-#pragma unroll
-            for (int k = 0; k < NP; ++k) pcur = (k == tid) ? prm[k] : pcur;
-            const bool live = sm.wpl[tid] > 0.0;
-            const double step = live ? sm.pdraw[(set * kMaxNp + tid) * 2 + 0] : 0.0;
-            double pl;
-            if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)pcur, step);
-            else pl = (double)__fadd_rn(pcur, (float)step);
-            sm.s_pl[tid] = pl;
-            sm.s_in[tid] = !live ? 0 : ((pl >= sm.blo[tid] && pl <= sm.bhi[tid]) ? 2 : 1);
-        }
         __syncthreads();
 
         // ---------------- A4: parameter moves, in sequence; one tile site per thread ----------------
+        if constexpr (STAT) {
+        // ---------------- A4, trapezoid rule: all parameter moves of the sweep from ONE reduction of sufficient statistics ----------------
+        // The V residual of term n -> n+1 is d_n - theta(p) . psi_n (psi_n = phi_n + phi_{n+1}, Model::theta / Model::regressors), so
+        //   Delta-A(p -> p') = (Rf_V / 2) [ (theta' - theta)^T Q (theta' + theta) - 2 (theta' - theta) . b ],  Q = sum psi psi^T, b = sum d psi:
+        // identical in exact arithmetic to re-evaluating the field over the whole path under p' (K2 + K3 once
+        // per parameter), but Q and b do not depend on p: 35 sums per sweep replace 7 model evaluations of every site and 7 grid-wide
+        // exchanges.  Every CTA decides every move from bit-identical totals; the cache is rebuilt once, under the final parameters.
+        if (a.do_params) {
+            const int n = s_ext + prm_iloc;
+            const bool can_eval = prm_iloc < n_ext && n <= M;
+            const bool owned = n >= s && n < e && n <= M - 1;
+            bool any = false;
+#pragma unroll
+            for (int l = 0; l < NP; ++l) any = any || sm.s_in[l] == 2;
+            if (any) {
+                // S1: the regressors of this thread's term
+                double ps[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) ps[k] = 0.0;
+                if (owned) {
+                    R xn[D], xq[D];
+                    lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
+                    lds_site<R, D>(sm.xs, 1 - prm_q, prm_j + prm_q, P, xq);
+                    double f0[7], f1[7];
+                    const double hdt = (double)prep.hdt;
+                    Model::regressors(xn, sm.Is[prm_iloc], hdt, f0);
+                    Model::regressors(xq, sm.Is[prm_iloc + 1], hdt, f1);
+#pragma unroll
+                    for (int k = 0; k < 7; ++k) ps[k] = f0[k] + f1[k];
+                    ps[7] = (double)xq[0] - (double)xn[0];
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) sm.st_psi[tid * 8 + k] = ps[k];
+                __syncwarp();
+                // S2: the 8 x 8 matrix Psi^T Psi (rows / columns psi_0..6, d) over the warp's own 32 sites, as eight FP64 tensor-core
+                // products of 4 sites each (mma.sync m8n8k4: a small but genuine contraction; fixed order, so every CTA that holds a
+                // site forms the same bits).  Lane (g = lane / 4, k = lane % 4) holds A[g][k] = B[k][g] = psi_g(site 4 step + k).
+                {
+                    const int lane = tid & 31, wbase = tid & ~31;
+                    double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                    for (int step = 0; step < 8; ++step) {
+                        const double e = sm.st_psi[(wbase + 4 * step + (lane & 3)) * 8 + (lane >> 2)];
+                        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(e), "d"(e));
+                    }
+                    double* dst = sm.st_part + (tid >> 5) * 64 + (lane >> 2) * 8 + 2 * (lane & 3);
+                    dst[0] = c0; dst[1] = c1;
+                }
+                __syncthreads();
+                // S3: this CTA's partial of statistic v (thread v; a reducer thread forms the same sum, in the same order, for itself)
+                const int nwp = T >> 5;
+                auto cta_partial = [&](int v) {
+                    const int e = kStatJ[v] * 8 + kStatK[v];
+                    double t = 0.0;
+                    for (int w = 0; w < nwp; ++w) t += sm.st_part[w * 64 + e];
+                    return t;
+                };
+                if (G == 1) {
+                    if (tid < kStatN) sm.st_tot[tid] = cta_partial(tid);
+                    __syncthreads();
+                } else {
+                    // Two hops through L2: tile b is the REDUCER of the statistics v = b, b + G, ...: it gathers that statistic's G partials
+                    // (one packet per thread), adds them in a fixed order and publishes the total; then everybody reads the 35 totals.
+                    // G * 35 + 35 packets are read per CTA instead of the G * 35 * G a flat all-gather of the vector would cost.
+                    const uint32_t tag = (uint32_t)(ar_count + 1ull);
+                    unsigned long long* rec = a.st_words + (size_t)(ar_count & 1ull) * kTileMaxCtas * 2 * kStatSlots * 2;
+                    const int cta0 = (int)chain * G;
+                    auto part_of = [&](int cta, int v) { return rec + (((size_t)cta * 2 + 0) * kStatSlots + v) * 2; };
+                    // the total of statistic v lives in its REDUCER's record: 35 totals in 35 different cache lines (packets that share a
+                    // line serialise in L2, and polls that arrive before a packet delay it: pimc_exchange_selftest)
+                    auto tot_of = [&](int v) { return rec + (((size_t)(cta0 + v % G) * 2 + 1) * kStatSlots + v) * 2; };
+                    if (tid < kStatN) ll_store_f64(part_of(cta0 + b, tid), cta_partial(tid), tag);
+                    const int nv = b < kStatN ? (kStatN - 1 - b) / G + 1 : 0;
+                    const long long until = clock64() + (long long)a.ar_hold;
+                    auto fetch = [&](int j, int v) -> double {      // tile j's partial of statistic v
+                        if (j == b) return cta_partial(v);
+                        while (clock64() < until) {}
+                        return ll_wait_f64(part_of(cta0 + j, v), tag, a.fault);
+                    };
+                    if (G >= kStatN) {          // one statistic per reducer: a block sum (fixed tree) of the G packets; every CTA passes here
+                        double val = 0.0;
+                        if (nv == 1) for (int j = tid; j < G; j += T) val += fetch(j, b);
+                        const double total = block_sum_db<NWMAX>(val, sm.red, red_phase);
+                        if (nv == 1 && tid == 0) ll_store_f64(tot_of(b), total, tag);
+                    } else {                    // few tiles: several statistics per reducer (nv G < 70 packets), each summed in index order by one thread
+                        for (int q = tid; q < nv * G; q += T) sm.st_red[q] = fetch(q % G, b + G * (q / G));
+                        __syncthreads();
+                        if (tid < nv) {
+                            const double* q = sm.st_red + tid * G;
+                            double t = 0.0;
+                            for (int j = 0; j < G; ++j) t += q[j];
+                            ll_store_f64(tot_of(b + G * tid), t, tag);
+                        }
+                    }
+                    // a total needs two hops and a block sum from the moment the last partial is out: hold the first poll.  Compute threads
+                    // only (they alone meet at the barrier below; a small CTA has fewer of them than there are statistics)
+                    if (tid < TC) {
+                        const long long until2 = until + 3ll * (long long)a.ar_hold;
+                        for (int v = tid; v < kStatN; v += TC) {
+                            while (clock64() < until2) {}
+                            sm.st_tot[v] = ll_wait_f64(tot_of(v), tag, a.fault);
+                        }
+                    }
+                    ar_count += 1ull;
+                    if (tid < TC) bar_compute(TC);      // the totals are for the compute warps; the producers go on to draw at once
+                }
+            }
+            // The compute warps decide; the producer warps draw the next sweep's random numbers meanwhile and take the result from shared memory.
+            bool params_changed = false;
+            if (tid < TC) {
+            // Decisions, in sequence, by every compute thread from the same totals.  With v = Q theta - b for the CURRENT parameters,
+            //   Delta-A = (Rf_V / 2) sum_j dtheta_j (2 v_j + (Q dtheta)_j),  and on accept  v += Q dtheta;
+            // a move of parameter l changes the monomials Model::theta_mask(l) only (compile-time: the loop over l is unrolled).
+            double S[kStatN];
+#pragma unroll
+            for (int v = 0; v < kStatN; ++v) S[v] = any ? sm.st_tot[v] : 0.0;
+            double ic = Model::theta_pre(prm);
+            double th[7], vv[7];
+            Model::theta_from(prm, ic, th);
+#pragma unroll
+            for (int j = 0; j < 7; ++j) {
+                double row = -S[28 + j];
+#pragma unroll
+                for (int k = 0; k < 7; ++k) row = fma(S[stat_qs(j, k)], th[k], row);
+                vv[j] = row;
+            }
+            const double half_rf = 0.5 * (double)rf(0);
+            unsigned n_prop = 0, n_acc = 0;        // bit fields: 4 bits per parameter are not enough -- one move per parameter and sweep, so 1 bit each
+            static_for<NP>([&](auto LC) {          // branch-free and unrolled: everything that does not hang on the previous decision is hoisted
+                constexpr int l = decltype(LC)::value;
+                constexpr unsigned mask = Model::theta_mask(l);
+                const int st = sm.s_in[l];
+                const double pl = sm.s_pl[l], logu = sm.pdraw[(set * kMaxNp + l) * 2 + 1];
+                R pp[NP];
+#pragma unroll
+                for (int k = 0; k < NP; ++k) pp[k] = (k == l) ? (R)pl : prm[k];
+                const double ic2 = mask == 0x7Fu ? Model::theta_pre(pp) : ic;
+                double th2[7], dth[7], qd[7];
+                Model::theta_from(pp, ic2, th2);
+#pragma unroll
+                for (int j = 0; j < 7; ++j) dth[j] = (mask >> j & 1u) ? th2[j] - th[j] : 0.0;
+#pragma unroll
+                for (int j = 0; j < 7; ++j) {
+                    double r = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 7; ++k) if (mask >> k & 1u) r = fma(S[stat_qs(j, k)], dth[k], r);
+                    qd[j] = r;
+                }
+                double acc = 0.0;
+#pragma unroll
+                for (int j = 0; j < 7; ++j) if (mask >> j & 1u) acc = fma(dth[j], fma(2.0, vv[j], qd[j]), acc);
+                const double dA = half_rf * acc;
+                const bool accept = st == 2 && logu < -dA;
+#pragma unroll
+                for (int j = 0; j < 7; ++j) {
+                    vv[j] = accept ? vv[j] + qd[j] : vv[j];
+                    if (mask >> j & 1u) th[j] = accept ? th2[j] : th[j];
+                }
+                ic = accept ? ic2 : ic;
+                params_changed = params_changed || accept;
+                prm[l] = accept ? (R)pl : prm[l];
+                n_prop |= (st != 0 ? 1u : 0u) << l;
+                n_acc |= (accept ? 1u : 0u) << l;
+                if (trace && b == 0 && tid == 0 && st != 0) {
+                    if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = st == 2 ? (R)dA : (R)__longlong_as_double(0x7FF8000000000000ll);
+                    if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = accept ? 1 : 0;
+                    if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = (R)pl;
+                }
+            });
+            if (tid < NP) { sm.s_pprop[tid] += n_prop >> tid & 1u; sm.s_pacc[tid] += n_acc >> tid & 1u; }
+            if (tid == 0) {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) sm.st_red[k] = (double)prm[k];
+                sm.st_red[NP] = params_changed ? 1.0 : 0.0;
+            }
+            } else if (i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull);
+            __syncthreads();
+            if (tid >= TC) {
+#pragma unroll
+                for (int k = 0; k < NP; ++k) prm[k] = (R)sm.st_red[k];
+                params_changed = sm.st_red[NP] != 0.0;
+            }
+            if (params_changed) {       // the cache under the final parameters: c_n = (dt/2) F(x_n, p), every tile site
+                prep = Model::prepare(prm, a.dt);
+                if (can_eval) {         // only the V entry depends on the parameters; the same expression as Model::half_rhs forms it
+                    R xn[D];
+                    lds_site<R, D>(sm.xs, prm_q, prm_j, P, xn);
+                    const R c0 = prep.hdt * Model::rhs_V(xn, prm, prep.inv_C, sm.Is[prm_iloc]);
+                    (cur ? sm.g1 : sm.g0)[(prm_q * D + 0) * P + prm_j] = fabs(xn[0]) < Model::kVmax ? c0 : (R)__longlong_as_double(0x7FF8000000000000ll);
+                }
+            }
+            __syncthreads();            // the next half-sweep reads the neighbours' cache entries; the producers overwrite pdraw
+            if (trace && b == 0 && tid == 0) {
+#pragma unroll
+                for (int l = 0; l < NP; ++l)
+                    if (!(sm.wpl[l] > 0.0)) {
+                        if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)__longlong_as_double(0x7FF8000000000000ll);
+                        if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = 0;
+                        if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = prm[l];
+                    }
+            }
+        }
+        } else
         if (a.do_params) {
             const int n = s_ext + prm_iloc;
             const bool can_eval = prm_iloc < n_ext && n <= (TRAP ? M : M - 1);

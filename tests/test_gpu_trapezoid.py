@@ -30,6 +30,8 @@ CASES = [
     ("cfg2_M333_1cta_global", 2, 333, (1, 96), True, 20, 1),
     ("cfg1_M999_7ctas_global", 1, 999, (7, 32), False, 20, 1),
     ("cfg1_M1000_auto", 1, 1000, None, False, 40, 0),
+    ("cfg2_M1201_38tiles_tile", 2, 1201, None, True, 20, 2),
+    ("cfg2_M4000_126tiles_of_64_tile", 2, 4000, (126, 64), True, 10, 2),
 ]
 
 
@@ -55,7 +57,11 @@ def test_teacher_forced_parity_trapezoid(P, name, cfg, M, launch, with_params, n
 
 
 @pytest.mark.parametrize("cfg,M,launch,engine", [(0, 256, None, 0), (2, 500, (4, 64), 1), (2, 500, (4, 192), 2), (1, 700, (3, 128), 1),
-                                                 (3, 4001, None, 0), (3, 4001, None, 1)])
+                                                 (3, 4001, None, 0), (3, 4001, None, 1),
+                                                 # the sufficient-statistics parameter moves of the tile engine in the shapes its exchange distinguishes:
+                                                 # 38 tiles of 64 threads (one statistic per reducer, fewer compute threads than statistics),
+                                                 # 126 tiles of 64 threads (more tiles than threads), 9 tiles (several statistics per reducer), one tile
+                                                 (2, 1201, None, 2), (2, 4000, (126, 64), 2), (2, 2000, (9, 256), 2), (2, 200, None, 2)])
 def test_free_running_uniform_bit_identical_trapezoid(P, cfg, M, launch, engine):
     w = make_workload(cfg, M=M)
     h = gpu_handle(w, kind=1, disc=TRAP)
