@@ -264,7 +264,7 @@ int pimc_run_host_ws(int model, int D, int L, int M, double dt, double Rm, const
  * or allocating library routine.  Arguments, results and error behaviour are those of pimc_run_host (HOST buffers in and out,
  * default stream, synchronises before returning).  Limits: pimc_run_host_workspace_bytes(shape) must not exceed
  * pimc_static_scratch_bytes(), else PIMC_EUNSUPPORTED with the two sizes in pimc_last_error(NULL) -- enough for one chain of
- * M = 32768 in fp64 (30.6 MiB; the headline workload) or any smaller single chain, not for 16 chains of M = 8192 (68 MiB).
+ * M = 32768 in fp64 (28.1 MiB; the headline workload) or any smaller single chain, not for 16 chains of M = 8192 (65 MiB).
  * The array is shared by every call on a device and keeps the last call's contents: each call clears the part it uses before
  * use (what must start at zero: epochs, mailbox tags, counters, moment sums), so calls one after the other are independent,
  * but two calls of this process that overlap on the same GPU (e.g. from two host threads) race on it -- serialise them

@@ -27,7 +27,7 @@ namespace pimc {
 constexpr int kMcGroup = 128;        // threads per group: four warps, one per scheduler
 constexpr int kMcTileMax = 256;      // tile sites incl. halos per group: one (even, odd) pair per thread
 constexpr int kMcPitch = 130;        // plane pitch: 128 pairs + the right neighbour of the last odd site
-constexpr int kMcMaxSlots = 1024;    // (chain, tile) pairs in flight per launch (mailbox slots)
+constexpr int kMcMaxSlots = 640;     // (chain, tile) pairs in flight per launch (mailbox slots): 148 SMs x 4 groups = 592 on a B200
 
 __device__ __forceinline__ void bar_group(int grp) { asm volatile("bar.sync %0, 128;" ::"r"(grp + 1) : "memory"); }
 

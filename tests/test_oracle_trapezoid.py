@@ -242,3 +242,54 @@ def test_the_replica_test_has_power():
     # a sampler whose model-error weight is 5 % off must fail the same statistic by a wide margin
     z_mean, z_var, var = _eigenmode_z(TRAPEZOID, K=12, n_samples=1500, weight_bug=1.05)
     assert np.abs(z_var).max() > 6.0, z_var
+
+
+# ------------------------------------------------------------------------------------------------------------
+# The identity the tile engine's trapezoid parameter moves rest on: with Eq. 7 the parameters enter
+# the action only through (dt/2) F_V = theta(p) . phi(x, I), seven monomials typed here from PAPER.md:256-260 Eq. 11, so
+#   Delta-A(p -> p') = (Rf_V / 2) [ (theta' - theta)^T Q (theta' + theta) - 2 (theta' - theta) . b ]
+# with Q = sum psi psi^T, b = sum d psi independent of p.  Checked against the oracle's direct sum over the path.
+# ------------------------------------------------------------------------------------------------------------
+def _theta(p):
+    gNa, gK, gL, ENa, EK, EL, C = [np.longdouble(v) for v in p]
+    return np.array([1, gNa, gNa * ENa, gK, gK * EK, gL, gL * EL], dtype=np.longdouble) / C
+
+
+def _phi(x, I, dt):
+    ld = np.longdouble
+    V, m, h, n = [x[:, c].astype(ld) for c in range(4)]
+    one = np.ones_like(V)
+    return ld(dt) / 2 * np.stack([I.astype(ld), -m**3 * h * V, m**3 * h, -n**4 * V, n**4, -V, one], axis=1)
+
+
+@pytest.mark.parametrize("kinetics", ["tanh", "classic"])
+def test_parameter_moves_are_a_quadratic_form_in_seven_monomials(kinetics):
+    w = make_workload(2, M=300, seed=9, kinetics=kinetics)
+    o = OracleChain.from_workload(w)
+    o.set_discretisation(TRAPEZOID)
+    rng = np.random.default_rng(4)
+    x, p = o.get_path()
+    x = x + 0.3 * rng.normal(size=x.shape) * np.array([1.0, 0.02, 0.02, 0.02])      # off the initial path: residuals of every size
+    o.set_path(x)
+    phi = _phi(x, w.I[0], w.dt)
+    psi = phi[:-1] + phi[1:]                                                        # terms n -> n+1, n = 0..M-1
+    d = (x[1:, 0] - x[:-1, 0]).astype(np.longdouble)
+    Q, b = psi.T @ psi, psi.T @ d
+    th = _theta(p)
+    # the cached V entries ARE theta . phi (the gate entries hold no parameter)
+    c = o.get_cache()
+    assert np.allclose(c[:, 0], np.asarray(phi @ th, dtype=np.float64), rtol=1e-13, atol=1e-15)
+    worst = 0.0
+    for l in range(7):
+        for scale in (1.0, 30.0, -200.0):
+            pl = p[l] + scale * w.w_param[l] * rng.normal()
+            p2 = p.copy(); p2[l] = pl
+            th2 = _theta(p2)
+            formula = float(np.longdouble(w.Rf[0]) / 2 * ((th2 - th) @ Q @ (th2 + th) - 2 * (th2 - th) @ b))
+            dA, S = o.param_delta_A(l, pl)
+            assert abs(formula - dA) <= 1e-12 * max(abs(dA), S), (kinetics, l, scale, formula, dA, S)
+            worst = max(worst, abs(formula - dA) / max(abs(dA), S))
+    # power: a dropped monomial or a wrong sign does not survive (gL EL missing from theta . phi)
+    bad = float(np.longdouble(w.Rf[0]) / 2 * ((th2 - th)[:6] @ Q[:6, :6] @ (th2 + th)[:6] - 2 * (th2 - th)[:6] @ b[:6]))
+    assert abs(bad - dA) > 1e-6 * max(abs(dA), S)
+    print("max |formula - oracle| / max(|dA|, S):", worst)

@@ -39,7 +39,7 @@ def test_run_host_static_matches_the_caller_scratch_path_on_calls_in_a_row():
     calls = [(make_workload(2, M=4096), 5, 30, 11, 1),      # tile-resident engine, 7 parameters, uniform proposals
              (make_workload(0, M=256), 3, 40, 12, 0),       # much smaller shape right after: the array holds the previous call's bytes
              (make_workload(2, M=4096), 5, 30, 11, 1),      # the first call again: same result as before
-             (make_workload(3), 0, 12, 13, 0)]              # config 3 at full size: 30.6 of the 32 MiB
+             (make_workload(3), 0, 12, 13, 0)]              # config 3 at full size: 28.1 of the 32 MiB
     first = None
     for i, (w, n_burn, n_sweeps, seed, kind) in enumerate(calls):
         ref = P.run_host(w, n_burn, n_sweeps, seed, kind=kind, want_path=True, scratch=P.run_host_scratch(w))
