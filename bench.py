@@ -386,7 +386,9 @@ def run_ours(args):
                 "a2_only": {"site_updates_per_s": a2_rate, "ms_per_launch": a2_ms, "frac": a2_frac,
                             "frac_oracle_work": tfl(a2_rate * w_site, 1.0) / peak_tflops},
                 "a4_only": {"param_evals_per_s": a4_rate, "ms_per_launch": a4_ms, "frac": a4_frac,
-                            "frac_oracle_work": tfl(a4_rate * w_eval, 1.0) / peak_tflops}}
+                            "frac_oracle_work": tfl(a4_rate * w_eval, 1.0) / peak_tflops,
+                            "note": ("trapezoid rule on the tile engine: the parameter moves are decided from one reduction of sufficient statistics per sweep "
+                                     "(DESIGN.md 6.1b); param_evals_per_s counts the evaluations the paper's K2/K3 would have made, none is executed") if (trap and tile and w.model != 0) else None}}
 
     # end to end through the C ABI on HOST buffers: H2D of y, I, x0, p0 + sweeps + D2H of the moments inside the timed region
     e2e = None

@@ -71,7 +71,9 @@ enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2, PIMC_
  *  TRAPEZOID (the paper's own rule, Eq. 7): r = x_{n+1} - x_n - (dt/2)[F(x_{n+1}) + F(x_n)], F the model's
  *            vector field with the current I_n at step n (LINEAR: F(x) = (A x - x)/dt); the cache holds
  *            c_n = (dt/2) F(x_n), n = 0..M (PAPER.md:189, 242 caches F_n).  One right-hand side per proposal instead of
- *            four.  Both engines support both discretisations. */
+ *            four.  Both engines support both discretisations.  On the TILE engine the Hodgkin-Huxley models decide ALL parameter
+ *            moves of a sweep from one grid-wide reduction of 35 path sums (the cached V term is linear in seven parameter
+ *            monomials): same decisions as the per-parameter evaluation, to rounding. */
 enum { PIMC_DISC_RK4MAP = 0, PIMC_DISC_TRAPEZOID = 1 };
 /* How a site is updated (Fig. 1 proposes all D components together; PAPER.md:226-230 keeps step sizes and
  * acceptance counters per component).  JOINT (default): x'_n = x_n + w o z, one decision per site.  COMPONENTWISE: for
