@@ -120,3 +120,37 @@ def test_edge_sizes_switching_and_engine_rule_trapezoid(P):
     assert h.get_cache().shape == (1, 300, 4)
     with pytest.raises(Pm.PimcError):
         h.set_discretisation(7)
+
+
+def test_sufficient_statistics_parameter_moves_edge_cases(P):
+    # tile engine, trapezoid rule: the parameter moves come from one reduction of path sums per sweep.  Several chains with
+    # several tiles each (one reducer set per chain), tight bounds (proposals outside are rejected unevaluated), a frozen parameter, the
+    # parameter record, both kinetics: chains bit-identical to the oracle's
+    import paper_1103_4887_b200 as Pm
+    for kinetics in ("tanh", "classic"):
+        w = make_workload(4, M=700, n_chains=3, kinetics=kinetics)
+        wp = w.w_param.copy(); wp[2] = 0.0                       # gL frozen
+        lo, hi = w.p0 - 1.5 * wp, w.p0 + 1.5 * wp                 # bounds 1.5 step sizes around the start: a good share of the proposals falls outside
+        lo[:, 2], hi[:, 2] = w.lo[:, 2], w.hi[:, 2]
+        h = gpu_handle(w, kind=1, disc=TRAP)
+        h.set_proposal(w.w_state, wp, 1)
+        h.set_bounds(lo, hi)
+        h.set_engine(Pm.ENGINE_TILE)
+        assert h.get_launch()["ctas_per_chain"] > 1
+        h.set_accum(True, 1); h.reset_moments()
+        rec = h.param_trace(25)
+        h.sweep(25, seed=21)
+        xg, pg = [a.cpu().numpy() for a in h.get_path()]
+        st = h.stats().cpu().numpy().astype(np.uint64)
+        for c, o in enumerate(oracle_chains(w, kind=1, disc=TRAP)):
+            o.set_proposal(w.w_state, wp, 1)
+            o.set_bounds(lo[c], hi[c])
+            o.set_accum(True, 1); o.reset_moments(); o.param_trace_enable(True)
+            o.sweep(25, seed=21)
+            xo, po = o.get_path()
+            assert np.array_equal(xg[c], xo) and np.array_equal(pg[c], po), (kinetics, c)
+            assert np.array_equal(st[c], o.stats()), (kinetics, c, st[c], o.stats())
+            assert np.array_equal(rec.cpu().numpy()[c], o.param_trace()), (kinetics, c)
+            acc, prop = o.stats()[0][4:], o.stats()[1][4:]
+            assert prop[2] == 0 and acc[2] == 0 and np.all(prop[[0, 1, 3, 4, 5, 6]] == 25)
+            assert 0 < acc.sum() < prop.sum()                     # some accepted, some rejected (incl. out of bounds)
