@@ -326,11 +326,12 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
     if (tid < NP) { sm.s_pacc[tid] = 0u; sm.s_pprop[tid] = 0u; }      // parameter-move counters live in shared memory (thread 0 counts)
 
     // ---- producers: fill RNG set `set` for sweep t ----
-    auto produce = [&](int set, unsigned long long t) {
-        const int j = tid - TC;
+    // (pair index j, site parities [par_lo, par_hi), and whether this call also draws the parameter moves' numbers: normally producer
+    //  thread j draws both sites of compute thread j; the trapezoid parameter phase splits the work, see there)
+    auto produce = [&](int set, unsigned long long t, int j, int par_lo, int par_hi, bool with_params) {
         if (a.do_states) {
 #pragma unroll 1
-            for (int parity = 0; parity < 2; ++parity) {
+            for (int parity = par_lo; parity < par_hi; ++parity) {
                 const int n = s_ext + 2 * j + parity;
                 if (n <= M && 2 * j + parity < n_ext) {
                     R* so_step = sm.rstep + (size_t)((set * 2 + parity) * npass) * D * RP + j;
@@ -350,7 +351,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 }
             }
         }
-        if (a.do_params && j < NP && sm.wpl[j] > 0.0) {
+        if (with_params && a.do_params && j < NP && sm.wpl[j] > 0.0) {
             const Words4 w = draw(a.seed, t, chain, (uint32_t)j, kStreamParam, 0);
             double step;
             if (a.kind == 1) step = __dmul_rn(sm.wpl[j], 2.0 * unit_open(w.w[0]) - 1.0);
@@ -360,7 +361,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
         }
     };
     __syncthreads();                               // the step sizes the producers read were loaded by other threads
-    if (tid >= TC) produce(0, a.t0);
+    if (tid >= TC) produce(0, a.t0, tid - TC, 0, 2, true);
     __syncthreads();
 
     // compute thread `tid` owns the local site pair (2 tid, 2 tid + 1); thread r of a parameter move evaluates local
@@ -541,7 +542,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             // ---------------- A1: proposals and uniforms of the next sweep (producer warps) ----------------
             // (trapezoid rule with parameter moves: a half-sweep is ONE field evaluation, shorter than the drawing of a sweep's random
             //  numbers, so there the producers draw while the compute warps wait for the statistics exchange and decide the moves)
-            if (i + 1 < a.n_sweeps && !(STAT && a.do_params)) produce(set ^ 1, t + 1ull);
+            if (i + 1 < a.n_sweeps && !(STAT && a.do_params)) produce(set ^ 1, t + 1ull, tid - TC, 0, 2, true);
         }
         if (a.do_states) k_phase += 2;               // every thread keeps the count: the hand-off below is CTA-uniform
         __syncthreads();
@@ -558,7 +559,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             const int n = s_ext + prm_iloc;
             const bool can_eval = prm_iloc < n_ext && n <= M;
             const bool owned = n >= s && n < e && n <= M - 1;
-            bool any = false;
+            bool any = false, drawn = false;
 #pragma unroll
             for (int l = 0; l < NP; ++l) any = any || sm.s_in[l] == 2;
             if (any) {
@@ -641,8 +642,11 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                             ll_store_f64(tot_of(b + G * tid), t, tag);
                         }
                     }
-                    // a total needs two hops and a block sum from the moment the last partial is out: hold the first poll.  Compute threads
-                    // only (they alone meet at the barrier below; a small CTA has fewer of them than there are statistics)
+                    // The totals need two hops and a block sum from the moment the last partial is out.  Meanwhile every compute thread draws
+                    // the next sweep's numbers of its ODD site (it is their only reader; the producer warps draw the even sites), which takes
+                    // about as long; then compute threads (they alone meet at the barrier below; a small CTA has fewer of them than there are
+                    // statistics) poll.
+                    if (tid < TC && i + 1 < a.n_sweeps) { produce(set ^ 1, t + 1ull, tid, 1, 2, false); drawn = true; }
                     if (tid < TC) {
                         const long long until2 = until + 3ll * (long long)a.ar_hold;
                         for (int v = tid; v < kStatN; v += TC) {
@@ -657,6 +661,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             // The compute warps decide; the producer warps draw the next sweep's random numbers meanwhile and take the result from shared memory.
             bool params_changed = false;
             if (tid < TC) {
+            if (!drawn && i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull, tid, 1, 2, false);      // no exchange this sweep: nothing to hide it behind
             // Decisions, in sequence, by every compute thread from the same totals.  With v = Q theta - b for the CURRENT parameters,
             //   Delta-A = (Rf_V / 2) sum_j dtheta_j (2 v_j + (Q dtheta)_j),  and on accept  v += Q dtheta;
             // a move of parameter l changes the monomials Model::theta_mask(l) only (compile-time: the loop over l is unrolled).
@@ -722,7 +727,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                 for (int k = 0; k < NP; ++k) sm.st_red[k] = (double)prm[k];
                 sm.st_red[NP] = params_changed ? 1.0 : 0.0;
             }
-            } else if (i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull);
+            } else if (i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull, tid - TC, 0, 1, true);     // even sites (and the parameter draws); the compute threads drew the odd ones
             __syncthreads();
             if (tid >= TC) {
 #pragma unroll
