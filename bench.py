@@ -145,14 +145,18 @@ OTHER_CONFIGS = [   # (config, dtype, sweeps per step, chains or None): every BA
     # variant, and FOUR independent chains of the headline shape in one launch (north_star: "HH chains at M=32768 sustaining >= 50 % of
     # the FP64 pipe for the checkerboard sweep": a single chain offers M/2 independent updates per half-sweep, several chains fill the SMs)
     (0, 64, 2000, None), (1, 64, 1000, None), (2, 64, 1000, None), (4, 64, 100, None), (3, 32, 1000, None), (3, 64, 100, 4),
+    # the paper's own trapezoid discretisation (Eq. 7): the headline shape, and the paper-shaped workload (config 5, not a BASELINE config)
+    (3, 64, 1000, None, "trapezoid"), (5, 64, 1000, None, "trapezoid"),
 ]
 
 
-def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=None, n_chains=None):
+def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=None, n_chains=None, disc="rk4"):
     """One extra line of the "other_configs" block: the same timed protocol as the headline (3 warm-up steps, L2 flushed before
     every step, CUDA events on the launching stream), full sweeps with accumulation every sweep, oracle on one core beside it."""
     w = w or (make_workload(cfg, n_chains=n_chains) if n_chains else make_workload(cfg))
     h = P.Pimc.from_workload(w, dtype=dtype)
+    if disc == "trapezoid":
+        h.set_discretisation(P.DISC_TRAPEZOID)
     h.set_accum(True, 1)
     h.reset_moments()
     stream = torch.cuda.current_stream()
@@ -184,7 +188,7 @@ def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=No
         torch.cuda.synchronize()
         a2 = units / (float(np.mean([a.elapsed_time(b) for a, b in ev2])) * 1e-3)
     fault = h.fault()
-    out = {"workload": w.name, "dtype": "f64" if dtype == 64 else "f32", "value": units / (ms * 1e-3), "unit": UNIT,
+    out = {"workload": w.name + ("_trapezoid" if disc == "trapezoid" else ""), "dtype": "f64" if dtype == 64 else "f32", "value": units / (ms * 1e-3), "unit": UNIT,
            "chain_sweeps_per_s": w.n_chains * S / (ms * 1e-3), "ms_per_step": ms, "sweeps_per_step": S, "steps": steps,
            "params_moved": int(np.count_nonzero(w.w_param)), "engine": ENGINE_NAMES[h.get_engine()["engine"]],
            "launch": h.get_launch(), "gpu_launches": int(gpu_launches), "fault": int(fault)}
@@ -194,7 +198,7 @@ def measure_other_config(P, torch, flush, cfg, dtype, S, steps, cpu_budget, w=No
         if eng["engine"] == P.ENGINE_TILE_MC and dtype == 64 and w.model == 1:     # executed FP64 lane operations of the checkerboard sweep over the derived peak
             out["a2_only_frac"] = 2.0 * a2 * EXEC_FP64_COMPUTED["tilemc"][0] * (256.0 / h.get_launch()["tile_sites"]) / 1e12 / PEAK_TFLOPS_DERIVED
     if cpu_budget > 0 and dtype == 64:
-        r, n, dt = oracle_rate(w, cpu_budget)
+        r, n, dt = oracle_rate(w, cpu_budget, disc=1 if disc == "trapezoid" else 0)
         out["oracle_1core"] = {"value": r, "unit": UNIT, "sample": f"{n} full sweeps of chain 0 in {dt:.1f} s"}
     del h
     return out
@@ -413,9 +417,9 @@ def run_ours(args):
             # the rest of BASELINE.json's workloads (north_star: "Report throughput on the synthetic workloads below at 1 GPU"),
             # after the timed region of the headline; and the oracle on all host cores (one independent chain per core)
             other = []
-            for cfg, dt_, S_, nch in OTHER_CONFIGS:
+            for cfg, dt_, S_, nch, *rest in OTHER_CONFIGS:
                 other.append(measure_other_config(P, torch, flush, cfg, dt_, S_, 3, min(args.cpu_budget, 2.0) if not nch else 0.0,
-                                                  w=w if (cfg == 3 and not nch) else None, n_chains=nch))
+                                                  w=w if (cfg == 3 and not nch) else None, n_chains=nch, disc=rest[0] if rest else "rk4"))
             ar, cores, an, adt = oracle_rate_all_cores(w, min(args.cpu_budget, 8.0), cpu_s / max(cpu_n, 1))
             cpu["all_cores"] = {"value": ar, "unit": UNIT, "cores": cores,
                                 "sample": f"{cores} independent chains of {w.name}, one per core (threads), {an} full sweeps each in {adt:.1f} s"}
