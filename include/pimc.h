@@ -309,6 +309,21 @@ int pimc_fp64_peak_selftest(int millis, double* lane_fma_per_s);
 int pimc_exchange_selftest(int mode, int n_ctas, int threads, int rounds, int work, double* cycles_per_round_host,
                            double* max_abs_err_host, int* n_distinct_host);
 
+/* Latency probes behind DESIGN.md 6.1a (what one inter-CTA message through L2 is made of).  out: host double[n_out], n_out >= 5.
+ *  what = 0: every SM (one CTA per SM, one thread) times dependent chains of ld.relaxed.gpu on each of `arg` lines (0 = 128, <= 256)
+ *            4 KB apart, i.e. the cost of an L2 HIT.  The (SM, line) latencies are split at the midpoint of their 10th / 90th
+ *            percentile into near and far; out = { mean near ticks, mean far ticks, SMs whose near-pattern agrees with the first
+ *            CTA's, the other SMs, fraction of near pairs }: on a two-die part the SMs fall into two equal groups.
+ *  what = 1..5: CTA 0 and CTA `arg` (0 = the last) play ping-pong with a tagged 16-byte packet, one reader per line, published with
+ *            1 st.relaxed.gpu.v2.u64, 2 two atom.exch.b64, 3 two red.max.u64, 4 st.volatile.v2.u64, 5 st.release.gpu.v2.u64;
+ *            out[0] = SM clock ticks one way (store -> the peer's successful poll).
+ *  what = 6: the same ping-pong (st.relaxed.gpu) on `arg` line pairs 1 MiB apart (0 = 16, <= 32), once between two CTAs of the same
+ *            SM group of what = 0 and once between two CTAs of different groups: out = { same-group min, same-group max, cross-group
+ *            min, cross-group max one-way ticks, fraction of the line pairs that are fast for the same-group pair }.  A packet is fast
+ *            only when writer, reader and the line's home are on one die; an all-gather always has to cross.
+ * Allocates and frees its own device memory, synchronises the device.  PIMC_EINVAL on a bad argument. */
+int pimc_latency_selftest(int what, int arg, double* out, int n_out);
+
 const char* pimc_last_error(const pimc_handle* h);   /* h may be NULL: last error of a failed pimc_init / static call */
 int pimc_destroy(pimc_handle* h);
 

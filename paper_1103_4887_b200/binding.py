@@ -64,6 +64,7 @@ _SIGNATURES = {
     "pimc_run_host_workspace_bytes": (C.c_size_t, [C.c_int] * 6),
     "pimc_run_host_ws": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _vp, _vp, _vp,
                                    _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp, _vp, C.c_size_t]),
+    "pimc_latency_selftest": (C.c_int, [C.c_int, C.c_int, _dp, C.c_int]),
     "pimc_static_scratch_bytes": (C.c_size_t, []),
     "pimc_run_host_static": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_int, C.c_int, _vp, _vp, _vp,
                                        _vp, _dp, _dp, _dp, _dp, C.c_int, C.c_longlong, C.c_longlong, C.c_ulonglong, _dp, _vp, _vp]),
@@ -445,6 +446,18 @@ def exchange_selftest(mode, n_ctas=0, threads=256, rounds=2000, work=0):
     cyc, err, nd = C.c_double(), C.c_double(), C.c_int()
     _check(lib().pimc_exchange_selftest(int(mode), int(n_ctas), int(threads), int(rounds), int(work), C.byref(cyc), C.byref(err), C.byref(nd)))
     return dict(cycles_per_round=cyc.value, max_abs_err=err.value, n_distinct=nd.value)
+
+
+def latency_selftest(what, arg=0):
+    """pimc_latency_selftest: what = 0 -> dict of the L2-hit map (near / far ticks, SM groups); 1..5 -> one-way ticks of a packet;
+    6 -> one-way ticks over many line addresses for a same-die and a cross-die pair of CTAs."""
+    out = (C.c_double * 5)()
+    _check(lib().pimc_latency_selftest(int(what), int(arg), out, 5))
+    if what == 0:
+        return dict(near=out[0], far=out[1], group_a=int(out[2]), group_b=int(out[3]), frac_near=out[4])
+    if what == 6:
+        return dict(same_min=out[0], same_max=out[1], cross_min=out[2], cross_max=out[3], frac_fast=out[4])
+    return out[0]
 
 
 def run_host_scratch(w, dtype=64):

@@ -3,6 +3,7 @@
 // is no CPU fallback.
 #include "../../include/pimc.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstdarg>
@@ -659,6 +660,52 @@ bool finite_all(const double* v, int n) {
     return true;
 }
 
+}  // namespace
+
+// ---- latency probes (pimc_latency_selftest): what one inter-CTA message through L2 is made of -------------------------------
+namespace {
+constexpr int kLatMaxLines = 256, kLatLineStrideWords = 512, kLatReps = 64;      // lines 4 KB apart
+// what = 0: every SM (one thread) times a dependent chain of ld.relaxed.gpu on each of n_lines lines: the cost of an L2 HIT from that SM
+__global__ void lat_l2map_kernel(unsigned long long* lines, int n_lines, float* out) {
+    if (threadIdx.x != 0) return;
+    for (int l = 0; l < n_lines; ++l) {
+        unsigned long long* p = lines + (size_t)l * kLatLineStrideWords;
+        unsigned long long v = 0;
+        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+        const long long t0 = clock64();
+        for (int r = 0; r < kLatReps; ++r)
+            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p + (v & 1ull)) : "memory");     // v == 0: same address, dependent
+        out[(size_t)blockIdx.x * n_lines + l] = (float)(clock64() - t0) / kLatReps + (float)(v & 1ull);
+    }
+}
+__device__ __forceinline__ void lat_publish(int how, unsigned long long* p, unsigned long long tag) {
+    unsigned long long o;
+    if (how == 1) asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(tag), "l"(tag) : "memory");
+    else if (how == 2) { asm volatile("atom.relaxed.gpu.global.exch.b64 %0, [%1], %2;" : "=l"(o) : "l"(p), "l"(tag) : "memory");
+                         asm volatile("atom.relaxed.gpu.global.exch.b64 %0, [%1], %2;" : "=l"(o) : "l"(p + 1), "l"(tag) : "memory"); }
+    else if (how == 3) { asm volatile("red.relaxed.gpu.global.max.u64 [%0], %1;" ::"l"(p), "l"(tag) : "memory");
+                         asm volatile("red.relaxed.gpu.global.max.u64 [%0], %1;" ::"l"(p + 1), "l"(tag) : "memory"); }
+    else if (how == 4) asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(tag), "l"(tag) : "memory");
+    else asm volatile("st.release.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(tag), "l"(tag) : "memory");
+}
+// what = 1..5: CTA 0 and CTA `peer` play ping-pong with a tagged 16-byte packet (one reader per line: no contention); one-way ticks
+__global__ void lat_pingpong_kernel(int how, int first_cta, int peer, int rounds, unsigned long long* box, long long* out) {
+    if (threadIdx.x != 0 || ((int)blockIdx.x != first_cta && (int)blockIdx.x != peer)) return;
+    const bool first = (int)blockIdx.x == first_cta;
+    unsigned long long* mine = box + (first ? 0 : 64);             // the pair's two lines are 512 B apart
+    const unsigned long long* theirs = box + (first ? 64 : 0);
+    long long t0 = 0;
+    for (int r = 1; r <= rounds; ++r) {
+        if (r == 11 && first) t0 = clock64();
+        if (first) lat_publish(how, mine, (unsigned long long)r);
+        unsigned long long a, b, spins = 0;
+        do {
+            asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(theirs) : "memory");
+        } while ((a < (unsigned long long)r || b < (unsigned long long)r) && ++spins < kSpinLimit);
+        if (!first) lat_publish(how, mine, (unsigned long long)r);
+    }
+    if (first) out[0] = (clock64() - t0) / (2 * (rounds - 10));
+}
 }  // namespace
 
 // ---- device scratch of the no-allocation entry point (pimc_run_host_static) -------------------------------------------------
@@ -1354,6 +1401,137 @@ int pimc_exchange_selftest(int mode, int n_ctas, int threads, int rounds, int wo
     }
     *max_abs_err_host = worst;
     *n_distinct_host = (mode >= 0 && mode != 3 && (mode < 7 || mode >= 10)) ? distinct : 1;
+    return PIMC_OK;
+}
+
+int pimc_latency_selftest(int what, int arg, double* out_host, int n_out) {
+    if (!out_host || n_out < 5 || what < 0 || what > 6) return fail(nullptr, PIMC_EINVAL, "bad argument");
+    int dev = 0, sms = 0;
+    PIMC_CUDA(nullptr, cudaGetDevice(&dev));
+    PIMC_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    for (int k = 0; k < n_out; ++k) out_host[k] = 0.0;
+    const size_t smem = 100 * 1024;               // one CTA per SM
+    if (what == 0) {
+        const int n_lines = arg <= 0 ? 128 : arg;
+        if (n_lines > kLatMaxLines) return fail(nullptr, PIMC_EINVAL, "at most %d lines", kLatMaxLines);
+        unsigned long long* lines = nullptr;
+        float* out = nullptr;
+        PIMC_CUDA(nullptr, cudaMalloc(&lines, (size_t)n_lines * kLatLineStrideWords * 8));
+        cudaError_t e = cudaMalloc(&out, (size_t)sms * n_lines * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemset(lines, 0, (size_t)n_lines * kLatLineStrideWords * 8);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)lat_l2map_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        void* params[] = {&lines, (void*)&n_lines, &out};
+        for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {          // the second pass is the measurement
+            e = cudaLaunchCooperativeKernel((const void*)lat_l2map_kernel, dim3((unsigned)sms), dim3(32), params, smem, 0);
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        }
+        std::vector<float> lat((size_t)sms * n_lines);
+        if (e == cudaSuccess) e = cudaMemcpy(lat.data(), out, lat.size() * sizeof(float), cudaMemcpyDeviceToHost);
+        cudaFree(lines); cudaFree(out);
+        if (e != cudaSuccess) return fail(nullptr, PIMC_ECUDA, "pimc_latency_selftest: %s", cudaGetErrorString(e));
+        // near / far: threshold half way between the 10th and the 90th percentile; SMs grouped by agreement with SM-slot 0's pattern
+        std::vector<float> sorted(lat);
+        std::sort(sorted.begin(), sorted.end());
+        const double thr = 0.5 * ((double)sorted[sorted.size() / 10] + (double)sorted[sorted.size() * 9 / 10]);
+        double s_near = 0, s_far = 0; size_t n_near = 0, n_far = 0;
+        int group_a = 0;
+        for (int b = 0; b < sms; ++b) {
+            int agree = 0;
+            for (int l = 0; l < n_lines; ++l) {
+                const double v = lat[(size_t)b * n_lines + l];
+                const bool near = v < thr, near0 = lat[l] < thr;
+                if (near) { s_near += v; ++n_near; } else { s_far += v; ++n_far; }
+                agree += near == near0;
+            }
+            group_a += 2 * agree > n_lines;
+        }
+        out_host[0] = n_near ? s_near / n_near : 0.0;
+        out_host[1] = n_far ? s_far / n_far : 0.0;
+        out_host[2] = group_a;
+        out_host[3] = sms - group_a;
+        out_host[4] = (double)n_near / (double)(n_near + n_far);
+        return PIMC_OK;
+    }
+    // one ping-pong measurement: CTAs a <-> b on the line pair at `box`; returns SM clock ticks one way (< 0: CUDA error)
+    auto pingpong = [&](int how, int a, int b, unsigned long long* box, long long* out) -> double {
+        int rounds = 1010;
+        cudaError_t e = cudaMemsetAsync(box, 0, 1024, 0);
+        void* params[] = {&how, &a, &b, &rounds, &box, &out};
+        if (e == cudaSuccess) e = cudaLaunchCooperativeKernel((const void*)lat_pingpong_kernel, dim3((unsigned)sms), dim3(32), params, smem, 0);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        long long cyc = 0;
+        if (e == cudaSuccess) e = cudaMemcpy(&cyc, out, sizeof cyc, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { fail(nullptr, PIMC_ECUDA, "pimc_latency_selftest: %s", cudaGetErrorString(e)); return -1.0; }
+        return (double)cyc;
+    };
+    PIMC_CUDA(nullptr, cudaFuncSetAttribute((const void*)lat_pingpong_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (what <= 5) {
+        const int peer = arg <= 0 ? sms - 1 : arg;
+        if (peer >= sms) return fail(nullptr, PIMC_EINVAL, "peer must be in [1, SM count)");
+        unsigned long long* box = nullptr;
+        PIMC_CUDA(nullptr, cudaMalloc(&box, 4096));
+        const double v = pingpong(what, 0, peer, box, (long long*)(box + 256));
+        cudaFree(box);
+        if (v < 0) return PIMC_ECUDA;
+        out_host[0] = v;
+        return PIMC_OK;
+    }
+    // what = 6: where the line lives matters.  `arg` line pairs 1 MiB apart (0 = 16, <= 32), a pair of CTAs on the same die and a pair
+    // across the dies (groups taken from the L2-hit map of what = 0), plain st.relaxed.gpu
+    const int n_pairs = arg <= 0 ? 16 : arg;
+    if (n_pairs > 32) return fail(nullptr, PIMC_EINVAL, "at most 32 line pairs");
+    double map[5];
+    int rc = pimc_latency_selftest(0, 64, map, 5);
+    if (rc != PIMC_OK) return rc;
+    // classify the CTAs again (the map call returns sizes only): CTA b is in CTA 0's group if its near-pattern agrees with CTA 0's
+    std::vector<int> same_group(sms, 1);
+    {
+        const int n_lines = 64;
+        unsigned long long* lines = nullptr; float* out = nullptr;
+        PIMC_CUDA(nullptr, cudaMalloc(&lines, (size_t)n_lines * kLatLineStrideWords * 8));
+        cudaError_t e = cudaMalloc(&out, (size_t)sms * n_lines * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemset(lines, 0, (size_t)n_lines * kLatLineStrideWords * 8);
+        void* params[] = {&lines, (void*)&n_lines, &out};
+        for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {
+            e = cudaLaunchCooperativeKernel((const void*)lat_l2map_kernel, dim3((unsigned)sms), dim3(32), params, smem, 0);
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        }
+        std::vector<float> lat((size_t)sms * n_lines);
+        if (e == cudaSuccess) e = cudaMemcpy(lat.data(), out, lat.size() * sizeof(float), cudaMemcpyDeviceToHost);
+        cudaFree(lines); cudaFree(out);
+        if (e != cudaSuccess) return fail(nullptr, PIMC_ECUDA, "pimc_latency_selftest: %s", cudaGetErrorString(e));
+        const double thr = 0.5 * (map[0] + map[1]);
+        for (int b = 0; b < sms; ++b) {
+            int agree = 0;
+            for (int l = 0; l < n_lines; ++l) agree += (lat[(size_t)b * n_lines + l] < thr) == (lat[l] < thr);
+            same_group[b] = 2 * agree > n_lines;
+        }
+    }
+    int same_peer = -1, cross_peer = -1;
+    for (int b = 1; b < sms; ++b) {
+        if (same_group[b] && same_peer < 0) same_peer = b;
+        if (!same_group[b] && cross_peer < 0) cross_peer = b;
+    }
+    if (same_peer < 0 || cross_peer < 0) return fail(nullptr, PIMC_EUNSUPPORTED, "the SMs of this device do not fall into two groups");
+    unsigned long long* big = nullptr;
+    PIMC_CUDA(nullptr, cudaMalloc(&big, (size_t)n_pairs << 20));
+    long long* outp = nullptr;
+    if (cudaMalloc(&outp, 64) != cudaSuccess) { cudaFree(big); return fail(nullptr, PIMC_ENOMEM, "cudaMalloc failed"); }
+    double smin = 1e30, smax = 0, cmin = 1e30, cmax = 0;
+    int n_fast = 0;
+    std::vector<double> sv(n_pairs);
+    bool ok = true;
+    for (int k = 0; k < n_pairs && ok; ++k) {
+        unsigned long long* box = big + (size_t)k * (1u << 17);
+        const double a = pingpong(1, 0, same_peer, box, outp), c = pingpong(1, 0, cross_peer, box, outp);
+        ok = a >= 0 && c >= 0;
+        sv[k] = a;
+        smin = std::min(smin, a); smax = std::max(smax, a); cmin = std::min(cmin, c); cmax = std::max(cmax, c);
+    }
+    cudaFree(big); cudaFree(outp);
+    if (!ok) return PIMC_ECUDA;
+    for (int k = 0; k < n_pairs; ++k) n_fast += sv[k] < 0.5 * (smin + smax);
+    out_host[0] = smin; out_host[1] = smax; out_host[2] = cmin; out_host[3] = cmax; out_host[4] = (double)n_fast / n_pairs;
     return PIMC_OK;
 }
 

@@ -49,3 +49,27 @@ def test_components_of_a_block_sum():
            for mode, name in ((7, "block_sum_db"), (8, "warp xor tree"), (9, "barrier + serial sum of 8"))}
     print("\ncycles each:", {k: round(v) for k, v in out.items()})
     assert 50 < out["warp xor tree"] < 1000 and out["block_sum_db"] > out["warp xor tree"]
+
+
+def test_latency_probes_l2_hit_map_and_one_way_packet():
+    # the two measurements DESIGN.md 6.1a rests its "the hop is the L2 path itself" on, re-runnable (pimc_latency_selftest).  The figures
+    # are SM clock ticks of a fixed TIME (an idle GPU that has not clocked up yet counts ~ 0.67x as many), so only ratios are asserted
+    import paper_1103_4887_b200 as Pm
+    Pm.fp64_peak(200)                                                # clock the SMs up
+    m = Pm.latency_selftest(0, 128)
+    print("L2 hit map:", m)
+    assert 100 < m["near"] < m["far"] < 1000 and m["far"] < 1.5 * m["near"], m     # an L2 hit: a few hundred ticks; the far die costs little more
+    assert m["group_a"] + m["group_b"] >= 100
+    one_way = {how: Pm.latency_selftest(how, 1) for how in (1, 2, 3, 4, 5)}
+    print("one-way ticks to the neighbouring SM (1 st.relaxed, 2 atom.exch, 3 red.max, 4 st.volatile, 5 st.release):", one_way)
+    far_peer = Pm.latency_selftest(1, 0)
+    print("one-way ticks to the last SM, st.relaxed:", far_peer)
+    for how in (1, 2, 3, 4):
+        assert 1.5 * m["far"] < one_way[how] < 10 * m["far"], (one_way, m)          # a packet needs several L2-hit times whatever publishes it ...
+    assert 0.7 < far_peer / one_way[1] < 1.4                                           # ... and wherever the peer sits: the hop is not the die crossing
+    assert one_way[5] > 1.2 * one_way[1]                                               # a release store is the slow way
+    # where the line lives: fast only when writer, reader and the line's home share a die; across the dies every line is slow
+    w = Pm.latency_selftest(6, 16)
+    print("line-address sweep:", w)
+    assert w["same_min"] < 0.8 * w["same_max"] and 0.2 <= w["frac_fast"] <= 0.8, w      # two classes of lines for a same-die pair
+    assert w["cross_min"] > 1.25 * w["same_min"] and w["cross_max"] < 1.3 * w["cross_min"], w   # one (slow) class across the dies
