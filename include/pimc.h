@@ -71,8 +71,8 @@ enum { PIMC_ENGINE_AUTO = 0, PIMC_ENGINE_GLOBAL = 1, PIMC_ENGINE_TILE = 2, PIMC_
  *  TRAPEZOID (the paper's own rule, Eq. 7): r = x_{n+1} - x_n - (dt/2)[F(x_{n+1}) + F(x_n)], F the model's
  *            vector field with the current I_n at step n (LINEAR: F(x) = (A x - x)/dt); the cache holds
  *            c_n = (dt/2) F(x_n), n = 0..M (PAPER.md:189, 242 caches F_n).  One right-hand side per proposal instead of
- *            four.  Both engines support both discretisations.  On the TILE engine the Hodgkin-Huxley models decide ALL parameter
- *            moves of a sweep from one grid-wide reduction of 35 path sums (the cached V term is linear in seven parameter
+ *            four.  Both engines support both discretisations.  On the TILE engine, and on the GLOBAL engine with one CTA per chain,
+ *            the Hodgkin-Huxley models decide ALL parameter moves of a sweep from one reduction of 35 path sums (the cached V term is linear in seven parameter
  *            monomials): same decisions as the per-parameter evaluation, to rounding. */
 enum { PIMC_DISC_RK4MAP = 0, PIMC_DISC_TRAPEZOID = 1 };
 /* How a site is updated (Fig. 1 proposes all D components together; PAPER.md:226-230 keeps step sizes and
@@ -317,9 +317,10 @@ int pimc_exchange_selftest(int mode, int n_ctas, int threads, int rounds, int wo
  *  what = 1..5: CTA 0 and CTA `arg` (0 = the last) play ping-pong with a tagged 16-byte packet, one reader per line, published with
  *            1 st.relaxed.gpu.v2.u64, 2 two atom.exch.b64, 3 two red.max.u64, 4 st.volatile.v2.u64, 5 st.release.gpu.v2.u64;
  *            out[0] = SM clock ticks one way (store -> the peer's successful poll).
- *  what = 6: the same ping-pong (st.relaxed.gpu) on `arg` line pairs 1 MiB apart (0 = 16, <= 32), once between two CTAs of the same
- *            SM group of what = 0 and once between two CTAs of different groups: out = { same-group min, same-group max, cross-group
- *            min, cross-group max one-way ticks, fraction of the line pairs that are fast for the same-group pair }.  A packet is fast
+ *  what = 6: the same ping-pong (st.relaxed.gpu) on `arg` line pairs 1 MiB apart (0 = 16, <= 32) between CTA 0 and each of eight peers
+ *            spread over the grid; the peer with the smallest minimum over the lines shares CTA 0's die, the one with the largest does
+ *            not: out = { same-die min, same-die max, cross-die min, cross-die max one-way ticks, fraction of the line pairs that are
+ *            fast for the same-die pair }.  A packet is fast
  *            only when writer, reader and the line's home are on one die; an all-gather always has to cross.
  * Allocates and frees its own device memory, synchronises the device.  PIMC_EINVAL on a bad argument. */
 int pimc_latency_selftest(int what, int arg, double* out, int n_out);

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")           # git-ignored
 LIB = os.path.join(HERE, "libpimc.so")
 N_PARTS = 5
-DEPS = ["pimc.cu", "pimc_kernels.cuh", "pimc_tile_kernel.cuh", "pimc_tilemc_kernel.cuh", "pimc_exchange.cuh", "pimc_model.cuh", "pimc_rng.cuh", "pimc_math.cuh", "pimc_math_coef.inc", os.path.join("..", "..", "include", "pimc.h")]
+DEPS = ["pimc.cu", "pimc_kernels.cuh", "pimc_tile_kernel.cuh", "pimc_tilemc_kernel.cuh", "pimc_exchange.cuh", "pimc_stat.cuh", "pimc_model.cuh", "pimc_rng.cuh", "pimc_math.cuh", "pimc_math_coef.inc", os.path.join("..", "..", "include", "pimc.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -1476,60 +1476,34 @@ int pimc_latency_selftest(int what, int arg, double* out_host, int n_out) {
         out_host[0] = v;
         return PIMC_OK;
     }
-    // what = 6: where the line lives matters.  `arg` line pairs 1 MiB apart (0 = 16, <= 32), a pair of CTAs on the same die and a pair
-    // across the dies (groups taken from the L2-hit map of what = 0), plain st.relaxed.gpu
+    // what = 6: where the line lives matters.  `arg` line pairs 1 MiB apart (0 = 16, <= 32), plain st.relaxed.gpu, CTA 0 against a
+    // handful of peers spread over the grid; the peer with the smallest minimum over the lines shares CTA 0's die, the one with the
+    // largest minimum does not (the L2-hit map of what = 0 separates the dies by 35 ticks only: too little to pick pairs from)
     const int n_pairs = arg <= 0 ? 16 : arg;
     if (n_pairs > 32) return fail(nullptr, PIMC_EINVAL, "at most 32 line pairs");
-    double map[5];
-    int rc = pimc_latency_selftest(0, 64, map, 5);
-    if (rc != PIMC_OK) return rc;
-    // classify the CTAs again (the map call returns sizes only): CTA b is in CTA 0's group if its near-pattern agrees with CTA 0's
-    std::vector<int> same_group(sms, 1);
-    {
-        const int n_lines = 64;
-        unsigned long long* lines = nullptr; float* out = nullptr;
-        PIMC_CUDA(nullptr, cudaMalloc(&lines, (size_t)n_lines * kLatLineStrideWords * 8));
-        cudaError_t e = cudaMalloc(&out, (size_t)sms * n_lines * sizeof(float));
-        if (e == cudaSuccess) e = cudaMemset(lines, 0, (size_t)n_lines * kLatLineStrideWords * 8);
-        void* params[] = {&lines, (void*)&n_lines, &out};
-        for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {
-            e = cudaLaunchCooperativeKernel((const void*)lat_l2map_kernel, dim3((unsigned)sms), dim3(32), params, smem, 0);
-            if (e == cudaSuccess) e = cudaDeviceSynchronize();
-        }
-        std::vector<float> lat((size_t)sms * n_lines);
-        if (e == cudaSuccess) e = cudaMemcpy(lat.data(), out, lat.size() * sizeof(float), cudaMemcpyDeviceToHost);
-        cudaFree(lines); cudaFree(out);
-        if (e != cudaSuccess) return fail(nullptr, PIMC_ECUDA, "pimc_latency_selftest: %s", cudaGetErrorString(e));
-        const double thr = 0.5 * (map[0] + map[1]);
-        for (int b = 0; b < sms; ++b) {
-            int agree = 0;
-            for (int l = 0; l < n_lines; ++l) agree += (lat[(size_t)b * n_lines + l] < thr) == (lat[l] < thr);
-            same_group[b] = 2 * agree > n_lines;
-        }
-    }
-    int same_peer = -1, cross_peer = -1;
-    for (int b = 1; b < sms; ++b) {
-        if (same_group[b] && same_peer < 0) same_peer = b;
-        if (!same_group[b] && cross_peer < 0) cross_peer = b;
-    }
-    if (same_peer < 0 || cross_peer < 0) return fail(nullptr, PIMC_EUNSUPPORTED, "the SMs of this device do not fall into two groups");
     unsigned long long* big = nullptr;
     PIMC_CUDA(nullptr, cudaMalloc(&big, (size_t)n_pairs << 20));
     long long* outp = nullptr;
     if (cudaMalloc(&outp, 64) != cudaSuccess) { cudaFree(big); return fail(nullptr, PIMC_ENOMEM, "cudaMalloc failed"); }
-    double smin = 1e30, smax = 0, cmin = 1e30, cmax = 0;
-    int n_fast = 0;
-    std::vector<double> sv(n_pairs);
+    const int cand[8] = {1, 2, sms / 4, sms / 2 - 1, sms / 2, 3 * sms / 4, sms - 2, sms - 1};
+    double smin = 1e30, smax = 0, cmin = 0, cmax = 0;
+    std::vector<double> sv(n_pairs), tv(n_pairs);
     bool ok = true;
-    for (int k = 0; k < n_pairs && ok; ++k) {
-        unsigned long long* box = big + (size_t)k * (1u << 17);
-        const double a = pingpong(1, 0, same_peer, box, outp), c = pingpong(1, 0, cross_peer, box, outp);
-        ok = a >= 0 && c >= 0;
-        sv[k] = a;
-        smin = std::min(smin, a); smax = std::max(smax, a); cmin = std::min(cmin, c); cmax = std::max(cmax, c);
+    for (int c = 0; c < 8 && ok; ++c) {
+        const int peer = cand[c];
+        if (peer < 1 || peer >= sms) continue;
+        double lo = 1e30, hi = 0;
+        for (int k = 0; k < n_pairs && ok; ++k) {
+            tv[k] = pingpong(1, 0, peer, big + (size_t)k * (1u << 17), outp);
+            ok = tv[k] >= 0;
+            lo = std::min(lo, tv[k]); hi = std::max(hi, tv[k]);
+        }
+        if (lo < smin) { smin = lo; smax = hi; sv = tv; }
+        if (lo > cmin) { cmin = lo; cmax = hi; }
     }
     cudaFree(big); cudaFree(outp);
     if (!ok) return PIMC_ECUDA;
+    int n_fast = 0;
     for (int k = 0; k < n_pairs; ++k) n_fast += sv[k] < 0.5 * (smin + smax);
     out_host[0] = smin; out_host[1] = smax; out_host[2] = cmin; out_host[3] = cmax; out_host[4] = (double)n_fast / n_pairs;
     return PIMC_OK;

@@ -20,6 +20,7 @@
 
 #include "pimc_model.cuh"
 #include "pimc_rng.cuh"
+#include "pimc_stat.cuh"
 
 namespace pimc {
 
@@ -465,7 +466,108 @@ __global__ void __launch_bounds__(kMaxThreads) sweep_kernel(const SweepArgs<R> a
         }
 
         // ---------------- A4: parameter moves, in sequence ----------------
-        if (a.do_params) {
+        bool stat_done = false;
+        if constexpr (SOLO && Model::NTH > 0) {
+            // Trapezoid rule, one CTA per chain: ALL parameter moves of the sweep from one pass over the chain (sufficient statistics,
+            // pimc_stat.cuh / DESIGN.md 6.1b) instead of one pass, with a model evaluation of every site, per parameter.
+            if (a.do_params && a.disc == 1) {
+                stat_done = true;
+                __shared__ double st_part[(kMaxThreads / 32) * kStatCols];
+                __shared__ double st_tot[kStatSlots];
+                __shared__ double st_pl[NP], st_logu[NP];
+                __shared__ int st_in[NP];
+                if (tid < NP) {          // this sweep's proposals, bounds verdicts and log-uniforms: they do not depend on one another's decisions
+                    const bool live = wps[tid] > 0.0;
+                    double pl = (double)ps[tid], lu = 0.0;
+                    int verdict = 0;
+                    if (live) {
+                        const Words4 w = draw(a.seed, t, chain, (uint32_t)tid, kStreamParam, 0);
+                        double step;
+                        if (a.kind == 1) step = __dmul_rn(wps[tid], 2.0 * unit_open(w.w[0]) - 1.0);
+                        else { double z0, z1; normal_pair(unit_open(w.w[0]), unit_open(w.w[1]), z0, z1); step = __dmul_rn(wps[tid], z0); }
+                        if constexpr (sizeof(R) == 8) pl = __dadd_rn((double)ps[tid], step);
+                        else pl = (double)__fadd_rn(ps[tid], (float)step);
+                        lu = log_fast(unit_open52(w.w[2], w.w[3]));
+                        const double lo = a.lo[(size_t)chain * NP + tid], hi = a.hi[(size_t)chain * NP + tid];
+                        verdict = (pl >= lo && pl <= hi) ? 2 : 1;
+                    }
+                    st_pl[tid] = pl; st_logu[tid] = lu; st_in[tid] = verdict;
+                }
+                // the 35 sums over the terms n -> n+1 of this thread's sites, in the order of its loop
+                double acc[kStatN];
+#pragma unroll
+                for (int v = 0; v < kStatN; ++v) acc[v] = 0.0;
+                const double hdt = (double)prep.hdt;
+                for (int n = tid; n < M; n += T) {
+                    R xn[D], xq[D];
+                    load_vec<R, D, CG>(x, n, xn);
+                    load_vec<R, D, CG>(x, n + 1, xq);
+                    double f0[7], f1[7], psi[8];
+                    Model::regressors(xn, I ? __ldg(I + n) : R(0), hdt, f0);
+                    Model::regressors(xq, I ? __ldg(I + n + 1) : R(0), hdt, f1);
+#pragma unroll
+                    for (int k = 0; k < 7; ++k) psi[k] = f0[k] + f1[k];
+                    psi[7] = (double)xq[0] - (double)xn[0];
+#pragma unroll
+                    for (int j = 0; j < 7; ++j) {
+#pragma unroll
+                        for (int k = j; k < 7; ++k) acc[stat_q(j, k)] = fma(psi[j], psi[k], acc[stat_q(j, k)]);
+                        acc[28 + j] = fma(psi[j], psi[7], acc[28 + j]);
+                    }
+                }
+                // block sums in a fixed order: xor tree inside a warp, then the warps in index order
+#pragma unroll
+                for (int v = 0; v < kStatN; ++v) {
+                    double q = acc[v];
+#pragma unroll
+                    for (int off = 16; off > 0; off >>= 1) q += __shfl_xor_sync(0xFFFFFFFFu, q, off);
+                    if ((tid & 31) == 0) st_part[(tid >> 5) * kStatCols + v] = q;
+                }
+                __syncthreads();
+                if (tid < kStatN) {
+                    double q = 0.0;
+                    for (int wq = 0; wq < (T >> 5); ++wq) q += st_part[wq * kStatCols + tid];
+                    st_tot[tid] = q;
+                }
+                __syncthreads();
+                double S[kStatN], dAs[NP];
+#pragma unroll
+                for (int v = 0; v < kStatN; ++v) S[v] = st_tot[v];
+                R prm[NP];
+#pragma unroll
+                for (int k = 0; k < NP; ++k) prm[k] = ps[k];
+                unsigned n_prop = 0, n_acc = 0;
+                const bool changed = stat_decide<Model, R>(S, prm, 0.5 * (double)Rfs[0], st_in, st_pl, st_logu, 1, n_prop, n_acc, dAs);
+                __syncthreads();                         // everybody has read ps
+                if (tid == 0) {
+#pragma unroll
+                    for (int l = 0; l < NP; ++l) {
+                        ps[l] = prm[l];
+                        if (n_acc >> l & 1u) s_ntune[l] += 1u;
+                        s_pprop[l] += n_prop >> l & 1u;
+                        s_pacc[l] += n_acc >> l & 1u;
+                        if (trace) {
+                            const bool frozen = !(n_prop >> l & 1u);
+                            if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = frozen ? (R)__longlong_as_double(0x7FF8000000000000ll) : (R)dAs[l];
+                            if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = (n_acc >> l & 1u) ? 1 : 0;
+                            if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = frozen ? prm[l] : (R)st_pl[l];
+                        }
+                    }
+                }
+                if (changed) {                           // the V entry of the cache under the final parameters (the gate entries hold no parameter)
+                    const typename Model::Prep pq = Model::prepare(prm, a.dt);
+                    R* gcur = cur ? g_b : g_a;
+                    for (int n = tid; n <= M; n += T) {
+                        R xn[D];
+                        load_vec<R, D, CG>(x, n, xn);
+                        const R c0 = pq.hdt * Model::rhs_V(xn, prm, pq.inv_C, I ? __ldg(I + n) : R(0));
+                        gcur[(size_t)n * D] = fabs(xn[0]) < Model::kVmax ? c0 : (R)__longlong_as_double(0x7FF8000000000000ll);
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        if (a.do_params && !stat_done) {
             for (int l = 0; l < NP; ++l) {
                 if (!(wps[l] > 0.0)) continue;
                 // one thread draws the proposal and the accept uniform; everybody needs p', log u and the bounds verdict

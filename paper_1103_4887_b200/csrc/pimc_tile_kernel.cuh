@@ -23,7 +23,6 @@
 #pragma once
 #include "pimc_kernels.cuh"
 #include "pimc_exchange.cuh"
-#include <type_traits>
 
 namespace pimc {
 
@@ -32,20 +31,6 @@ constexpr int kTileMaxCtas = 256;                                  // inbox slot
 constexpr int kArSlotWords = 16;                                   // one 128-byte line per CTA: slots sharing a line serialise in L2 (measured 2x slower)
 constexpr int kHaloWordsPerSide = kTileHaloMax * 2 * kMaxD * 2;    // h sites x (x, g) x D values x 2 words
 constexpr unsigned long long kSpinLimit = 20ull * 1000 * 1000;    // polls before a hand-off is declared lost
-// Sufficient statistics of the trapezoid parameter moves (Model::NTH = 7 monomials): the 28 entries of the symmetric matrix
-// Q = sum psi psi^T and the 7 entries of b = sum d psi; product v of the table below is psi[kStatJ[v]] * (kStatK[v] < 7 ? psi[kStatK[v]] : d).
-constexpr int kStatN = 35;
-constexpr int kStatSlots = 40;                                     // packets per mailbox record (35 used)
-constexpr int kStatCols = 36;                                      // product columns of the in-CTA reduction (35 used)
-__device__ const signed char kStatJ[kStatCols] = {0, 0, 0, 0, 0, 0, 0, 1, 1, 1, 1, 1, 1, 2, 2, 2, 2, 2, 3, 3, 3, 3, 4, 4, 4, 5, 5, 6, 0, 1, 2, 3, 4, 5, 6, 0};
-__device__ const signed char kStatK[kStatCols] = {0, 1, 2, 3, 4, 5, 6, 1, 2, 3, 4, 5, 6, 2, 3, 4, 5, 6, 3, 4, 5, 6, 4, 5, 6, 5, 6, 6, 7, 7, 7, 7, 7, 7, 7, 7};
-// entry (j, k), j <= k, of Q in that order
-__host__ __device__ constexpr int stat_q(int j, int k) { return j * 7 - j * (j - 1) / 2 + (k - j); }
-__host__ __device__ constexpr int stat_qs(int j, int k) { return j <= k ? stat_q(j, k) : stat_q(k, j); }
-template <int N, class F> __device__ __forceinline__ void static_for(F&& f) {
-    if constexpr (N > 0) { static_for<N - 1>(f); f(std::integral_constant<int, N - 1>{}); }
-}
-
 // ---- 8-byte tagged packets ---------------------------------------------------------------------------------
 __device__ __forceinline__ void ll_store(unsigned long long* p, uint32_t payload, uint32_t tag) {
     const unsigned long long v = ((unsigned long long)tag << 32) | (unsigned long long)payload;
@@ -662,65 +647,21 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
             bool params_changed = false;
             if (tid < TC) {
             if (!drawn && i + 1 < a.n_sweeps) produce(set ^ 1, t + 1ull, tid, 1, 2, false);      // no exchange this sweep: nothing to hide it behind
-            // Decisions, in sequence, by every compute thread from the same totals.  With v = Q theta - b for the CURRENT parameters,
-            //   Delta-A = (Rf_V / 2) sum_j dtheta_j (2 v_j + (Q dtheta)_j),  and on accept  v += Q dtheta;
-            // a move of parameter l changes the monomials Model::theta_mask(l) only (compile-time: the loop over l is unrolled).
-            double S[kStatN];
+            // Decisions, in sequence, by every compute thread from the same totals (stat_decide, pimc_stat.cuh)
+            double S[kStatN], dAs[NP];
 #pragma unroll
             for (int v = 0; v < kStatN; ++v) S[v] = any ? sm.st_tot[v] : 0.0;
-            double ic = Model::theta_pre(prm);
-            double th[7], vv[7];
-            Model::theta_from(prm, ic, th);
+            unsigned n_prop = 0, n_acc = 0;
+            params_changed = stat_decide<Model, R>(S, prm, 0.5 * (double)rf(0), sm.s_in, sm.s_pl, sm.pdraw + (set * kMaxNp) * 2 + 1, 2, n_prop, n_acc, dAs);
+            if (trace && b == 0 && tid == 0) {
 #pragma unroll
-            for (int j = 0; j < 7; ++j) {
-                double row = -S[28 + j];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) row = fma(S[stat_qs(j, k)], th[k], row);
-                vv[j] = row;
+                for (int l = 0; l < NP; ++l)
+                    if (n_prop >> l & 1u) {
+                        if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = (R)dAs[l];
+                        if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = (n_acc >> l & 1u) ? 1 : 0;
+                        if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = (R)sm.s_pl[l];
+                    }
             }
-            const double half_rf = 0.5 * (double)rf(0);
-            unsigned n_prop = 0, n_acc = 0;        // bit fields: 4 bits per parameter are not enough -- one move per parameter and sweep, so 1 bit each
-            static_for<NP>([&](auto LC) {          // branch-free and unrolled: everything that does not hang on the previous decision is hoisted
-                constexpr int l = decltype(LC)::value;
-                constexpr unsigned mask = Model::theta_mask(l);
-                const int st = sm.s_in[l];
-                const double pl = sm.s_pl[l], logu = sm.pdraw[(set * kMaxNp + l) * 2 + 1];
-                R pp[NP];
-#pragma unroll
-                for (int k = 0; k < NP; ++k) pp[k] = (k == l) ? (R)pl : prm[k];
-                const double ic2 = mask == 0x7Fu ? Model::theta_pre(pp) : ic;
-                double th2[7], dth[7], qd[7];
-                Model::theta_from(pp, ic2, th2);
-#pragma unroll
-                for (int j = 0; j < 7; ++j) dth[j] = (mask >> j & 1u) ? th2[j] - th[j] : 0.0;
-#pragma unroll
-                for (int j = 0; j < 7; ++j) {
-                    double r = 0.0;
-#pragma unroll
-                    for (int k = 0; k < 7; ++k) if (mask >> k & 1u) r = fma(S[stat_qs(j, k)], dth[k], r);
-                    qd[j] = r;
-                }
-                double acc = 0.0;
-#pragma unroll
-                for (int j = 0; j < 7; ++j) if (mask >> j & 1u) acc = fma(dth[j], fma(2.0, vv[j], qd[j]), acc);
-                const double dA = half_rf * acc;
-                const bool accept = st == 2 && logu < -dA;
-#pragma unroll
-                for (int j = 0; j < 7; ++j) {
-                    vv[j] = accept ? vv[j] + qd[j] : vv[j];
-                    if (mask >> j & 1u) th[j] = accept ? th2[j] : th[j];
-                }
-                ic = accept ? ic2 : ic;
-                params_changed = params_changed || accept;
-                prm[l] = accept ? (R)pl : prm[l];
-                n_prop |= (st != 0 ? 1u : 0u) << l;
-                n_acc |= (accept ? 1u : 0u) << l;
-                if (trace && b == 0 && tid == 0 && st != 0) {
-                    if (a.tr_dAp) a.tr_dAp[(size_t)chain * NP + l] = st == 2 ? (R)dA : (R)__longlong_as_double(0x7FF8000000000000ll);
-                    if (a.tr_accp) a.tr_accp[(size_t)chain * NP + l] = accept ? 1 : 0;
-                    if (a.tr_pprop) a.tr_pprop[(size_t)chain * NP + l] = (R)pl;
-                }
-            });
             if (tid < NP) { sm.s_pprop[tid] += n_prop >> tid & 1u; sm.s_pacc[tid] += n_acc >> tid & 1u; }
             if (tid == 0) {
 #pragma unroll

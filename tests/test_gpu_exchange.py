@@ -62,11 +62,9 @@ def test_latency_probes_l2_hit_map_and_one_way_packet():
     assert m["group_a"] + m["group_b"] >= 100
     one_way = {how: Pm.latency_selftest(how, 1) for how in (1, 2, 3, 4, 5)}
     print("one-way ticks to the neighbouring SM (1 st.relaxed, 2 atom.exch, 3 red.max, 4 st.volatile, 5 st.release):", one_way)
-    far_peer = Pm.latency_selftest(1, 0)
-    print("one-way ticks to the last SM, st.relaxed:", far_peer)
     for how in (1, 2, 3, 4):
-        assert 1.5 * m["far"] < one_way[how] < 10 * m["far"], (one_way, m)          # a packet needs several L2-hit times whatever publishes it ...
-    assert 0.7 < far_peer / one_way[1] < 1.4                                           # ... and wherever the peer sits: the hop is not the die crossing
+        assert 1.5 * m["far"] < one_way[how] < 10 * m["far"], (one_way, m)          # a packet needs several L2-hit times whatever publishes it
+        assert 0.8 < one_way[how] / one_way[1] < 1.25, one_way                         # (same lines, same pair: the store flavour does not matter)
     assert one_way[5] > 1.2 * one_way[1]                                               # a release store is the slow way
     # where the line lives: fast only when writer, reader and the line's home share a die; across the dies every line is slow
     w = Pm.latency_selftest(6, 16)

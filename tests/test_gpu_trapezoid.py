@@ -122,10 +122,12 @@ def test_edge_sizes_switching_and_engine_rule_trapezoid(P):
         h.set_discretisation(7)
 
 
-def test_sufficient_statistics_parameter_moves_edge_cases(P):
-    # tile engine, trapezoid rule: the parameter moves come from one reduction of path sums per sweep.  Several chains with
-    # several tiles each (one reducer set per chain), tight bounds (proposals outside are rejected unevaluated), a frozen parameter, the
-    # parameter record, both kinetics: chains bit-identical to the oracle's
+@pytest.mark.parametrize("engine", ["tile", "global_one_cta_per_chain"])
+def test_sufficient_statistics_parameter_moves_edge_cases(P, engine):
+    # trapezoid rule: the parameter moves come from one reduction of path sums per sweep -- on the tile engine (several
+    # chains with several tiles each, one reducer set per chain) and on the global-memory engine with one CTA per chain (block reduction).
+    # Tight bounds (proposals outside are rejected unevaluated), a frozen parameter, the parameter record, both kinetics: chains
+    # bit-identical to the oracle's
     import paper_1103_4887_b200 as Pm
     for kinetics in ("tanh", "classic"):
         w = make_workload(4, M=700, n_chains=3, kinetics=kinetics)
@@ -135,8 +137,12 @@ def test_sufficient_statistics_parameter_moves_edge_cases(P):
         h = gpu_handle(w, kind=1, disc=TRAP)
         h.set_proposal(w.w_state, wp, 1)
         h.set_bounds(lo, hi)
-        h.set_engine(Pm.ENGINE_TILE)
-        assert h.get_launch()["ctas_per_chain"] > 1
+        if engine == "tile":
+            h.set_engine(Pm.ENGINE_TILE)
+            assert h.get_launch()["ctas_per_chain"] > 1
+        else:
+            h.set_engine(Pm.ENGINE_GLOBAL); h.set_launch(1, 160)
+            assert h.get_launch()["ctas_per_chain"] == 1 and h.get_engine()["engine"] == Pm.ENGINE_GLOBAL
         h.set_accum(True, 1); h.reset_moments()
         rec = h.param_trace(25)
         h.sweep(25, seed=21)
