@@ -146,7 +146,7 @@ OTHER_CONFIGS = [   # (config, dtype, sweeps per step, chains or None): every BA
     # the FP64 pipe for the checkerboard sweep": a single chain offers M/2 independent updates per half-sweep, several chains fill the SMs)
     (0, 64, 2000, None), (1, 64, 1000, None), (2, 64, 1000, None), (4, 64, 100, None), (3, 32, 1000, None), (3, 64, 100, 4),
     # the paper's own trapezoid discretisation (Eq. 7): the headline shape, and the paper-shaped workload (config 5, not a BASELINE config)
-    (3, 64, 1000, None, "trapezoid"), (5, 64, 1000, None, "trapezoid"),
+    (3, 64, 1000, None, "trapezoid"), (5, 64, 1000, None, "trapezoid"), (4, 64, 50, None, "trapezoid"),
 ]
 
 
