@@ -609,8 +609,7 @@ __global__ void __launch_bounds__(MAXT, 1) tile_sweep_kernel(const SweepArgs<R> 
                     const long long until = clock64() + (long long)a.ar_hold;
                     auto fetch = [&](int j, int v) -> double {      // tile j's partial of statistic v
                         if (j == b) return cta_partial(v);
-                        while (clock64() < until) {}
-                        return ll_wait_f64(part_of(cta0 + j, v), tag, a.fault);
+                        return ll_wait_f64(part_of(cta0 + j, v), tag, a.fault);     // one reader per packet: no first-poll hold here (measured: it only delays)
                     };
                     if (G >= kStatN) {          // one statistic per reducer: a block sum (fixed tree) of the G packets; every CTA passes here
                         double val = 0.0;
