@@ -78,10 +78,24 @@ __device__ __forceinline__ void bar_compute(int n_threads) {     // named barrie
 // The warp partials are added as a fixed balanced tree (depth 3 for 8 warps), not one after the other: a dependent FP64 add
 // costs ~17 cycles here (measured, pimc_exchange_selftest modes 7-9: xor tree 207 cycles, barrier + serial 8-sum 307), and
 // this sum sits on the critical path of every parameter move twice.  NW = the most warps a CTA of this kernel can have.
+// Sum over the 32 lanes of a warp on the FP64 tensor cores: with A[row = lane / 4][k = lane % 4] = v and B = ones, one mma.sync.m8n8k4 leaves the
+// sum of each group of four lanes in that group; one shuffle level moves the eight group sums onto the k index, two more products with ones
+// add them: a dependent chain of three products and one shuffle instead of five shuffle + add levels.  Same bits in every lane, fixed order.
+__device__ __forceinline__ double warp_sum_mma(double v) {
+    const int lane = threadIdx.x & 31;
+    double c0 = 0.0, c1 = 0.0;
+    const double one = 1.0;
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(v), "d"(one));
+    const double lo = __shfl_sync(0xFFFFFFFFu, c0, 4 * (lane & 3)), hi = __shfl_sync(0xFFFFFFFFu, c0, 16 + 4 * (lane & 3));
+    double d0 = 0.0, d1 = 0.0;
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(lo), "d"(one));
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(hi), "d"(one));
+    return d0;
+}
+
 template <int NW = 16>
 __device__ __forceinline__ double block_sum_db(double v, double* red /* 64 doubles */, unsigned& phase) {
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+    v = warp_sum_mma(v);
     double* buf = red + (phase & 1u) * 32;
     phase ^= 1u;
     const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;

@@ -33,8 +33,7 @@ __device__ __forceinline__ void bar_group(int grp) { asm volatile("bar.sync %0, 
 
 // Deterministic sum over the 128 threads of a group with ONE named barrier (alternating buffers as in block_sum_db).
 __device__ __forceinline__ double group_sum(double v, double* red /* [2][4] */, unsigned& phase, int grp, int j) {
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, off);
+    v = warp_sum_mma(v);
     double* buf = red + (phase & 1u) * 4;
     phase ^= 1u;
     if ((j & 31) == 0) buf[j >> 5] = v;
