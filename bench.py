@@ -41,13 +41,14 @@ W_EVAL_ORACLE = 666.0
 #     reciprocal series instead of two divides per gate, cached first-stage gate rates in parameter moves), so the useful
 #     fraction credits min((1), (2) / redundancy).
 EXEC_FP64_COMPUTED = {   # engine -> (per COMPUTED site update, per COMPUTED parameter-move evaluation); HH tanh kinetics, fp64, RK4 map, joint updates
-    "tile": (520.1, 264.9),      # tile_sweep_kernel, profiles/r02_work_counts.md: 595.0 and 303.1 per OWNED unit at cfg3 / (254 / 222)
+    "tile": (519.4, 252.2),      # tile_sweep_kernel, profiles/r02_head_verification.md: 594.2 and 288.5 per OWNED unit at cfg3 / (254 / 222)
+                                 # (303.1 per evaluation until the warp sums of the block reductions moved to the FP64 tensor cores)
     "tilemc": (502.4, 255.4),    # tilemc_sweep_kernel (many-chain tile-resident engine), profiles/r02_tilemc.md: 545 and 277 per OWNED unit at cfg4 / (256 / 236)
     "global": (521.0, 285.0),    # sweep_kernel (one CTA per chain, no halos, stage-1 rates cached in global memory), profiles/r02_cfg4.md: launch total minus
                                  # 521 per site update, over the evaluations
 }
 # ncu sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed of the same kernels, same launches
-NCU_PIPE_FP64_ACTIVE = {3: {"full_sweep": 0.310, "a2_only": 0.427, "a4_only": 0.274, "source": "profiles/r02_final.md"},
+NCU_PIPE_FP64_ACTIVE = {3: {"full_sweep": 0.310, "a2_only": 0.431, "a4_only": 0.272, "source": "profiles/r02_head_verification.md"},
                         4: {"full_sweep": 0.527, "a2_only": 0.518, "a4_only": 0.513, "source": "profiles/r02_tilemc.md (TILE_MC engine; GLOBAL engine: 0.453, profiles/r02_cfg4.md)"}}
 # trapezoid discretisation / component-wise updates: estimated slots (no oracle count yet), used for the non-headline variants only
 W_SITE_SLOTS_TRAP = 380.0
