@@ -377,7 +377,7 @@ def run_ours(args):
                 "pipe_fp64_active_ncu": NCU_PIPE_FP64_ACTIVE.get(args.config) if exec_counts else None,
                 "target": ("north_star: >= 50 % of the FP64 pipe for the checkerboard sweep (A2), judged on ncu's sm__pipe_fp64_cycles_active: ONE chain of M = 32768 "
                            "(config 3, this line's workload when --config 3): 42.7 %, NOT reached (M/2 independent updates per half-sweep are one warp per scheduler); "
-                           "many chains per launch (config 4 on the TILE_MC engine): 51.8 %, reached (profiles/r02_tilemc.md)"),
+                           "several chains per launch on the TILE_MC engine: 54.3 % for four chains of M = 32768, 51.8 % for config 4: reached (profiles/r02_tilemc.md)"),
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (headline and args.dtype == 64) else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full, profiles/r02_work_counts.md (tile loaded once, written back once: independent of the sweeps per launch)",
                 "peak_source": ("derived: 148 SM x 64 FP64 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md); no FP64 figure in MEASURED_PEAKS.json" if args.dtype == 64 else "derived: 148 SM x 128 FP32 lanes/clk x 1.965 GHz x 2 FLOP (DESIGN.md)"),
